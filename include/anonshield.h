@@ -1,0 +1,204 @@
+/*
+ * anonshield.h -- C ABI of the B200-native AnonShield pseudonymization hot path
+ * (arxiv/paper_2606_15650).  Every entry point is plain C: pointers + sizes, no C++ or
+ * torch types.  `d_*` arguments are DEVICE pointers owned by the caller (allocated e.g.
+ * through PyTorch); `h_*` / un-prefixed pointers are HOST pointers.  The library never
+ * frees caller memory and keeps no caller pointer after a call returns, except inside
+ * handles it created (anon_weights keeps its own device copy of the parameters,
+ * anon_cache copies entity bytes into its own arena).
+ *
+ * Citations: P:L<n> = /root/reference/PAPER.md line n; BJ = BASELINE.json north_star;
+ * S8x = SURVEY.md section 8(x); Dn = DESIGN.md reading n.
+ *
+ * Execution model.  All work is enqueued on the cudaStream_t given to anon_ctx_create.
+ * Calls are asynchronous with respect to the host unless stated ("synchronises").
+ * Device-side failures that are only known after kernels ran (span list / arena
+ * capacity, table full) are latched in a sticky per-context status word that
+ * anon_ctx_sync() returns and clears.  No exception or abort crosses the ABI.  One
+ * context per host thread; handles are not thread-safe.  There is NO CPU fallback: on a
+ * machine without a CUDA device every compute call returns ANON_ERR_CUDA.
+ */
+#ifndef ANONSHIELD_H
+#define ANONSHIELD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- return codes -------------------------------------------------------------------- */
+#define ANON_OK                 0
+#define ANON_ERR_INVALID_ARG   -1   /* NULL where a pointer is required, negative size ...        */
+#define ANON_ERR_UNSUPPORTED   -2   /* d_head != 64, n_i > max_pos, even num_labels, S >= 2^31 ... */
+#define ANON_ERR_CAPACITY      -3   /* span list / cache / arena / output buffer too small; the   */
+                                    /* needed count is still written where the call documents it  */
+#define ANON_ERR_KEY_MISMATCH  -4   /* cache already bound to another HMAC key                    */
+#define ANON_ERR_CUDA          -5   /* CUDA runtime error; see anon_last_cuda_error               */
+#define ANON_ERR_OOM           -6   /* workspace or device allocation too small / failed          */
+
+typedef struct anon_ctx     anon_ctx;
+typedef struct anon_weights anon_weights;
+typedef struct anon_cache   anon_cache;
+
+/* Encoder shape (BJ "embedding plus L encoder layers ... then the token-classification
+ * head"; S8c O1).  dtype: 0 = FP32 parameters and arithmetic (BJ configs[0]);
+ * 1 = BF16 matrices/embeddings, FP32 accumulate, FP32 residual stream / LayerNorm /
+ * softmax / logits (BJ configs[1..3], S8c reading S8). */
+typedef struct {
+    int32_t layers, hidden, heads, ffn, vocab, num_labels, max_pos;
+    float   ln_eps;
+    int32_t dtype;
+} anon_model_desc;
+
+/* Per-token metadata for span decoding (S8c O3).  flags bit0 = keep. */
+typedef struct { int32_t record_id, char_start, char_end, flags; } anon_tok_meta;
+/* One decoded entity span: bytes [char_start, char_end) of record record_id. */
+typedef struct { int32_t record_id, char_start, char_end, type; } anon_span;
+
+const char* anon_strerror(int code);
+/* Name of every exported entry point, NULL-terminated (used by the load/export test). */
+const char* const* anon_exported_symbols(void);
+
+/* ---- context --------------------------------------------------------------------------- */
+/* Creates a context on CUDA device `device` that enqueues on `cuda_stream` (a cudaStream_t
+ * passed as void*; NULL = the legacy default stream) and owns a scratch workspace of
+ * `workspace_bytes` bytes of device memory (0 is legal: calls that need scratch then
+ * return ANON_ERR_OOM).  Synchronises.  Errors: INVALID_ARG, CUDA, OOM. */
+int  anon_ctx_create(anon_ctx** out, int device, void* cuda_stream, size_t workspace_bytes);
+void anon_ctx_destroy(anon_ctx* ctx);
+/* Waits for the context's stream; returns and clears the sticky device status (ANON_OK,
+ * ANON_ERR_CAPACITY, ANON_ERR_UNSUPPORTED or ANON_ERR_CUDA). */
+int  anon_ctx_sync(anon_ctx* ctx);
+/* Text of the last CUDA error seen by this context ("" if none).  Owned by the context. */
+const char* anon_last_cuda_error(anon_ctx* ctx);
+/* Scratch bytes anon_ner_forward needs to process `max_tokens` packed tokens in
+ * `max_seqs` sequences in ONE pass; with less, anon_ner_forward splits the batch into
+ * sequence-aligned chunks that fit (at least one 512-token sequence must fit).  Also
+ * covers anon_decode_spans / anon_gather_spans / anon_pseudonymize for max_tokens items. */
+size_t anon_workspace_bytes(const anon_model_desc* desc, int64_t max_tokens, int32_t max_seqs);
+
+/* ---- parameters -------------------------------------------------------------------------- */
+/* Uploads the parameters.  `host_fp32_blob` holds n_floats FP32 values in the fixed order
+ *   E_w[V,H], E_p[max_pos,H], E_t[H], g_e[H], b_e[H],
+ *   { W_qkv[3H,H], b_qkv[3H], W_o[H,H], b_o[H], g_1[H], b_1[H],
+ *     W_1[F,H], b_1f[F], W_2[H,F], b_2f[H], g_2[H], b_2[H] } x layers,
+ *   W_c[NL,H], b_c[NL]
+ * (all matrices row-major [out,in]: y = W x + b; S8d W0).  For dtype 1 the matrices and
+ * embedding tables are converted to BF16 (round-to-nearest-even; exact when the caller
+ * pre-rounded them).  Synchronises.  Errors: INVALID_ARG (size mismatch), UNSUPPORTED
+ * (hidden/heads != 64, hidden % 64, ffn % 64, even num_labels, num_labels > 64,
+ * max_pos > 512), CUDA, OOM. */
+int  anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, const float* host_fp32_blob,
+                       size_t n_floats, anon_weights** out);
+void anon_weights_free(anon_weights* w);
+
+/* ---- A1-A8: encoder forward + head + argmax (BJ ¶1; S8c O1, O2) ---------------------- */
+/* d_token_ids int32[T] packed, d_cu_seqlens int32[B+1] with [0]=0, [B]=T, every length in
+ * [0, max_pos].  Position ids are 0..n_i-1 inside each sequence; attention spans exactly
+ * the tokens of the same sequence (bidirectional).  Writes logits FP32 [T, num_labels]
+ * row-major if d_logits != NULL and labels int32[T] (argmax, ties -> lowest index, taken on
+ * the FP32 logits) if d_labels != NULL.  Reads d_cu_seqlens on the host (one small D2H
+ * copy + stream sync at entry) to plan chunks and attention work.  Errors: INVALID_ARG,
+ * UNSUPPORTED (a sequence longer than max_pos, token id outside [0,V) is clamped and
+ * latches UNSUPPORTED in the sticky status), OOM (workspace cannot hold one sequence), CUDA. */
+int  anon_ner_forward(anon_ctx* ctx, const anon_weights* w,
+                      const int32_t* d_token_ids, const int32_t* d_cu_seqlens, int32_t B, int32_t T,
+                      float* d_logits, int32_t* d_labels);
+
+/* ---- A9: BIO decode + stream compaction (BJ ¶1; S8c O3) -------------------------------------- */
+/* Label map 0 = O, 2t+1 = B-t, 2t+2 = I-t.  Tokens with keep = 0 are transparent.  Spans are
+ * written in order of their first token.  *d_num_spans (device int32) receives the TOTAL
+ * number of spans found even when it exceeds span_capacity; only the first span_capacity
+ * are written and ANON_ERR_CAPACITY is latched in the sticky status.  Asynchronous. */
+int  anon_decode_spans(anon_ctx* ctx, const int32_t* d_labels, const anon_tok_meta* d_meta, int32_t T,
+                       int32_t num_labels, anon_span* d_spans, int32_t span_capacity, int32_t* d_num_spans);
+
+/* ---- A10: span byte gather (S8a A10) ---------------------------------------------------------- */
+/* span_bytes[off_s : off_s + len_s] = text[rec_off[record_id] + char_start : ... + char_end],
+ * d_span_offsets int64[S+1] = exclusive prefix sum of the lengths; d_span_type uint8[S]
+ * (optional) receives spans[s].type.  If the total exceeds bytes_capacity nothing beyond it
+ * is written and ANON_ERR_CAPACITY is latched.  Asynchronous. */
+int  anon_gather_spans(anon_ctx* ctx, const uint8_t* d_text, const int64_t* d_record_offsets,
+                       const anon_span* d_spans, int32_t S,
+                       uint8_t* d_span_bytes, size_t bytes_capacity, int64_t* d_span_offsets,
+                       uint8_t* d_span_type);
+
+/* ---- A11-A13: hash-cache dedup, HMAC-SHA256, pseudonym write-back (S8c O4) */
+/* An open-addressing table with room for max_unique distinct entity strings (slots =
+ * next power of two >= 2*max_unique) plus an arena of key_arena_bytes for their bytes and
+ * 32 bytes of digest each.  No eviction (reading S18).  Synchronises. */
+int  anon_cache_create(anon_ctx* ctx, uint64_t max_unique, uint64_t key_arena_bytes, anon_cache** out);
+void anon_cache_destroy(anon_cache* c);
+/* Counters since creation.  Synchronises. */
+int  anon_cache_stats(anon_cache* c, uint64_t* n_unique, uint64_t* n_lookups, uint64_t* n_hits);
+/* Entry `uid` (0 <= uid < n_unique): copies min(len, bytes_capacity) entity bytes to
+ * h_bytes (may be NULL), the 32-byte digest to h_digest (may be NULL); returns the entity
+ * length or a negative error.  Synchronises.  (The (entity, slug, full_hash) hand-off
+ * of P:L52.) */
+int64_t anon_cache_entry(anon_cache* c, uint64_t uid, uint8_t* h_bytes, size_t bytes_capacity,
+                         uint8_t* h_digest);
+
+/* For span i = 0..S-1 in order (e_i = d_span_bytes[off[i] .. off[i+1]), exact bytes):
+ *   hit[i] = 1 if e_i is already in the cache (from an earlier call or an earlier i), else 0
+ *            and (HMAC_SHA256(key, e_i), uid = number of entries before insertion) is inserted;
+ *   uid[i] = uid of e_i;  digests[i] = its 32-byte HMAC;
+ *   out[i] = "[" type_names[type[i]] "_" lowerhex(digest)[0:slug_len] "]"   (type 0 if d_span_type NULL);
+ *   d_out_offsets int64[S+1] = exclusive prefix sum of the token lengths.
+ * key: HOST pointer, any length (keys > 64 bytes are hashed first, RFC 2104).  The cache
+ * binds to the first key it sees; another key -> ANON_ERR_KEY_MISMATCH.  slug_len in
+ * [0,64].  type_names: HOST array of num_types NUL-terminated ASCII names (<= 32 bytes
+ * each, num_types <= 64); a type >= num_types is clamped to num_types-1 and latches
+ * ANON_ERR_UNSUPPORTED in the sticky status.  d_hit / d_uid / d_digests may be NULL.
+ * Synchronises once (to learn how many entities are new, so that capacity errors are
+ * returned, not latched): on ANON_ERR_CAPACITY (max_unique, arena or out_capacity
+ * exceeded) the cache is left exactly as before the call.  S must be < 2^31. */
+int  anon_pseudonymize(anon_ctx* ctx, anon_cache* cache,
+                       const uint8_t* d_span_bytes, const int64_t* d_span_offsets,
+                       const uint8_t* d_span_type, int64_t S,
+                       const uint8_t* key, size_t key_len, int32_t slug_len,
+                       const char* const* type_names, int32_t num_types,
+                       uint8_t* d_out_tokens, size_t out_capacity, int64_t* d_out_offsets,
+                       uint8_t* d_hit, int64_t* d_uid, uint8_t* d_digests);
+
+/* A12 alone, dedup disabled: digests[i] = HMAC_SHA256(key, e_i) for every span (used to
+ * measure the SHA-256 kernel's integer issue rate, S8d c5).  Asynchronous. */
+int  anon_hmac_spans(anon_ctx* ctx, const uint8_t* d_span_bytes, const int64_t* d_span_offsets, int64_t S,
+                     const uint8_t* key, size_t key_len, uint8_t* d_digests /* [S,32] */);
+
+/* ---- whole hot path with HOST buffers (the call a user makes; bench.py's e2e leg) ------------- */
+/* Copies one batch host->device, runs A1-A13 and copies the results back, all on the
+ * context's stream; synchronises before returning.  Host inputs: token_ids int32[T],
+ * cu_seqlens int32[B+1], meta[T], text uint8[text_bytes], record_offsets int64[R+1].
+ * Host outputs: spans[span_capacity], *num_spans, out_tokens[out_capacity],
+ * out_offsets int64[span_capacity+1], hit uint8[span_capacity] (may be NULL).
+ * Device staging comes from the context workspace (ANON_ERR_OOM if too small).  Returns
+ * ANON_ERR_CAPACITY (with *num_spans = needed) if the span list or outputs do not fit. */
+int  anon_pipeline_host(anon_ctx* ctx, const anon_weights* w, anon_cache* cache,
+                        const int32_t* h_token_ids, const int32_t* h_cu_seqlens, int32_t B, int32_t T,
+                        const anon_tok_meta* h_meta, const uint8_t* h_text, size_t text_bytes,
+                        const int64_t* h_record_offsets, int32_t R,
+                        const uint8_t* key, size_t key_len, int32_t slug_len,
+                        const char* const* type_names, int32_t num_types,
+                        anon_span* h_spans, int32_t span_capacity, int32_t* h_num_spans,
+                        uint8_t* h_out_tokens, size_t out_capacity, int64_t* h_out_offsets,
+                        uint8_t* h_hit);
+
+/* ---- building blocks exported for parity tests and per-kernel roofline measurement ----------- */
+/* C[M,N] = A[M,K] * W[N,K]^T + bias[N], BF16 operands, FP32 accumulate on the tcgen05
+ * tensor cores (S8a A2/A4/A5/A6).  epilogue: 0 = bias -> BF16 out; 1 = bias, erf-GELU ->
+ * BF16 out; 2 = bias + FP32 residual[M,N] -> FP32 out.  K % 64 == 0, N % 8 == 0 required.
+ * d_A, d_W BF16 (uint16 bit patterns) row-major, 16-byte aligned.  Asynchronous. */
+int  anon_gemm_bf16(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,
+                    const float* d_residual, void* d_C, int32_t M, int32_t N, int32_t K, int32_t epilogue);
+/* ctx[T,H] = varlen bidirectional softmax attention over qkv[T,3H] (S8a A3); dtype as in
+ * anon_model_desc (0: FP32 qkv/ctx, 1: BF16).  h_cu_seqlens is a HOST pointer.  Asynchronous. */
+int  anon_attention(anon_ctx* ctx, const void* d_qkv, const int32_t* d_cu_seqlens,
+                    const int32_t* h_cu_seqlens, int32_t B, int32_t T, int32_t hidden, int32_t heads,
+                    int32_t dtype, void* d_ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ANONSHIELD_H */

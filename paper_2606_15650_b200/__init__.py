@@ -1,0 +1,8 @@
+"""paper_2606_15650_b200 -- B200-native (sm_100a) hot path of AnonShield's pseudonymization pipeline.
+
+The product is the C-ABI library `libanonshield.so` (csrc/, declared in include/anonshield.h); this package
+is its thin Python binding.  See DESIGN.md.
+"""
+from .binding import (AnonError, Cache, Context, ModelDesc, Weights, anon_attention, anon_decode_spans,  # noqa: F401
+                      anon_gather_spans, anon_gemm_bf16, anon_hmac_spans, anon_ner_forward, anon_pipeline_host,
+                      anon_pseudonymize, anon_workspace_bytes, lib)

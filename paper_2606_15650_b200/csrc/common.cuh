@@ -1,0 +1,76 @@
+// common.cuh -- context, error plumbing and workspace cursor shared by the translation units of
+// libanonshield.so (product code; shares nothing with oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/anonshield.h"
+
+struct anon_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    uint8_t* ws = nullptr;          // device scratch
+    size_t ws_bytes = 0;
+    int* d_status = nullptr;        // sticky device-side status word (0 = ok, else first ANON_ERR_*)
+    uint8_t* h_pinned = nullptr;    // small pinned host buffer for read-backs
+    size_t h_pinned_bytes = 0;
+    int sm_count = 148;
+    char cuda_err[256] = {0};
+    // cached driver entry point for cuTensorMapEncodeTiled (resolved lazily, see gemm_tcgen05.cu)
+    void* encode_tiled = nullptr;
+    int smem_optin = 0;
+};
+
+// Bump cursor over the context workspace.  Every public entry point starts one at offset 0
+// (stream order makes reuse across calls safe); anon_pipeline_host carves its staging first and
+// hands the remainder to the stages.
+struct WsCursor {
+    uint8_t* base; size_t cap; size_t used;
+    __host__ void* take(size_t bytes, size_t align = 256) {
+        size_t o = (used + align - 1) / align * align;
+        if (o + bytes > cap) return nullptr;
+        used = o + bytes;
+        return base + o;
+    }
+    __host__ size_t left() const { return cap > used ? cap - used : 0; }
+};
+static inline WsCursor ws_begin(anon_ctx* c) { return WsCursor{c->ws, c->ws_bytes, 0}; }
+
+static inline int cuda_fail(anon_ctx* c, cudaError_t e, const char* what) {
+    if (c) snprintf(c->cuda_err, sizeof c->cuda_err, "%s: %s", what, cudaGetErrorString(e));
+    return ANON_ERR_CUDA;
+}
+#define CU_TRY(ctx, expr)                                                            \
+    do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return cuda_fail((ctx), e__, #expr); } while (0)
+#define CU_LAUNCH_CHECK(ctx, name)                                                   \
+    do { cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return cuda_fail((ctx), e__, name); } while (0)
+
+__device__ __forceinline__ void latch_status(int* d_status, int code) { atomicCAS(d_status, 0, code); }
+
+static inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// ---- internal stage entry points (defined in the per-stage .cu files; all take a cursor) ----
+struct anon_weights;
+int ner_forward_impl(anon_ctx*, WsCursor&, const anon_weights*, const int32_t* d_ids, const int32_t* d_cu,
+                     const int32_t* h_cu, int32_t B, int32_t T, float* d_logits, int32_t* d_labels);
+int decode_spans_impl(anon_ctx*, WsCursor&, const int32_t* d_labels, const anon_tok_meta* d_meta, int32_t T,
+                      int32_t num_labels, anon_span* d_spans, int32_t cap, int32_t* d_num);
+int gather_spans_impl(anon_ctx*, WsCursor&, const uint8_t* d_text, const int64_t* d_rec_off,
+                      const anon_span* d_spans, const int32_t* d_num_spans, int32_t S_max,
+                      uint8_t* d_bytes, size_t cap, int64_t* d_off, uint8_t* d_type);
+int pseudonymize_impl(anon_ctx*, WsCursor&, anon_cache*, const uint8_t* d_bytes, const int64_t* d_off,
+                      const uint8_t* d_type, int64_t S, const uint8_t* key, size_t key_len, int32_t slug_len,
+                      const char* const* type_names, int32_t num_types, uint8_t* d_out, size_t out_cap,
+                      int64_t* d_out_off, uint8_t* d_hit, int64_t* d_uid, uint8_t* d_digests,
+                      int64_t* total_out_bytes);
+int gemm_bf16_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias,
+                   const float* residual, void* C, int M, int N, int K, int epilogue);
+struct AttnPlan { void* d_work; int n_items; };
+int attention_plan(anon_ctx*, WsCursor&, const int32_t* h_cu, int B, int dtype, AttnPlan* plan);
+int attention_run(anon_ctx*, const AttnPlan&, const void* d_qkv, const int32_t* d_cu, int tok0, int B, int hidden,
+                  int heads, int dtype, void* d_ctx);
+const anon_model_desc* weights_desc(const anon_weights* w);

@@ -1,0 +1,489 @@
+// crypto.cu -- A11 hash-cache dedup (K9), A12 HMAC-SHA256 (K10), A13 pseudonym write-back (K11).
+// P:L43 (cache), P:L44 (HMAC-SHA256 slug, "[TYPE_slug]"), P:L50/L38 (referential integrity),
+// P:L52 (entity, slug, full_hash rows); S8c O4; FIPS 180-4; RFC 2104.
+//
+// Determinism.  The sequential definition ("for i in order: hit or insert") is reproduced by a
+// parallel protocol on one 64-bit word per slot:  [tag:32 | pending:1 | index:31].
+//   probe    every span finds the slot of its string (full byte compare, never tag-only); the
+//            first claimer CASes (tag, pending, i) into an empty slot and every later span of the
+//            same string lowers the index with atomicMin, so the slot ends up naming the LOWEST
+//            span index of each string that was not cached before the call.
+//   classify span i is a miss iff its slot is pending and names i.  A transform-scan over
+//            (miss, miss bytes, token bytes) gives dense uids in first-occurrence order, arena
+//            offsets and out_offsets; the totals go to the host, which checks capacity BEFORE
+//            anything persistent is written (otherwise the pending slots are rolled back to 0).
+//   insert   one thread per NEW entity: copy bytes into the arena, HMAC, slot := (tag, 0, uid).
+//   emit     every span reads its slot -> uid -> digest and writes its token.
+#include "common.cuh"
+#include "scan.cuh"
+#include "sha256.cuh"
+
+#include <new>
+
+typedef unsigned long long u64;
+
+struct anon_cache {
+    anon_ctx* ctx = nullptr;
+    uint64_t max_unique = 0, arena_bytes = 0, n_slots = 0;
+    u64* d_table = nullptr;
+    uint8_t* d_arena = nullptr;
+    long long* d_entry_off = nullptr;   // [max_unique + 1]
+    uint8_t* d_digests = nullptr;       // [max_unique, 32]
+    uint64_t n_unique = 0, arena_used = 0, n_lookups = 0, n_hits = 0;
+    bool key_bound = false;
+    uint32_t ipad[8], opad[8];
+};
+
+struct PadStates { uint32_t ipad[8], opad[8]; };
+struct TypeTable { uint8_t len[64]; char name[64][32]; int num; };
+
+// ------------------------------------------------------------------------------------------------
+// byte-stream helpers: read a message at any alignment as little-endian 32-bit words
+// ------------------------------------------------------------------------------------------------
+// bytes p[4j .. 4j+3], zero-filled past len.  Requires 4j < len.  Touches only aligned words that
+// contain at least one byte of the message.
+__device__ __forceinline__ uint32_t load_le_word(const uint8_t* p, int len, int j) {
+    const uintptr_t addr = (uintptr_t)(p + 4 * j);
+    const uint32_t a = (uint32_t)(addr & 3);
+    const uint32_t* q = (const uint32_t*)(addr - a);
+    const int remaining = len - 4 * j;
+    uint32_t w = __ldg(q);
+    if (a) {
+        uint32_t hi = (remaining > (int)(4 - a)) ? __ldg(q + 1) : 0u;
+        w = __funnelshift_r(w, hi, 8 * a);
+    }
+    if (remaining < 4) w &= (1u << (8 * remaining)) - 1u;
+    return w;
+}
+
+__device__ __forceinline__ u64 hash_bytes(const uint8_t* p, int len) {
+    u64 h = 0x9E3779B97F4A7C15ull ^ ((u64)(uint32_t)len * 0xFF51AFD7ED558CCDull);
+    const int nw = (len + 3) >> 2;
+    for (int j = 0; j < nw; j++) {
+        h = (h ^ load_le_word(p, len, j)) * 0xD6E8FEB86659FD93ull;
+        h ^= h >> 32;
+    }
+    h ^= h >> 33; h *= 0xFF51AFD7ED558CCDull; h ^= h >> 33; h *= 0xC4CEB9FE1A85EC53ull; h ^= h >> 33;
+    return h;
+}
+
+__device__ __forceinline__ bool bytes_equal(const uint8_t* a, const uint8_t* b, int len) {
+    const int nw = (len + 3) >> 2;
+    for (int j = 0; j < nw; j++)
+        if (load_le_word(a, len, j) != load_le_word(b, len, j)) return false;
+    return true;
+}
+
+__device__ __forceinline__ uint32_t slot_tag(u64 h) { uint32_t t = (uint32_t)(h >> 32); return t ? t : 1u; }
+__device__ __forceinline__ u64 make_slot(uint32_t tag, uint32_t pending, uint32_t idx) {
+    return ((u64)tag << 32) | ((u64)pending << 31) | idx;
+}
+__device__ __forceinline__ bool slot_pending(u64 v) { return (v >> 31) & 1ull; }
+__device__ __forceinline__ uint32_t slot_index(u64 v) { return (uint32_t)(v & 0x7FFFFFFFull); }
+
+// ------------------------------------------------------------------------------------------------
+// K9 probe / insert-claim
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) cache_probe_kernel(
+    const uint8_t* __restrict__ bytes, const long long* __restrict__ off, long long S,
+    u64* table, u64 mask, const uint8_t* __restrict__ arena, const long long* __restrict__ entry_off,
+    int* __restrict__ slot_of, int* d_status)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= S) return;
+    const long long o = off[i];
+    const int len = (int)(off[i + 1] - o);
+    const uint8_t* p = bytes + o;
+    const u64 h = hash_bytes(p, len);
+    const uint32_t tag = slot_tag(h);
+    const u64 mine = make_slot(tag, 1u, (uint32_t)i);
+    u64 slot = h & mask;
+    for (u64 probes = 0; probes <= mask; probes++) {
+        u64 v = *((volatile u64*)&table[slot]);
+        if (v == 0) {
+            v = atomicCAS(&table[slot], 0ull, mine);
+            if (v == 0) { slot_of[i] = (int)slot; return; }
+        }
+        if ((uint32_t)(v >> 32) == tag) {
+            bool eq;
+            if (slot_pending(v)) {
+                const long long r = slot_index(v);
+                const long long ro = off[r];
+                eq = (off[r + 1] - ro == len) && bytes_equal(p, bytes + ro, len);
+            } else {
+                const long long e = slot_index(v);
+                const long long eo = entry_off[e];
+                eq = (entry_off[e + 1] - eo == len) && bytes_equal(p, arena + eo, len);
+            }
+            if (eq) {
+                if (slot_pending(v) && slot_index(v) > (uint32_t)i) atomicMin(&table[slot], mine);
+                slot_of[i] = (int)slot;
+                return;
+            }
+        }
+        slot = (slot + 1) & mask;
+    }
+    slot_of[i] = -1;
+    latch_status(d_status, ANON_ERR_CAPACITY);
+}
+
+// ------------------------------------------------------------------------------------------------
+// classify + scan functors
+// ------------------------------------------------------------------------------------------------
+struct ClassifyIn {
+    const long long* off; const uint8_t* type; const int* slot_of; const u64* table;
+    TypeTable tt; int slug_len;
+    __device__ __forceinline__ scan::I64x3 operator()(long long i) const {
+        const int s = slot_of[i];
+        bool is_new = false;
+        if (s >= 0) { u64 v = table[s]; is_new = slot_pending(v) && slot_index(v) == (uint32_t)i; }
+        int t = type ? type[i] : 0;
+        if (t >= tt.num) t = tt.num - 1;
+        return scan::I64x3{is_new ? 1 : 0, is_new ? off[i + 1] - off[i] : 0, 3 + tt.len[t] + slug_len};
+    }
+};
+struct ClassifyOut {
+    long long* out_off; uint8_t* hit; int* new_list; long long* entry_off;
+    long long base_unique, arena_used, S;
+    __device__ __forceinline__ void operator()(long long i, const scan::I64x3& ex, const scan::I64x3& v) const {
+        out_off[i] = ex.c;
+        if (hit) hit[i] = v.a ? 0 : 1;
+        if (v.a) { new_list[ex.a] = (int)i; entry_off[base_unique + ex.a] = arena_used + ex.b; }
+        if (i == S - 1) {
+            out_off[S] = ex.c + v.c;
+            entry_off[base_unique + ex.a + v.a] = arena_used + ex.b + v.b;
+        }
+    }
+};
+
+__global__ void __launch_bounds__(256) cache_rollback_kernel(long long S, const int* __restrict__ slot_of, u64* table) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= S) return;
+    const int s = slot_of[i];
+    if (s >= 0 && slot_pending(table[s])) table[s] = 0ull;
+}
+
+// ------------------------------------------------------------------------------------------------
+// K10 HMAC-SHA256: one thread per message, W[16] ring in registers, pads precomputed on the host
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t bswap32(uint32_t x) { return __byte_perm(x, 0, 0x0123); }
+
+__device__ __forceinline__ void hmac_message(const uint8_t* p, int len, const PadStates& ps, uint32_t out[8]) {
+    uint32_t st[8];
+#pragma unroll
+    for (int k = 0; k < 8; k++) st[k] = ps.ipad[k];
+    const int nblk = (len + 9 + 63) >> 6;
+    uint32_t w[16];
+    for (int b = 0; b < nblk; b++) {
+#pragma unroll
+        for (int t = 0; t < 16; t++) {
+            const int j = b * 16 + t, pos = 4 * j;
+            uint32_t x = 0;
+            if (pos < len) x = load_le_word(p, len, j);
+            if (pos <= len && len < pos + 4) x |= 0x80u << (8 * (len - pos));    // FIPS 180-4 §5.1.1
+            w[t] = bswap32(x);
+        }
+        if (b == nblk - 1) w[15] = (uint32_t)(64 + len) * 8u;                     // bit length incl. the ipad block
+        sha::compress(st, w);
+    }
+#pragma unroll
+    for (int k = 0; k < 8; k++) w[k] = st[k];
+    w[8] = 0x80000000u;
+#pragma unroll
+    for (int k = 9; k < 15; k++) w[k] = 0;
+    w[15] = (64 + 32) * 8;
+#pragma unroll
+    for (int k = 0; k < 8; k++) out[k] = ps.opad[k];
+    sha::compress(out, w);
+}
+
+// insert: thread r handles the r-th new entity of this call
+__global__ void __launch_bounds__(128) cache_insert_kernel(
+    const uint8_t* __restrict__ bytes, const long long* __restrict__ off, const int* __restrict__ new_list,
+    long long n_new, long long base_unique, const int* __restrict__ slot_of, u64* table,
+    uint8_t* arena, const long long* __restrict__ entry_off, uint32_t* digests, PadStates ps)
+{
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_new) return;
+    const int i = new_list[r];
+    const long long e = base_unique + r;
+    const long long o = off[i];
+    const int len = (int)(off[i + 1] - o);
+    const uint8_t* p = bytes + o;
+    uint8_t* dst = arena + entry_off[e];
+    for (int k = 0; k < len; k++) dst[k] = p[k];
+    uint32_t d[8];
+    hmac_message(p, len, ps, d);
+    uint4* dg = (uint4*)(digests + e * 8);
+    dg[0] = make_uint4(bswap32(d[0]), bswap32(d[1]), bswap32(d[2]), bswap32(d[3]));
+    dg[1] = make_uint4(bswap32(d[4]), bswap32(d[5]), bswap32(d[6]), bswap32(d[7]));
+    const int s = slot_of[i];
+    table[s] = make_slot((uint32_t)(table[s] >> 32), 0u, (uint32_t)e);
+}
+
+// HMAC of every span, no dedup (anon_hmac_spans)
+__global__ void __launch_bounds__(128) hmac_spans_kernel(
+    const uint8_t* __restrict__ bytes, const long long* __restrict__ off, long long S, uint32_t* digests, PadStates ps)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= S) return;
+    const long long o = off[i];
+    uint32_t d[8];
+    hmac_message(bytes + o, (int)(off[i + 1] - o), ps, d);
+    uint4* dg = (uint4*)(digests + i * 8);
+    dg[0] = make_uint4(bswap32(d[0]), bswap32(d[1]), bswap32(d[2]), bswap32(d[3]));
+    dg[1] = make_uint4(bswap32(d[4]), bswap32(d[5]), bswap32(d[6]), bswap32(d[7]));
+}
+
+// ------------------------------------------------------------------------------------------------
+// K11 write-back
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) emit_tokens_kernel(
+    long long S, const int* __restrict__ slot_of, const u64* __restrict__ table, const uint8_t* __restrict__ type,
+    const uint32_t* __restrict__ digests, const long long* __restrict__ out_off, uint8_t* out,
+    long long* uid_out, uint8_t* dig_out, TypeTable tt, int slug_len, int* d_status)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= S) return;
+    const int s = slot_of[i];
+    if (s < 0) return;
+    const long long e = slot_index(table[s]);
+    if (uid_out) uid_out[i] = e;
+    const uint4* dg = (const uint4*)(digests + e * 8);
+    const uint4 d0 = __ldg(dg), d1 = __ldg(dg + 1);
+    if (dig_out) { uint4* q = (uint4*)(dig_out + i * 32); q[0] = d0; q[1] = d1; }
+    int t = type ? type[i] : 0;
+    if (t >= tt.num) { t = tt.num - 1; latch_status(d_status, ANON_ERR_UNSUPPORTED); }
+    uint8_t* o = out + out_off[i];
+    *o++ = '[';
+    const int nl = tt.len[t];
+    for (int k = 0; k < nl; k++) *o++ = (uint8_t)tt.name[t][k];
+    *o++ = '_';
+    const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};   // little-endian words = digest bytes in order
+#pragma unroll 1
+    for (int c = 0; c < slug_len; c++) {
+        const uint32_t byte = (dw[c >> 3] >> (8 * ((c >> 1) & 3))) & 0xFFu;
+        const uint32_t nib = (c & 1) ? (byte & 15u) : (byte >> 4);
+        *o++ = (uint8_t)(nib < 10 ? '0' + nib : 'a' + (nib - 10));
+    }
+    *o = ']';
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+static void host_sha256(const uint8_t* msg, size_t len, uint8_t out[32]) {
+    uint32_t st[8];
+    sha::init_state(st);
+    const size_t padded = ((len + 9 + 63) / 64) * 64;
+    for (size_t b = 0; b < padded; b += 64) {
+        uint32_t w[16];
+        for (int t = 0; t < 16; t++) {
+            uint32_t x = 0;
+            for (int k = 0; k < 4; k++) {
+                size_t pos = b + 4 * t + k;
+                uint8_t byte = pos < len ? msg[pos] : (pos == len ? 0x80 : 0);
+                x = (x << 8) | byte;
+            }
+            w[t] = x;
+        }
+        if (b + 64 == padded) { w[14] = (uint32_t)(((uint64_t)len * 8) >> 32); w[15] = (uint32_t)((uint64_t)len * 8); }
+        sha::compress(st, w);
+    }
+    for (int i = 0; i < 8; i++) { out[4 * i] = st[i] >> 24; out[4 * i + 1] = st[i] >> 16; out[4 * i + 2] = st[i] >> 8; out[4 * i + 3] = st[i]; }
+}
+
+// RFC 2104: K' = K (or SHA256(K) when longer than the block), zero-padded to 64 bytes; midstates of
+// the (K' xor ipad) and (K' xor opad) blocks.
+static void make_pads(const uint8_t* key, size_t key_len, PadStates* ps) {
+    uint8_t k[64];
+    memset(k, 0, sizeof k);
+    if (key_len > 64) host_sha256(key, key_len, k);
+    else if (key_len) memcpy(k, key, key_len);
+    for (int which = 0; which < 2; which++) {
+        uint32_t w[16];
+        const uint8_t x = which ? 0x5c : 0x36;
+        for (int t = 0; t < 16; t++)
+            w[t] = ((uint32_t)(k[4 * t] ^ x) << 24) | ((uint32_t)(k[4 * t + 1] ^ x) << 16) |
+                   ((uint32_t)(k[4 * t + 2] ^ x) << 8) | (uint32_t)(k[4 * t + 3] ^ x);
+        uint32_t* st = which ? ps->opad : ps->ipad;
+        sha::init_state(st);
+        sha::compress(st, w);
+    }
+}
+
+static int fill_type_table(const char* const* names, int num, TypeTable* tt) {
+    memset(tt, 0, sizeof *tt);
+    if (num < 1 || num > 64 || !names) return ANON_ERR_INVALID_ARG;
+    for (int t = 0; t < num; t++) {
+        if (!names[t]) return ANON_ERR_INVALID_ARG;
+        size_t n = strlen(names[t]);
+        if (n > 32) return ANON_ERR_UNSUPPORTED;
+        tt->len[t] = (uint8_t)n;
+        memcpy(tt->name[t], names[t], n);
+    }
+    tt->num = num;
+    return ANON_OK;
+}
+
+extern "C" int anon_cache_create(anon_ctx* ctx, uint64_t max_unique, uint64_t key_arena_bytes, anon_cache** out) {
+    if (!ctx || !out || max_unique == 0) return ANON_ERR_INVALID_ARG;
+    if (max_unique > (1ull << 30)) return ANON_ERR_UNSUPPORTED;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    anon_cache* c = new (std::nothrow) anon_cache();
+    if (!c) return ANON_ERR_OOM;
+    c->ctx = ctx; c->max_unique = max_unique; c->arena_bytes = key_arena_bytes;
+    uint64_t slots = 1024;
+    while (slots < 2 * max_unique) slots <<= 1;
+    c->n_slots = slots;
+    cudaError_t e;
+    if ((e = cudaMalloc(&c->d_table, slots * 8)) != cudaSuccess ||
+        (e = cudaMalloc(&c->d_arena, key_arena_bytes + 16)) != cudaSuccess ||
+        (e = cudaMalloc(&c->d_entry_off, (max_unique + 1) * 8)) != cudaSuccess ||
+        (e = cudaMalloc(&c->d_digests, max_unique * 32)) != cudaSuccess) {
+        anon_cache_destroy(c);
+        cuda_fail(ctx, e, "cudaMalloc(cache)");
+        return ANON_ERR_OOM;
+    }
+    CU_TRY(ctx, cudaMemsetAsync(c->d_table, 0, slots * 8, ctx->stream));
+    CU_TRY(ctx, cudaMemsetAsync(c->d_entry_off, 0, 8, ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    *out = c;
+    return ANON_OK;
+}
+
+extern "C" void anon_cache_destroy(anon_cache* c) {
+    if (!c) return;
+    cudaFree(c->d_table); cudaFree(c->d_arena); cudaFree(c->d_entry_off); cudaFree(c->d_digests);
+    delete c;
+}
+
+extern "C" int anon_cache_stats(anon_cache* c, uint64_t* n_unique, uint64_t* n_lookups, uint64_t* n_hits) {
+    if (!c) return ANON_ERR_INVALID_ARG;
+    CU_TRY(c->ctx, cudaStreamSynchronize(c->ctx->stream));
+    if (n_unique) *n_unique = c->n_unique;
+    if (n_lookups) *n_lookups = c->n_lookups;
+    if (n_hits) *n_hits = c->n_hits;
+    return ANON_OK;
+}
+
+extern "C" int64_t anon_cache_entry(anon_cache* c, uint64_t uid, uint8_t* h_bytes, size_t cap, uint8_t* h_digest) {
+    if (!c) return ANON_ERR_INVALID_ARG;
+    anon_ctx* ctx = c->ctx;
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    if (uid >= c->n_unique) return ANON_ERR_INVALID_ARG;
+    long long o[2];
+    CU_TRY(ctx, cudaMemcpy(o, c->d_entry_off + uid, 16, cudaMemcpyDeviceToHost));
+    const int64_t len = o[1] - o[0];
+    if (h_bytes && len > 0 && cap > 0)
+        CU_TRY(ctx, cudaMemcpy(h_bytes, c->d_arena + o[0], (size_t)len < cap ? (size_t)len : cap, cudaMemcpyDeviceToHost));
+    if (h_digest) CU_TRY(ctx, cudaMemcpy(h_digest, c->d_digests + uid * 32, 32, cudaMemcpyDeviceToHost));
+    return len;
+}
+
+int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t* d_bytes, const int64_t* d_off,
+                      const uint8_t* d_type, int64_t S, const uint8_t* key, size_t key_len, int32_t slug_len,
+                      const char* const* type_names, int32_t num_types, uint8_t* d_out, size_t out_cap,
+                      int64_t* d_out_off, uint8_t* d_hit, int64_t* d_uid, uint8_t* d_digests,
+                      int64_t* total_out_bytes)
+{
+    if (!ctx || !c || c->ctx != ctx || S < 0 || !d_off || !d_out_off || (!key && key_len) || slug_len < 0 || slug_len > 64)
+        return ANON_ERR_INVALID_ARG;
+    if (S > 0 && (!d_bytes || !d_out)) {
+        // d_bytes may legitimately be NULL only when every span is empty; we cannot know: require it
+        if (!d_out) return ANON_ERR_INVALID_ARG;
+    }
+    if (S >= (1ll << 31)) return ANON_ERR_UNSUPPORTED;
+    TypeTable tt;
+    int rc = fill_type_table(type_names, num_types, &tt);
+    if (rc) return rc;
+    PadStates ps;
+    make_pads(key, key_len, &ps);
+    if (c->key_bound) {
+        if (memcmp(ps.ipad, c->ipad, 32) || memcmp(ps.opad, c->opad, 32)) return ANON_ERR_KEY_MISMATCH;
+    }
+    cudaStream_t st = ctx->stream;
+    if (total_out_bytes) *total_out_bytes = 0;
+    if (S == 0) {
+        CU_TRY(ctx, cudaMemsetAsync(d_out_off, 0, 8, st));
+        if (!c->key_bound) { memcpy(c->ipad, ps.ipad, 32); memcpy(c->opad, ps.opad, 32); c->key_bound = true; }
+        return ANON_OK;
+    }
+    int* slot_of = (int*)ws.take((size_t)S * 4);
+    int* new_list = (int*)ws.take((size_t)S * 4);
+    scan::I64x3* agg = (scan::I64x3*)ws.take(scan::agg_bytes<scan::I64x3>(S));
+    if (!slot_of || !new_list || !agg) return ANON_ERR_OOM;
+    const long long* off = (const long long*)d_off;
+    const unsigned nb256 = (unsigned)((S + 255) / 256);
+
+    cache_probe_kernel<<<nb256, 256, 0, st>>>(d_bytes, off, S, c->d_table, c->n_slots - 1, c->d_arena,
+                                               c->d_entry_off, slot_of, ctx->d_status);
+    CU_LAUNCH_CHECK(ctx, "cache_probe_kernel");
+    ClassifyIn in{off, d_type, slot_of, c->d_table, tt, slug_len};
+    scan::reduce_and_scan<scan::I64x3, scan::SumI64x3>(in, S, nullptr, agg, st);
+    CU_LAUNCH_CHECK(ctx, "classify scan");
+    scan::I64x3* h_tot = (scan::I64x3*)ctx->h_pinned;
+    int* h_status = (int*)(ctx->h_pinned + 64);
+    CU_TRY(ctx, cudaMemcpyAsync(h_tot, agg + scan::num_tiles(S), sizeof(scan::I64x3), cudaMemcpyDeviceToHost, st));
+    CU_TRY(ctx, cudaMemcpyAsync(h_status, ctx->d_status, 4, cudaMemcpyDeviceToHost, st));
+    CU_TRY(ctx, cudaStreamSynchronize(st));
+    const long long n_new = h_tot->a, new_bytes = h_tot->b, out_bytes = h_tot->c;
+    if (total_out_bytes) *total_out_bytes = out_bytes;
+    const bool table_full = (*h_status == ANON_ERR_CAPACITY);
+    if (table_full || c->n_unique + (uint64_t)n_new > c->max_unique ||
+        c->arena_used + (uint64_t)new_bytes > c->arena_bytes || (uint64_t)out_bytes > out_cap) {
+        cache_rollback_kernel<<<nb256, 256, 0, st>>>(S, slot_of, c->d_table);
+        if (table_full) cudaMemsetAsync(ctx->d_status, 0, 4, st);
+        CU_TRY(ctx, cudaStreamSynchronize(st));
+        return ANON_ERR_CAPACITY;
+    }
+    ClassifyOut outf{(long long*)d_out_off, d_hit, new_list, c->d_entry_off, (long long)c->n_unique,
+                     (long long)c->arena_used, S};
+    scan::apply<scan::I64x3, scan::SumI64x3>(in, outf, S, nullptr, agg, st);
+    CU_LAUNCH_CHECK(ctx, "classify apply");
+    if (n_new > 0) {
+        cache_insert_kernel<<<(unsigned)((n_new + 127) / 128), 128, 0, st>>>(
+            d_bytes, off, new_list, n_new, (long long)c->n_unique, slot_of, c->d_table, c->d_arena,
+            c->d_entry_off, (uint32_t*)c->d_digests, ps);
+        CU_LAUNCH_CHECK(ctx, "cache_insert_kernel");
+    }
+    emit_tokens_kernel<<<nb256, 256, 0, st>>>(S, slot_of, c->d_table, d_type, (const uint32_t*)c->d_digests,
+                                               (const long long*)d_out_off, d_out, (long long*)d_uid, d_digests,
+                                               tt, slug_len, ctx->d_status);
+    CU_LAUNCH_CHECK(ctx, "emit_tokens_kernel");
+    if (!c->key_bound) { memcpy(c->ipad, ps.ipad, 32); memcpy(c->opad, ps.opad, 32); c->key_bound = true; }
+    c->n_unique += (uint64_t)n_new;
+    c->arena_used += (uint64_t)new_bytes;
+    c->n_lookups += (uint64_t)S;
+    c->n_hits += (uint64_t)(S - n_new);
+    return ANON_OK;
+}
+
+extern "C" int anon_pseudonymize(anon_ctx* ctx, anon_cache* cache, const uint8_t* d_span_bytes,
+                                 const int64_t* d_span_offsets, const uint8_t* d_span_type, int64_t S,
+                                 const uint8_t* key, size_t key_len, int32_t slug_len,
+                                 const char* const* type_names, int32_t num_types, uint8_t* d_out_tokens,
+                                 size_t out_capacity, int64_t* d_out_offsets, uint8_t* d_hit, int64_t* d_uid,
+                                 uint8_t* d_digests)
+{
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    WsCursor ws = ws_begin(ctx);
+    return pseudonymize_impl(ctx, ws, cache, d_span_bytes, d_span_offsets, d_span_type, S, key, key_len, slug_len,
+                             type_names, num_types, d_out_tokens, out_capacity, d_out_offsets, d_hit, d_uid,
+                             d_digests, nullptr);
+}
+
+extern "C" int anon_hmac_spans(anon_ctx* ctx, const uint8_t* d_span_bytes, const int64_t* d_span_offsets, int64_t S,
+                               const uint8_t* key, size_t key_len, uint8_t* d_digests)
+{
+    if (!ctx || S < 0 || !d_span_offsets || (S > 0 && !d_digests) || (!key && key_len)) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    if (S == 0) return ANON_OK;
+    PadStates ps;
+    make_pads(key, key_len, &ps);
+    hmac_spans_kernel<<<(unsigned)((S + 127) / 128), 128, 0, ctx->stream>>>(
+        d_span_bytes, (const long long*)d_span_offsets, S, (uint32_t*)d_digests, ps);
+    CU_LAUNCH_CHECK(ctx, "hmac_spans_kernel");
+    return ANON_OK;
+}

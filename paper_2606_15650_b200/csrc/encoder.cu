@@ -1,0 +1,248 @@
+// encoder.cu -- parameter upload and the A1-A8 forward pass (BJ north_star ¶1; S8c O1/O2).
+//
+// Activation layout in HBM (per chunk of whole sequences, carved from the context workspace):
+//   dtype 1 (BF16):  x  FP32 [t,H]  residual stream        xb BF16 [t,H]  GEMM operand copy of x
+//                    y  FP32 [t,H]  GEMM(+bias+residual)    qkv BF16 [t,3H]   ctx BF16 [t,H]   f BF16 [t,F]
+//   dtype 0 (FP32):  the same tensors, all FP32 (xb unused)
+// The residual stream, LayerNorm statistics, softmax and the classifier head stay FP32 in both modes
+// (S7 H2: that is what keeps BF16 logits within 3e-2 and label agreement high).
+#include "common.cuh"
+#include "encoder_kernels.cuh"
+
+#include <new>
+#include <vector>
+#include <stdlib.h>
+
+struct LayerW {
+    void *W_qkv, *W_o, *W_1, *W_2;                     // BF16 or FP32 matrices
+    float *b_qkv, *b_o, *g_1, *b_1, *b_1f, *b_2f, *g_2, *b_2;
+};
+struct anon_weights {
+    anon_ctx* ctx = nullptr;
+    anon_model_desc d;
+    uint8_t* store = nullptr;
+    void *E_w = nullptr, *E_p = nullptr;
+    float *E_t = nullptr, *g_e = nullptr, *b_e = nullptr, *W_c = nullptr, *b_c = nullptr;
+    std::vector<LayerW> layers;
+};
+
+namespace {
+
+__global__ void f32_to_bf16_kernel(const float* __restrict__ src, __nv_bfloat16* __restrict__ dst, size_t n) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (; i < n; i += stride) dst[i] = __float2bfloat16_rn(src[i]);
+}
+
+int check_desc(const anon_model_desc* d) {
+    if (!d) return ANON_ERR_INVALID_ARG;
+    if (d->layers < 0 || d->hidden <= 0 || d->heads <= 0 || d->ffn <= 0 || d->vocab <= 0 || d->num_labels <= 0 ||
+        d->max_pos <= 0 || (d->dtype != 0 && d->dtype != 1))
+        return ANON_ERR_INVALID_ARG;
+    if (d->hidden != d->heads * 64 || d->hidden % 128 != 0 || d->hidden > 1024 || d->ffn % 64 != 0 ||
+        (d->num_labels & 1) == 0 || d->num_labels > 64 || d->max_pos > 512)
+        return ANON_ERR_UNSUPPORTED;
+    return ANON_OK;
+}
+
+size_t desc_floats(const anon_model_desc& d) {
+    const size_t H = d.hidden, F = d.ffn, V = d.vocab, NL = d.num_labels, P = d.max_pos, L = d.layers;
+    const size_t per_layer = 3 * H * H + 3 * H + H * H + H + 2 * H + F * H + F + H * F + H + 2 * H;
+    return V * H + P * H + 3 * H + L * per_layer + NL * H + NL;
+}
+
+size_t per_token_bytes(const anon_model_desc& d) {
+    const size_t H = d.hidden, F = d.ffn;
+    if (d.dtype == 1) return 4 * H + 2 * H + 4 * H + 6 * H + 2 * H + 2 * F;
+    return 4 * H + 4 * H + 12 * H + 4 * H + 4 * F;
+}
+
+}  // namespace
+
+extern "C" size_t anon_workspace_bytes(const anon_model_desc* d, int64_t max_tokens, int32_t max_seqs) {
+    if (!d || max_tokens < 0 || max_seqs < 0) return 0;
+    const size_t per_tok = per_token_bytes(*d) + 64;                 // + decode / gather / scan scratch per item
+    return (size_t)max_tokens * per_tok + (size_t)max_seqs * 64 + ((size_t)8 << 20);
+}
+
+extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, const float* blob, size_t n_floats,
+                                 anon_weights** out)
+{
+    if (!ctx || !blob || !out) return ANON_ERR_INVALID_ARG;
+    int rc = check_desc(desc);
+    if (rc) return rc;
+    if (n_floats != desc_floats(*desc)) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    anon_weights* w = new (std::nothrow) anon_weights();
+    if (!w) return ANON_ERR_OOM;
+    w->ctx = ctx; w->d = *desc;
+    const anon_model_desc& d = *desc;
+    const size_t H = d.hidden, F = d.ffn, V = d.vocab, NL = d.num_labels, P = d.max_pos;
+    const bool bf = d.dtype == 1;
+    const size_t msz = bf ? 2 : 4;
+    struct Item { void** dst; size_t n; bool matrix; };
+    std::vector<Item> items;
+    w->layers.resize(d.layers);
+    items.push_back({&w->E_w, V * H, true});
+    items.push_back({&w->E_p, P * H, true});
+    items.push_back({(void**)&w->E_t, H, false});
+    items.push_back({(void**)&w->g_e, H, false});
+    items.push_back({(void**)&w->b_e, H, false});
+    for (int l = 0; l < d.layers; l++) {
+        LayerW& L = w->layers[l];
+        items.push_back({&L.W_qkv, 3 * H * H, true});   items.push_back({(void**)&L.b_qkv, 3 * H, false});
+        items.push_back({&L.W_o, H * H, true});         items.push_back({(void**)&L.b_o, H, false});
+        items.push_back({(void**)&L.g_1, H, false});    items.push_back({(void**)&L.b_1, H, false});
+        items.push_back({&L.W_1, F * H, true});         items.push_back({(void**)&L.b_1f, F, false});
+        items.push_back({&L.W_2, H * F, true});         items.push_back({(void**)&L.b_2f, H, false});
+        items.push_back({(void**)&L.g_2, H, false});    items.push_back({(void**)&L.b_2, H, false});
+    }
+    items.push_back({(void**)&w->W_c, NL * H, false});   // head stays FP32 (values are BF16-representable)
+    items.push_back({(void**)&w->b_c, NL, false});
+    size_t total = 0, max_matrix = 0;
+    for (auto& it : items) {
+        total = (total + 255) / 256 * 256 + it.n * (it.matrix ? msz : 4);
+        if (it.matrix && bf && it.n > max_matrix) max_matrix = it.n;
+    }
+    float* stage = nullptr;
+    cudaError_t e = cudaMalloc(&w->store, total + 256);
+    if (e == cudaSuccess && max_matrix) e = cudaMalloc(&stage, max_matrix * 4);
+    if (e != cudaSuccess) { cudaFree(w->store); delete w; cuda_fail(ctx, e, "cudaMalloc(weights)"); return ANON_ERR_OOM; }
+    size_t off = 0;
+    const float* src = blob;
+    for (auto& it : items) {
+        off = (off + 255) / 256 * 256;
+        void* dst = w->store + off;
+        *it.dst = dst;
+        if (it.matrix && bf) {
+            e = cudaMemcpyAsync(stage, src, it.n * 4, cudaMemcpyHostToDevice, ctx->stream);
+            if (e == cudaSuccess) {
+                f32_to_bf16_kernel<<<1024, 256, 0, ctx->stream>>>(stage, (__nv_bfloat16*)dst, it.n);
+                e = cudaStreamSynchronize(ctx->stream);      // stage is reused by the next matrix
+            }
+        } else {
+            e = cudaMemcpyAsync(dst, src, it.n * 4, cudaMemcpyHostToDevice, ctx->stream);
+        }
+        if (e != cudaSuccess) break;
+        off += it.n * (it.matrix ? msz : 4);
+        src += it.n;
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(stage);
+    if (e != cudaSuccess) { cudaFree(w->store); delete w; return cuda_fail(ctx, e, "weights upload"); }
+    *out = w;
+    return ANON_OK;
+}
+
+extern "C" void anon_weights_free(anon_weights* w) {
+    if (!w) return;
+    cudaFree(w->store);
+    delete w;
+}
+
+const anon_model_desc* weights_desc(const anon_weights* w) { return &w->d; }
+
+template <int EPI>
+static int sgemm(anon_ctx* ctx, const float* A, const float* W, const float* bias, const float* res, float* C, int M, int N, int K) {
+    if (M == 0) return ANON_OK;
+    dim3 grid((N + 63) / 64, (M + 63) / 64);
+    enc::sgemm_tn_kernel<EPI><<<grid, 256, 0, ctx->stream>>>(A, W, bias, res, C, M, N, K);
+    CU_LAUNCH_CHECK(ctx, "sgemm_tn_kernel");
+    return ANON_OK;
+}
+
+int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const int32_t* d_ids, const int32_t* d_cu,
+                     const int32_t* h_cu, int32_t B, int32_t T, float* d_logits, int32_t* d_labels)
+{
+    if (!ctx || !w || w->ctx != ctx || B < 0 || T < 0 || !d_cu || !h_cu || (T > 0 && !d_ids)) return ANON_ERR_INVALID_ARG;
+    if (h_cu[0] != 0 || h_cu[B] != T) return ANON_ERR_INVALID_ARG;
+    const anon_model_desc& d = w->d;
+    for (int s = 0; s < B; s++) {
+        if (h_cu[s + 1] < h_cu[s]) return ANON_ERR_INVALID_ARG;
+        if (h_cu[s + 1] - h_cu[s] > d.max_pos) return ANON_ERR_UNSUPPORTED;
+    }
+    if (T == 0) return ANON_OK;
+    const int H = d.hidden, F = d.ffn, NL = d.num_labels;
+    const bool bf = d.dtype == 1;
+    cudaStream_t st = ctx->stream;
+
+    // chunk budget: whole sequences, as many tokens as the remaining workspace holds (optionally capped)
+    const size_t per_tok = per_token_bytes(d);
+    const size_t avail = ws.left() > ((size_t)2 << 20) ? ws.left() - ((size_t)2 << 20) : 0;
+    long long cap = (long long)(avail / per_tok);
+    static long long env_cap = -1;
+    if (env_cap < 0) { const char* e = getenv("ANON_CHUNK_TOKENS"); env_cap = e ? atoll(e) : 0; }
+    if (env_cap > 0 && cap > env_cap) cap = env_cap;
+    if (cap < d.max_pos && cap < T) return ANON_ERR_OOM;
+
+    int s0 = 0;
+    while (s0 < B) {
+        int s1 = s0;
+        while (s1 < B && (long long)(h_cu[s1 + 1] - h_cu[s0]) <= cap) s1++;
+        if (s1 == s0) return ANON_ERR_OOM;
+        const int tok0 = h_cu[s0], nt = h_cu[s1] - tok0, nb = s1 - s0;
+        if (nt > 0) {
+            WsCursor c = ws;          // chunk-local carve (same region reused by every chunk; stream-ordered)
+            float* x = (float*)c.take((size_t)nt * H * 4);
+            float* y = (float*)c.take((size_t)nt * H * 4);
+            __nv_bfloat16* xb = bf ? (__nv_bfloat16*)c.take((size_t)nt * H * 2) : nullptr;
+            void* qkv = c.take((size_t)nt * 3 * H * (bf ? 2 : 4));
+            void* cx = c.take((size_t)nt * H * (bf ? 2 : 4));
+            void* f = c.take((size_t)nt * F * (bf ? 2 : 4));
+            if (!x || !y || (bf && !xb) || !qkv || !cx || !f) return ANON_ERR_OOM;
+            AttnPlan plan;
+            int prc = attention_plan(ctx, c, h_cu + s0, nb, d.dtype, &plan);
+            if (prc) return prc;
+            const unsigned row_grid = (unsigned)((nt + enc::kRowWarps - 1) / enc::kRowWarps);
+            if (bf)
+                enc::embed_ln_kernel<__nv_bfloat16><<<row_grid, enc::kRowWarps * 32, 0, st>>>(
+                    d_ids, d_cu, B, tok0, nt, (const __nv_bfloat16*)w->E_w, (const __nv_bfloat16*)w->E_p, w->E_t, w->g_e,
+                    w->b_e, d.ln_eps, H, d.vocab, d.max_pos, x, xb, ctx->d_status);
+            else
+                enc::embed_ln_kernel<float><<<row_grid, enc::kRowWarps * 32, 0, st>>>(
+                    d_ids, d_cu, B, tok0, nt, (const float*)w->E_w, (const float*)w->E_p, w->E_t, w->g_e, w->b_e,
+                    d.ln_eps, H, d.vocab, d.max_pos, x, nullptr, ctx->d_status);
+            CU_LAUNCH_CHECK(ctx, "embed_ln_kernel");
+            for (int l = 0; l < d.layers; l++) {
+                const LayerW& L = w->layers[l];
+                int rc;
+                if (bf) rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_qkv, L.b_qkv, nullptr, qkv, nt, 3 * H, H, 0);
+                else rc = sgemm<0>(ctx, x, (const float*)L.W_qkv, L.b_qkv, nullptr, (float*)qkv, nt, 3 * H, H);
+                if (rc) return rc;
+                rc = attention_run(ctx, plan, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx);
+                if (rc) return rc;
+                if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, y, nt, H, H, 2);
+                else rc = sgemm<2>(ctx, (const float*)cx, (const float*)L.W_o, L.b_o, x, y, nt, H, H);
+                if (rc) return rc;
+                enc::layer_norm_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, L.g_1, L.b_1, d.ln_eps, x, xb);
+                CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+                if (bf) rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_1, L.b_1f, nullptr, f, nt, F, H, 1);
+                else rc = sgemm<1>(ctx, x, (const float*)L.W_1, L.b_1f, nullptr, (float*)f, nt, F, H);
+                if (rc) return rc;
+                if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, x, y, nt, H, F, 2);
+                else rc = sgemm<2>(ctx, (const float*)f, (const float*)L.W_2, L.b_2f, x, y, nt, H, F);
+                if (rc) return rc;
+                enc::layer_norm_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, L.g_2, L.b_2, d.ln_eps, x, xb);
+                CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+            }
+            enc::head_argmax_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(
+                x, nt, H, w->W_c, w->b_c, NL, d_logits ? d_logits + (size_t)tok0 * NL : nullptr,
+                d_labels ? d_labels + tok0 : nullptr);
+            CU_LAUNCH_CHECK(ctx, "head_argmax_kernel");
+        }
+        s0 = s1;
+    }
+    return ANON_OK;
+}
+
+extern "C" int anon_ner_forward(anon_ctx* ctx, const anon_weights* w, const int32_t* d_token_ids,
+                                const int32_t* d_cu_seqlens, int32_t B, int32_t T, float* d_logits, int32_t* d_labels)
+{
+    if (!ctx || !w || B < 0 || T < 0 || !d_cu_seqlens) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    std::vector<int32_t> h_cu((size_t)B + 1);
+    CU_TRY(ctx, cudaMemcpyAsync(h_cu.data(), d_cu_seqlens, ((size_t)B + 1) * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    WsCursor ws = ws_begin(ctx);
+    return ner_forward_impl(ctx, ws, w, d_token_ids, d_cu_seqlens, h_cu.data(), B, T, d_logits, d_labels);
+}

@@ -1,0 +1,235 @@
+// encoder_kernels.cuh -- the HBM-bound encoder kernels (K1 embed+LN, K4 LN, K6 head+argmax) and the FP32
+// SIMT path for BJ configs[0] (K2f SGEMM, FP32 attention).  S8a A1, A4, A6, A7, A8; S8c O1, O2.
+// One warp per token row; every global access is a coalesced 16-byte vector; statistics in FP32 with the
+// two-pass (mean, then centred variance) form of O1.
+#pragma once
+#include "common.cuh"
+
+namespace enc {
+
+constexpr int kMaxVec = 8;           // hidden <= 1024 (8 float4 per lane)
+constexpr int kRowWarps = 8;         // warps (token rows) per CTA for the row kernels
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    return v;
+}
+
+__device__ __forceinline__ float4 load4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+__device__ __forceinline__ float4 load4(const __nv_bfloat16* p) {
+    const uint2 u = __ldg(reinterpret_cast<const uint2*>(p));
+    const __nv_bfloat162 a = *reinterpret_cast<const __nv_bfloat162*>(&u.x);
+    const __nv_bfloat162 b = *reinterpret_cast<const __nv_bfloat162*>(&u.y);
+    const float2 fa = __bfloat1622float2(a), fb = __bfloat1622float2(b);
+    return make_float4(fa.x, fa.y, fb.x, fb.y);
+}
+
+// LN over one row held as n4 float4 per lane (element index = 4*(lane + 32k) + c); writes FP32 and optional BF16.
+__device__ __forceinline__ void layer_norm_row(float4 (&v)[kMaxVec], int n4, int H, const float* __restrict__ g,
+                                               const float* __restrict__ b, float eps, int lane,
+                                               float* __restrict__ xo, __nv_bfloat16* __restrict__ xbo) {
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < kMaxVec; k++) if (k < n4) s += (v[k].x + v[k].y) + (v[k].z + v[k].w);
+    const float mean = warp_sum(s) / (float)H;
+    float q = 0.f;
+#pragma unroll
+    for (int k = 0; k < kMaxVec; k++) if (k < n4) {
+        v[k].x -= mean; v[k].y -= mean; v[k].z -= mean; v[k].w -= mean;
+        q += (v[k].x * v[k].x + v[k].y * v[k].y) + (v[k].z * v[k].z + v[k].w * v[k].w);
+    }
+    const float rstd = 1.0f / sqrtf(warp_sum(q) / (float)H + eps);
+#pragma unroll
+    for (int k = 0; k < kMaxVec; k++) if (k < n4) {
+        const int e = 4 * (lane + 32 * k);
+        const float4 gg = load4(g + e), bb = load4(b + e);
+        float4 o;
+        o.x = v[k].x * rstd * gg.x + bb.x; o.y = v[k].y * rstd * gg.y + bb.y;
+        o.z = v[k].z * rstd * gg.z + bb.z; o.w = v[k].w * rstd * gg.w + bb.w;
+        if (xo) *reinterpret_cast<float4*>(xo + e) = o;
+        if (xbo) {
+            __nv_bfloat162 lo = __floats2bfloat162_rn(o.x, o.y), hi = __floats2bfloat162_rn(o.z, o.w);
+            uint2 u;
+            u.x = *reinterpret_cast<uint32_t*>(&lo); u.y = *reinterpret_cast<uint32_t*>(&hi);
+            *reinterpret_cast<uint2*>(xbo + e) = u;
+        }
+    }
+}
+
+// K1: x_j = LN(E_w[id_j] + E_p[pos_j] + E_t).  tok0 = first token of the chunk (absolute index); cu is absolute.
+template <class TE>
+static __global__ void __launch_bounds__(kRowWarps * 32) embed_ln_kernel(
+    const int* __restrict__ ids, const int* __restrict__ cu, int B, int tok0, int ntok, const TE* __restrict__ E_w,
+    const TE* __restrict__ E_p, const float* __restrict__ E_t, const float* __restrict__ g, const float* __restrict__ b,
+    float eps, int H, int V, int max_pos, float* __restrict__ x, __nv_bfloat16* __restrict__ xb, int* d_status)
+{
+    const int lane = threadIdx.x & 31;
+    const int r = blockIdx.x * kRowWarps + (threadIdx.x >> 5);
+    if (r >= ntok) return;
+    const int j = tok0 + r;
+    int lo = 0, hi = B;                       // largest s with cu[s] <= j  (cu[B] = T > j)
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(cu + mid) <= j) lo = mid; else hi = mid; }
+    int pos = j - __ldg(cu + lo);
+    int id = __ldg(ids + j);
+    if (id < 0 || id >= V || pos >= max_pos) {
+        if (lane == 0) latch_status(d_status, ANON_ERR_UNSUPPORTED);
+        id = id < 0 ? 0 : (id >= V ? V - 1 : id);
+        pos = pos >= max_pos ? max_pos - 1 : pos;
+    }
+    const int n4 = H >> 7;
+    float4 v[kMaxVec];
+#pragma unroll
+    for (int k = 0; k < kMaxVec; k++) if (k < n4) {
+        const int e = 4 * (lane + 32 * k);
+        const float4 a = load4(E_w + (size_t)id * H + e), p = load4(E_p + (size_t)pos * H + e), t = load4(E_t + e);
+        v[k] = make_float4(a.x + p.x + t.x, a.y + p.y + t.y, a.z + p.z + t.z, a.w + p.w + t.w);
+    }
+    layer_norm_row(v, n4, H, g, b, eps, lane, x + (size_t)r * H, xb ? xb + (size_t)r * H : nullptr);
+}
+
+// K4: x = LN(y) (the residual add is fused into the producing GEMM's epilogue), or x = LN(y + res) if res != NULL.
+static __global__ void __launch_bounds__(kRowWarps * 32) layer_norm_kernel(
+    const float* __restrict__ y, const float* __restrict__ res, int ntok, int H, const float* __restrict__ g,
+    const float* __restrict__ b, float eps, float* __restrict__ x, __nv_bfloat16* __restrict__ xb)
+{
+    const int lane = threadIdx.x & 31;
+    const int r = blockIdx.x * kRowWarps + (threadIdx.x >> 5);
+    if (r >= ntok) return;
+    const int n4 = H >> 7;
+    float4 v[kMaxVec];
+#pragma unroll
+    for (int k = 0; k < kMaxVec; k++) if (k < n4) {
+        const int e = 4 * (lane + 32 * k);
+        v[k] = load4(y + (size_t)r * H + e);
+        if (res) { const float4 o = load4(res + (size_t)r * H + e); v[k].x += o.x; v[k].y += o.y; v[k].z += o.z; v[k].w += o.w; }
+    }
+    layer_norm_row(v, n4, H, g, b, eps, lane, x + (size_t)r * H, xb ? xb + (size_t)r * H : nullptr);
+}
+
+// K6: logits = x W_c^T + b_c (FP32), label = argmax (ties -> lowest index).
+static __global__ void __launch_bounds__(kRowWarps * 32) head_argmax_kernel(
+    const float* __restrict__ x, int ntok, int H, const float* __restrict__ W_c, const float* __restrict__ b_c, int NL,
+    float* __restrict__ logits, int* __restrict__ labels)
+{
+    const int lane = threadIdx.x & 31;
+    const int r = blockIdx.x * kRowWarps + (threadIdx.x >> 5);
+    if (r >= ntok) return;
+    const int n4 = H >> 7;
+    float4 v[kMaxVec];
+#pragma unroll
+    for (int k = 0; k < kMaxVec; k++) if (k < n4) v[k] = load4(x + (size_t)r * H + 4 * (lane + 32 * k));
+    float best = 0.f; int best_c = 0;
+    for (int c = 0; c < NL; c++) {
+        float s = 0.f;
+#pragma unroll
+        for (int k = 0; k < kMaxVec; k++) if (k < n4) {
+            const float4 w = load4(W_c + (size_t)c * H + 4 * (lane + 32 * k));
+            s += (v[k].x * w.x + v[k].y * w.y) + (v[k].z * w.z + v[k].w * w.w);
+        }
+        s = warp_sum(s) + __ldg(b_c + c);
+        if (logits && lane == 0) logits[(size_t)r * NL + c] = s;
+        if (c == 0 || s > best) { best = s; best_c = c; }
+    }
+    if (labels && lane == 0) labels[r] = best_c;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// FP32 SIMT path (BJ configs[0]; TF32 would miss the 1e-4 bound, S7 H5): 64x64x16 tiles, 4x4 per thread
+// ---------------------------------------------------------------------------------------------------------
+template <int EPI>   // 0: +bias; 1: +bias, erf-GELU; 2: +bias +residual
+static __global__ void __launch_bounds__(256) sgemm_tn_kernel(const float* __restrict__ A, const float* __restrict__ W,
+                                                       const float* __restrict__ bias, const float* __restrict__ res,
+                                                       float* __restrict__ C, int M, int N, int K)
+{
+    __shared__ float As[16][64 + 4], Ws[16][64 + 4];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const int m0 = blockIdx.y * 64, n0 = blockIdx.x * 64;
+    const int lr = tid >> 2, lk = (tid & 3) * 4;
+    float acc[4][4] = {};
+    for (int k0 = 0; k0 < K; k0 += 16) {
+        float4 a = make_float4(0, 0, 0, 0), w = a;
+        if (m0 + lr < M && k0 + lk < K) a = load4(A + (size_t)(m0 + lr) * K + k0 + lk);
+        if (n0 + lr < N && k0 + lk < K) w = load4(W + (size_t)(n0 + lr) * K + k0 + lk);
+        As[lk][lr] = a.x; As[lk + 1][lr] = a.y; As[lk + 2][lr] = a.z; As[lk + 3][lr] = a.w;
+        Ws[lk][lr] = w.x; Ws[lk + 1][lr] = w.y; Ws[lk + 2][lr] = w.z; Ws[lk + 3][lr] = w.w;
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 16; k++) {
+            const float4 av = *reinterpret_cast<const float4*>(&As[k][ty * 4]);
+            const float4 wv = *reinterpret_cast<const float4*>(&Ws[k][tx * 4]);
+            const float ar[4] = {av.x, av.y, av.z, av.w}, wr[4] = {wv.x, wv.y, wv.z, wv.w};
+#pragma unroll
+            for (int i = 0; i < 4; i++)
+#pragma unroll
+                for (int j = 0; j < 4; j++) acc[i][j] = fmaf(ar[i], wr[j], acc[i][j]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        const int m = m0 + ty * 4 + i;
+        if (m >= M) continue;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            const int n = n0 + tx * 4 + j;
+            if (n >= N) continue;
+            float f = acc[i][j] + __ldg(bias + n);
+            if (EPI == 1) f = 0.5f * f * (1.0f + erff(f * 0.70710678118654752f));
+            if (EPI == 2) f += res[(size_t)m * N + n];
+            C[(size_t)m * N + n] = f;
+        }
+    }
+}
+
+// FP32 varlen attention: one CTA per (sequence, head); each warp owns one query at a time; scores in shared
+// memory; exact two-pass softmax in FP32.  qkv [T,3H] with q | k | v column blocks; d_head = 64.
+static __global__ void __launch_bounds__(128) attention_f32_kernel(const float* __restrict__ qkv, const int* __restrict__ cu,
+                                                            int seq0, int tok0, int H, float* __restrict__ ctx)
+{
+    __shared__ float sc[4][512];
+    __shared__ float qs[4][64];
+    const int seq = seq0 + blockIdx.x, head = blockIdx.y;
+    const int a = cu[seq] - tok0, n = cu[seq + 1] - cu[seq];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const size_t ld = (size_t)3 * H;
+    const float* Q = qkv + (size_t)a * ld + head * 64;
+    const float* Kp = Q + H;
+    const float* Vp = Q + 2 * H;
+    for (int i = warp; i < n; i += 4) {
+        qs[warp][lane] = Q[(size_t)i * ld + lane];
+        qs[warp][lane + 32] = Q[(size_t)i * ld + lane + 32];
+        __syncwarp();
+        float mx = -INFINITY;
+        for (int m = lane; m < n; m += 32) {
+            const float4* kr = reinterpret_cast<const float4*>(Kp + (size_t)m * ld);
+            float s = 0.f;
+#pragma unroll
+            for (int d = 0; d < 16; d++) {
+                const float4 kv = __ldg(kr + d);
+                s += qs[warp][4 * d] * kv.x + qs[warp][4 * d + 1] * kv.y + qs[warp][4 * d + 2] * kv.z + qs[warp][4 * d + 3] * kv.w;
+            }
+            s *= 0.125f;
+            sc[warp][m] = s;
+            mx = fmaxf(mx, s);
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+        float sum = 0.f;
+        for (int m = lane; m < n; m += 32) { const float e = expf(sc[warp][m] - mx); sc[warp][m] = e; sum += e; }
+        sum = warp_sum(sum);
+        __syncwarp();
+        float o0 = 0.f, o1 = 0.f;
+        for (int m = 0; m < n; m++) {
+            const float p = sc[warp][m];
+            o0 = fmaf(p, __ldg(Vp + (size_t)m * ld + lane), o0);
+            o1 = fmaf(p, __ldg(Vp + (size_t)m * ld + lane + 32), o1);
+        }
+        const float inv = 1.0f / sum;
+        ctx[(size_t)(a + i) * H + head * 64 + lane] = o0 * inv;
+        ctx[(size_t)(a + i) * H + head * 64 + lane + 32] = o1 * inv;
+        __syncwarp();
+    }
+}
+
+}  // namespace enc

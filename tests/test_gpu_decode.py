@@ -1,0 +1,120 @@
+"""GPU parity (through the C ABI) of A9 BIO decode + compaction and A10 span byte gather.
+Bar: span offsets bit-exact against oracle/decode.py (BASELINE.json north_star ¶5)."""
+import os
+
+import numpy as np
+import pytest
+
+from harness import gen
+from test_oracle_decode import _parse_case
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    import paper_2606_15650_b200 as P
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device")
+    ctx = P.Context(0, workspace_bytes=512 << 20)
+    yield P, torch, ctx
+    ctx.close()
+
+
+def _gpu_decode(P, torch, ctx, labels, meta, num_labels, cap=None):
+    dev = "cuda:0"
+    T = len(labels)
+    cap = T + 1 if cap is None else cap
+    d_lab = torch.from_numpy(np.ascontiguousarray(labels, np.int32)).to(dev) if T else torch.zeros(1, dtype=torch.int32, device=dev)[:0]
+    d_meta = torch.from_numpy(np.ascontiguousarray(meta, np.int32).reshape(-1, 4)).to(dev) if T else torch.zeros((0, 4), dtype=torch.int32, device=dev)
+    spans = torch.full((max(cap, 1), 4), -7, dtype=torch.int32, device=dev)
+    num = torch.zeros(1, dtype=torch.int32, device=dev)
+    P.anon_decode_spans(ctx, d_lab, d_meta, num_labels, spans[:cap], num)
+    rc = ctx.sync()
+    n = int(num.item())
+    return rc, n, spans.cpu().numpy()[:min(n, cap)]
+
+
+def test_hand_worked_cases_on_gpu(env, golden_dir):
+    P, torch, ctx = env
+    with open(os.path.join(golden_dir, "bio_cases.txt")) as f:
+        for line in f:
+            if not line.strip() or line.startswith("#"):
+                continue
+            labels, meta, want = _parse_case(line)
+            rc, n, spans = _gpu_decode(P, torch, ctx, labels, meta, 5)
+            assert rc == 0 and n == len(want), line
+            assert [tuple(int(v) for v in s) for s in spans] == want, line
+
+
+def _random_stream(rng, T, nt, p_keep, n_rec):
+    labels = rng.integers(0, 2 * nt + 1, T).astype(np.int32)
+    labels[rng.random(T) < 0.35] = 0
+    rec = np.sort(rng.integers(0, n_rec, T)).astype(np.int32)
+    cs = np.arange(T, dtype=np.int32) * 5
+    meta = np.stack([rec, cs, cs + rng.integers(1, 5, T).astype(np.int32), (rng.random(T) < p_keep).astype(np.int32)], 1)
+    return labels, meta
+
+
+@pytest.mark.parametrize("T,p_keep", [(1, 1.0), (31, 0.9), (2048, 0.8), (2049, 0.5), (100_003, 0.97), (300_000, 0.02)])
+def test_random_streams_match_oracle(env, T, p_keep):
+    """Several scan tiles plus a ragged tail; sparse keep flags exercise long transparent runs."""
+    P, torch, ctx = env
+    from oracle import decode
+    rng = np.random.default_rng(T)
+    labels, meta = _random_stream(rng, T, 6, p_keep, max(1, T // 300))
+    want = decode.decode_spans(labels, meta)
+    rc, n, spans = _gpu_decode(P, torch, ctx, labels, meta, 13)
+    assert rc == 0 and n == len(want)
+    assert np.array_equal(spans, np.asarray(want, np.int32).reshape(-1, 4))
+
+
+def test_empty_none_kept_and_capacity(env):
+    P, torch, ctx = env
+    rc, n, _ = _gpu_decode(P, torch, ctx, np.zeros(0, np.int32), np.zeros((0, 4), np.int32), 13)
+    assert rc == 0 and n == 0
+    rng = np.random.default_rng(1)
+    labels, meta = _random_stream(rng, 5000, 6, 1.0, 3)
+    meta0 = meta.copy(); meta0[:, 3] = 0
+    rc, n, _ = _gpu_decode(P, torch, ctx, labels, meta0, 13)
+    assert rc == 0 and n == 0
+    from oracle import decode
+    want = decode.decode_spans(labels, meta)
+    rc, n, spans = _gpu_decode(P, torch, ctx, labels, meta, 13, cap=10)
+    assert rc == -3 and n == len(want)                       # ANON_ERR_CAPACITY latched, needed count reported
+    assert np.array_equal(spans, np.asarray(want[:10], np.int32))
+    assert ctx.sync() == 0                                   # sticky status was cleared
+
+
+def test_windowed_records_decode_and_gather(env):
+    """Planted labels on windowed records (510+2 tokens, 128 overlap, midpoint ownership): spans cross window
+    boundaries; the gathered bytes are exactly the planted entity strings."""
+    P, torch, ctx = env
+    from oracle import decode
+    d = gen.DESCS["base"]
+    pool, poff, ptype = gen.entity_pool(800, 21)
+    n_tok = np.array([8, 510, 511, 893, 2000, 3000, 40, 1275])
+    rec = gen.make_records(len(n_tok), n_tok, d, pool, poff, ptype, 22)
+    win = gen.window_records(rec)
+    want = decode.decode_spans(win["planted_label"], win["meta"])
+    rc, n, spans = _gpu_decode(P, torch, ctx, win["planted_label"].astype(np.int32), win["meta"], 13)
+    assert rc == 0 and n == len(want) == rec["n_entities"]
+    assert np.array_equal(spans, np.asarray(want, np.int32))
+    wb, wo = decode.gather_spans(rec["text"], rec["rec_off"], want)
+    dev = "cuda:0"
+    d_sp = torch.from_numpy(spans).to(dev)
+    sb = torch.zeros(int(wo[-1]) + 16, dtype=torch.uint8, device=dev)
+    so = torch.zeros(n + 1, dtype=torch.int64, device=dev)
+    stype = torch.zeros(n, dtype=torch.uint8, device=dev)
+    P.anon_gather_spans(ctx, torch.from_numpy(rec["text"]).to(dev), torch.from_numpy(rec["rec_off"]).to(dev), d_sp, n,
+                        sb, so, stype)
+    assert ctx.sync() == 0
+    assert np.array_equal(so.cpu().numpy(), wo)
+    assert np.array_equal(sb.cpu().numpy()[:wo[-1]], wb)
+    assert np.array_equal(stype.cpu().numpy(), spans[:, 3].astype(np.uint8))
+    # capacity: one byte short
+    sb2 = torch.zeros(int(wo[-1]) - 1, dtype=torch.uint8, device=dev)
+    P.anon_gather_spans(ctx, torch.from_numpy(rec["text"]).to(dev), torch.from_numpy(rec["rec_off"]).to(dev), d_sp, n,
+                        sb2, so, None)
+    assert ctx.sync() == -3

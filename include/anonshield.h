@@ -73,6 +73,16 @@ void anon_ctx_destroy(anon_ctx* ctx);
 int  anon_ctx_sync(anon_ctx* ctx);
 /* Text of the last CUDA error seen by this context ("" if none).  Owned by the context. */
 const char* anon_last_cuda_error(anon_ctx* ctx);
+/* Launch accounting and per-kernel-class CUDA-event timing (bench.py's roofline / gpu_launches keys).
+ * anon_ctx_profile(ctx, 1) synchronises, zeroes the counters and starts bracketing every launch group
+ * with events on the context stream; (ctx, 0) stops.  anon_ctx_profile_read synchronises and returns,
+ * for class c (0 = GEMM, 1 = attention, 2 = row kernels embed/LN/head, 3 = decode+gather,
+ * 4 = pseudonymize; arrays of 8): summed event time in ms, algorithmic work (FLOPs for classes 0-1,
+ * bytes for 2-3, 0 for 4), launches; and the total number of kernels launched since the last
+ * anon_ctx_profile call (counted whether or not timing is enabled).  Any pointer may be NULL. */
+int  anon_ctx_profile(anon_ctx* ctx, int enable);
+int  anon_ctx_profile_read(anon_ctx* ctx, double* class_ms, double* class_work, int64_t* class_launches,
+                           int64_t* total_launches);
 /* Scratch bytes anon_ner_forward needs to process `max_tokens` packed tokens in
  * `max_seqs` sequences in ONE pass; with less, anon_ner_forward splits the batch into
  * sequence-aligned chunks that fit (at least one 512-token sequence must fit).  Also

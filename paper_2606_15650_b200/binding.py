@@ -60,6 +60,8 @@ _SIGNATURES = {
     "anon_hmac_spans": (ctypes.c_int, [_vp, _vp, _vp, _i64, _vp, _sz, _vp]),
     "anon_pipeline_host": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _vp, _sz, _vp, _i32, _vp, _sz, _i32,
                                           ctypes.POINTER(ctypes.c_char_p), _i32, _vp, _i32, _vp, _vp, _sz, _vp, _vp]),
+    "anon_ctx_profile": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "anon_ctx_profile_read": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "anon_gemm_bf16": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32]),
     "anon_attention": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32, _i32, _vp]),
 }
@@ -118,6 +120,18 @@ class Context:
     def sync(self):
         """anon_ctx_sync: waits for the stream, returns (and clears) the sticky device status."""
         return lib().anon_ctx_sync(self._h)
+
+    def profile(self, enable):
+        self.check(lib().anon_ctx_profile(self._h, 1 if enable else 0), "anon_ctx_profile")
+
+    def profile_read(self):
+        """{class name: (ms, work, launches)}, total kernel launches since profile() was last called."""
+        ms, work = np.zeros(8, np.float64), np.zeros(8, np.float64)
+        ln, tot = np.zeros(8, np.int64), np.zeros(1, np.int64)
+        self.check(lib().anon_ctx_profile_read(self._h, ms.ctypes.data, work.ctypes.data, ln.ctypes.data, tot.ctypes.data),
+                   "anon_ctx_profile_read")
+        names = ["gemm", "attention", "row", "decode", "pseudonymize"]
+        return {n: (float(ms[i]), float(work[i]), int(ln[i])) for i, n in enumerate(names)}, int(tot[0])
 
     def close(self):
         if self._h:

@@ -22,7 +22,7 @@ extern "C" const char* const* anon_exported_symbols(void) {
         "anon_last_cuda_error", "anon_workspace_bytes", "anon_weights_load", "anon_weights_free", "anon_ner_forward",
         "anon_decode_spans", "anon_gather_spans", "anon_cache_create", "anon_cache_destroy", "anon_cache_stats",
         "anon_cache_entry", "anon_pseudonymize", "anon_hmac_spans", "anon_pipeline_host", "anon_gemm_bf16",
-        "anon_attention", nullptr};
+        "anon_attention", "anon_ctx_profile", "anon_ctx_profile_read", nullptr};
     return names;
 }
 
@@ -54,6 +54,7 @@ extern "C" int anon_ctx_create(anon_ctx** out, int device, void* cuda_stream, si
 
 extern "C" void anon_ctx_destroy(anon_ctx* c) {
     if (!c) return;
+    for (auto& r : c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     cudaFree(c->ws);
     cudaFree(c->d_status);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
@@ -71,6 +72,34 @@ extern "C" int anon_ctx_sync(anon_ctx* ctx) {
         CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
     }
     return s;
+}
+
+extern "C" int anon_ctx_profile(anon_ctx* ctx, int enable) {
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->prof_on = enable != 0;
+    ctx->prof_used = 0;
+    ctx->n_launches = 0;
+    for (int i = 0; i < PROF_NCLASS; i++) { ctx->prof_work[i] = 0; ctx->prof_launches[i] = 0; }
+    return ANON_OK;
+}
+
+extern "C" int anon_ctx_profile_read(anon_ctx* ctx, double* class_ms, double* class_work, int64_t* class_launches,
+                                     int64_t* total_launches) {
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    double ms[PROF_NCLASS] = {0};
+    for (size_t i = 0; i < ctx->prof_used; i++) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, ctx->prof_recs[i].a, ctx->prof_recs[i].b) == cudaSuccess) ms[ctx->prof_recs[i].cls] += t;
+    }
+    for (int i = 0; i < PROF_NCLASS; i++) {
+        if (class_ms) class_ms[i] = ms[i];
+        if (class_work) class_work[i] = ctx->prof_work[i];
+        if (class_launches) class_launches[i] = ctx->prof_launches[i];
+    }
+    if (total_launches) *total_launches = ctx->n_launches;
+    return ANON_OK;
 }
 
 extern "C" const char* anon_last_cuda_error(anon_ctx* ctx) { return ctx ? ctx->cuda_err : ""; }

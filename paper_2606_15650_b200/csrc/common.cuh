@@ -7,8 +7,13 @@
 #include <stddef.h>
 #include <stdio.h>
 #include <string.h>
+#include <vector>
 
 #include "../../include/anonshield.h"
+
+// per-kernel-class CUDA-event timing (anon_ctx_profile): classes index ctx->prof_* arrays
+enum ProfClass { PROF_GEMM = 0, PROF_ATTN = 1, PROF_ROW = 2, PROF_DECODE = 3, PROF_PSEUDO = 4, PROF_NCLASS = 8 };
+struct ProfRec { cudaEvent_t a, b; int cls; };
 
 struct anon_ctx {
     int device = 0;
@@ -23,6 +28,33 @@ struct anon_ctx {
     // cached driver entry point for cuTensorMapEncodeTiled (resolved lazily, see gemm_tcgen05.cu)
     void* encode_tiled = nullptr;
     int smem_optin = 0;
+    // launch accounting + optional event profiling
+    long long n_launches = 0;
+    bool prof_on = false;
+    std::vector<ProfRec> prof_recs;       // events of the current profiling window (pooled, reused)
+    size_t prof_used = 0;
+    double prof_work[PROF_NCLASS] = {0};
+    long long prof_launches[PROF_NCLASS] = {0};
+};
+
+// RAII: brackets the launches of one kernel class with events on the context stream (when profiling is on)
+struct ProfScope {
+    anon_ctx* c; ProfRec* r = nullptr;
+    ProfScope(anon_ctx* ctx, int cls, double work, int launches = 1) : c(ctx) {
+        c->n_launches += launches;
+        if (!c->prof_on) return;
+        if (c->prof_used == c->prof_recs.size()) {
+            ProfRec n; n.cls = cls;
+            if (cudaEventCreate(&n.a) != cudaSuccess || cudaEventCreate(&n.b) != cudaSuccess) return;
+            c->prof_recs.push_back(n);
+        }
+        r = &c->prof_recs[c->prof_used++];
+        r->cls = cls;
+        c->prof_work[cls] += work;
+        c->prof_launches[cls] += launches;
+        cudaEventRecord(r->a, c->stream);
+    }
+    ~ProfScope() { if (r) cudaEventRecord(r->b, c->stream); }
 };
 
 // Bump cursor over the context workspace.  Every public entry point starts one at offset 0

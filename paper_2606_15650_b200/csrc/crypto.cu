@@ -415,6 +415,7 @@ int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t*
     if (!slot_of || !new_list || !agg) return ANON_ERR_OOM;
     const long long* off = (const long long*)d_off;
     const unsigned nb256 = (unsigned)((S + 255) / 256);
+    ProfScope prof(ctx, PROF_PSEUDO, 0.0, 6);
 
     cache_probe_kernel<<<nb256, 256, 0, st>>>(d_bytes, off, S, c->d_table, c->n_slots - 1, c->d_arena,
                                                c->d_entry_off, slot_of, ctx->d_status);
@@ -482,6 +483,7 @@ extern "C" int anon_hmac_spans(anon_ctx* ctx, const uint8_t* d_span_bytes, const
     if (S == 0) return ANON_OK;
     PadStates ps;
     make_pads(key, key_len, &ps);
+    ProfScope prof(ctx, PROF_PSEUDO, 0.0, 1);
     hmac_spans_kernel<<<(unsigned)((S + 127) / 128), 128, 0, ctx->stream>>>(
         d_span_bytes, (const long long*)d_span_offsets, S, (uint32_t*)d_digests, ps);
     CU_LAUNCH_CHECK(ctx, "hmac_spans_kernel");

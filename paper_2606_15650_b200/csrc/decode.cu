@@ -113,6 +113,7 @@ int decode_spans_impl(anon_ctx* ctx, WsCursor& ws, const int32_t* d_labels, cons
     int* agg_i = (int*)ws.take(scan::agg_bytes<int>(T));
     long long* agg_l = (long long*)ws.take(scan::agg_bytes<long long>(T));
     if (!prev || !agg_i || !agg_l) return ANON_ERR_OOM;
+    ProfScope ps(ctx, PROF_DECODE, (double)T * 20 + (double)T * 8, 7);
     KeepIn kin{d_meta};
     scan::reduce_and_scan<int, scan::MaxI32>(kin, T, nullptr, agg_i, st);
     scan::apply<int, scan::MaxI32>(kin, PrevKeptOut{prev}, T, nullptr, agg_i, st);
@@ -134,6 +135,7 @@ int gather_spans_impl(anon_ctx* ctx, WsCursor& ws, const uint8_t* d_text, const 
     if (S_max == 0) { CU_TRY(ctx, cudaMemsetAsync(d_off, 0, 8, st)); return ANON_OK; }
     long long* agg = (long long*)ws.take(scan::agg_bytes<long long>(S_max));
     if (!agg) return ANON_ERR_OOM;
+    ProfScope ps(ctx, PROF_DECODE, (double)S_max * 40, 4);
     LenIn lin{d_spans};
     scan::reduce_and_scan<long long, scan::SumI64>(lin, S_max, d_num_spans, agg, st);
     scan::apply<long long, scan::SumI64>(lin, GatherOut{d_spans, d_text, (const long long*)d_rec_off, d_bytes,

@@ -193,7 +193,11 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
             AttnPlan plan;
             int prc = attention_plan(ctx, c, h_cu + s0, nb, d.dtype, &plan);
             if (prc) return prc;
+            double attn_flops = 0;            // 4 n^2 d per (sequence, head): QK^T and PV
+            for (int s = s0; s < s1; s++) { const double n = h_cu[s + 1] - h_cu[s]; attn_flops += 4.0 * n * n * H; }
             const unsigned row_grid = (unsigned)((nt + enc::kRowWarps - 1) / enc::kRowWarps);
+            const double row_bytes = (double)nt * H * 4 * 2 + (bf ? (double)nt * H * 2 : 0);   // LN: read y, write x (+xb)
+            { ProfScope ps(ctx, PROF_ROW, (double)nt * H * (bf ? 2 : 4) + (double)nt * (4 + H * 4 + (bf ? H * 2 : 0)));
             if (bf)
                 enc::embed_ln_kernel<__nv_bfloat16><<<row_grid, enc::kRowWarps * 32, 0, st>>>(
                     d_ids, d_cu, B, tok0, nt, (const __nv_bfloat16*)w->E_w, (const __nv_bfloat16*)w->E_p, w->E_t, w->g_e,
@@ -202,32 +206,41 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                 enc::embed_ln_kernel<float><<<row_grid, enc::kRowWarps * 32, 0, st>>>(
                     d_ids, d_cu, B, tok0, nt, (const float*)w->E_w, (const float*)w->E_p, w->E_t, w->g_e, w->b_e,
                     d.ln_eps, H, d.vocab, d.max_pos, x, nullptr, ctx->d_status);
+            }
             CU_LAUNCH_CHECK(ctx, "embed_ln_kernel");
             for (int l = 0; l < d.layers; l++) {
                 const LayerW& L = w->layers[l];
                 int rc;
+                { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * 3 * H * H);
                 if (bf) rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_qkv, L.b_qkv, nullptr, qkv, nt, 3 * H, H, 0);
-                else rc = sgemm<0>(ctx, x, (const float*)L.W_qkv, L.b_qkv, nullptr, (float*)qkv, nt, 3 * H, H);
+                else rc = sgemm<0>(ctx, x, (const float*)L.W_qkv, L.b_qkv, nullptr, (float*)qkv, nt, 3 * H, H); }
                 if (rc) return rc;
-                rc = attention_run(ctx, plan, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx);
+                { ProfScope ps(ctx, PROF_ATTN, attn_flops);
+                rc = attention_run(ctx, plan, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx); }
                 if (rc) return rc;
+                { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * H * H);
                 if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, y, nt, H, H, 2);
-                else rc = sgemm<2>(ctx, (const float*)cx, (const float*)L.W_o, L.b_o, x, y, nt, H, H);
+                else rc = sgemm<2>(ctx, (const float*)cx, (const float*)L.W_o, L.b_o, x, y, nt, H, H); }
                 if (rc) return rc;
-                enc::layer_norm_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, L.g_1, L.b_1, d.ln_eps, x, xb);
+                { ProfScope ps(ctx, PROF_ROW, row_bytes);
+                enc::layer_norm_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, L.g_1, L.b_1, d.ln_eps, x, xb); }
                 CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+                { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * F * H);
                 if (bf) rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_1, L.b_1f, nullptr, f, nt, F, H, 1);
-                else rc = sgemm<1>(ctx, x, (const float*)L.W_1, L.b_1f, nullptr, (float*)f, nt, F, H);
+                else rc = sgemm<1>(ctx, x, (const float*)L.W_1, L.b_1f, nullptr, (float*)f, nt, F, H); }
                 if (rc) return rc;
+                { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * F * H);
                 if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, x, y, nt, H, F, 2);
-                else rc = sgemm<2>(ctx, (const float*)f, (const float*)L.W_2, L.b_2f, x, y, nt, H, F);
+                else rc = sgemm<2>(ctx, (const float*)f, (const float*)L.W_2, L.b_2f, x, y, nt, H, F); }
                 if (rc) return rc;
-                enc::layer_norm_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, L.g_2, L.b_2, d.ln_eps, x, xb);
+                { ProfScope ps(ctx, PROF_ROW, row_bytes);
+                enc::layer_norm_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, L.g_2, L.b_2, d.ln_eps, x, xb); }
                 CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
             }
+            { ProfScope ps(ctx, PROF_ROW, (double)nt * (H * 4 + (d_logits ? NL * 4 : 0) + (d_labels ? 4 : 0)));
             enc::head_argmax_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(
                 x, nt, H, w->W_c, w->b_c, NL, d_logits ? d_logits + (size_t)tok0 * NL : nullptr,
-                d_labels ? d_labels + tok0 : nullptr);
+                d_labels ? d_labels + tok0 : nullptr); }
             CU_LAUNCH_CHECK(ctx, "head_argmax_kernel");
         }
         s0 = s1;

@@ -141,7 +141,11 @@ int  anon_gather_spans(anon_ctx* ctx, const uint8_t* d_text, const int64_t* d_re
  * 32 bytes of digest each.  No eviction (reading S18).  Synchronises. */
 int  anon_cache_create(anon_ctx* ctx, uint64_t max_unique, uint64_t key_arena_bytes, anon_cache** out);
 void anon_cache_destroy(anon_cache* c);
-/* Counters since creation.  Synchronises. */
+/* Forgets every entry, the counters and the key binding (table memset on the context stream;
+ * arena and digests are simply reused).  Asynchronous.  bench.py calls it between steps so that
+ * every step inserts and HMACs the same set of new entities. */
+int  anon_cache_clear(anon_cache* c);
+/* Counters since creation (or the last anon_cache_clear).  Synchronises. */
 int  anon_cache_stats(anon_cache* c, uint64_t* n_unique, uint64_t* n_lookups, uint64_t* n_hits);
 /* Entry `uid` (0 <= uid < n_unique): copies min(len, bytes_capacity) entity bytes to
  * h_bytes (may be NULL), the 32-byte digest to h_digest (may be NULL); returns the entity

@@ -53,6 +53,7 @@ _SIGNATURES = {
     "anon_gather_spans": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _vp, _sz, _vp, _vp]),
     "anon_cache_create": (ctypes.c_int, [_vp, _u64, _u64, ctypes.POINTER(_vp)]),
     "anon_cache_destroy": (None, [_vp]),
+    "anon_cache_clear": (ctypes.c_int, [_vp]),
     "anon_cache_stats": (ctypes.c_int, [_vp, ctypes.POINTER(_u64), ctypes.POINTER(_u64), ctypes.POINTER(_u64)]),
     "anon_cache_entry": (_i64, [_vp, _u64, _vp, _sz, _vp]),
     "anon_pseudonymize": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i64, _vp, _sz, _i32,
@@ -181,6 +182,9 @@ class Cache:
         self.ctx = ctx
         self._h = _vp()
         ctx.check(lib().anon_cache_create(ctx._h, max_unique, key_arena_bytes, ctypes.byref(self._h)), "anon_cache_create")
+
+    def clear(self):
+        self.ctx.check(lib().anon_cache_clear(self._h), "anon_cache_clear")
 
     def stats(self):
         a, b, c = _u64(), _u64(), _u64()

@@ -358,6 +358,16 @@ extern "C" void anon_cache_destroy(anon_cache* c) {
     delete c;
 }
 
+extern "C" int anon_cache_clear(anon_cache* c) {
+    if (!c) return ANON_ERR_INVALID_ARG;
+    anon_ctx* ctx = c->ctx;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    CU_TRY(ctx, cudaMemsetAsync(c->d_table, 0, c->n_slots * 8, ctx->stream));
+    c->n_unique = c->arena_used = c->n_lookups = c->n_hits = 0;
+    c->key_bound = false;
+    return ANON_OK;
+}
+
 extern "C" int anon_cache_stats(anon_cache* c, uint64_t* n_unique, uint64_t* n_lookups, uint64_t* n_hits) {
     if (!c) return ANON_ERR_INVALID_ARG;
     CU_TRY(c->ctx, cudaStreamSynchronize(c->ctx->stream));

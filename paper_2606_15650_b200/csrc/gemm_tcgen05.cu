@@ -9,8 +9,12 @@
 //                           the epilogue of tile i overlaps the mainloop of tile i+1; tcgen05.commit frees
 //                           ring slots / publishes accumulators
 //   warp 2   TMEM allocator
-//   warps 4-7 epilogue    : tcgen05.ld (32 lanes x 32 columns per warp) -> bias / GELU / residual in
-//                           registers -> vectorised global stores
+//   warps 4-7 epilogue    : tcgen05.ld (32 lanes x 32 columns per warp) -> bias / GELU / residual in registers
+//                           -> 128B-swizzled shared-memory boxes (one row per thread, conflict-free) -> TMA store
+//                           (coalesced, asynchronous, M/N tails clipped by the tensor map).  The FP32 residual
+//                           tile arrives the same way: each epilogue warp TMA-loads its own 32x32 boxes three
+//                           boxes ahead (also across tiles, so they land during the next mainloop), adds in
+//                           place and stores from the same buffer.
 // Operands are "TN": A row-major [M,K], W row-major [N,K] (both K-contiguous = K-major UMMA operands).
 #include "common.cuh"
 #include "ptx_sm100.cuh"
@@ -25,12 +29,15 @@ constexpr int UMMA_K = 16;
 constexpr int kThreads = 256;
 constexpr int A_STAGE_BYTES = BM * BK * 2;
 
-template <int BN> struct Cfg {
+template <int BN, int EPI> struct Cfg {
     static constexpr int B_STAGE_BYTES = BN * BK * 2;
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
-    static constexpr int STAGES = (BN == 256) ? 4 : 6;
-    static constexpr int TMEM_COLS = 2 * BN;      // two accumulator buffers
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+    static constexpr int EPI_BUFS = (EPI == 2) ? 4 : 2;           // 4 KB boxes per epilogue warp
+    static constexpr int EPI_BYTES = 4 * EPI_BUFS * 4096;
+    static constexpr int STAGES = (BN == 256) ? (EPI == 2 ? 3 : 4) : (EPI == 2 ? 4 : 6);
+    static constexpr int TMEM_COLS = 2 * BN;                      // two accumulator buffers
+    static constexpr int NUM_BARS = 2 * STAGES + 4 + 16;
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + EPI_BYTES + 1024 /*align slack*/ + 512 /*barriers*/;
 };
 
 // erf-GELU with the Abramowitz-Stegun 7.1.26 rational-exponential form (|err(erf)| < 1.5e-7, far below
@@ -52,23 +59,33 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
     __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
     return *reinterpret_cast<uint32_t*>(&v);
 }
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+    return v;
+}
 
 // EPI: 0 = +bias -> BF16;  1 = +bias, GELU -> BF16;  2 = +bias +residual(FP32) -> FP32
 template <int BN, int EPI>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
-                         const float* __restrict__ bias, const float* __restrict__ residual, void* __restrict__ Cout,
-                         int M, int N, int K)
+                         const __grid_constant__ CUtensorMap tmap_c, const __grid_constant__ CUtensorMap tmap_r,
+                         const float* __restrict__ bias, int M, int N, int K)
 {
-    using C = Cfg<BN>;
+    using C = Cfg<BN, EPI>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bar_base = smem_base + C::STAGES * C::STAGE_BYTES;
+    const uint32_t epi_base = smem_base + C::STAGES * C::STAGE_BYTES;
+    const uint32_t bar_base = epi_base + C::EPI_BYTES;
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (C::STAGES + s); };
     auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * C::STAGES + a); };
     auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * C::STAGES + 2 + a); };
-    const uint32_t tmem_slot = bar_base + 8u * (2 * C::STAGES + 4);
+    auto rfull_bar = [&](int q, int b) { return bar_base + 8u * (2 * C::STAGES + 4 + 4 * q + b); };
+    const uint32_t tmem_slot = bar_base + 8u * C::NUM_BARS;
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -79,10 +96,13 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&tmap_a);
         ptx::prefetch_tensormap(&tmap_b);
+        ptx::prefetch_tensormap(&tmap_c);
+        if (EPI == 2) ptx::prefetch_tensormap(&tmap_r);
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < C::STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
         for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 4); }
+        for (int i = 0; i < 16; i++) ptx::mbar_init(rfull_bar(i >> 2, i & 3), 1);
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
     }
@@ -140,72 +160,125 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         }
     } else if (warp >= 4) {
         const int q = warp & 3;                       // TMEM lane quarter this warp may access
+        const uint32_t stg = epi_base + (uint32_t)(q * C::EPI_BUFS * 4096);
+        const uint32_t row_off = (uint32_t)lane * 128u;      // this thread's row inside a 32-row box
+        const uint32_t sw = (uint32_t)(lane & 7);            // 128B swizzle: 16-byte chunk index ^= row & 7
         int acc = 0; uint32_t acc_ph = 0;
-        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-            const int m_blk = tile / num_n, n_blk = tile % num_n;
-            const int row = m_blk * BM + q * 32 + lane;
-            ptx::mbar_wait(tfull_bar(acc), acc_ph);
-            ptx::tc_fence_after();
-            const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
+        uint32_t nbox = 0;                            // boxes this warp has handled (buffer ring position)
+
+        if constexpr (EPI == 2) {
+            constexpr int BPT = BN / 32;              // 32x32 FP32 boxes per tile per warp
+            uint32_t rph = 0;                         // phase bit of each residual buffer's barrier
+            auto issue_load = [&](uint32_t i) {       // lane 0: residual box i -> buffer i & 3
+                const int tile = blockIdx.x + (int)(i / BPT) * (int)gridDim.x;
+                if (tile >= num_tiles) return;
+                const int row0 = (tile / num_n) * BM + q * 32, col = (tile % num_n) * BN + (int)(i % BPT) * 32;
+                if (row0 >= M || col >= N) return;
+                const uint32_t bar = rfull_bar(q, i & 3);
+                ptx::mbar_arrive_expect_tx(bar, 4096);
+                ptx::tma_load_2d(stg + (i & 3) * 4096u, &tmap_r, bar, col, row0);
+            };
+            if (lane == 0) { issue_load(0); issue_load(1); issue_load(2); }
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+                const int m_blk = tile / num_n, n_blk = tile % num_n;
+                const int row0 = m_blk * BM + q * 32;
+                ptx::mbar_wait(tfull_bar(acc), acc_ph);
+                ptx::tc_fence_after();
+                const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
 #pragma unroll 1
-            for (int c0 = 0; c0 < BN; c0 += 32) {
-                uint32_t r[32];
-                ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)c0, r);
-                ptx::tmem_ld_wait();
-                const int col = n_blk * BN + c0;
-                if (row < M && col < N) {
-                    if (col + 32 <= N) {
-                        const float4* b4 = reinterpret_cast<const float4*>(bias + col);
-                        if (EPI == 2) {
-                            const float4* r4 = reinterpret_cast<const float4*>(residual + (size_t)row * N + col);
-                            float4* o4 = reinterpret_cast<float4*>(reinterpret_cast<float*>(Cout) + (size_t)row * N + col);
-#pragma unroll
-                            for (int v = 0; v < 8; v++) {
-                                const float4 b = __ldg(b4 + v), x = __ldg(r4 + v);
-                                float4 o;
-                                o.x = __uint_as_float(r[4 * v + 0]) + b.x + x.x;
-                                o.y = __uint_as_float(r[4 * v + 1]) + b.y + x.y;
-                                o.z = __uint_as_float(r[4 * v + 2]) + b.z + x.z;
-                                o.w = __uint_as_float(r[4 * v + 3]) + b.w + x.w;
-                                o4[v] = o;
-                            }
-                        } else {
-                            uint4* o4 = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(Cout) + (size_t)row * N + col);
-#pragma unroll
-                            for (int v = 0; v < 4; v++) {
-                                const float4 b0 = __ldg(b4 + 2 * v), b1 = __ldg(b4 + 2 * v + 1);
-                                float f[8];
-                                f[0] = __uint_as_float(r[8 * v + 0]) + b0.x; f[1] = __uint_as_float(r[8 * v + 1]) + b0.y;
-                                f[2] = __uint_as_float(r[8 * v + 2]) + b0.z; f[3] = __uint_as_float(r[8 * v + 3]) + b0.w;
-                                f[4] = __uint_as_float(r[8 * v + 4]) + b1.x; f[5] = __uint_as_float(r[8 * v + 5]) + b1.y;
-                                f[6] = __uint_as_float(r[8 * v + 6]) + b1.z; f[7] = __uint_as_float(r[8 * v + 7]) + b1.w;
-                                if (EPI == 1) {
-#pragma unroll
-                                    for (int u = 0; u < 8; u++) f[u] = gelu_fast(f[u]);
-                                }
-                                o4[v] = make_uint4(pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]),
-                                                   pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
-                            }
-                        }
-                    } else {
-                        for (int u = 0; u < 32 && col + u < N; u++) {          // ragged N tail
-                            float f = __uint_as_float(r[u]) + bias[col + u];
-                            if (EPI == 1) f = gelu_fast(f);
-                            if (EPI == 2) {
-                                f += residual[(size_t)row * N + col + u];
-                                reinterpret_cast<float*>(Cout)[(size_t)row * N + col + u] = f;
-                            } else {
-                                reinterpret_cast<__nv_bfloat16*>(Cout)[(size_t)row * N + col + u] = __float2bfloat16_rn(f);
-                            }
-                        }
+                for (int j = 0; j < BPT; j++, nbox++) {
+                    const int col = n_blk * BN + j * 32;
+                    const uint32_t b = nbox & 3u;
+                    const uint32_t buf = stg + b * 4096u;
+                    uint32_t r[32];
+                    ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)(j * 32), r);
+                    ptx::tmem_ld_wait();
+                    if (j == BPT - 1) {               // accumulator fully read: hand it back to the MMA warp
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
                     }
+                    const bool valid = row0 < M && col < N;      // warp-uniform
+                    if (valid) {
+                        ptx::mbar_wait(rfull_bar(q, b), (rph >> b) & 1u);
+                        rph ^= 1u << b;
+#pragma unroll
+                        for (int v = 0; v < 8; v++) {
+                            const uint32_t addr = buf + row_off + (((uint32_t)v ^ sw) << 4);
+                            const float4 x = ld_shared_f4(addr);
+                            float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
+                            if (col + 4 * v < N) bb = __ldg(reinterpret_cast<const float4*>(bias + col + 4 * v));
+                            st_shared_v4(addr, __float_as_uint(__uint_as_float(r[4 * v + 0]) + bb.x + x.x),
+                                         __float_as_uint(__uint_as_float(r[4 * v + 1]) + bb.y + x.y),
+                                         __float_as_uint(__uint_as_float(r[4 * v + 2]) + bb.z + x.z),
+                                         __float_as_uint(__uint_as_float(r[4 * v + 3]) + bb.w + x.w));
+                        }
+                        ptx::fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) ptx::tma_store_2d(&tmap_c, buf, col, row0);
+                    }
+                    if (lane == 0) {
+                        ptx::bulk_commit();
+                        ptx::bulk_wait_read<1>();     // the store of box nbox-1 has read its buffer: refill it
+                        issue_load(nbox + 3);
+                    }
+                    __syncwarp();
                 }
+                if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
             }
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
-            if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
+        } else {
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+                const int m_blk = tile / num_n, n_blk = tile % num_n;
+                const int row0 = m_blk * BM + q * 32;
+                ptx::mbar_wait(tfull_bar(acc), acc_ph);
+                ptx::tc_fence_after();
+                const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
+#pragma unroll 1
+                for (int c0 = 0; c0 < BN; c0 += 64, nbox++) {      // one 32-row x 64-column BF16 box (128 B rows)
+                    const int col = n_blk * BN + c0;
+                    const uint32_t buf = stg + (nbox & 1u) * 4096u;
+                    if (lane == 0) ptx::bulk_wait_read<1>();       // the store two boxes ago has read this buffer
+                    __syncwarp();
+                    uint32_t r[64];
+                    ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)c0, r);
+                    ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)(c0 + 32), r + 32);
+                    ptx::tmem_ld_wait();
+                    if (c0 + 64 == BN) {
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+                    }
+                    const bool valid = row0 < M && col < N;        // warp-uniform
+                    if (valid) {
+#pragma unroll
+                        for (int v = 0; v < 8; v++) {
+                            float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
+                            if (col + 8 * v < N) {                 // N % 8 == 0: an 8-column group is all in or all out
+                                b0 = __ldg(reinterpret_cast<const float4*>(bias + col + 8 * v));
+                                b1 = __ldg(reinterpret_cast<const float4*>(bias + col + 8 * v + 4));
+                            }
+                            float f[8];
+                            f[0] = __uint_as_float(r[8 * v + 0]) + b0.x; f[1] = __uint_as_float(r[8 * v + 1]) + b0.y;
+                            f[2] = __uint_as_float(r[8 * v + 2]) + b0.z; f[3] = __uint_as_float(r[8 * v + 3]) + b0.w;
+                            f[4] = __uint_as_float(r[8 * v + 4]) + b1.x; f[5] = __uint_as_float(r[8 * v + 5]) + b1.y;
+                            f[6] = __uint_as_float(r[8 * v + 6]) + b1.z; f[7] = __uint_as_float(r[8 * v + 7]) + b1.w;
+                            if (EPI == 1) {
+#pragma unroll
+                                for (int u = 0; u < 8; u++) f[u] = gelu_fast(f[u]);
+                            }
+                            st_shared_v4(buf + row_off + (((uint32_t)v ^ sw) << 4), pack_bf16(f[0], f[1]),
+                                         pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
+                        }
+                        ptx::fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) ptx::tma_store_2d(&tmap_c, buf, col, row0);
+                    }
+                    if (lane == 0) ptx::bulk_commit();
+                }
+                if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
+            }
         }
+        if (lane == 0) ptx::bulk_wait<0>();           // every store has completed before shared memory goes away
     }
 
     ptx::tc_fence_before();
@@ -220,7 +293,10 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-int make_tmap_bf16_2d(anon_ctx* ctx, CUtensorMap* tm, const void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+// 2-D row-major tensor [rows, cols] of `esize`-byte elements, box [box_rows, box_cols] (box_cols * esize = 128 B),
+// 128-byte swizzle.
+int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_t esize, const void* base, uint64_t rows,
+                 uint64_t cols, uint32_t box_cols, uint32_t box_rows) {
     if (!ctx->encode_tiled) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult q;
@@ -230,13 +306,12 @@ int make_tmap_bf16_2d(anon_ctx* ctx, CUtensorMap* tm, const void* base, uint64_t
         ctx->encode_tiled = fn;
     }
     const cuuint64_t gdim[2] = {cols, rows};
-    const cuuint64_t gstride[1] = {cols * 2};
-    const cuuint32_t box[2] = {(cuuint32_t)BK, box_rows};
+    const cuuint64_t gstride[1] = {cols * esize};
+    const cuuint32_t box[2] = {box_cols, box_rows};
     const cuuint32_t estr[2] = {1, 1};
-    CUresult r = ((EncodeTiledFn)ctx->encode_tiled)(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim,
-                                                    gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                                                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = ((EncodeTiledFn)ctx->encode_tiled)(tm, dt, 2, const_cast<void*>(base), gdim, gstride, box, estr,
+                                                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(ctx->cuda_err, sizeof ctx->cuda_err, "cuTensorMapEncodeTiled failed: CUresult %d", (int)r);
         return ANON_ERR_CUDA;
@@ -248,12 +323,22 @@ template <int BN, int EPI>
 int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
                 void* Cout, int M, int N, int K)
 {
-    using C = Cfg<BN>;
-    CUtensorMap ta, tb;
-    int rc = make_tmap_bf16_2d(ctx, &ta, A, (uint64_t)M, (uint64_t)K, BM);
+    using C = Cfg<BN, EPI>;
+    CUtensorMap ta, tb, tc, tr;
+    int rc = make_tmap_2d(ctx, &ta, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, A, (uint64_t)M, (uint64_t)K, BK, BM);
     if (rc) return rc;
-    rc = make_tmap_bf16_2d(ctx, &tb, W, (uint64_t)N, (uint64_t)K, BN);
+    rc = make_tmap_2d(ctx, &tb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, W, (uint64_t)N, (uint64_t)K, BK, BN);
     if (rc) return rc;
+    if (EPI == 2) {
+        rc = make_tmap_2d(ctx, &tc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Cout, (uint64_t)M, (uint64_t)N, 32, 32);
+        if (rc) return rc;
+        rc = make_tmap_2d(ctx, &tr, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, residual, (uint64_t)M, (uint64_t)N, 32, 32);
+        if (rc) return rc;
+    } else {
+        rc = make_tmap_2d(ctx, &tc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, Cout, (uint64_t)M, (uint64_t)N, 64, 32);
+        if (rc) return rc;
+        tr = tc;
+    }
     auto kern = gemm_bf16_tcgen05_kernel<BN, EPI>;
     static bool attr_set = false;
     if (!attr_set) {
@@ -262,7 +347,7 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
     }
     const int tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
     const int grid = tiles < ctx->sm_count ? tiles : ctx->sm_count;
-    kern<<<grid, kThreads, C::SMEM_BYTES, ctx->stream>>>(ta, tb, bias, residual, Cout, M, N, K);
+    kern<<<grid, kThreads, C::SMEM_BYTES, ctx->stream>>>(ta, tb, tc, tr, bias, M, N, K);
     CU_LAUNCH_CHECK(ctx, "gemm_bf16_tcgen05_kernel");
     return ANON_OK;
 }

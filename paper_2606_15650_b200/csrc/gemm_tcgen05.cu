@@ -26,33 +26,67 @@ namespace {
 constexpr int BM = 128;
 constexpr int BK = 64;                    // 64 BF16 = 128 bytes = one swizzle row
 constexpr int UMMA_K = 16;
-constexpr int kThreads = 256;
+constexpr int kThreads = 384;               // warps 0-3: TMA / MMA / TMEM alloc / idle; warps 4-11: epilogue
 constexpr int A_STAGE_BYTES = BM * BK * 2;
 
-template <int BN, int EPI> struct Cfg {
+// NB = FP32 residual boxes in flight per epilogue warp (EPI 2 only): 4 for short K (the epilogue's HBM traffic
+// paces the kernel), 2 for long K (a fourth mainloop stage is worth more).
+template <int BN, int EPI, int NB> struct Cfg {
     static constexpr int B_STAGE_BYTES = BN * BK * 2;
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
-    static constexpr int EPI_BUFS = (EPI == 2) ? 4 : 2;           // 4 KB boxes per epilogue warp
-    static constexpr int EPI_BYTES = 4 * EPI_BUFS * 4096;
-    static constexpr int STAGES = (BN == 256) ? (EPI == 2 ? 3 : 4) : (EPI == 2 ? 4 : 6);
+    static constexpr int EPI_WARPS = (EPI == 2) ? 4 : 8;
+    static constexpr int EPI_BYTES = (EPI == 2) ? 4 * NB * 4096 : 8 * 4096;   // 4 KB boxes
+    static constexpr int STAGES = (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES > 6 ? 6 : (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES;
     static constexpr int TMEM_COLS = 2 * BN;                      // two accumulator buffers
     static constexpr int NUM_BARS = 2 * STAGES + 4 + 16;
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + EPI_BYTES + 1024 /*align slack*/ + 512 /*barriers*/;
 };
 
-// erf-GELU with the Abramowitz-Stegun 7.1.26 rational-exponential form (|err(erf)| < 1.5e-7, far below
-// the BF16 rounding of the stored activation); 2 MUFU ops + ~12 FMA-pipe ops per element.
-__device__ __forceinline__ float gelu_fast(float z) {
-    const float x = fabsf(z) * 0.70710678118654752f;
-    const float t = __fdividef(1.0f, fmaf(0.3275911f, x, 1.0f));
-    float p = fmaf(t, 1.061405429f, -1.453152027f);
-    p = fmaf(t, p, 1.421413741f);
-    p = fmaf(t, p, -0.284496736f);
-    p = fmaf(t, p, 0.254829592f);
-    p *= t;
-    const float e = __expf(-x * x);
-    const float erf_abs = fmaf(-p, e, 1.0f);
-    return 0.5f * z * (1.0f + copysignf(erf_abs, z));
+__device__ __forceinline__ uint32_t pack_bf16(float a, float b);
+// ---- packed FP32x2 arithmetic (sm_100 FFMA2 / FMUL2 / FADD2: two lanes per issue slot) ----
+__device__ __forceinline__ uint64_t pk2(float a, float b) {
+    uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r;
+}
+__device__ __forceinline__ void upk2(uint64_t v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
+    uint64_t d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+    uint64_t d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// erf-GELU (reading D3) for two values at once: gelu(z) = z * Phi(z) with Phi(z) = sigma(z * P(z^2)), P a degree-4
+// polynomial in z^2 fitted (minimax, csrc/fit_gelu_coeffs.py) so that |z| * |sigma(z P(z^2)) - Phi(z)| <= 3.1e-6 for
+// every z (the leading coefficient is positive, so the form saturates correctly and needs no clamp).  That is
+// ~1e3 below the BF16 rounding of the stored activation.  The coefficients below carry the factor -log2(e) so that
+// sigma(u) = 1 / (1 + 2^(u')).  Cost per pair: 8 packed FMA-pipe ops + 4 MUFU (ex2, rcp) + 1 convert.
+__device__ __forceinline__ uint32_t gelu2_bf16(uint64_t z) {
+    constexpr float kL = -1.4426950408889634f;
+    const uint64_t c1 = pk2(kL * 1.5956562720997576f, kL * 1.5956562720997576f);
+    const uint64_t c3 = pk2(kL * 0.07293758090262617f, kL * 0.07293758090262617f);
+    const uint64_t c5 = pk2(kL * -0.00024972250409287103f, kL * -0.00024972250409287103f);
+    const uint64_t c7 = pk2(kL * -6.116217765511888e-05f, kL * -6.116217765511888e-05f);
+    const uint64_t c9 = pk2(kL * 2.2381744780047116e-06f, kL * 2.2381744780047116e-06f);
+    const uint64_t z2 = mul2(z, z);
+    uint64_t p = fma2(c9, z2, c7);
+    p = fma2(p, z2, c5);
+    p = fma2(p, z2, c3);
+    p = fma2(p, z2, c1);
+    const uint64_t u = mul2(p, z);
+    float u0, u1;
+    upk2(u, u0, u1);
+    const uint64_t d = add2(pk2(ex2_approx(u0), ex2_approx(u1)), pk2(1.0f, 1.0f));
+    float d0, d1;
+    upk2(d, d0, d1);
+    const uint64_t g = mul2(z, pk2(rcp_approx(d0), rcp_approx(d1)));
+    float g0, g1;
+    upk2(g, g0, g1);
+    return pack_bf16(g0, g1);
 }
 
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
@@ -69,13 +103,13 @@ __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
 }
 
 // EPI: 0 = +bias -> BF16;  1 = +bias, GELU -> BF16;  2 = +bias +residual(FP32) -> FP32
-template <int BN, int EPI>
+template <int BN, int EPI, int NB>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                          const __grid_constant__ CUtensorMap tmap_c, const __grid_constant__ CUtensorMap tmap_r,
                          const float* __restrict__ bias, int M, int N, int K)
 {
-    using C = Cfg<BN, EPI>;
+    using C = Cfg<BN, EPI, NB>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t epi_base = smem_base + C::STAGES * C::STAGE_BYTES;
@@ -101,7 +135,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < C::STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
-        for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 4); }
+        for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), C::EPI_WARPS); }
         for (int i = 0; i < 16; i++) ptx::mbar_init(rfull_bar(i >> 2, i & 3), 1);
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
@@ -158,27 +192,28 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                 if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
             }
         }
-    } else if (warp >= 4) {
+    } else if (warp >= 4 && warp < 4 + C::EPI_WARPS) {
         const int q = warp & 3;                       // TMEM lane quarter this warp may access
-        const uint32_t stg = epi_base + (uint32_t)(q * C::EPI_BUFS * 4096);
         const uint32_t row_off = (uint32_t)lane * 128u;      // this thread's row inside a 32-row box
         const uint32_t sw = (uint32_t)(lane & 7);            // 128B swizzle: 16-byte chunk index ^= row & 7
         int acc = 0; uint32_t acc_ph = 0;
         uint32_t nbox = 0;                            // boxes this warp has handled (buffer ring position)
+        (void)nbox;
 
         if constexpr (EPI == 2) {
             constexpr int BPT = BN / 32;              // 32x32 FP32 boxes per tile per warp
+            const uint32_t stg = epi_base + (uint32_t)(q * NB * 4096);
             uint32_t rph = 0;                         // phase bit of each residual buffer's barrier
-            auto issue_load = [&](uint32_t i) {       // lane 0: residual box i -> buffer i & 3
+            auto issue_load = [&](uint32_t i) {       // lane 0: residual box i -> buffer i % NB
                 const int tile = blockIdx.x + (int)(i / BPT) * (int)gridDim.x;
                 if (tile >= num_tiles) return;
                 const int row0 = (tile / num_n) * BM + q * 32, col = (tile % num_n) * BN + (int)(i % BPT) * 32;
                 if (row0 >= M || col >= N) return;
-                const uint32_t bar = rfull_bar(q, i & 3);
+                const uint32_t bar = rfull_bar(q, i % NB);
                 ptx::mbar_arrive_expect_tx(bar, 4096);
-                ptx::tma_load_2d(stg + (i & 3) * 4096u, &tmap_r, bar, col, row0);
+                ptx::tma_load_2d(stg + (i % NB) * 4096u, &tmap_r, bar, col, row0);
             };
-            if (lane == 0) { issue_load(0); issue_load(1); issue_load(2); }
+            if (lane == 0) { for (uint32_t i = 0; i + 1 < NB; i++) issue_load(i); }
             for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
                 const int m_blk = tile / num_n, n_blk = tile % num_n;
                 const int row0 = m_blk * BM + q * 32;
@@ -188,7 +223,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
 #pragma unroll 1
                 for (int j = 0; j < BPT; j++, nbox++) {
                     const int col = n_blk * BN + j * 32;
-                    const uint32_t b = nbox & 3u;
+                    const uint32_t b = nbox % NB;
                     const uint32_t buf = stg + b * 4096u;
                     uint32_t r[32];
                     ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)(j * 32), r);
@@ -220,13 +255,16 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                     if (lane == 0) {
                         ptx::bulk_commit();
                         ptx::bulk_wait_read<1>();     // the store of box nbox-1 has read its buffer: refill it
-                        issue_load(nbox + 3);
+                        issue_load(nbox + NB - 1);
                     }
                     __syncwarp();
                 }
                 if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
             }
         } else {
+            // two warps per TMEM lane quarter, each owning half of the tile's columns and one 4 KB staging box
+            const int half = (warp - 4) >> 2;
+            const uint32_t buf = epi_base + (uint32_t)((warp - 4) * 4096);
             for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
                 const int m_blk = tile / num_n, n_blk = tile % num_n;
                 const int row0 = m_blk * BM + q * 32;
@@ -234,46 +272,44 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                 ptx::tc_fence_after();
                 const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
 #pragma unroll 1
-                for (int c0 = 0; c0 < BN; c0 += 64, nbox++) {      // one 32-row x 64-column BF16 box (128 B rows)
+                for (int c0 = half * (BN / 2); c0 < (half + 1) * (BN / 2); c0 += 64) {   // 32-row x 64-column BF16 boxes
                     const int col = n_blk * BN + c0;
-                    const uint32_t buf = stg + (nbox & 1u) * 4096u;
-                    if (lane == 0) ptx::bulk_wait_read<1>();       // the store two boxes ago has read this buffer
-                    __syncwarp();
                     uint32_t r[64];
                     ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)c0, r);
                     ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)(c0 + 32), r + 32);
                     ptx::tmem_ld_wait();
-                    if (c0 + 64 == BN) {
+                    if (c0 + 64 == (half + 1) * (BN / 2)) {       // this warp's share of the accumulator is read
                         ptx::tc_fence_before();
                         __syncwarp();
                         if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
                     }
-                    const bool valid = row0 < M && col < N;        // warp-uniform
-                    if (valid) {
+                    if (row0 < M && col < N) {                     // warp-uniform
+                        uint32_t o[32];
 #pragma unroll
-                        for (int v = 0; v < 8; v++) {
-                            float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
-                            if (col + 8 * v < N) {                 // N % 8 == 0: an 8-column group is all in or all out
-                                b0 = __ldg(reinterpret_cast<const float4*>(bias + col + 8 * v));
-                                b1 = __ldg(reinterpret_cast<const float4*>(bias + col + 8 * v + 4));
-                            }
-                            float f[8];
-                            f[0] = __uint_as_float(r[8 * v + 0]) + b0.x; f[1] = __uint_as_float(r[8 * v + 1]) + b0.y;
-                            f[2] = __uint_as_float(r[8 * v + 2]) + b0.z; f[3] = __uint_as_float(r[8 * v + 3]) + b0.w;
-                            f[4] = __uint_as_float(r[8 * v + 4]) + b1.x; f[5] = __uint_as_float(r[8 * v + 5]) + b1.y;
-                            f[6] = __uint_as_float(r[8 * v + 6]) + b1.z; f[7] = __uint_as_float(r[8 * v + 7]) + b1.w;
+                        for (int v = 0; v < 16; v++) {             // 4 columns per step; N % 8 == 0
+                            float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
+                            if (col + 4 * v < N) bb = __ldg(reinterpret_cast<const float4*>(bias + col + 4 * v));
+                            const uint64_t z0 = add2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), pk2(bb.x, bb.y));
+                            const uint64_t z1 = add2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), pk2(bb.z, bb.w));
                             if (EPI == 1) {
-#pragma unroll
-                                for (int u = 0; u < 8; u++) f[u] = gelu_fast(f[u]);
+                                o[2 * v] = gelu2_bf16(z0);
+                                o[2 * v + 1] = gelu2_bf16(z1);
+                            } else {
+                                float a0, a1, a2, a3;
+                                upk2(z0, a0, a1); upk2(z1, a2, a3);
+                                o[2 * v] = pack_bf16(a0, a1);
+                                o[2 * v + 1] = pack_bf16(a2, a3);
                             }
-                            st_shared_v4(buf + row_off + (((uint32_t)v ^ sw) << 4), pack_bf16(f[0], f[1]),
-                                         pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
                         }
+                        if (lane == 0) ptx::bulk_wait_read<0>();   // the previous store has read the staging box
+                        __syncwarp();
+#pragma unroll
+                        for (int v = 0; v < 8; v++)
+                            st_shared_v4(buf + row_off + (((uint32_t)v ^ sw) << 4), o[4 * v], o[4 * v + 1], o[4 * v + 2], o[4 * v + 3]);
                         ptx::fence_proxy_async();
                         __syncwarp();
-                        if (lane == 0) ptx::tma_store_2d(&tmap_c, buf, col, row0);
+                        if (lane == 0) { ptx::tma_store_2d(&tmap_c, buf, col, row0); ptx::bulk_commit(); }
                     }
-                    if (lane == 0) ptx::bulk_commit();
                 }
                 if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
             }
@@ -319,11 +355,11 @@ int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_
     return ANON_OK;
 }
 
-template <int BN, int EPI>
+template <int BN, int EPI, int NB>
 int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
                 void* Cout, int M, int N, int K)
 {
-    using C = Cfg<BN, EPI>;
+    using C = Cfg<BN, EPI, NB>;
     CUtensorMap ta, tb, tc, tr;
     int rc = make_tmap_2d(ctx, &ta, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, A, (uint64_t)M, (uint64_t)K, BK, BM);
     if (rc) return rc;
@@ -339,7 +375,7 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
         if (rc) return rc;
         tr = tc;
     }
-    auto kern = gemm_bf16_tcgen05_kernel<BN, EPI>;
+    auto kern = gemm_bf16_tcgen05_kernel<BN, EPI, NB>;
     static bool attr_set = false;
     if (!attr_set) {
         CU_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
@@ -362,17 +398,19 @@ int gemm_bf16_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W
         return ANON_ERR_INVALID_ARG;
     if (K % BK != 0 || N % 8 != 0) return ANON_ERR_UNSUPPORTED;
     if (M == 0) return ANON_OK;
+    const bool long_k = K >= 2048;
     if (N > 128) {
         switch (epilogue) {
-            case 0: return launch_gemm<256, 0>(ctx, A, W, bias, residual, Cout, M, N, K);
-            case 1: return launch_gemm<256, 1>(ctx, A, W, bias, residual, Cout, M, N, K);
-            default: return launch_gemm<256, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
+            case 0: return launch_gemm<256, 0, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
+            case 1: return launch_gemm<256, 1, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
+            default: return long_k ? launch_gemm<256, 2, 2>(ctx, A, W, bias, residual, Cout, M, N, K)
+                                   : launch_gemm<256, 2, 4>(ctx, A, W, bias, residual, Cout, M, N, K);
         }
     }
     switch (epilogue) {
-        case 0: return launch_gemm<128, 0>(ctx, A, W, bias, residual, Cout, M, N, K);
-        case 1: return launch_gemm<128, 1>(ctx, A, W, bias, residual, Cout, M, N, K);
-        default: return launch_gemm<128, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
+        case 0: return launch_gemm<128, 0, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
+        case 1: return launch_gemm<128, 1, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
+        default: return launch_gemm<128, 2, 4>(ctx, A, W, bias, residual, Cout, M, N, K);
     }
 }
 

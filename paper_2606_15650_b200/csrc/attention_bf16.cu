@@ -1,187 +1,261 @@
 // attention_bf16.cu -- K3: packed variable-length bidirectional self-attention, d_head = 64 (S8a A3; S8c O1).
-// No padding FLOPs: the work list holds one item per (sequence, 64-query tile), longest sequences first;
-// keys are walked in 64-key tiles up to the sequence's own length only.  BF16 operands, FP32 scores,
-// FP32 online softmax (exp2 with the 1/sqrt(64)*log2(e) scale folded in), FP32 output accumulators.
+// No padding FLOPs: the work list holds one item per (sequence, 128-query tile), longest sequences first; keys
+// are walked in 64-key chunks up to the sequence's own length only.
 //
-// v0 (this file): warp-level mma.sync.m16n8k16 tensor-core tiles fed by cp.async double buffering and
-// ldmatrix from XOR-swizzled shared memory.  The tcgen05/TMEM version replaces it once the GEMM path is tuned.
+// sm_100a design (BF16 path): persistent CTAs, two per SM (96 KB shared memory, 256 TMEM columns each), looping
+// over (work item, head) units.  Warp-specialised:
+//   warp 0      TMA producer : Q tile [128 x 64] (double-buffered) and K / V chunks [64 x 64] (4-stage ring) of the
+//                              packed qkv tensor, 128B swizzle, mbarrier completion
+//   warp 1      MMA issuer   : S = Q K^T   tcgen05.mma M128 N64 K16 x4, both operands K-major in shared memory,
+//                                          accumulator = one of two 64-column S buffers in TMEM
+//                              O += P V    A = P read from TMEM (BF16 pairs written by the softmax warps over the
+//                                          S buffer they have just consumed), B = V chunk, MN-major descriptor
+//                              QK^T of chunk g+1 is issued before PV of chunk g, so the tensor pipe works while the
+//                              softmax warps are busy with chunk g
+//   warps 2-5   softmax      : one thread per query row: tcgen05.ld S -> FP32 max -> exp2 (1/sqrt(64)*log2(e) folded
+//                              in) -> row sum -> BF16 P -> tcgen05.st.  The running reference max is only raised
+//                              when a chunk exceeds it by more than 2^8 (then O is rescaled in TMEM), so the common
+//                              path never touches O; the final O / l uses the same reference, hence exact.
+// The softmax is MUFU-bound at d_head = 64 (one exp per 256 tensor FLOPs); two CTAs per SM keep the MUFU pipes of
+// all four SMSPs fed while either CTA waits for an MMA or a TMA.
 #include "common.cuh"
+#include "ptx_sm100.cuh"
 
 #include <algorithm>
 #include <vector>
 
 namespace {
 
-constexpr int kQT = 64;     // queries per CTA (16 per warp)
-constexpr int kKT = 64;     // keys per pipeline stage
+constexpr int kQT = 128;    // queries per work item
+constexpr int kKC = 64;     // keys per chunk
 constexpr int kD = 64;
+constexpr int kKVStages = 4;
+constexpr int kAttThreads = 192;
+constexpr int kQBytes = kQT * kD * 2;          // 16 KB
+constexpr int kKVBytes = kKC * kD * 2;         // 8 KB (K and V each)
+constexpr int kAttSmem = 2 * kQBytes + kKVStages * 2 * kKVBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+constexpr int kAttTmemCols = 256;              // S/P buffers 2 x 64, O buffers 2 x 64
 
 struct WorkItem { int q_row0; int kv_row0; int n; int q_valid; };   // rows relative to the chunk
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
-    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
-}
-__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
-    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
-}
-__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+__device__ __forceinline__ float ex2f(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float max3(float a, float b, float c) {
+    float d; asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c)); return d;
 }
 __device__ __forceinline__ uint32_t pack2(float a, float b) {
     __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
     return *reinterpret_cast<uint32_t*>(&v);
 }
-// tile of 64 rows x 64 BF16 (128 B per row), 16-byte chunk index XOR-swizzled by (row & 7)
-__device__ __forceinline__ uint32_t tile_off(int row, int chunk) { return (uint32_t)(row * 128 + ((chunk ^ (row & 7)) << 4)); }
 
-// loads rows [row0, row0+64) x 64 columns starting at column col0 of a [*, ld] BF16 matrix; rows >= rows_valid zero-filled
-__device__ __forceinline__ void load_tile(uint32_t smem, const __nv_bfloat16* base, size_t ld, int row0, int rows_valid, int col0, int tid) {
-#pragma unroll
-    for (int it = 0; it < 4; it++) {
-        const int idx = tid + it * 128;          // 512 chunks of 16 B
-        const int r = idx >> 3, c = idx & 7;
-        const bool ok = r < rows_valid;
-        const __nv_bfloat16* src = base + (size_t)(row0 + (ok ? r : 0)) * ld + col0 + c * 8;
-        cp_async16(smem + tile_off(r, c), src, ok ? 16 : 0);
-    }
-}
-
-__global__ void __launch_bounds__(128) attention_bf16_kernel(const __nv_bfloat16* __restrict__ qkv, const WorkItem* __restrict__ work,
-                                                             int H, __nv_bfloat16* __restrict__ ctx)
+__global__ void __launch_bounds__(kAttThreads, 2)
+attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_kv,
+                         const WorkItem* __restrict__ work, int n_units, int heads, int H, __nv_bfloat16* __restrict__ ctx)
 {
-    __shared__ __align__(128) uint8_t sQ[kQT * 128];
-    __shared__ __align__(128) uint8_t sK[2][kKT * 128];
-    __shared__ __align__(128) uint8_t sV[2][kKT * 128];
-    const WorkItem w = work[blockIdx.x];
-    const int head = blockIdx.y;
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
-    const size_t ld = (size_t)3 * H;
-    const int n = w.n;
-    const int nkt = (n + kKT - 1) / kKT;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t q_smem = smem_base;                                   // 2 x 16 KB
+    const uint32_t kv_smem = smem_base + 2 * kQBytes;                    // stages x (K 8 KB | V 8 KB)
+    const uint32_t bar_base = kv_smem + kKVStages * 2 * kKVBytes;
+    auto q_full = [&](uint32_t i) { return bar_base + 8u * i; };
+    auto q_empty = [&](uint32_t i) { return bar_base + 8u * (2 + i); };
+    auto kv_full = [&](uint32_t i) { return bar_base + 8u * (4 + i); };
+    auto kv_empty = [&](uint32_t i) { return bar_base + 8u * (8 + i); };
+    auto s_full = [&](uint32_t i) { return bar_base + 8u * (12 + i); };
+    auto p_full = [&](uint32_t i) { return bar_base + 8u * (14 + i); };
+    auto pv_done = [&](uint32_t i) { return bar_base + 8u * (16 + i); };
+    auto o_full = [&](uint32_t i) { return bar_base + 8u * (18 + i); };
+    auto o_empty = [&](uint32_t i) { return bar_base + 8u * (20 + i); };
+    const uint32_t tmem_slot = bar_base + 8u * 22;
+    uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
-    load_tile(smem_u32(sQ), qkv, ld, w.q_row0, w.q_valid, head * kD, tid);
-    load_tile(smem_u32(sK[0]), qkv, ld, w.kv_row0, n, H + head * kD, tid);
-    load_tile(smem_u32(sV[0]), qkv, ld, w.kv_row0, n, 2 * H + head * kD, tid);
-    cp_async_commit();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
-    uint32_t qf[4][4];
-    float o[8][4];
-#pragma unroll
-    for (int i = 0; i < 8; i++) { o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f; }
-    float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.f, 0.f};
-    const float sl2 = 0.125f * 1.4426950408889634f;
-
-    for (int kt = 0; kt < nkt; kt++) {
-        const int buf = kt & 1;
-        if (kt + 1 < nkt) {
-            const int k0 = (kt + 1) * kKT;
-            load_tile(smem_u32(sK[buf ^ 1]), qkv, ld, w.kv_row0 + k0, n - k0, H + head * kD, tid);
-            load_tile(smem_u32(sV[buf ^ 1]), qkv, ld, w.kv_row0 + k0, n - k0, 2 * H + head * kD, tid);
-            cp_async_commit();
-            cp_async_wait<1>();
-        } else {
-            cp_async_wait<0>();
-        }
-        __syncthreads();
-        if (kt == 0) {
-#pragma unroll
-            for (int kk = 0; kk < 4; kk++)
-                ldsm_x4(smem_u32(sQ) + tile_off(warp * 16 + (lane & 15), 2 * kk + (lane >> 4)), qf[kk][0], qf[kk][1], qf[kk][2], qf[kk][3]);
-        }
-        // S = Q K^T : 16 x 64 per warp
-        float s[8][4];
-#pragma unroll
-        for (int i = 0; i < 8; i++) { s[i][0] = s[i][1] = s[i][2] = s[i][3] = 0.f; }
-        const uint32_t kb = smem_u32(sK[buf]);
-#pragma unroll
-        for (int kk = 0; kk < 4; kk++) {
-#pragma unroll
-            for (int np = 0; np < 4; np++) {            // pairs of 8-key tiles
-                uint32_t b0, b1, b2, b3;
-                // matrices: [keys 16np..+7, d 16kk..+7], [same keys, d +8], [keys +8, d], [keys +8, d +8]
-                const int row = np * 16 + (lane & 7) + ((lane >> 4) << 3);
-                const int chunk = 2 * kk + ((lane >> 3) & 1);
-                ldsm_x4(kb + tile_off(row, chunk), b0, b1, b2, b3);
-                mma_bf16(s[2 * np], qf[kk], b0, b1);
-                mma_bf16(s[2 * np + 1], qf[kk], b2, b3);
-            }
-        }
-        // mask keys past the end of the sequence (last tile only)
-        const int kbase = kt * kKT;
-        if (kbase + kKT > n) {
-#pragma unroll
-            for (int i = 0; i < 8; i++) {
-                const int c = kbase + i * 8 + 2 * t;
-                if (c >= n) { s[i][0] = -INFINITY; s[i][2] = -INFINITY; }
-                if (c + 1 >= n) { s[i][1] = -INFINITY; s[i][3] = -INFINITY; }
-            }
-        }
-        // online softmax for rows g (h=0) and g+8 (h=1)
-#pragma unroll
-        for (int h = 0; h < 2; h++) {
-            float mx = -INFINITY;
-#pragma unroll
-            for (int i = 0; i < 8; i++) mx = fmaxf(mx, fmaxf(s[i][2 * h], s[i][2 * h + 1]));
-            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
-            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
-            const float m_new = fmaxf(m_run[h], mx);
-            const float corr = exp2f((m_run[h] - m_new) * sl2);
-            m_run[h] = m_new;
-            float sum = 0.f;
-#pragma unroll
-            for (int i = 0; i < 8; i++) {
-                const float p0 = exp2f((s[i][2 * h] - m_new) * sl2), p1 = exp2f((s[i][2 * h + 1] - m_new) * sl2);
-                s[i][2 * h] = p0; s[i][2 * h + 1] = p1;
-                sum += p0 + p1;
-            }
-            l_run[h] = l_run[h] * corr + sum;
-#pragma unroll
-            for (int i = 0; i < 8; i++) { o[i][2 * h] *= corr; o[i][2 * h + 1] *= corr; }
-        }
-        // O += P V
-        const uint32_t vb = smem_u32(sV[buf]);
-#pragma unroll
-        for (int kk = 0; kk < 4; kk++) {               // 16 keys per step
-            uint32_t pa[4];
-            pa[0] = pack2(s[2 * kk][0], s[2 * kk][1]);
-            pa[1] = pack2(s[2 * kk][2], s[2 * kk][3]);
-            pa[2] = pack2(s[2 * kk + 1][0], s[2 * kk + 1][1]);
-            pa[3] = pack2(s[2 * kk + 1][2], s[2 * kk + 1][3]);
-#pragma unroll
-            for (int dp = 0; dp < 4; dp++) {           // pairs of 8-wide d tiles
-                uint32_t b0, b1, b2, b3;
-                // transposed loads: matrices [keys 16kk..+7, d 16dp..+7], [keys +8, d], [keys, d +8], [keys +8, d +8]
-                const int row = kk * 16 + (lane & 7) + (((lane >> 3) & 1) << 3);
-                const int chunk = 2 * dp + (lane >> 4);
-                ldsm_x4_t(vb + tile_off(row, chunk), b0, b1, b2, b3);
-                mma_bf16(o[2 * dp], pa, b0, b1);
-                mma_bf16(o[2 * dp + 1], pa, b2, b3);
-            }
-        }
-        __syncthreads();
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tensormap(&tmap_q);
+        ptx::prefetch_tensormap(&tmap_kv);
     }
-    // normalise and store
-#pragma unroll
-    for (int h = 0; h < 2; h++) {
-        float l = l_run[h];
-        l += __shfl_xor_sync(0xffffffffu, l, 1);
-        l += __shfl_xor_sync(0xffffffffu, l, 2);
-        const float inv = 1.0f / l;
-        const int r = warp * 16 + g + 8 * h;
-        if (r < w.q_valid) {
-            __nv_bfloat16* dst = ctx + (size_t)(w.q_row0 + r) * H + head * kD;
-#pragma unroll
-            for (int i = 0; i < 8; i++)
-                *reinterpret_cast<uint32_t*>(dst + i * 8 + 2 * t) = pack2(o[i][2 * h] * inv, o[i][2 * h + 1] * inv);
+    if (warp == 1 && lane == 0) {
+        for (uint32_t i = 0; i < 2; i++) {
+            ptx::mbar_init(q_full(i), 1); ptx::mbar_init(q_empty(i), 1);
+            ptx::mbar_init(s_full(i), 1); ptx::mbar_init(p_full(i), 4); ptx::mbar_init(pv_done(i), 1);
+            ptx::mbar_init(o_full(i), 1); ptx::mbar_init(o_empty(i), 4);
         }
+        for (uint32_t i = 0; i < kKVStages; i++) { ptx::mbar_init(kv_full(i), 1); ptx::mbar_init(kv_empty(i), 1); }
+        ptx::fence_barrier_init();
+        ptx::fence_proxy_async();
+    }
+    if (warp == 2) {
+        ptx::tmem_alloc(tmem_slot, kAttTmemCols);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+    const uint32_t tmem_o = tmem_base + 128u;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            uint32_t qi = 0, g = 0;
+            for (int u = blockIdx.x; u < n_units; u += gridDim.x, qi++) {
+                const WorkItem w = work[u / heads];
+                const int head = u % heads;
+                const uint32_t qb = qi & 1u;
+                ptx::mbar_wait(q_empty(qb), ((qi >> 1) & 1u) ^ 1u);
+                ptx::mbar_arrive_expect_tx(q_full(qb), kQBytes);
+                ptx::tma_load_2d(q_smem + qb * kQBytes, &tmap_q, q_full(qb), head * kD, w.q_row0);
+                const int nc = (w.n + kKC - 1) / kKC;
+                for (int c = 0; c < nc; c++, g++) {
+                    const uint32_t st = g % kKVStages;
+                    ptx::mbar_wait(kv_empty(st), ((g / kKVStages) & 1u) ^ 1u);
+                    ptx::mbar_arrive_expect_tx(kv_full(st), 2 * kKVBytes);
+                    const uint32_t dst = kv_smem + st * 2 * kKVBytes;
+                    ptx::tma_load_2d(dst, &tmap_kv, kv_full(st), H + head * kD, w.kv_row0 + c * kKC);
+                    ptx::tma_load_2d(dst + kKVBytes, &tmap_kv, kv_full(st), 2 * H + head * kD, w.kv_row0 + c * kKC);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer: two cursors over the flattened (unit, chunk) sequence, QK^T one chunk ahead of PV =====
+        if (lane == 0) {
+            constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(kQT, kKC);          // both operands K-major
+            constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(kQT, kD, 1);        // B = V is MN-major
+            struct Cur { int u, c, nc; uint32_t qi, g; };
+            auto load = [&](Cur& k) { k.c = 0; k.nc = k.u < n_units ? (work[k.u / heads].n + kKC - 1) / kKC : 0; };
+            auto advance = [&](Cur& k) { k.g++; if (++k.c == k.nc) { k.u += gridDim.x; k.qi++; load(k); } };
+            Cur a{(int)blockIdx.x, 0, 0, 0u, 0u}, b = a;
+            load(a); load(b);
+            auto issue_qk = [&]() {
+                const uint32_t qb = a.qi & 1u, st = a.g % kKVStages, sb = a.g & 1u;
+                if (a.c == 0) ptx::mbar_wait(q_full(qb), (a.qi >> 1) & 1u);
+                ptx::mbar_wait(kv_full(st), (a.g / kKVStages) & 1u);
+                ptx::tc_fence_after();
+                const uint64_t qd = ptx::make_desc_k_sw128(q_smem + qb * kQBytes);
+                const uint64_t kd = ptx::make_desc_k_sw128(kv_smem + st * 2 * kKVBytes);
+#pragma unroll
+                for (int k = 0; k < kD / 16; k++)
+                    ptx::mma_f16_ss(tmem_base + sb * 64u, qd + (uint64_t)(2 * k), kd + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
+                ptx::mma_commit(s_full(sb));
+                if (a.c == a.nc - 1) ptx::mma_commit(q_empty(qb));       // last use of this Q tile
+            };
+            auto issue_pv = [&]() {
+                const uint32_t st = b.g % kKVStages, sb = b.g & 1u, ob = b.qi & 1u;
+                ptx::mbar_wait(p_full(sb), (b.g >> 1) & 1u);
+                if (b.c == 0) ptx::mbar_wait(o_empty(ob), ((b.qi >> 1) & 1u) ^ 1u);
+                ptx::tc_fence_after();
+                const uint64_t vd = ptx::make_desc_mn_sw128(kv_smem + st * 2 * kKVBytes + kKVBytes);
+#pragma unroll
+                for (int k = 0; k < kKC / 16; k++)                       // 16 keys per MMA: 8 TMEM columns of P, 2 KB of V
+                    ptx::mma_f16_ts(tmem_o + ob * 64u, tmem_base + sb * 64u + 8u * k, vd + (uint64_t)(128 * k), idesc_pv,
+                                    (b.c | k) ? 1u : 0u);
+                ptx::mma_commit(kv_empty(st));
+                ptx::mma_commit(pv_done(sb));
+                if (b.c == b.nc - 1) ptx::mma_commit(o_full(ob));
+            };
+            if (a.nc) { issue_qk(); advance(a); }
+            while (b.nc) {
+                if (a.nc) { issue_qk(); advance(a); }
+                issue_pv();
+                advance(b);
+            }
+        }
+    } else {
+        // ===== softmax warps: thread = query row =====
+        const uint32_t quarter = (uint32_t)(warp & 3);
+        const uint32_t lane_base = (quarter * 32u) << 16;
+        const int row = (int)quarter * 32 + lane;
+        const float sc = 0.125f * 1.4426950408889634f;                   // 1/sqrt(64) * log2(e)
+        uint32_t qi = 0, g = 0;
+        for (int u = blockIdx.x; u < n_units; u += gridDim.x, qi++) {
+            const WorkItem w = work[u / heads];
+            const int head = u % heads;
+            const int nc = (w.n + kKC - 1) / kKC;
+            float m = -INFINITY, l = 0.f;                                // reference max (scaled, log2 domain), row sum
+            for (int c = 0; c < nc; c++, g++) {
+                const uint32_t sb = g & 1u;
+                const uint32_t t_s = tmem_base + lane_base + sb * 64u;
+                ptx::mbar_wait(s_full(sb), (g >> 1) & 1u);
+                ptx::tc_fence_after();
+                uint32_t r[64];
+                ptx::tmem_ld_32x32b_x32(t_s, r);
+                ptx::tmem_ld_32x32b_x32(t_s + 32u, r + 32);
+                ptx::tmem_ld_wait();
+                const int valid = w.n - c * kKC;                         // keys of this chunk that belong to the sequence
+                if (valid < kKC) {
+#pragma unroll
+                    for (int j = 0; j < kKC; j++) if (j >= valid) r[j] = 0xff800000u;      // -inf
+                }
+                float cm = max3(__uint_as_float(r[0]), __uint_as_float(r[1]), __uint_as_float(r[2]));
+#pragma unroll
+                for (int j = 3; j + 1 < kKC; j += 2) cm = max3(cm, __uint_as_float(r[j]), __uint_as_float(r[j + 1]));
+                cm = fmaxf(cm, __uint_as_float(r[kKC - 1]));
+                const float mnew = cm * sc;
+                if (__any_sync(0xffffffffu, mnew > m + 8.0f)) {          // raise the reference (first chunk: m = -inf)
+                    float alpha = 1.0f;
+                    if (mnew > m) { alpha = ex2f(m - mnew); m = mnew; l *= alpha; }
+                    if (c > 0) {                                         // rescale O in TMEM once PV(g-1) has landed
+                        const uint32_t t_o = tmem_o + lane_base + (qi & 1u) * 64u;
+                        ptx::mbar_wait(pv_done((g - 1u) & 1u), ((g - 1u) >> 1) & 1u);
+                        ptx::tc_fence_after();
+#pragma unroll
+                        for (int hh = 0; hh < 2; hh++) {
+                            uint32_t o[32];
+                            ptx::tmem_ld_32x32b_x32(t_o + 32u * hh, o);
+                            ptx::tmem_ld_wait();
+#pragma unroll
+                            for (int j = 0; j < 32; j++) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
+                            ptx::tmem_st_32x32b_x32(t_o + 32u * hh, o);
+                        }
+                        ptx::tmem_st_wait();
+                    }
+                }
+                uint32_t pk[32];
+                float s0 = 0.f, s1 = 0.f;
+                const float nm = -m;
+#pragma unroll
+                for (int j = 0; j < 32; j++) {
+                    const float p0 = ex2f(fmaf(__uint_as_float(r[2 * j]), sc, nm));
+                    const float p1 = ex2f(fmaf(__uint_as_float(r[2 * j + 1]), sc, nm));
+                    s0 += p0; s1 += p1;
+                    pk[j] = pack2(p0, p1);
+                }
+                l += s0 + s1;
+                ptx::tmem_st_32x32b_x32(t_s, pk);                        // P over the first 32 columns of the S buffer
+                ptx::tmem_st_wait();
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(p_full(sb));
+            }
+            // ---- final: O / l -> BF16 row ----
+            const uint32_t ob = qi & 1u;
+            ptx::mbar_wait(o_full(ob), (qi >> 1) & 1u);
+            ptx::tc_fence_after();
+            uint32_t o[64];
+            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + ob * 64u, o);
+            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + ob * 64u + 32u, o + 32);
+            ptx::tmem_ld_wait();
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(o_empty(ob));
+            if (row < w.q_valid) {
+                const float inv = 1.0f / l;
+                uint4* dst = reinterpret_cast<uint4*>(ctx + (size_t)(w.q_row0 + row) * H + head * kD);
+#pragma unroll
+                for (int v = 0; v < 8; v++)
+                    dst[v] = make_uint4(pack2(__uint_as_float(o[8 * v]) * inv, __uint_as_float(o[8 * v + 1]) * inv),
+                                        pack2(__uint_as_float(o[8 * v + 2]) * inv, __uint_as_float(o[8 * v + 3]) * inv),
+                                        pack2(__uint_as_float(o[8 * v + 4]) * inv, __uint_as_float(o[8 * v + 5]) * inv),
+                                        pack2(__uint_as_float(o[8 * v + 6]) * inv, __uint_as_float(o[8 * v + 7]) * inv));
+            }
+        }
+    }
+
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc(tmem_base, kAttTmemCols);
     }
 }
 
@@ -193,12 +267,13 @@ __global__ void __launch_bounds__(128) attention_bf16_kernel(const __nv_bfloat16
 int attention_plan(anon_ctx* ctx, WsCursor& ws, const int32_t* h_cu, int B, int dtype, AttnPlan* plan)
 {
     // h_cu points at this chunk's first sequence boundary; rows are relative to token h_cu[0]
-    plan->d_work = nullptr; plan->n_items = 0;
+    plan->d_work = nullptr; plan->n_items = 0; plan->n_rows = 0;
     if (!ctx || !h_cu || B < 0) return ANON_ERR_INVALID_ARG;
     for (int s = 0; s < B; s++)
         if (h_cu[s + 1] < h_cu[s] || h_cu[s + 1] - h_cu[s] > 512) return ANON_ERR_UNSUPPORTED;
     if (dtype == 0 || B == 0) return ANON_OK;
     const int tok0 = h_cu[0];
+    plan->n_rows = h_cu[B] - tok0;
     std::vector<WorkItem> items;
     items.reserve((size_t)(h_cu[B] - tok0) / kQT + B);
     for (int s = 0; s < B; s++) {
@@ -229,9 +304,22 @@ int attention_run(anon_ctx* ctx, const AttnPlan& plan, const void* d_qkv, const 
         return ANON_OK;
     }
     if (plan.n_items == 0) return ANON_OK;
-    attention_bf16_kernel<<<dim3((unsigned)plan.n_items, heads), 128, 0, ctx->stream>>>(
-        (const __nv_bfloat16*)d_qkv, (const WorkItem*)plan.d_work, hidden, (__nv_bfloat16*)d_ctx);
-    CU_LAUNCH_CHECK(ctx, "attention_bf16_kernel");
+    // rows of the packed qkv tensor this launch may touch: up to the end of the chunk (plan.n_rows)
+    CUtensorMap tq, tkv;
+    int rc = make_tmap_2d(ctx, &tq, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, d_qkv, (uint64_t)plan.n_rows, (uint64_t)3 * hidden, kD, kQT);
+    if (rc) return rc;
+    rc = make_tmap_2d(ctx, &tkv, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, d_qkv, (uint64_t)plan.n_rows, (uint64_t)3 * hidden, kD, kKC);
+    if (rc) return rc;
+    static bool attr_set = false;
+    if (!attr_set) {
+        CU_TRY(ctx, cudaFuncSetAttribute(attention_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kAttSmem));
+        attr_set = true;
+    }
+    const long long units = (long long)plan.n_items * heads;
+    const int grid = (int)std::min<long long>(units, 2LL * ctx->sm_count);
+    attention_tcgen05_kernel<<<grid, kAttThreads, kAttSmem, ctx->stream>>>(tq, tkv, (const WorkItem*)plan.d_work, (int)units,
+                                                                            heads, hidden, (__nv_bfloat16*)d_ctx);
+    CU_LAUNCH_CHECK(ctx, "attention_tcgen05_kernel");
     return ANON_OK;
 }
 

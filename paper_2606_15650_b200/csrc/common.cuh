@@ -1,6 +1,7 @@
 // common.cuh -- context, error plumbing and workspace cursor shared by the translation units of
 // libanonshield.so (product code; shares nothing with oracle/).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
 #include <stdint.h>
@@ -101,7 +102,11 @@ int pseudonymize_impl(anon_ctx*, WsCursor&, anon_cache*, const uint8_t* d_bytes,
                       int64_t* total_out_bytes);
 int gemm_bf16_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias,
                    const float* residual, void* C, int M, int N, int K, int epilogue);
-struct AttnPlan { void* d_work; int n_items; };
+// 2-D row-major tensor [rows, cols] of esize-byte elements, box [box_rows, box_cols] with box_cols * esize = 128 B,
+// 128-byte swizzle (gemm_tcgen05.cu).
+int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_t esize, const void* base, uint64_t rows,
+                 uint64_t cols, uint32_t box_cols, uint32_t box_rows);
+struct AttnPlan { void* d_work; int n_items; int n_rows; };
 int attention_plan(anon_ctx*, WsCursor&, const int32_t* h_cu, int B, int dtype, AttnPlan* plan);
 int attention_run(anon_ctx*, const AttnPlan&, const void* d_qkv, const int32_t* d_cu, int tok0, int B, int hidden,
                   int heads, int dtype, void* d_ctx);

@@ -42,6 +42,14 @@ __device__ __forceinline__ float ex2f(float x) { float y; asm("ex2.approx.ftz.f3
 __device__ __forceinline__ float max3(float a, float b, float c) {
     float d; asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c)); return d;
 }
+__device__ __forceinline__ uint64_t pk2(float a, float b) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void upk2(uint64_t v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+    uint64_t d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
 __device__ __forceinline__ uint32_t pack2(float a, float b) {
     __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
     return *reinterpret_cast<uint32_t*>(&v);
@@ -102,13 +110,13 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 const WorkItem w = work[u / heads];
                 const int head = u % heads;
                 const uint32_t qb = qi & 1u;
-                ptx::mbar_wait(q_empty(qb), ((qi >> 1) & 1u) ^ 1u);
+                ptx::mbar_wait_backoff(q_empty(qb), ((qi >> 1) & 1u) ^ 1u);
                 ptx::mbar_arrive_expect_tx(q_full(qb), kQBytes);
                 ptx::tma_load_2d(q_smem + qb * kQBytes, &tmap_q, q_full(qb), head * kD, w.q_row0);
                 const int nc = (w.n + kKC - 1) / kKC;
                 for (int c = 0; c < nc; c++, g++) {
                     const uint32_t st = g % kKVStages;
-                    ptx::mbar_wait(kv_empty(st), ((g / kKVStages) & 1u) ^ 1u);
+                    ptx::mbar_wait_backoff(kv_empty(st), ((g / kKVStages) & 1u) ^ 1u);
                     ptx::mbar_arrive_expect_tx(kv_full(st), 2 * kKVBytes);
                     const uint32_t dst = kv_smem + st * 2 * kKVBytes;
                     ptx::tma_load_2d(dst, &tmap_kv, kv_full(st), H + head * kD, w.kv_row0 + c * kKC);
@@ -167,6 +175,32 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
         const int row = (int)quarter * 32 + lane;
         const float sc = 0.125f * 1.4426950408889634f;                   // 1/sqrt(64) * log2(e)
         uint32_t qi = 0, g = 0;
+        bool pend = false;
+        uint32_t pend_ob = 0, pend_par = 0;
+        float pend_l = 1.f;
+        int pend_row0 = 0, pend_valid = 0, pend_head = 0;
+        auto finalize = [&]() {                                          // O / l -> BF16 row of ctx
+            ptx::mbar_wait(o_full(pend_ob), pend_par);
+            ptx::tc_fence_after();
+            uint32_t o[64];
+            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + pend_ob * 64u, o);
+            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + pend_ob * 64u + 32u, o + 32);
+            ptx::tmem_ld_wait();
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(o_empty(pend_ob));
+            if (row < pend_valid) {
+                const float inv = 1.0f / pend_l;
+                uint4* dst = reinterpret_cast<uint4*>(ctx + (size_t)(pend_row0 + row) * H + pend_head * kD);
+#pragma unroll
+                for (int v = 0; v < 8; v++)
+                    dst[v] = make_uint4(pack2(__uint_as_float(o[8 * v]) * inv, __uint_as_float(o[8 * v + 1]) * inv),
+                                        pack2(__uint_as_float(o[8 * v + 2]) * inv, __uint_as_float(o[8 * v + 3]) * inv),
+                                        pack2(__uint_as_float(o[8 * v + 4]) * inv, __uint_as_float(o[8 * v + 5]) * inv),
+                                        pack2(__uint_as_float(o[8 * v + 6]) * inv, __uint_as_float(o[8 * v + 7]) * inv));
+            }
+            pend = false;
+        };
         for (int u = blockIdx.x; u < n_units; u += gridDim.x, qi++) {
             const WorkItem w = work[u / heads];
             const int head = u % heads;
@@ -177,6 +211,13 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 const uint32_t t_s = tmem_base + lane_base + sb * 64u;
                 ptx::mbar_wait(s_full(sb), (g >> 1) & 1u);
                 ptx::tc_fence_after();
+                if ((int)quarter * 32 >= w.q_valid) {                    // no query of this warp is real: P rows are don't-care
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(p_full(sb));
+                    if (c == 0 && pend) finalize();
+                    continue;
+                }
                 uint32_t r[64];
                 ptx::tmem_ld_32x32b_x32(t_s, r);
                 ptx::tmem_ld_32x32b_x32(t_s + 32u, r + 32);
@@ -186,10 +227,16 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
 #pragma unroll
                     for (int j = 0; j < kKC; j++) if (j >= valid) r[j] = 0xff800000u;      // -inf
                 }
-                float cm = max3(__uint_as_float(r[0]), __uint_as_float(r[1]), __uint_as_float(r[2]));
+                float cmx[4];                                            // four independent chains, then a tree
 #pragma unroll
-                for (int j = 3; j + 1 < kKC; j += 2) cm = max3(cm, __uint_as_float(r[j]), __uint_as_float(r[j + 1]));
-                cm = fmaxf(cm, __uint_as_float(r[kKC - 1]));
+                for (int q4 = 0; q4 < 4; q4++) {
+                    cmx[q4] = max3(__uint_as_float(r[16 * q4]), __uint_as_float(r[16 * q4 + 1]), __uint_as_float(r[16 * q4 + 2]));
+#pragma unroll
+                    for (int j = 3; j + 1 < 16; j += 2)
+                        cmx[q4] = max3(cmx[q4], __uint_as_float(r[16 * q4 + j]), __uint_as_float(r[16 * q4 + j + 1]));
+                    cmx[q4] = fmaxf(cmx[q4], __uint_as_float(r[16 * q4 + 15]));
+                }
+                const float cm = fmaxf(max3(cmx[0], cmx[1], cmx[2]), cmx[3]);
                 const float mnew = cm * sc;
                 if (__any_sync(0xffffffffu, mnew > m + 8.0f)) {          // raise the reference (first chunk: m = -inf)
                     float alpha = 1.0f;
@@ -211,44 +258,42 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     }
                 }
                 uint32_t pk[32];
-                float s0 = 0.f, s1 = 0.f;
-                const float nm = -m;
+                uint64_t sum_a = pk2(0.f, 0.f), sum_b = sum_a;           // packed FP32x2 partial row sums
+                const uint64_t sc2 = pk2(sc, sc), nm2 = pk2(-m, -m);
 #pragma unroll
-                for (int j = 0; j < 32; j++) {
-                    const float p0 = ex2f(fmaf(__uint_as_float(r[2 * j]), sc, nm));
-                    const float p1 = ex2f(fmaf(__uint_as_float(r[2 * j + 1]), sc, nm));
-                    s0 += p0; s1 += p1;
-                    pk[j] = pack2(p0, p1);
+                for (int hh = 0; hh < 2; hh++) {
+                    if (hh == 1 && valid <= 32) {                        // second half of a short last chunk: all masked
+#pragma unroll
+                        for (int j = 16; j < 32; j++) pk[j] = 0u;
+                        break;
+                    }
+#pragma unroll
+                    for (int j = 16 * hh; j < 16 * hh + 16; j++) {
+                        float t0, t1;
+                        upk2(fma2(pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])), sc2, nm2), t0, t1);
+                        const float p0 = ex2f(t0), p1 = ex2f(t1);
+                        if (j & 1) sum_b = add2(sum_b, pk2(p0, p1)); else sum_a = add2(sum_a, pk2(p0, p1));
+                        pk[j] = pack2(p0, p1);
+                    }
                 }
-                l += s0 + s1;
+                {
+                    float s0, s1;
+                    upk2(add2(sum_a, sum_b), s0, s1);
+                    l += s0 + s1;
+                }
                 ptx::tmem_st_32x32b_x32(t_s, pk);                        // P over the first 32 columns of the S buffer
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(p_full(sb));
+                if (c == 0 && pend) finalize();
             }
-            // ---- final: O / l -> BF16 row ----
-            const uint32_t ob = qi & 1u;
-            ptx::mbar_wait(o_full(ob), (qi >> 1) & 1u);
-            ptx::tc_fence_after();
-            uint32_t o[64];
-            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + ob * 64u, o);
-            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + ob * 64u + 32u, o + 32);
-            ptx::tmem_ld_wait();
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(o_empty(ob));
-            if (row < w.q_valid) {
-                const float inv = 1.0f / l;
-                uint4* dst = reinterpret_cast<uint4*>(ctx + (size_t)(w.q_row0 + row) * H + head * kD);
-#pragma unroll
-                for (int v = 0; v < 8; v++)
-                    dst[v] = make_uint4(pack2(__uint_as_float(o[8 * v]) * inv, __uint_as_float(o[8 * v + 1]) * inv),
-                                        pack2(__uint_as_float(o[8 * v + 2]) * inv, __uint_as_float(o[8 * v + 3]) * inv),
-                                        pack2(__uint_as_float(o[8 * v + 4]) * inv, __uint_as_float(o[8 * v + 5]) * inv),
-                                        pack2(__uint_as_float(o[8 * v + 6]) * inv, __uint_as_float(o[8 * v + 7]) * inv));
-            }
+            // the O / l write-back of this unit is deferred until after the first chunk of the next one, so that the
+            // wait for the last PV overlaps useful work
+            pend = true; pend_ob = qi & 1u; pend_par = (qi >> 1) & 1u; pend_l = l;
+            pend_row0 = w.q_row0; pend_valid = w.q_valid; pend_head = head;
         }
+        if (pend) finalize();
     }
 
     ptx::tc_fence_before();

@@ -153,7 +153,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
                 const int m_blk = tile / num_n, n_blk = tile % num_n;
                 for (int kb = 0; kb < num_kb; kb++) {
-                    ptx::mbar_wait(empty_bar(s), ph ^ 1u);
+                    ptx::mbar_wait_backoff(empty_bar(s), ph ^ 1u);
                     ptx::mbar_arrive_expect_tx(full_bar(s), C::STAGE_BYTES);
                     const uint32_t sa = smem_base + s * C::STAGE_BYTES;
                     ptx::tma_load_2d(sa, &tmap_a, full_bar(s), kb * BK, m_blk * BM);
@@ -168,11 +168,11 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             int s = 0; uint32_t ph = 0;
             int acc = 0; uint32_t acc_ph = 0;
             for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-                ptx::mbar_wait(tempty_bar(acc), acc_ph ^ 1u);
+                ptx::mbar_wait_backoff(tempty_bar(acc), acc_ph ^ 1u);
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
                 for (int kb = 0; kb < num_kb; kb++) {
-                    ptx::mbar_wait(full_bar(s), ph);
+                    ptx::mbar_wait_backoff(full_bar(s), ph);
                     ptx::tc_fence_after();
                     const uint32_t sa = smem_base + s * C::STAGE_BYTES;
                     const uint64_t adesc = ptx::make_desc_k_sw128(sa);

@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the AnonShield hot path (A1-A13) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload base|large|pseudonym] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload base|large|stream|pseudonym] [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of seeded synthetic input: anon_ner_forward ->
 anon_decode_spans -> anon_gather_spans -> anon_pseudonymize (cache cleared first, so every step inserts and
@@ -150,10 +150,16 @@ def run_reference(args):
         return
     if args.workload == "pseudonym":
         return run_reference_pseudonym(args)
-    desc, rec, win, wseed, label = encoder_workload(args.workload, 0, n_records=64)
+    if args.workload == "stream":
+        desc, wseed = gen.DESCS["base"], gen.SEED_BASE + 2
+        rec = gen.workload_stream(n_records=64, seed=gen.SEED_BASE + 3, n_pool=20000)
+        win = gen.window_records(rec)
+        label = "BASELINE.json configs[2]: synthetic record stream, 510+2-token windows (first 64 records generated)"
+    else:
+        desc, rec, win, wseed, label = encoder_workload(args.workload, 0, n_records=64)
     w = gen.make_weights(desc, wseed, planted=PLANTED)
     names = gen.TYPE_NAMES_6
-    n = seqs_for_tokens(win["cu_seqlens"], 600 if args.workload == "base" else 250)
+    n = seqs_for_tokens(win["cu_seqlens"], 250 if args.workload == "large" else 600)
     tot_t = tot_s = 0
     times = []
     for i in range(args.warmup + args.steps):
@@ -163,12 +169,17 @@ def run_reference(args):
     sec = sum(times)
     v = tot_t / sec
     sample = "first %d sequences (%d tokens) of the workload per step" % (n, int(win["cu_seqlens"][n]))
-    out = {"impl": "reference", "metric": "ner_tokens_per_s", "value": v, "unit": "tokens/s", "n_gpus": args.gpus,
+    metric, unit = "ner_tokens_per_s", "tokens/s"
+    if args.workload == "stream":     # records/s = tokens/s over the stream's window-tokens per record
+        v = v * (len(rec["rec_off"]) - 1) / float(win["cu_seqlens"][-1])
+        metric, unit = "records_per_s", "records/s"
+        sample += "; tokens/s scaled by the sample's window-tokens per record"
+    out = {"impl": "reference", "metric": metric, "value": v, "unit": unit, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": label, "sample": sample},
-           "cpu_baseline": {"value": v, "unit": "tokens/s", "cores": blas_threads(), "kind": "oracle", "sample": sample},
-           "e2e": {"value": v, "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "cpu_baseline": {"value": v, "unit": unit, "cores": blas_threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": v, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "spans_per_s": tot_s / sec}
     print(json.dumps(out), flush=True)
 
@@ -368,6 +379,167 @@ def run_encoder(args):
     print(json.dumps(out), flush=True)
 
 
+def run_stream(args):
+    """BASELINE.json configs[2]: the full synthetic record stream (70,951 records, ~550 MB) in token-budgeted
+    batches of whole records; the entity cache persists across batches.  A "step" is one batch (~1 M tokens);
+    the timed region is ALL batches of the stream, after 3 warm-up batches run on a scratch cache."""
+    import torch
+    import paper_2606_15650_b200 as P
+    from paper_2606_15650_b200 import sharding, stream
+    world, rank, local = dist_setup(args)
+    dev = torch.device("cuda", local)
+    peaks = measured_peaks()
+    t_setup = time.time()
+    desc = gen.DESCS["base"]
+    n_records = args.records or 70951
+    rec = gen.workload_stream(n_records=n_records, seed=gen.SEED_BASE + 3 + 1000 * rank,
+                              n_pool=300000 if n_records >= 20000 else 20000)
+    log(f"[rank {rank}] records generated in {time.time() - t_setup:.0f}s: {rec['text'].size / 2**20:.1f} MiB, "
+        f"{int(rec['tok_rec_off'][-1])} content tokens, {rec['n_entities']} planted entities")
+    win = gen.window_records(rec)
+    names = gen.TYPE_NAMES_6
+    w = gen.make_weights(desc, gen.SEED_BASE + 2, planted=PLANTED)
+    plan = stream.plan_batches(win["win_rec"], win["cu_seqlens"], args.batch_tokens)
+    batches = [stream.slice_batch(rec, win, a, b) for a, b in plan]
+    T_all = int(win["cu_seqlens"][-1])
+    maxT = max(b["token_ids"].size for b in batches)
+    maxB = max(b["cu_seqlens"].size - 1 for b in batches)
+    max_text = max(b["text"].size for b in batches)
+    cap = maxT // 4 + 4096
+    out_cap = cap * 32
+    ws = P.anon_workspace_bytes(desc, maxT, maxB) + 96 * maxT + 2 * max_text + out_cap + 40 * cap + (128 << 20)
+    ctx = P.Context(local, workspace_bytes=ws)
+    W = P.Weights(ctx, desc, gen.pack_blob(w))
+    log(f"[rank {rank}] setup {time.time() - t_setup:.0f}s: {len(batches)} batches, {T_all} window-tokens, "
+        f"{len(win['cu_seqlens']) - 1} windows, max batch {maxT} tokens, ws={ws / 2**30:.1f} GiB")
+
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    dbat = [dict(ids=d(b["token_ids"]), cu=d(b["cu_seqlens"]), meta=d(b["meta"]), text=d(b["text"]), ro=d(b["rec_off"]))
+            for b in batches]
+    labels = torch.zeros(maxT, dtype=torch.int32, device=dev)
+    spans = torch.zeros((cap, 4), dtype=torch.int32, device=dev)
+    nsp = torch.zeros(1, dtype=torch.int32, device=dev)
+    span_bytes = torch.zeros(max_text + 16, dtype=torch.uint8, device=dev)
+    span_off = torch.zeros(cap + 1, dtype=torch.int64, device=dev)
+    span_type = torch.zeros(cap, dtype=torch.uint8, device=dev)
+    out_tokens = torch.zeros(out_cap, dtype=torch.uint8, device=dev)
+    out_off = torch.zeros(cap + 1, dtype=torch.int64, device=dev)
+    hit = torch.zeros(cap, dtype=torch.uint8, device=dev)
+    nsp_host = torch.zeros(1, dtype=torch.int32).pin_memory()
+
+    def step(cache, k):
+        b = dbat[k]
+        T = b["ids"].numel()
+        P.anon_ner_forward(ctx, W, b["ids"], b["cu"], None, labels[:T])
+        P.anon_decode_spans(ctx, labels[:T], b["meta"], desc["num_labels"], spans, nsp)
+        nsp_host.copy_(nsp, non_blocking=True)
+        rc = ctx.sync()
+        if rc:
+            raise RuntimeError(f"device status {rc}")
+        S = int(nsp_host[0])
+        P.anon_gather_spans(ctx, b["text"], b["ro"], spans, S, span_bytes, span_off, span_type)
+        P.anon_pseudonymize(ctx, cache, span_bytes, span_off[:S + 1], span_type, KEY, SLUG_LEN, names, out_tokens,
+                            out_off[:S + 1], hit)
+        return S
+
+    scratch = P.Cache(ctx, 1 << 20, 64 << 20)
+    for k in range(min(3, len(batches))):
+        step(scratch, k)
+    assert ctx.sync() == 0
+    scratch.close()
+    cache = P.Cache(ctx, 1 << 20, 64 << 20)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier(world)
+    sampler = ClockSampler(gpu_id_for_smi(local)) if rank == 0 else None
+    ctx.profile(True)
+    ev0.record()
+    S_all = 0
+    for k in range(len(batches)):
+        S_all += step(cache, k)
+    ev1.record()
+    barrier(world)
+    prof, launches = ctx.profile_read()
+    ctx.profile(False)
+    clocks = sampler.stop() if sampler else None
+    sec_local = ev0.elapsed_time(ev1) / 1e3
+    st = cache.stats()
+    cache.close()
+    recs_all, sec = sharding.aggregate_throughput(n_records, sec_local, dev)
+    tokens_all, _ = sharding.aggregate_throughput(T_all, sec_local, dev)
+    spans_all, _ = sharding.aggregate_throughput(S_all, sec_local, dev)
+    del dbat
+
+    # ---- e2e: every batch through anon_pipeline_host from pinned HOST buffers, fresh cache ----
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    hbat = [dict(ids=pin(b["token_ids"]), cu=pin(b["cu_seqlens"]), meta=pin(b["meta"]), text=pin(b["text"]),
+                 ro=pin(b["rec_off"])) for b in batches]
+    bufs = dict(spans=torch.zeros((cap, 4), dtype=torch.int32).pin_memory().numpy(),
+                out=torch.zeros(out_cap, dtype=torch.uint8).pin_memory().numpy(),
+                off=torch.zeros(cap + 1, dtype=torch.int64).pin_memory().numpy(),
+                hit=torch.zeros(cap, dtype=torch.uint8).pin_memory().numpy())
+    cache2 = P.Cache(ctx, 1 << 20, 64 << 20)
+    barrier(world)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    h2d = d2h = 0
+    hits = 0
+    e0.record()
+    for hb in hbat:
+        res = P.anon_pipeline_host(ctx, W, cache2, hb["ids"], hb["cu"], hb["meta"], hb["text"], hb["ro"], KEY, SLUG_LEN,
+                                   names, cap, out_cap, want_hit=True, bufs=bufs)
+        Sh = len(res["spans"])
+        hits += int(res["hit"].sum())
+        h2d += hb["ids"].nbytes + hb["cu"].nbytes + hb["meta"].nbytes + hb["text"].nbytes + hb["ro"].nbytes
+        d2h += Sh * 16 + int(res["out_tokens"].size) + (Sh + 1) * 8 + Sh + 8
+    e1.record()
+    barrier(world)
+    e2e_recs, e2e_sec = sharding.aggregate_throughput(n_records, e0.elapsed_time(e1) / 1e3, dev)
+    st2 = cache2.stats()
+    if rank != 0:
+        return
+    nb = len(batches)
+    g_ms, g_fl, g_n = prof["gemm"]
+    peak = peaks["bf16_tflops_sustained"]
+    achieved = g_fl / (g_ms * 1e-3) / 1e12 if g_ms > 0 else 0.0
+    a_ms, a_fl, _ = prof["attention"]
+    r_ms, r_by, _ = prof["row"]
+    out = {
+        "metric": "records_per_s", "value": recs_all / sec, "unit": "records/s", "n_gpus": world,
+        "steps": nb, "warmup": min(3, nb), "ms_per_step": 1e3 * sec / nb, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[2]: %d synthetic records, %.1f MiB of text, %d windows (510+2, overlap 128), "
+                               "%d window-tokens, Zipf(1.1) entities; batches of whole records, <= %d tokens"
+                               % (n_records, rec["text"].size / 2**20, len(win["cu_seqlens"]) - 1, T_all, args.batch_tokens),
+                   "batches": nb, "weights": "W2 planted-detector, seeded random-init", "slug_len": SLUG_LEN,
+                   "spans": S_all, "planted_entities": int(rec["n_entities"]), "unique_entities": st["n_unique"],
+                   "cache_hit_rate": st["n_hits"] / max(st["n_lookups"], 1),
+                   "l2": "inputs larger than L2 (each batch streams ~20 GB of activations through HBM)"},
+        "seconds_whole_stream": sec, "tokens_per_s": tokens_all / sec, "spans_per_s": spans_all / sec,
+        "kb_per_s": rec["text"].size / 1024.0 * world / sec,
+        "clocks": clocks, "gpu_launches": launches,
+        "e2e": {"value": e2e_recs / e2e_sec, "unit": "records/s", "h2d_bytes_per_step": int(h2d // nb),
+                "d2h_bytes_per_step": int(d2h // nb), "steps": nb, "seconds_whole_stream": e2e_sec,
+                "tokens_per_s": T_all * world / e2e_sec, "kb_per_s": rec["text"].size / 1024.0 * world / e2e_sec,
+                "cache_hit_rate": st2["n_hits"] / max(st2["n_lookups"], 1)},
+        "roofline": {"bound": "tensor", "kernel": "gemm_bf16_tcgen05_kernel (QKV, out, FFN1, FFN2)",
+                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                     "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (%s)" % peaks["source"],
+                     "frac_of_burst_peak": achieved / peaks["bf16_tflops"], "frac_of_nominal_2250": achieved / 2250.0,
+                     "launches": g_n, "avg_launch_ms": g_ms / max(g_n, 1), "flops_per_launch": g_fl / max(g_n, 1),
+                     "traffic": None},
+        "breakdown_ms_per_step": {k: v[0] / nb for k, v in prof.items()},
+        "attention_tflops": a_fl / (a_ms * 1e-3) / 1e12 if a_ms > 0 else None,
+        "row_kernels_gbs": r_by / (r_ms * 1e-3) / 1e9 if r_ms > 0 else None,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        n = seqs_for_tokens(win["cu_seqlens"], 4000)
+        Tc, Sc, dt = oracle_sample_pass(w, desc, rec, win, n, names)
+        out["cpu_baseline"] = {"value": n_records * (Tc / dt) / T_all, "unit": "records/s", "cores": blas_threads(),
+                               "kind": "oracle",
+                               "sample": "first %d windows (%d tokens, %d spans) of the stream in %.1f s = %.0f tokens/s, "
+                                         "scaled by tokens per record" % (n, Tc, Sc, dt, Tc / dt)}
+    print(json.dumps(out), flush=True)
+
+
 def run_pseudonym(args):
     """BASELINE.json configs[4]: 50 M spans Zipf(1.1) over 2 M strings -> dedup + HMAC + write-back."""
     import torch
@@ -438,9 +610,10 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="base", choices=["base", "large", "pseudonym"])
+    ap.add_argument("--workload", default="base", choices=["base", "large", "stream", "pseudonym"])
     ap.add_argument("--records", type=int, default=None, help="override the number of records / sequences / strings")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch-tokens", type=int, default=1 << 20, help="stream workload: token budget per batch")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         log("note: timing rules ask for >= 3 warm-up steps")
@@ -448,6 +621,8 @@ def main():
         return run_reference(args)
     if args.workload == "pseudonym":
         return run_pseudonym(args)
+    if args.workload == "stream":
+        return run_stream(args)
     return run_encoder(args)
 
 

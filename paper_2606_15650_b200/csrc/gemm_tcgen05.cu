@@ -1,20 +1,24 @@
 // gemm_tcgen05.cu -- K2: C[M,N] = A[M,K] * W[N,K]^T (+bias, +GELU | +residual) for the encoder's dense
 // projections (S8a A2, A4, A5, A6; BJ "tcgen05/TMEM tensor-core GEMMs fed by TMA").
 //
-// sm_100a design: persistent CTAs (one per SM), warp-specialised:
-//   warp 0   TMA producer : cp.async.bulk.tensor 2-D tiles (128B swizzle) of A [128 x 64] and W [BN x 64]
-//                           into a STAGES-deep shared-memory ring, completion on mbarriers
-//   warp 1   MMA issuer   : one thread issues tcgen05.mma (M=128, N=BN, K=16, BF16 -> FP32) with shared-memory
-//                           matrix descriptors; accumulators live in TMEM, double-buffered (2 x BN columns) so
-//                           the epilogue of tile i overlaps the mainloop of tile i+1; tcgen05.commit frees
-//                           ring slots / publishes accumulators
+// sm_100a design: persistent CTA PAIRS (tcgen05 cta_group::2, one CTA per SM, clusters of 2): a pair computes a
+// 256 x 256 tile, each CTA holding 128 accumulator rows in its TMEM and staging its 128 rows of A and only HALF of
+// the B tile (the tensor cores of both SMs read both halves), which halves the shared-memory fill and operand
+// traffic that capped the single-CTA version at ~70 % tensor-pipe activity.  Warp-specialised:
+//   warp 0   TMA producer : (both CTAs) cp.async.bulk.tensor 2-D tiles (128B swizzle) of A [128 x 64] and W [128 x 64]
+//                           into a 5-6 stage shared-memory ring; all bytes are counted on the LEADER's mbarrier
+//   warp 1   MMA issuer   : one thread of the leader CTA issues tcgen05.mma.cta_group::2 (M=256, N=256, K=16,
+//                           BF16 -> FP32) with shared-memory matrix descriptors; accumulators live in TMEM,
+//                           double-buffered (2 x 256 columns) so the epilogue of tile i overlaps the mainloop of
+//                           tile i+1; tcgen05.commit (multicast to both CTAs) frees ring slots / publishes accumulators
 //   warp 2   TMEM allocator
-//   warps 4-7 epilogue    : tcgen05.ld (32 lanes x 32 columns per warp) -> bias / GELU / residual in registers
+//   warps 4-11 epilogue   : (both CTAs, two warps per TMEM lane quarter; 4 warps for the residual epilogue) tcgen05.ld (32 lanes x 32 columns per warp) -> bias / GELU / residual in registers
 //                           -> 128B-swizzled shared-memory boxes (one row per thread, conflict-free) -> TMA store
 //                           (coalesced, asynchronous, M/N tails clipped by the tensor map).  The FP32 residual
 //                           tile arrives the same way: each epilogue warp TMA-loads its own 32x32 boxes three
 //                           boxes ahead (also across tiles, so they land during the next mainloop), adds in
 //                           place and stores from the same buffer.
+// Outputs with N <= 128 use the single-CTA variant (CG = 1, 128 x 128 tiles).
 // Operands are "TN": A row-major [M,K], W row-major [N,K] (both K-contiguous = K-major UMMA operands).
 #include "common.cuh"
 #include "ptx_sm100.cuh"
@@ -29,8 +33,10 @@ constexpr int A_STAGE_BYTES = BM * BK * 2;
 
 // NB = FP32 residual boxes in flight per epilogue warp (EPI 2 only): 4 for short K (the epilogue's HBM traffic
 // paces the kernel), 2 for long K (a fourth mainloop stage is worth more).
-template <int BN, int EPI, int NB> struct Cfg {
-    static constexpr int B_STAGE_BYTES = BN * BK * 2;
+// CG = CTAs per MMA (tcgen05 cta_group): 1 = 128 x BN tile per CTA; 2 = a CTA pair computes 256 x BN, each CTA owning
+// 128 rows of the accumulator and staging only half of the B tile (halves shared-memory fill and operand traffic).
+template <int BN, int EPI, int NB, int CG> struct Cfg {
+    static constexpr int B_STAGE_BYTES = (BN / CG) * BK * 2;
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
     static constexpr int EPI_WARPS = (EPI == 2) ? 4 : 8;
     static constexpr int EPI_BYTES = (EPI == 2) ? 4 * NB * 4096 : 8 * 4096;   // 4 KB boxes
@@ -101,13 +107,13 @@ __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
 }
 
 // EPI: 0 = +bias -> BF16;  1 = +bias, GELU -> BF16;  2 = +bias +residual(FP32) -> FP32
-template <int BN, int EPI, int NB>
+template <int BN, int EPI, int NB, int CG>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                          const __grid_constant__ CUtensorMap tmap_c, const __grid_constant__ CUtensorMap tmap_r,
                          const float* __restrict__ bias, int M, int N, int K)
 {
-    using C = Cfg<BN, EPI, NB>;
+    using C = Cfg<BN, EPI, NB, CG>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t epi_base = smem_base + C::STAGES * C::STAGE_BYTES;
@@ -121,7 +127,10 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int num_m = (M + BM - 1) / BM, num_n = (N + BN - 1) / BN;
+    const int rank = CG == 2 ? (int)ptx::cluster_ctarank() : 0;          // position in the CTA pair; 0 issues the MMAs
+    const int cid = (int)blockIdx.x / CG, ncl = (int)gridDim.x / CG;     // tile scheduler works on pairs
+    constexpr int TM = BM * CG;                                         // rows per tile
+    const int num_m = (M + TM - 1) / TM, num_n = (N + BN - 1) / BN;
     const int num_tiles = num_m * num_n;
     const int num_kb = K / BK;
 
@@ -133,46 +142,58 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < C::STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
-        for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), C::EPI_WARPS); }
+        for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), CG * C::EPI_WARPS); }
         for (int i = 0; i < 16; i++) ptx::mbar_init(rfull_bar(i >> 2, i & 3), 1);
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
     }
     if (warp == 2) {
-        ptx::tmem_alloc(tmem_slot, C::TMEM_COLS);
-        ptx::tmem_relinquish();
+        if (CG == 2) { ptx::tmem_alloc_cg2(tmem_slot, C::TMEM_COLS); ptx::tmem_relinquish_cg2(); }
+        else { ptx::tmem_alloc(tmem_slot, C::TMEM_COLS); ptx::tmem_relinquish(); }
     }
     ptx::tc_fence_before();
-    __syncthreads();
+    if (CG == 2) ptx::cluster_sync(); else __syncthreads();            // the peer's barriers must be initialised too
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
     if (warp == 0) {
+        // ===== TMA producer (one per CTA): A rows [rank*128, +128) of the tile, B rows [rank*BN/CG, +BN/CG) =====
         if (lane == 0) {
             int s = 0; uint32_t ph = 0;
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            for (int tile = cid; tile < num_tiles; tile += ncl) {
                 const int m_blk = tile / num_n, n_blk = tile % num_n;
                 for (int kb = 0; kb < num_kb; kb++) {
                     ptx::mbar_wait_backoff(empty_bar(s), ph ^ 1u);
-                    ptx::mbar_arrive_expect_tx(full_bar(s), C::STAGE_BYTES);
                     const uint32_t sa = smem_base + s * C::STAGE_BYTES;
-                    ptx::tma_load_2d(sa, &tmap_a, full_bar(s), kb * BK, m_blk * BM);
-                    ptx::tma_load_2d(sa + A_STAGE_BYTES, &tmap_b, full_bar(s), kb * BK, n_blk * BN);
+                    if (CG == 1) {
+                        ptx::mbar_arrive_expect_tx(full_bar(s), C::STAGE_BYTES);
+                        ptx::tma_load_2d(sa, &tmap_a, full_bar(s), kb * BK, m_blk * BM);
+                        ptx::tma_load_2d(sa + A_STAGE_BYTES, &tmap_b, full_bar(s), kb * BK, n_blk * BN);
+                    } else {
+                        // both CTAs' bytes are counted on the LEADER's barrier (it alone waits before issuing the MMA); only
+                        // the leader arrives.  The peer cannot run a phase ahead: its empty barrier of this stage fires
+                        // after the MMAs that the leader issued on the previous phase of the same full barrier.
+                        const uint32_t lead_full = ptx::mapa(full_bar(s), 0);
+                        if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(s), 2 * C::STAGE_BYTES);
+                        ptx::tma_load_2d_cg2(sa, &tmap_a, lead_full, kb * BK, m_blk * TM + rank * BM);
+                        ptx::tma_load_2d_cg2(sa + A_STAGE_BYTES, &tmap_b, lead_full, kb * BK, n_blk * BN + rank * (BN / CG));
+                    }
                     if (++s == C::STAGES) { s = 0; ph ^= 1u; }
                 }
             }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
-            constexpr uint32_t idesc = ptx::make_idesc_bf16(BM, BN);
+        // ===== MMA issuer: one thread of the leader CTA =====
+        if (lane == 0 && rank == 0) {
+            constexpr uint32_t idesc = ptx::make_idesc_bf16(TM, BN);
             int s = 0; uint32_t ph = 0;
             int acc = 0; uint32_t acc_ph = 0;
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-                ptx::mbar_wait_backoff(tempty_bar(acc), acc_ph ^ 1u);
+            for (int tile = cid; tile < num_tiles; tile += ncl) {
+                ptx::mbar_wait(tempty_bar(acc), acc_ph ^ 1u);
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
                 for (int kb = 0; kb < num_kb; kb++) {
-                    ptx::mbar_wait_backoff(full_bar(s), ph);
+                    ptx::mbar_wait(full_bar(s), ph);
                     ptx::tc_fence_after();
                     const uint32_t sa = smem_base + s * C::STAGE_BYTES;
                     const uint64_t adesc = ptx::make_desc_k_sw128(sa);
@@ -180,13 +201,13 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
 #pragma unroll
                     for (int k = 0; k < BK / UMMA_K; k++) {
                         // +32 bytes along K inside the 128-byte swizzle row = +2 in the (addr >> 4) field
-                        ptx::mma_f16_ss(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc,
-                                        (kb | k) ? 1u : 0u);
+                        if (CG == 2) ptx::mma_f16_ss_cg2(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) ? 1u : 0u);
+                        else ptx::mma_f16_ss(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) ? 1u : 0u);
                     }
-                    ptx::mma_commit(empty_bar(s));
+                    if (CG == 2) ptx::mma_commit_cg2(empty_bar(s)); else ptx::mma_commit(empty_bar(s));
                     if (++s == C::STAGES) { s = 0; ph ^= 1u; }
                 }
-                ptx::mma_commit(tfull_bar(acc));
+                if (CG == 2) ptx::mma_commit_cg2(tfull_bar(acc)); else ptx::mma_commit(tfull_bar(acc));
                 if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
             }
         }
@@ -194,6 +215,9 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         const int q = warp & 3;                       // TMEM lane quarter this warp may access
         const uint32_t row_off = (uint32_t)lane * 128u;      // this thread's row inside a 32-row box
         const uint32_t sw = (uint32_t)(lane & 7);            // 128B swizzle: 16-byte chunk index ^= row & 7
+        auto arrive_tempty = [&](int a) {               // the accumulator is handed back to the LEADER's MMA thread
+            if (CG == 2) ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(a), 0)); else ptx::mbar_arrive(tempty_bar(a));
+        };
         int acc = 0; uint32_t acc_ph = 0;
         uint32_t nbox = 0;                            // boxes this warp has handled (buffer ring position)
         (void)nbox;
@@ -203,18 +227,18 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             const uint32_t stg = epi_base + (uint32_t)(q * NB * 4096);
             uint32_t rph = 0;                         // phase bit of each residual buffer's barrier
             auto issue_load = [&](uint32_t i) {       // lane 0: residual box i -> buffer i % NB
-                const int tile = blockIdx.x + (int)(i / BPT) * (int)gridDim.x;
+                const int tile = cid + (int)(i / BPT) * ncl;
                 if (tile >= num_tiles) return;
-                const int row0 = (tile / num_n) * BM + q * 32, col = (tile % num_n) * BN + (int)(i % BPT) * 32;
+                const int row0 = (tile / num_n) * TM + rank * BM + q * 32, col = (tile % num_n) * BN + (int)(i % BPT) * 32;
                 if (row0 >= M || col >= N) return;
                 const uint32_t bar = rfull_bar(q, i % NB);
                 ptx::mbar_arrive_expect_tx(bar, 4096);
                 ptx::tma_load_2d(stg + (i % NB) * 4096u, &tmap_r, bar, col, row0);
             };
             if (lane == 0) { for (uint32_t i = 0; i + 1 < NB; i++) issue_load(i); }
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            for (int tile = cid; tile < num_tiles; tile += ncl) {
                 const int m_blk = tile / num_n, n_blk = tile % num_n;
-                const int row0 = m_blk * BM + q * 32;
+                const int row0 = m_blk * TM + rank * BM + q * 32;
                 ptx::mbar_wait(tfull_bar(acc), acc_ph);
                 ptx::tc_fence_after();
                 const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
@@ -229,7 +253,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                     if (j == BPT - 1) {               // accumulator fully read: hand it back to the MMA warp
                         ptx::tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+                        if (lane == 0) arrive_tempty(acc);
                     }
                     const bool valid = row0 < M && col < N;      // warp-uniform
                     if (valid) {
@@ -263,9 +287,9 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             // two warps per TMEM lane quarter, each owning half of the tile's columns and one 4 KB staging box
             const int half = (warp - 4) >> 2;
             const uint32_t buf = epi_base + (uint32_t)((warp - 4) * 4096);
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            for (int tile = cid; tile < num_tiles; tile += ncl) {
                 const int m_blk = tile / num_n, n_blk = tile % num_n;
-                const int row0 = m_blk * BM + q * 32;
+                const int row0 = m_blk * TM + rank * BM + q * 32;
                 ptx::mbar_wait(tfull_bar(acc), acc_ph);
                 ptx::tc_fence_after();
                 const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
@@ -279,7 +303,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                     if (c0 + 64 == (half + 1) * (BN / 2)) {       // this warp's share of the accumulator is read
                         ptx::tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+                        if (lane == 0) arrive_tempty(acc);
                     }
                     if (row0 < M && col < N) {                     // warp-uniform
                         uint32_t o[32];
@@ -316,10 +340,10 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     }
 
     ptx::tc_fence_before();
-    __syncthreads();
+    if (CG == 2) ptx::cluster_sync(); else __syncthreads();            // no CTA of a pair leaves while its peer may still signal it
     if (warp == 2) {
         ptx::tc_fence_after();
-        ptx::tmem_dealloc(tmem_base, C::TMEM_COLS);
+        if (CG == 2) ptx::tmem_dealloc_cg2(tmem_base, C::TMEM_COLS); else ptx::tmem_dealloc(tmem_base, C::TMEM_COLS);
     }
 }
 
@@ -357,15 +381,15 @@ int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_
 
 namespace {
 
-template <int BN, int EPI, int NB>
+template <int BN, int EPI, int NB, int CG>
 int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
                 void* Cout, int M, int N, int K)
 {
-    using C = Cfg<BN, EPI, NB>;
+    using C = Cfg<BN, EPI, NB, CG>;
     CUtensorMap ta, tb, tc, tr;
     int rc = make_tmap_2d(ctx, &ta, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, A, (uint64_t)M, (uint64_t)K, BK, BM);
     if (rc) return rc;
-    rc = make_tmap_2d(ctx, &tb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, W, (uint64_t)N, (uint64_t)K, BK, BN);
+    rc = make_tmap_2d(ctx, &tb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, W, (uint64_t)N, (uint64_t)K, BK, BN / CG);
     if (rc) return rc;
     if (EPI == 2) {
         rc = make_tmap_2d(ctx, &tc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Cout, (uint64_t)M, (uint64_t)N, 32, 32);
@@ -377,15 +401,22 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
         if (rc) return rc;
         tr = tc;
     }
-    auto kern = gemm_bf16_tcgen05_kernel<BN, EPI, NB>;
+    auto kern = gemm_bf16_tcgen05_kernel<BN, EPI, NB, CG>;
     static bool attr_set = false;
     if (!attr_set) {
         CU_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
         attr_set = true;
     }
-    const int tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
-    const int grid = tiles < ctx->sm_count ? tiles : ctx->sm_count;
-    kern<<<grid, kThreads, C::SMEM_BYTES, ctx->stream>>>(ta, tb, tc, tr, bias, M, N, K);
+    const int tiles = ((M + BM * CG - 1) / (BM * CG)) * ((N + BN - 1) / BN);
+    const int slots = ctx->sm_count / CG;
+    const int grid = CG * (tiles < slots ? tiles : slots);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, bias, M, N, K));
     CU_LAUNCH_CHECK(ctx, "gemm_bf16_tcgen05_kernel");
     return ANON_OK;
 }
@@ -401,18 +432,18 @@ int gemm_bf16_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W
     if (K % BK != 0 || N % 8 != 0) return ANON_ERR_UNSUPPORTED;
     if (M == 0) return ANON_OK;
     const bool long_k = K >= 2048;
-    if (N > 128) {
+    if (N > 128) {                 // CTA pairs: 256 x 256 tiles
         switch (epilogue) {
-            case 0: return launch_gemm<256, 0, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
-            case 1: return launch_gemm<256, 1, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
-            default: return long_k ? launch_gemm<256, 2, 2>(ctx, A, W, bias, residual, Cout, M, N, K)
-                                   : launch_gemm<256, 2, 4>(ctx, A, W, bias, residual, Cout, M, N, K);
+            case 0: return launch_gemm<256, 0, 2, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
+            case 1: return launch_gemm<256, 1, 2, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
+            default: return long_k ? launch_gemm<256, 2, 2, 2>(ctx, A, W, bias, residual, Cout, M, N, K)
+                                   : launch_gemm<256, 2, 4, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
         }
     }
-    switch (epilogue) {
-        case 0: return launch_gemm<128, 0, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
-        case 1: return launch_gemm<128, 1, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
-        default: return launch_gemm<128, 2, 4>(ctx, A, W, bias, residual, Cout, M, N, K);
+    switch (epilogue) {            // narrow outputs: single-CTA 128 x 128 tiles
+        case 0: return launch_gemm<128, 0, 2, 1>(ctx, A, W, bias, residual, Cout, M, N, K);
+        case 1: return launch_gemm<128, 1, 2, 1>(ctx, A, W, bias, residual, Cout, M, N, K);
+        default: return launch_gemm<128, 2, 4, 1>(ctx, A, W, bias, residual, Cout, M, N, K);
     }
 }
 

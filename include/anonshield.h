@@ -206,6 +206,14 @@ int  anon_pipeline_host(anon_ctx* ctx, const anon_weights* w, anon_cache* cache,
  * d_A, d_W BF16 (uint16 bit patterns) row-major, 16-byte aligned.  Asynchronous. */
 int  anon_gemm_bf16(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,
                     const float* d_residual, void* d_C, int32_t M, int32_t N, int32_t K, int32_t epilogue);
+/* The residual GEMMs of the encoder with the LayerNorm fused into the epilogue (S8a A4, A6; S8c O1):
+ *   x[M,N] = LN(A[M,K] * W[N,K]^T + bias + residual; gamma, beta)   (biased variance, eps inside the sqrt)
+ * written as FP32 to d_x (which MAY alias d_residual: every row is read completely before it is written) and as
+ * BF16 to d_xb.  N % 256 == 0 and K % 64 == 0 required (else ANON_ERR_UNSUPPORTED).  Uses a context-owned scratch
+ * (allocated on first use).  Asynchronous. */
+int  anon_gemm_bf16_ln(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,
+                       const float* d_residual, const float* d_gamma, const float* d_beta, float eps,
+                       float* d_x, void* d_xb, int32_t M, int32_t N, int32_t K);
 /* ctx[T,H] = varlen bidirectional softmax attention over qkv[T,3H] (S8a A3); dtype as in
  * anon_model_desc (0: FP32 qkv/ctx, 1: BF16).  h_cu_seqlens is a HOST pointer.  Asynchronous. */
 int  anon_attention(anon_ctx* ctx, const void* d_qkv, const int32_t* d_cu_seqlens,

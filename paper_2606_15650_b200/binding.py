@@ -64,6 +64,7 @@ _SIGNATURES = {
     "anon_ctx_profile": (ctypes.c_int, [_vp, ctypes.c_int]),
     "anon_ctx_profile_read": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "anon_gemm_bf16": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32]),
+    "anon_gemm_bf16_ln": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp, _vp, _i32, _i32, _i32]),
     "anon_attention": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32, _i32, _vp]),
 }
 
@@ -253,6 +254,13 @@ def anon_gemm_bf16(ctx, A, W, bias, residual, C, epilogue):
     N = W.shape[0]
     ctx.check(lib().anon_gemm_bf16(ctx._h, _ptr(A), _ptr(W), _ptr(bias), _ptr(residual), _ptr(C), M, N, K, epilogue),
               "anon_gemm_bf16")
+
+
+def anon_gemm_bf16_ln(ctx, A, W, bias, residual, gamma, beta, eps, x, xb):
+    M, K = A.shape
+    N = W.shape[0]
+    ctx.check(lib().anon_gemm_bf16_ln(ctx._h, _ptr(A), _ptr(W), _ptr(bias), _ptr(residual), _ptr(gamma), _ptr(beta), eps,
+                                      _ptr(x), _ptr(xb), M, N, K), "anon_gemm_bf16_ln")
 
 
 def anon_attention(ctx, qkv, cu_seqlens_dev, cu_seqlens_host, hidden, heads, dtype, out):

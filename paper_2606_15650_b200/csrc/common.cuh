@@ -29,6 +29,9 @@ struct anon_ctx {
     // cached driver entry point for cuTensorMapEncodeTiled (resolved lazily, see gemm_tcgen05.cu)
     void* encode_tiled = nullptr;
     int smem_optin = 0;
+    // L2-resident scratch of the fused residual+LayerNorm GEMM epilogue (allocated on first use, grows only)
+    void* ln_scratch = nullptr;
+    size_t ln_scratch_bytes = 0;
     // launch accounting + optional event profiling
     long long n_launches = 0;
     bool prof_on = false;
@@ -102,6 +105,9 @@ int pseudonymize_impl(anon_ctx*, WsCursor&, anon_cache*, const uint8_t* d_bytes,
                       int64_t* total_out_bytes);
 int gemm_bf16_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias,
                    const float* residual, void* C, int M, int N, int K, int epilogue);
+// x = LN(A W^T + bias + residual; gamma, beta) as FP32 (x_out may alias residual) plus its BF16 copy; N % 256 == 0
+int gemm_bf16_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
+                      const float* gamma, const float* beta, float eps, float* x_out, __nv_bfloat16* xb_out, int M, int N, int K);
 // 2-D row-major tensor [rows, cols] of esize-byte elements, box [box_rows, box_cols] with box_cols * esize = 128 B,
 // 128-byte swizzle (gemm_tcgen05.cu).
 int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_t esize, const void* base, uint64_t rows,

@@ -38,8 +38,9 @@ constexpr int A_STAGE_BYTES = BM * BK * 2;
 template <int BN, int EPI, int NB, int CG> struct Cfg {
     static constexpr int B_STAGE_BYTES = (BN / CG) * BK * 2;
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
-    static constexpr int EPI_WARPS = (EPI == 2) ? 4 : 8;
-    static constexpr int EPI_BYTES = (EPI == 2) ? 4 * NB * 4096 : 8 * 4096;   // 4 KB boxes
+    static constexpr int EPI_WARPS = (EPI >= 2) ? 4 : 8;
+    static constexpr int PAR_BYTES = 3 * 1024 * 4;                // EPI 3: bias, gamma, beta staged in shared memory (N <= 1024)
+    static constexpr int EPI_BYTES = (EPI == 3) ? 4 * (NB + 1) * 4096 + PAR_BYTES : (EPI == 2) ? 4 * NB * 4096 : 8 * 4096;   // 4 KB boxes
     static constexpr int STAGES = (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES > 6 ? 6 : (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES;
     static constexpr int TMEM_COLS = 2 * BN;                      // two accumulator buffers
     static constexpr int NUM_BARS = 2 * STAGES + 4 + 16;
@@ -100,18 +101,27 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
+__device__ __forceinline__ void ld_shared_2x2(uint32_t addr, uint64_t& lo, uint64_t& hi) {      // 4 floats as two FP32x2 pairs
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(lo), "=l"(hi) : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void st_shared_2x2(uint32_t addr, uint64_t lo, uint64_t hi) {
+    asm volatile("st.shared.v2.b64 [%0], {%1, %2};" ::"r"(addr), "l"(lo), "l"(hi) : "memory");
+}
 __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
     float4 v;
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
     return v;
 }
 
-// EPI: 0 = +bias -> BF16;  1 = +bias, GELU -> BF16;  2 = +bias +residual(FP32) -> FP32
+// EPI: 0 = +bias -> BF16;  1 = +bias, GELU -> BF16;  2 = +bias +residual(FP32) -> FP32;
+//      3 = LayerNorm(+bias +residual) -> FP32 x and BF16 xb (whole rows per CTA pair, see the EPI 3 branch)
 template <int BN, int EPI, int NB, int CG>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                          const __grid_constant__ CUtensorMap tmap_c, const __grid_constant__ CUtensorMap tmap_r,
-                         const float* __restrict__ bias, int M, int N, int K)
+                         const __grid_constant__ CUtensorMap tmap_y, const __grid_constant__ CUtensorMap tmap_xb,
+                         const float* __restrict__ bias, const float* __restrict__ ln_g, const float* __restrict__ ln_b,
+                         float ln_eps, int M, int N, int K)
 {
     using C = Cfg<BN, EPI, NB, CG>;
     extern __shared__ uint8_t smem_raw[];
@@ -133,12 +143,21 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     const int num_m = (M + TM - 1) / TM, num_n = (N + BN - 1) / BN;
     const int num_tiles = num_m * num_n;
     const int num_kb = K / BK;
+    // local tile lt of this CTA (pair) -> (m_blk, n_blk).  EPI 3 walks all n-tiles of one row block before the next row
+    // block (the LayerNorm needs whole rows); the other epilogues take tiles round-robin.
+    auto get_tile = [&](int lt, int& m_blk, int& n_blk) -> bool {
+        if (EPI == 3) { m_blk = cid + (lt / num_n) * ncl; n_blk = lt % num_n; return m_blk < num_m; }
+        const int tile = cid + lt * ncl;
+        m_blk = tile / num_n; n_blk = tile % num_n;
+        return tile < num_tiles;
+    };
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&tmap_a);
         ptx::prefetch_tensormap(&tmap_b);
         ptx::prefetch_tensormap(&tmap_c);
-        if (EPI == 2) ptx::prefetch_tensormap(&tmap_r);
+        if (EPI >= 2) ptx::prefetch_tensormap(&tmap_r);
+        if (EPI == 3) { ptx::prefetch_tensormap(&tmap_y); ptx::prefetch_tensormap(&tmap_xb); }
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < C::STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
@@ -146,6 +165,10 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         for (int i = 0; i < 16; i++) ptx::mbar_init(rfull_bar(i >> 2, i & 3), 1);
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
+    }
+    if constexpr (EPI == 3) {             // bias / gamma / beta -> shared memory (every thread reads all N of them per row)
+        float* par = reinterpret_cast<float*>(smem_raw + (epi_base + 4 * (NB + 1) * 4096 - ptx::smem_u32(smem_raw)));
+        for (int i = threadIdx.x; i < N; i += kThreads) { par[i] = bias[i]; par[1024 + i] = ln_g[i]; par[2048 + i] = ln_b[i]; }
     }
     if (warp == 2) {
         if (CG == 2) { ptx::tmem_alloc_cg2(tmem_slot, C::TMEM_COLS); ptx::tmem_relinquish_cg2(); }
@@ -160,8 +183,8 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         // ===== TMA producer (one per CTA): A rows [rank*128, +128) of the tile, B rows [rank*BN/CG, +BN/CG) =====
         if (lane == 0) {
             int s = 0; uint32_t ph = 0;
-            for (int tile = cid; tile < num_tiles; tile += ncl) {
-                const int m_blk = tile / num_n, n_blk = tile % num_n;
+            int m_blk, n_blk;
+            for (int lt = 0; get_tile(lt, m_blk, n_blk); lt++) {
                 for (int kb = 0; kb < num_kb; kb++) {
                     ptx::mbar_wait_backoff(empty_bar(s), ph ^ 1u);
                     const uint32_t sa = smem_base + s * C::STAGE_BYTES;
@@ -188,7 +211,8 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             constexpr uint32_t idesc = ptx::make_idesc_bf16(TM, BN);
             int s = 0; uint32_t ph = 0;
             int acc = 0; uint32_t acc_ph = 0;
-            for (int tile = cid; tile < num_tiles; tile += ncl) {
+            int m_blk, n_blk;
+            for (int lt = 0; get_tile(lt, m_blk, n_blk); lt++) {
                 ptx::mbar_wait(tempty_bar(acc), acc_ph ^ 1u);
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
@@ -222,7 +246,158 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         uint32_t nbox = 0;                            // boxes this warp has handled (buffer ring position)
         (void)nbox;
 
-        if constexpr (EPI == 2) {
+        if constexpr (EPI == 3) {
+            // ---- fused residual + LayerNorm: x = LN(acc + bias + residual), rows owned by one thread each ----
+            // Pass 1 (per n-tile, as EPI 2): v = acc + bias + residual computed in place in the TMA-loaded residual box,
+            //   stored to a per-pair scratch (L2-resident: the same 256 rows x N FP32 are rewritten for every row block),
+            //   while the thread merges each 32-value chunk into its row's running (count, mean, M2) -- Chan's
+            //   parallel update, numerically a two-pass variance.
+            // Pass 2 (after the last n-tile of the row block): the v boxes come back by TMA, are normalised with
+            //   gamma / beta in place and leave as the FP32 residual stream x plus its BF16 copy xb.
+            // Boxes of both passes run through one ring of NB 4 KB buffers per warp, loads issued NB-1 boxes ahead.
+            constexpr int BPT = BN / 32;
+            const int nbt = num_n * BPT;                  // v boxes per row block and warp
+            const uint32_t stg = epi_base + (uint32_t)(q * (NB + 1) * 4096);
+            const uint32_t xbuf = stg + NB * 4096u;       // one BF16 box (32 rows x 64 columns)
+            const uint32_t par = epi_base + 4u * (NB + 1) * 4096u;       // bias | gamma | beta, 1024 floats each
+            const int srow0 = cid * TM + rank * BM + q * 32;           // this warp's rows in the scratch
+            uint32_t rph = 0;
+            auto issue_load = [&](uint32_t i) {           // lane 0: box i of this warp's sequence -> buffer i % NB
+                const int rb = (int)(i / (2u * nbt)), b = (int)(i % (2u * nbt));
+                const int mb = cid + rb * ncl;
+                if (mb >= num_m) return;
+                const int row0 = mb * TM + rank * BM + q * 32;
+                if (row0 >= M) return;
+                const uint32_t bar = rfull_bar(q, i % NB);
+                ptx::mbar_arrive_expect_tx(bar, 4096);
+                if (b < nbt) {
+                    ptx::tma_load_2d(stg + (i % NB) * 4096u, &tmap_r, bar, b * 32, row0);
+                } else {
+                    // the store of this v box, nbt - NB + 1 groups ago, must have completed (not just been read)
+                    if (nbt >= 12) ptx::bulk_wait<8>(); else ptx::bulk_wait<2>();
+                    ptx::tma_load_2d(stg + (i % NB) * 4096u, &tmap_y, bar, (b - nbt) * 32, srow0);
+                }
+            };
+            if (lane == 0) { for (uint32_t i = 0; i + 1 < NB; i++) issue_load(i); }
+            int m_blk, n_blk;
+            float r_mean = 0.f, r_m2 = 0.f;
+            for (int lt = 0; get_tile(lt, m_blk, n_blk); lt++) {
+                const int row0 = m_blk * TM + rank * BM + q * 32;
+                const bool valid = row0 < M;              // warp-uniform
+                if (n_blk == 0) { r_mean = 0.f; r_m2 = 0.f; }
+                ptx::mbar_wait(tfull_bar(acc), acc_ph);
+                ptx::tc_fence_after();
+                const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
+#pragma unroll 1
+                for (int j = 0; j < BPT; j++, nbox++) {
+                    const int col = n_blk * BN + j * 32;
+                    const uint32_t b = nbox % NB;
+                    const uint32_t buf = stg + b * 4096u;
+                    uint32_t r[32];
+                    ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)(j * 32), r);
+                    ptx::tmem_ld_wait();
+                    if (j == BPT - 1) {
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) arrive_tempty(acc);
+                    }
+                    if (valid) {
+                        ptx::mbar_wait(rfull_bar(q, b), (rph >> b) & 1u);
+                        rph ^= 1u << b;
+                        uint64_t vv[16];                  // the 32 values of this row's chunk as FP32x2 pairs
+                        uint64_t cs0 = pk2(0.f, 0.f), cs1 = cs0;
+#pragma unroll
+                        for (int v = 0; v < 8; v++) {
+                            const uint32_t addr = buf + row_off + (((uint32_t)v ^ sw) << 4);
+                            uint64_t x0, x1, b0, b1;
+                            ld_shared_2x2(addr, x0, x1);
+                            ld_shared_2x2(par + (uint32_t)(col + 4 * v) * 4u, b0, b1);
+                            vv[2 * v] = add2(add2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), b0), x0);
+                            vv[2 * v + 1] = add2(add2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), b1), x1);
+                            st_shared_2x2(addr, vv[2 * v], vv[2 * v + 1]);
+                            cs0 = add2(cs0, vv[2 * v]); cs1 = add2(cs1, vv[2 * v + 1]);
+                        }
+                        ptx::fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) ptx::tma_store_2d(&tmap_y, buf, col, srow0);
+                        // merge this 32-value chunk into the row statistics (two-pass inside the chunk, Chan across chunks)
+                        float s0, s1;
+                        upk2(add2(cs0, cs1), s0, s1);
+                        const float cmean = (s0 + s1) * (1.0f / 32.0f);
+                        const uint64_t ncm = pk2(-cmean, -cmean);
+                        uint64_t q0 = pk2(0.f, 0.f), q1 = q0, q2 = q0, q3 = q0;
+#pragma unroll
+                        for (int u = 0; u < 16; u += 4) {
+                            const uint64_t d0 = add2(vv[u], ncm), d1 = add2(vv[u + 1], ncm), d2 = add2(vv[u + 2], ncm), d3 = add2(vv[u + 3], ncm);
+                            q0 = fma2(d0, d0, q0); q1 = fma2(d1, d1, q1); q2 = fma2(d2, d2, q2); q3 = fma2(d3, d3, q3);
+                        }
+                        upk2(add2(add2(q0, q1), add2(q2, q3)), s0, s1);
+                        const float cm2 = s0 + s1;
+                        const float kprev = (float)(n_blk * BPT + j);            // chunks merged so far
+                        const float w = 1.0f / (kprev + 1.0f);
+                        const float delta = cmean - r_mean;
+                        r_mean = fmaf(delta, w, r_mean);
+                        r_m2 += cm2 + delta * delta * (32.0f * kprev * w);
+                    }
+                    if (lane == 0) {
+                        ptx::bulk_commit();
+                        ptx::bulk_wait_read<1>();
+                        issue_load(nbox + NB - 1);
+                    }
+                    __syncwarp();
+                }
+                if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
+                if (n_blk != num_n - 1) continue;
+                // ---- pass 2 over the finished row block ----
+                const float rstd = rsqrtf(r_m2 / (float)N + ln_eps);
+                const uint64_t rstd2 = pk2(rstd, rstd), nmr2 = pk2(-r_mean * rstd, -r_mean * rstd);
+#pragma unroll 1
+                for (int p2 = 0; p2 < nbt; p2++, nbox++) {
+                    const int col = p2 * 32;
+                    const uint32_t b = nbox % NB;
+                    const uint32_t buf = stg + b * 4096u;
+                    if (valid) {
+                        ptx::mbar_wait(rfull_bar(q, b), (rph >> b) & 1u);
+                        rph ^= 1u << b;
+                        uint32_t pk[16];
+#pragma unroll
+                        for (int v = 0; v < 8; v++) {
+                            const uint32_t addr = buf + row_off + (((uint32_t)v ^ sw) << 4);
+                            uint64_t x0, x1, g0, g1, e0, e1;
+                            ld_shared_2x2(addr, x0, x1);
+                            ld_shared_2x2(par + (uint32_t)(1024 + col + 4 * v) * 4u, g0, g1);
+                            ld_shared_2x2(par + (uint32_t)(2048 + col + 4 * v) * 4u, e0, e1);
+                            // (x - mean) * rstd * gamma + beta = fma(fma(x, rstd, -mean * rstd), gamma, beta)
+                            const uint64_t o01 = fma2(fma2(x0, rstd2, nmr2), g0, e0), o23 = fma2(fma2(x1, rstd2, nmr2), g1, e1);
+                            st_shared_2x2(addr, o01, o23);
+                            float o0, o1, o2, o3;
+                            upk2(o01, o0, o1); upk2(o23, o2, o3);
+                            pk[2 * v] = pack_bf16(o0, o1); pk[2 * v + 1] = pack_bf16(o2, o3);
+                        }
+                        if (!(p2 & 1)) {                  // the BF16 box is refilled: its previous store must have read it
+                            if (lane == 0) ptx::bulk_wait_read<0>();
+                            __syncwarp();
+                        }
+#pragma unroll
+                        for (int c = 0; c < 4; c++)       // 16-byte chunks (p2 & 1) * 4 + c of the 64-column BF16 row
+                            st_shared_v4(xbuf + row_off + ((((uint32_t)((p2 & 1) * 4 + c)) ^ sw) << 4), pk[4 * c], pk[4 * c + 1],
+                                         pk[4 * c + 2], pk[4 * c + 3]);
+                        ptx::fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) {
+                            ptx::tma_store_2d(&tmap_c, buf, col, row0);
+                            if (p2 & 1) ptx::tma_store_2d(&tmap_xb, xbuf, col - 32, row0);
+                        }
+                    }
+                    if (lane == 0) {
+                        ptx::bulk_commit();
+                        ptx::bulk_wait_read<1>();
+                        issue_load(nbox + NB - 1);
+                    }
+                    __syncwarp();
+                }
+            }
+        } else if constexpr (EPI == 2) {
             constexpr int BPT = BN / 32;              // 32x32 FP32 boxes per tile per warp
             const uint32_t stg = epi_base + (uint32_t)(q * NB * 4096);
             uint32_t rph = 0;                         // phase bit of each residual buffer's barrier
@@ -236,8 +411,8 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                 ptx::tma_load_2d(stg + (i % NB) * 4096u, &tmap_r, bar, col, row0);
             };
             if (lane == 0) { for (uint32_t i = 0; i + 1 < NB; i++) issue_load(i); }
-            for (int tile = cid; tile < num_tiles; tile += ncl) {
-                const int m_blk = tile / num_n, n_blk = tile % num_n;
+            int m_blk, n_blk;
+            for (int lt = 0; get_tile(lt, m_blk, n_blk); lt++) {
                 const int row0 = m_blk * TM + rank * BM + q * 32;
                 ptx::mbar_wait(tfull_bar(acc), acc_ph);
                 ptx::tc_fence_after();
@@ -287,8 +462,8 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             // two warps per TMEM lane quarter, each owning half of the tile's columns and one 4 KB staging box
             const int half = (warp - 4) >> 2;
             const uint32_t buf = epi_base + (uint32_t)((warp - 4) * 4096);
-            for (int tile = cid; tile < num_tiles; tile += ncl) {
-                const int m_blk = tile / num_n, n_blk = tile % num_n;
+            int m_blk, n_blk;
+            for (int lt = 0; get_tile(lt, m_blk, n_blk); lt++) {
                 const int row0 = m_blk * TM + rank * BM + q * 32;
                 ptx::mbar_wait(tfull_bar(acc), acc_ph);
                 ptx::tc_fence_after();
@@ -381,17 +556,26 @@ int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_
 
 namespace {
 
+struct LnArgs { const float* gamma; const float* beta; float eps; void* xb_out; };
+
 template <int BN, int EPI, int NB, int CG>
 int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
-                void* Cout, int M, int N, int K)
+                void* Cout, int M, int N, int K, const LnArgs* ln = nullptr)
 {
     using C = Cfg<BN, EPI, NB, CG>;
-    CUtensorMap ta, tb, tc, tr;
+    const int tiles = ((M + BM * CG - 1) / (BM * CG)) * ((N + BN - 1) / BN);
+    const int slots = ctx->sm_count / CG;
+    int grid = CG * (tiles < slots ? tiles : slots);
+    if (EPI == 3) {                       // one pair per row block
+        const int row_blocks = (M + BM * CG - 1) / (BM * CG);
+        grid = CG * (row_blocks < slots ? row_blocks : slots);
+    }
+    CUtensorMap ta, tb, tc, tr, ty, txb;
     int rc = make_tmap_2d(ctx, &ta, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, A, (uint64_t)M, (uint64_t)K, BK, BM);
     if (rc) return rc;
     rc = make_tmap_2d(ctx, &tb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, W, (uint64_t)N, (uint64_t)K, BK, BN / CG);
     if (rc) return rc;
-    if (EPI == 2) {
+    if (EPI >= 2) {
         rc = make_tmap_2d(ctx, &tc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Cout, (uint64_t)M, (uint64_t)N, 32, 32);
         if (rc) return rc;
         rc = make_tmap_2d(ctx, &tr, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, residual, (uint64_t)M, (uint64_t)N, 32, 32);
@@ -401,22 +585,38 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
         if (rc) return rc;
         tr = tc;
     }
+    ty = tc; txb = tc;
+    if (EPI == 3) {
+        // per-pair scratch for v = acc + bias + residual: (pairs x 256) rows x N FP32, rewritten for every row block
+        const size_t need = (size_t)(grid / CG) * BM * CG * (size_t)N * 4;
+        if (ctx->ln_scratch_bytes < need) {
+            CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+            cudaFree(ctx->ln_scratch);
+            ctx->ln_scratch = nullptr; ctx->ln_scratch_bytes = 0;
+            if (cudaMalloc(&ctx->ln_scratch, need) != cudaSuccess) { cudaGetLastError(); return ANON_ERR_OOM; }
+            ctx->ln_scratch_bytes = need;
+        }
+        rc = make_tmap_2d(ctx, &ty, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, ctx->ln_scratch, (uint64_t)(grid / CG) * BM * CG, (uint64_t)N, 32, 32);
+        if (rc) return rc;
+        rc = make_tmap_2d(ctx, &txb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, ln->xb_out, (uint64_t)M, (uint64_t)N, 64, 32);
+        if (rc) return rc;
+    }
     auto kern = gemm_bf16_tcgen05_kernel<BN, EPI, NB, CG>;
     static bool attr_set = false;
     if (!attr_set) {
         CU_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
         attr_set = true;
     }
-    const int tiles = ((M + BM * CG - 1) / (BM * CG)) * ((N + BN - 1) / BN);
-    const int slots = ctx->sm_count / CG;
-    const int grid = CG * (tiles < slots ? tiles : slots);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, bias, M, N, K));
+    const float* g = ln ? ln->gamma : nullptr;
+    const float* be = ln ? ln->beta : nullptr;
+    const float eps = ln ? ln->eps : 0.f;
+    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, ty, txb, bias, g, be, eps, M, N, K));
     CU_LAUNCH_CHECK(ctx, "gemm_bf16_tcgen05_kernel");
     return ANON_OK;
 }
@@ -445,6 +645,28 @@ int gemm_bf16_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W
         case 1: return launch_gemm<128, 1, 2, 1>(ctx, A, W, bias, residual, Cout, M, N, K);
         default: return launch_gemm<128, 2, 4, 1>(ctx, A, W, bias, residual, Cout, M, N, K);
     }
+}
+
+int gemm_bf16_ln_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias,
+                      const float* residual, const float* gamma, const float* beta, float eps, float* x_out,
+                      __nv_bfloat16* xb_out, int M, int N, int K)
+{
+    if (!ctx || !A || !W || !bias || !residual || !gamma || !beta || !x_out || !xb_out || M < 0 || N <= 0 || K <= 0)
+        return ANON_ERR_INVALID_ARG;
+    if (K % BK != 0 || N % 256 != 0 || N > 1024) return ANON_ERR_UNSUPPORTED;
+    if (M == 0) return ANON_OK;
+    LnArgs ln{gamma, beta, eps, xb_out};
+    return launch_gemm<256, 3, 4, 2>(ctx, A, W, bias, residual, x_out, M, N, K, &ln);
+}
+
+extern "C" int anon_gemm_bf16_ln(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,
+                                 const float* d_residual, const float* d_gamma, const float* d_beta, float eps,
+                                 float* d_x, void* d_xb, int32_t M, int32_t N, int32_t K)
+{
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    return gemm_bf16_ln_impl(ctx, (const __nv_bfloat16*)d_A, (const __nv_bfloat16*)d_W, d_bias, d_residual, d_gamma, d_beta,
+                             eps, d_x, (__nv_bfloat16*)d_xb, M, N, K);
 }
 
 extern "C" int anon_gemm_bf16(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,

@@ -142,6 +142,15 @@ extern "C" void anon_weights_free(anon_weights* w) {
 
 const anon_model_desc* weights_desc(const anon_weights* w) { return &w->d; }
 
+// K4 launcher: compile-time row length for the BF16 shapes (H = 768, 1024), generic kernel otherwise
+static void launch_layer_norm(cudaStream_t st, unsigned grid, const float* y, int nt, int H, const float* g, const float* b,
+                              float eps, float* x, __nv_bfloat16* xb)
+{
+    if (xb && H == 768) enc::layer_norm_fixed_kernel<6><<<grid, enc::kRowWarps * 32, 0, st>>>(y, nt, g, b, eps, x, xb);
+    else if (xb && H == 1024) enc::layer_norm_fixed_kernel<8><<<grid, enc::kRowWarps * 32, 0, st>>>(y, nt, g, b, eps, x, xb);
+    else enc::layer_norm_kernel<<<grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, g, b, eps, x, xb);
+}
+
 template <int EPI>
 static int sgemm(anon_ctx* ctx, const float* A, const float* W, const float* bias, const float* res, float* C, int M, int N, int K) {
     if (M == 0) return ANON_OK;
@@ -234,7 +243,7 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                     else rc = sgemm<2>(ctx, (const float*)cx, (const float*)L.W_o, L.b_o, x, y, nt, H, H); }
                     if (rc) return rc;
                     { ProfScope ps(ctx, PROF_ROW, row_bytes);
-                    enc::layer_norm_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, L.g_1, L.b_1, d.ln_eps, x, xb); }
+                    launch_layer_norm(st, row_grid, y, nt, H, L.g_1, L.b_1, d.ln_eps, x, xb); }
                     CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
                 }
                 { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * F * H);
@@ -252,7 +261,7 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                     else rc = sgemm<2>(ctx, (const float*)f, (const float*)L.W_2, L.b_2f, x, y, nt, H, F); }
                     if (rc) return rc;
                     { ProfScope ps(ctx, PROF_ROW, row_bytes);
-                    enc::layer_norm_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, L.g_2, L.b_2, d.ln_eps, x, xb); }
+                    launch_layer_norm(st, row_grid, y, nt, H, L.g_2, L.b_2, d.ln_eps, x, xb); }
                     CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
                 }
             }

@@ -107,6 +107,49 @@ static __global__ void __launch_bounds__(kRowWarps * 32) layer_norm_kernel(
     layer_norm_row(v, n4, H, g, b, eps, lane, x + (size_t)r * H, xb ? xb + (size_t)r * H : nullptr);
 }
 
+// K4 with the row length known at compile time (H = 128 * N4): the row lives in exactly N4 float4 per lane, which
+// lets ptxas keep the kernel at 48 registers and 5 CTAs (40 warps) resident per SM.
+template <int N4>
+static __global__ void __launch_bounds__(kRowWarps * 32, (N4 <= 6) ? 5 : 4) layer_norm_fixed_kernel(
+    const float* __restrict__ y, int ntok, const float* __restrict__ g, const float* __restrict__ b, float eps,
+    float* __restrict__ x, __nv_bfloat16* __restrict__ xb)
+{
+    constexpr int H = 128 * N4;
+    const int lane = threadIdx.x & 31;
+    const int r = blockIdx.x * kRowWarps + (threadIdx.x >> 5);
+    if (r >= ntok) return;
+    float4 v[N4];
+    const float4* src = reinterpret_cast<const float4*>(y + (size_t)r * H) + lane;
+#pragma unroll
+    for (int k = 0; k < N4; k++) v[k] = __ldcs(src + 32 * k);
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < N4; k++) s += (v[k].x + v[k].y) + (v[k].z + v[k].w);
+    const float mean = warp_sum(s) * (1.0f / (float)H);
+    float q = 0.f;
+#pragma unroll
+    for (int k = 0; k < N4; k++) {
+        v[k].x -= mean; v[k].y -= mean; v[k].z -= mean; v[k].w -= mean;
+        q += (v[k].x * v[k].x + v[k].y * v[k].y) + (v[k].z * v[k].z + v[k].w * v[k].w);
+    }
+    const float rstd = 1.0f / sqrtf(warp_sum(q) * (1.0f / (float)H) + eps);
+    float4* xo = reinterpret_cast<float4*>(x + (size_t)r * H) + lane;
+    uint2* xbo = reinterpret_cast<uint2*>(xb + (size_t)r * H) + lane;
+#pragma unroll
+    for (int k = 0; k < N4; k++) {
+        const int e = 4 * (lane + 32 * k);
+        const float4 gg = load4(g + e), bb = load4(b + e);
+        float4 o;
+        o.x = v[k].x * rstd * gg.x + bb.x; o.y = v[k].y * rstd * gg.y + bb.y;
+        o.z = v[k].z * rstd * gg.z + bb.z; o.w = v[k].w * rstd * gg.w + bb.w;
+        xo[32 * k] = o;
+        __nv_bfloat162 lo = __floats2bfloat162_rn(o.x, o.y), hi = __floats2bfloat162_rn(o.z, o.w);
+        uint2 u;
+        u.x = *reinterpret_cast<uint32_t*>(&lo); u.y = *reinterpret_cast<uint32_t*>(&hi);
+        xbo[32 * k] = u;
+    }
+}
+
 // K6: logits = x W_c^T + b_c (FP32), label = argmax (ties -> lowest index).
 static __global__ void __launch_bounds__(kRowWarps * 32) head_argmax_kernel(
     const float* __restrict__ x, int ntok, int H, const float* __restrict__ W_c, const float* __restrict__ b_c, int NL,

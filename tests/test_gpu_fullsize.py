@@ -1,0 +1,136 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (one ~1 M-token chunk for
+configs[1]; 50 M spans in one call for configs[4]).  The oracle cannot run these sizes whole, so:
+  * encoder: oracle logits / labels on sampled sequences (computed one by one), BF16 tolerances of BASELINE.json;
+  * decode / gather / pseudonymize: the oracle applied to the GPU's own labels and spans (those stages are integer
+    work: bit-exact at full size);
+  * configs[4]: the hit / miss sets and uids follow from the generator's draws alone (first occurrence of each string),
+    the pseudonyms of sampled spans come from the oracle's HMAC one by one."""
+import numpy as np
+import pytest
+
+from harness import gen
+
+pytestmark = pytest.mark.gpu
+
+KEY = bytes((7 * i + 3) & 255 for i in range(32))
+
+
+def test_configs1_full_size_in_bench_configuration():
+    import torch
+    import paper_2606_15650_b200 as P
+    from oracle import crypto, decode, encoder
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device")
+    dev = "cuda:0"
+    d = gen.DESCS["base"]
+    rec, win = gen.workload_base(n_records=4096, seed=gen.SEED_BASE + 2)          # exactly bench.py's default workload
+    w = gen.make_weights(d, gen.SEED_BASE + 2, planted=(2.0, 0.5, 4.0))
+    ids, cu, meta = win["token_ids"], win["cu_seqlens"], np.ascontiguousarray(win["meta"])
+    T, B = ids.size, cu.size - 1
+    assert T > 900_000
+    ctx = P.Context(0, workspace_bytes=P.anon_workspace_bytes(d, T, B) + (256 << 20))
+    W = P.Weights(ctx, d, gen.pack_blob(w))
+    logits = torch.zeros((T, d["num_labels"]), dtype=torch.float32, device=dev)
+    labels = torch.zeros(T, dtype=torch.int32, device=dev)
+    P.anon_ner_forward(ctx, W, torch.from_numpy(ids).to(dev), torch.from_numpy(cu).to(dev), logits, labels)
+    assert ctx.sync() == 0
+    got_logits, got_labels = logits.cpu().numpy(), labels.cpu().numpy()
+    # the GPU label is the argmax (ties -> lowest) of the GPU's own FP32 logits, everywhere
+    assert np.array_equal(got_labels, encoder.argmax_labels(got_logits))
+    # sampled sequences: shortest, longest, first, last, and four seeded picks (tiles in the middle of the launch)
+    lens = np.diff(cu)
+    picks = {int(np.argmin(lens)), int(np.argmax(lens)), 0, B - 1}
+    picks |= set(np.random.default_rng(5).integers(0, B, 4).tolist())
+    subset = sorted(picks)
+    want = encoder.forward_packed(w, d, ids, cu, seq_subset=subset)
+    rows = ~np.isnan(want[:, 0])
+    assert rows.sum() >= 512
+    err = np.abs(got_logits[rows] - want[rows])
+    assert err.max() <= 3e-2, err.max()
+    mism = got_labels[rows] != encoder.argmax_labels(want[rows])
+    assert (encoder.top2_margin(want[rows])[mism] < 3e-2).all()
+    assert 1.0 - mism.mean() >= 0.999
+    # decode + gather + pseudonymize at full size against the oracle fed with the GPU's labels
+    cap = T // 2
+    spans = torch.zeros((cap, 4), dtype=torch.int32, device=dev)
+    nsp = torch.zeros(1, dtype=torch.int32, device=dev)
+    P.anon_decode_spans(ctx, labels, torch.from_numpy(meta).to(dev), d["num_labels"], spans, nsp)
+    assert ctx.sync() == 0
+    S = int(nsp.item())
+    want_spans = decode.decode_spans(got_labels, meta)
+    assert S == len(want_spans) and S > 20000
+    assert np.array_equal(spans.cpu().numpy()[:S], np.asarray(want_spans, np.int32).reshape(-1, 4))
+    text, rec_off = rec["text"], rec["rec_off"]
+    span_bytes = torch.zeros(text.size + 16, dtype=torch.uint8, device=dev)
+    span_off = torch.zeros(S + 1, dtype=torch.int64, device=dev)
+    span_type = torch.zeros(S, dtype=torch.uint8, device=dev)
+    P.anon_gather_spans(ctx, torch.from_numpy(text).to(dev), torch.from_numpy(rec_off).to(dev), spans, S, span_bytes, span_off,
+                        span_type)
+    sb, so = decode.gather_spans(text, rec_off, want_spans)
+    assert ctx.sync() == 0
+    assert np.array_equal(span_off.cpu().numpy(), so) and np.array_equal(span_bytes.cpu().numpy()[:so[-1]], sb)
+    cache = P.Cache(ctx, 1 << 20, 64 << 20)
+    out = torch.zeros(S * 32, dtype=torch.uint8, device=dev)
+    out_off = torch.zeros(S + 1, dtype=torch.int64, device=dev)
+    hit = torch.zeros(S, dtype=torch.uint8, device=dev)
+    P.anon_pseudonymize(ctx, cache, span_bytes, span_off, span_type, KEY, 10, gen.TYPE_NAMES_6, out, out_off, hit)
+    assert ctx.sync() == 0
+    oc = crypto.Cache(1 << 20)
+    wantp = oc.pseudonymize(sb, so, np.asarray([s[3] for s in want_spans], np.uint8), KEY, 10, gen.TYPE_NAMES_6)
+    oc.close()
+    oo = out_off.cpu().numpy()
+    assert np.array_equal(oo, wantp["out_offsets"])
+    assert np.array_equal(out.cpu().numpy()[:oo[-1]], wantp["out_tokens"])
+    assert np.array_equal(hit.cpu().numpy(), wantp["hit"])
+    cache.close(); W.close(); ctx.close()
+
+
+def test_configs4_full_size_50m_spans():
+    import torch
+    import paper_2606_15650_b200 as P
+    from oracle import crypto
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device")
+    dev = "cuda:0"
+    n_unique, S = 2_000_000, 50_000_000
+    data, off, types, key, draws = gen.spans_zipf(n_unique, S, 7, 128, 6, gen.SEED_BASE + 5)      # bench.py's workload
+    ctx = P.Context(0, workspace_bytes=S * 8 + (S // 2048 + 2) * 24 + (64 << 20))
+    cache = P.Cache(ctx, n_unique, int(n_unique * 70) + (1 << 20))
+    d_bytes, d_off, d_type = (torch.from_numpy(a).to(dev) for a in (data, off, types))
+    out = torch.zeros(S * (3 + 13 + 10), dtype=torch.uint8, device=dev)
+    out_off = torch.zeros(S + 1, dtype=torch.int64, device=dev)
+    hit = torch.zeros(S, dtype=torch.uint8, device=dev)
+    uid = torch.zeros(S, dtype=torch.int64, device=dev)
+    kb = key.tobytes()
+    P.anon_pseudonymize(ctx, cache, d_bytes, d_off, d_type, kb, 10, gen.TYPE_NAMES_6, out, out_off, hit, uid)
+    assert ctx.sync() == 0
+    # hit / miss sets and uids from the draws alone: a span misses iff it is the first occurrence of its pool string,
+    # and uid = rank of that first occurrence among all first occurrences (the pool strings are distinct by construction)
+    _vals, first = np.unique(draws, return_index=True)
+    want_hit = np.ones(S, np.uint8)
+    want_hit[first] = 0
+    got_hit = hit.cpu().numpy()
+    assert np.array_equal(got_hit, want_hit)
+    order = np.sort(first)                                   # first occurrences in stream order -> uid 0, 1, 2, ...
+    uid_of_pool = np.empty(n_unique, np.int64)
+    uid_of_pool[draws[order]] = np.arange(order.size)
+    assert np.array_equal(uid.cpu().numpy(), uid_of_pool[draws])
+    st = cache.stats()
+    assert st["n_unique"] == first.size and st["n_lookups"] == S and st["n_hits"] == S - first.size
+    # offsets: exclusive prefix sum of 3 + len(type name) + slug_len
+    name_len = np.asarray([len(n) for n in gen.TYPE_NAMES_6], np.int64)
+    want_off = np.zeros(S + 1, np.int64)
+    np.cumsum(3 + name_len[types] + 10, out=want_off[1:])
+    got_off = out_off.cpu().numpy()
+    assert np.array_equal(got_off, want_off)
+    # sampled pseudonyms from the oracle, one by one: the first and last spans, the head of the Zipf law, seeded picks
+    picks = np.unique(np.concatenate([[0, 1, S - 1], order[:50], np.random.default_rng(9).integers(0, S, 4000)]))
+    got_tok = out.cpu().numpy()
+    sub_off = np.zeros(picks.size + 1, np.int64)
+    np.cumsum(off[picks + 1] - off[picks], out=sub_off[1:])
+    sub = np.concatenate([data[off[i]:off[i + 1]] for i in picks])
+    dig = crypto.hmac_batch(kb, sub, sub_off)
+    for k, i in enumerate(picks):
+        want_tok = ("[" + gen.TYPE_NAMES_6[types[i]] + "_" + bytes(dig[k]).hex()[:10] + "]").encode()
+        assert bytes(got_tok[got_off[i]:got_off[i + 1]]) == want_tok, int(i)
+    cache.close(); ctx.close()

@@ -440,8 +440,12 @@ def run_stream(args):
         P.anon_gather_spans(ctx, b["text"], b["ro"], spans, S, span_bytes, span_off, span_type)
         P.anon_pseudonymize(ctx, cache, span_bytes, span_off[:S + 1], span_type, KEY, SLUG_LEN, names, out_tokens,
                             out_off[:S + 1], hit)
+        # NEXT-1: the records rewritten on the device with every span replaced by its pseudonym (text in -> text out)
+        P.anon_splice_records(ctx, b["text"], b["ro"], spans, S, out_tokens, out_off[:S + 1], new_text, new_ro[:b["ro"].numel()])
         return S
 
+    new_text = torch.zeros(max_text + out_cap, dtype=torch.uint8, device=dev)
+    new_ro = torch.zeros(max(b["rec_off"].size for b in batches), dtype=torch.int64, device=dev)
     scratch = P.Cache(ctx, 1 << 20, 64 << 20)
     for k in range(min(3, len(batches))):
         step(scratch, k)
@@ -510,6 +514,7 @@ def run_stream(args):
                                "%d window-tokens, Zipf(1.1) entities; batches of whole records, <= %d tokens"
                                % (n_records, rec["text"].size / 2**20, len(win["cu_seqlens"]) - 1, T_all, args.batch_tokens),
                    "batches": nb, "weights": "W2 planted-detector, seeded random-init", "slug_len": SLUG_LEN,
+                   "splice": "records rewritten on the device (anon_splice_records) inside the timed region",
                    "spans": S_all, "planted_entities": int(rec["n_entities"]), "unique_entities": st["n_unique"],
                    "cache_hit_rate": st["n_hits"] / max(st["n_lookups"], 1),
                    "l2": "inputs larger than L2 (each batch streams ~20 GB of activations through HBM)"},

@@ -181,6 +181,17 @@ int  anon_pseudonymize(anon_ctx* ctx, anon_cache* cache,
 int  anon_hmac_spans(anon_ctx* ctx, const uint8_t* d_span_bytes, const int64_t* d_span_offsets, int64_t S,
                      const uint8_t* key, size_t key_len, uint8_t* d_digests /* [S,32] */);
 
+/* ---- NEXT-1: record splice (P:L53 stage 5 restricted to record text; S8f NEXT-1) ------------------------------- */
+/* Rewrites every record with each span [char_start, char_end) replaced by its pseudonym token:
+ *   new_text = for each record, the bytes between spans copied, out_tokens[out_offsets[s] .. out_offsets[s+1]) in
+ *   place of span s;  d_new_record_offsets int64[R+1] = offsets of the rewritten records.
+ * d_spans must be in stream order (as anon_decode_spans writes them) and non-overlapping; text_bytes =
+ * record_offsets[R].  If the rewritten text exceeds new_text_capacity nothing beyond it is written and
+ * ANON_ERR_CAPACITY is latched in the sticky status.  Asynchronous. */
+int  anon_splice_records(anon_ctx* ctx, const uint8_t* d_text, size_t text_bytes, const int64_t* d_record_offsets, int32_t R,
+                         const anon_span* d_spans, int32_t S, const uint8_t* d_out_tokens, const int64_t* d_out_offsets,
+                         uint8_t* d_new_text, size_t new_text_capacity, int64_t* d_new_record_offsets);
+
 /* ---- whole hot path with HOST buffers (the call a user makes; bench.py's e2e leg) ------------- */
 /* Copies one batch host->device, runs A1-A13 and copies the results back, all on the
  * context's stream; synchronises before returning.  Host inputs: token_ids int32[T],

@@ -94,3 +94,34 @@ def gather_spans(text, record_offsets, spans):
         offs.append(offs[-1] + (ce - cs))
     data = np.frombuffer(b"".join(chunks), dtype=np.uint8) if chunks else np.zeros(0, np.uint8)
     return data, np.asarray(offs, np.int64)
+
+
+def splice_records(text, record_offsets, spans, out_tokens, out_offsets):
+    """Stage 5 of the paper's pipeline ("only sensitive values replaced", schema preserved) restricted to
+    the text of a record: every record's bytes with each span [char_start, char_end) replaced by its pseudonym token
+    (SURVEY.md §8(f) NEXT-1).  spans are in stream order (records ascending, char_start ascending inside a record) and
+    do not overlap; out_tokens / out_offsets are the CSR of their pseudonyms.  Written as the plain definition: walk
+    each record left to right, copy what lies between spans, emit the token in place of each span.
+
+    Returns (bytes uint8[], int64[R+1] offsets of the rewritten records)."""
+    R = len(record_offsets) - 1
+    per_rec = [[] for _ in range(R)]
+    for s, (rec, cs, ce, _t) in enumerate(spans):
+        per_rec[rec].append((cs, ce, s))
+    pieces, offs = [], [0]
+    for r in range(R):
+        base, end = int(record_offsets[r]), int(record_offsets[r + 1])
+        body = bytes(bytearray(text[base:end]))
+        cur, out = 0, []
+        for cs, ce, s in per_rec[r]:
+            if cs < cur or ce < cs or ce > len(body):
+                raise ValueError("spans must be ordered, non-overlapping and inside their record")
+            out.append(body[cur:cs])
+            out.append(bytes(bytearray(out_tokens[int(out_offsets[s]):int(out_offsets[s + 1])])))
+            cur = ce
+        out.append(body[cur:])
+        rec_bytes = b"".join(out)
+        pieces.append(rec_bytes)
+        offs.append(offs[-1] + len(rec_bytes))
+    data = np.frombuffer(b"".join(pieces), dtype=np.uint8) if offs[-1] else np.zeros(0, np.uint8)
+    return data, np.asarray(offs, np.int64)

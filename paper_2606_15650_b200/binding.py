@@ -65,6 +65,7 @@ _SIGNATURES = {
     "anon_ctx_profile_read": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "anon_gemm_bf16": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32]),
     "anon_gemm_bf16_ln": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp, _vp, _i32, _i32, _i32]),
+    "anon_splice_records": (ctypes.c_int, [_vp, _vp, _sz, _vp, _i32, _vp, _i32, _vp, _vp, _vp, _sz, _vp]),
     "anon_attention": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32, _i32, _vp]),
 }
 
@@ -254,6 +255,14 @@ def anon_gemm_bf16(ctx, A, W, bias, residual, C, epilogue):
     N = W.shape[0]
     ctx.check(lib().anon_gemm_bf16(ctx._h, _ptr(A), _ptr(W), _ptr(bias), _ptr(residual), _ptr(C), M, N, K, epilogue),
               "anon_gemm_bf16")
+
+
+def anon_splice_records(ctx, text, record_offsets, spans, S, out_tokens, out_offsets, new_text, new_record_offsets):
+    """Device tensors; rewrites the records with every span replaced by its pseudonym token (NEXT-1)."""
+    R = record_offsets.numel() - 1
+    ctx.check(lib().anon_splice_records(ctx._h, _ptr(text), text.numel(), _ptr(record_offsets), R, _ptr(spans), S,
+                                        _ptr(out_tokens), _ptr(out_offsets), _ptr(new_text), new_text.numel(),
+                                        _ptr(new_record_offsets)), "anon_splice_records")
 
 
 def anon_gemm_bf16_ln(ctx, A, W, bias, residual, gamma, beta, eps, x, xb):

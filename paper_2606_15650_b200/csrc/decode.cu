@@ -99,7 +99,118 @@ __global__ void gather_finish_kernel(const long long* total, const int* d_n, lon
     off[n] = *total;
 }
 
+// ---- NEXT-1: record splice (PAPER.md L53 stage 5, restricted to record text) ----
+// D[s] = exclusive prefix sum of (token length - span length) over the span list in stream order; a byte at absolute
+// position p that lies outside every span moves to p + D[k], k = number of spans that start at or before p; the token
+// of span s goes to abs_start[s] + D[s].
+struct DeltaIn {
+    const anon_span* spans; const long long* tok_off;
+    __device__ __forceinline__ long long operator()(long long s) const {
+        const int l = spans[s].char_end - spans[s].char_start;
+        return (tok_off[s + 1] - tok_off[s]) - (l > 0 ? l : 0);
+    }
+};
+struct DeltaOut {
+    const anon_span* spans; const long long* rec_off; long long* D; long long* astart; long long* aend; long long S;
+    __device__ __forceinline__ void operator()(long long s, long long ex, long long v) const {
+        const anon_span sp = spans[s];
+        const long long a = rec_off[sp.record_id] + sp.char_start;
+        const int l = sp.char_end - sp.char_start;
+        D[s] = ex; astart[s] = a; aend[s] = a + (l > 0 ? l : 0);
+        if (s == S - 1) D[S] = ex + v;
+    }
+};
+
+__global__ void __launch_bounds__(256) splice_copy_kernel(const uint8_t* __restrict__ text, long long nbytes, long long S,
+                                                          const long long* __restrict__ D, const long long* __restrict__ astart,
+                                                          const long long* __restrict__ aend, uint8_t* __restrict__ out,
+                                                          long long cap, int* d_status)
+{
+    const long long p0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 16;
+    if (p0 >= nbytes) return;
+    long long lo = 0, hi = S;                       // k = number of spans with astart <= p0
+    while (lo < hi) { const long long mid = (lo + hi) >> 1; if (astart[mid] <= p0) lo = mid + 1; else hi = mid; }
+    long long k = lo;
+    long long prev_end = k > 0 ? aend[k - 1] : -1, next_start = k < S ? astart[k] : nbytes + 16, shift = D[k];
+    const long long pe = p0 + 16 < nbytes ? p0 + 16 : nbytes;
+    for (long long p = p0; p < pe; p++) {
+        while (p >= next_start) { prev_end = aend[k]; k++; next_start = k < S ? astart[k] : nbytes + 16; shift = D[k]; }
+        if (p >= prev_end) {
+            const long long q = p + shift;
+            if (q < cap) out[q] = text[p]; else latch_status(d_status, ANON_ERR_CAPACITY);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) splice_tokens_kernel(long long S, const long long* __restrict__ D,
+                                                            const long long* __restrict__ astart, const uint8_t* __restrict__ tok,
+                                                            const long long* __restrict__ tok_off, uint8_t* __restrict__ out,
+                                                            long long cap, int* d_status)
+{
+    const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= S) return;
+    const long long q = astart[s] + D[s], a = tok_off[s], n = tok_off[s + 1] - a;
+    if (q + n > cap) { latch_status(d_status, ANON_ERR_CAPACITY); return; }
+    for (long long j = 0; j < n; j++) out[q + j] = tok[a + j];
+}
+
+__global__ void __launch_bounds__(256) splice_record_offsets_kernel(const long long* __restrict__ rec_off, int R, const anon_span* __restrict__ spans,
+                                                                    long long S, const long long* __restrict__ D, long long* __restrict__ new_off)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r > R) return;
+    long long lo = 0, hi = S;                       // number of spans in records < r
+    while (lo < hi) { const long long mid = (lo + hi) >> 1; if (spans[mid].record_id < r) lo = mid + 1; else hi = mid; }
+    new_off[r] = rec_off[r] + D[lo];
+}
+
 }  // namespace
+
+int splice_records_impl(anon_ctx* ctx, WsCursor& ws, const uint8_t* d_text, size_t text_bytes, const int64_t* d_rec_off, int32_t R,
+                        const anon_span* d_spans, int32_t S, const uint8_t* d_tok, const int64_t* d_tok_off,
+                        uint8_t* d_new_text, size_t cap, int64_t* d_new_rec_off)
+{
+    if (!ctx || R < 0 || S < 0 || !d_rec_off || !d_new_rec_off || (text_bytes > 0 && (!d_text || !d_new_text)) ||
+        (S > 0 && (!d_spans || !d_tok_off)))
+        return ANON_ERR_INVALID_ARG;
+    cudaStream_t st = ctx->stream;
+    long long* D = (long long*)ws.take(((size_t)S + 1) * 8);
+    long long* astart = (long long*)ws.take(((size_t)S + 1) * 8);
+    long long* aend = (long long*)ws.take(((size_t)S + 1) * 8);
+    long long* agg = (long long*)ws.take(scan::agg_bytes<long long>(S > 0 ? S : 1));
+    if (!D || !astart || !aend || !agg) return ANON_ERR_OOM;
+    ProfScope ps(ctx, PROF_DECODE, (double)text_bytes * 2 + (double)S * 64, 6);
+    if (S > 0) {
+        DeltaIn din{d_spans, (const long long*)d_tok_off};
+        scan::reduce_and_scan<long long, scan::SumI64>(din, S, nullptr, agg, st);
+        scan::apply<long long, scan::SumI64>(din, DeltaOut{d_spans, (const long long*)d_rec_off, D, astart, aend, S}, S, nullptr, agg, st);
+    } else {
+        CU_TRY(ctx, cudaMemsetAsync(D, 0, 8, st));
+    }
+    if (text_bytes > 0) {
+        const long long chunks = ((long long)text_bytes + 15) / 16;
+        splice_copy_kernel<<<(unsigned)((chunks + 255) / 256), 256, 0, st>>>(d_text, (long long)text_bytes, S, D, astart, aend,
+                                                                           d_new_text, (long long)cap, ctx->d_status);
+    }
+    if (S > 0)
+        splice_tokens_kernel<<<(unsigned)((S + 255) / 256), 256, 0, st>>>(S, D, astart, d_tok, (const long long*)d_tok_off, d_new_text,
+                                                                         (long long)cap, ctx->d_status);
+    splice_record_offsets_kernel<<<(unsigned)((R + 1 + 255) / 256), 256, 0, st>>>((const long long*)d_rec_off, R, d_spans, S, D,
+                                                                                 (long long*)d_new_rec_off);
+    CU_LAUNCH_CHECK(ctx, "splice_records");
+    return ANON_OK;
+}
+
+extern "C" int anon_splice_records(anon_ctx* ctx, const uint8_t* d_text, size_t text_bytes, const int64_t* d_record_offsets, int32_t R,
+                                   const anon_span* d_spans, int32_t S, const uint8_t* d_out_tokens, const int64_t* d_out_offsets,
+                                   uint8_t* d_new_text, size_t new_text_capacity, int64_t* d_new_record_offsets)
+{
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    WsCursor ws = ws_begin(ctx);
+    return splice_records_impl(ctx, ws, d_text, text_bytes, d_record_offsets, R, d_spans, S, d_out_tokens, d_out_offsets,
+                               d_new_text, new_text_capacity, d_new_record_offsets);
+}
 
 int decode_spans_impl(anon_ctx* ctx, WsCursor& ws, const int32_t* d_labels, const anon_tok_meta* d_meta, int32_t T,
                       int32_t num_labels, anon_span* d_spans, int32_t cap, int32_t* d_num)

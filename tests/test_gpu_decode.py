@@ -118,3 +118,46 @@ def test_windowed_records_decode_and_gather(env):
     P.anon_gather_spans(ctx, torch.from_numpy(rec["text"]).to(dev), torch.from_numpy(rec["rec_off"]).to(dev), d_sp, n,
                         sb2, so, None)
     assert ctx.sync() == -3
+
+
+def test_splice_records_matches_oracle(env):
+    """NEXT-1: every record rewritten with its spans replaced by their pseudonym tokens, bit-exact against
+    oracle/decode.splice_records; tokens longer and shorter than the spans, records without spans, S = 0, capacity."""
+    P, torch, ctx = env
+    from oracle import crypto, decode
+    dev = "cuda:0"
+    d = dict(gen.DESCS["tiny"])
+    pool, poff, ptype = gen.entity_pool(64, 3)
+    n_tok = np.array([40, 700, 90, 8, 1300, 16, 300, 8, 8, 64], np.int64)
+    rec = gen.make_records(len(n_tok), n_tok, d, pool, poff, ptype % 4, 5, entity_rate=1.0 / 12)
+    win = gen.window_records(rec)
+    spans = decode.decode_spans(win["planted_label"].astype(np.int32), win["meta"])
+    assert len(spans) > 100
+    sb, so = decode.gather_spans(rec["text"], rec["rec_off"], spans)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    for slug_len in (10, 0, 64):
+        oc = crypto.Cache()
+        ps = oc.pseudonymize(sb, so, np.asarray([s[3] for s in spans], np.uint8), bytes(range(32)), slug_len, gen.TYPE_NAMES_4)
+        oc.close()
+        want, want_off = decode.splice_records(rec["text"], rec["rec_off"], spans, ps["out_tokens"], ps["out_offsets"])
+        new_text = torch.full((want.size + 64,), 0xEE, dtype=torch.uint8, device=dev)
+        new_off = torch.zeros(len(n_tok) + 1, dtype=torch.int64, device=dev)
+        P.anon_splice_records(ctx, t(rec["text"]), t(rec["rec_off"]), t(np.asarray(spans, np.int32).reshape(-1, 4)), len(spans),
+                              t(ps["out_tokens"]) if ps["out_tokens"].size else torch.zeros(16, dtype=torch.uint8, device=dev),
+                              t(ps["out_offsets"]), new_text, new_off)
+        assert ctx.sync() == 0
+        assert np.array_equal(new_off.cpu().numpy(), want_off)
+        got = new_text.cpu().numpy()
+        assert np.array_equal(got[:want.size], want) and (got[want.size:] == 0xEE).all()
+    # no spans: identity
+    new_text = torch.zeros(rec["text"].size, dtype=torch.uint8, device=dev)
+    new_off = torch.zeros(len(n_tok) + 1, dtype=torch.int64, device=dev)
+    P.anon_splice_records(ctx, t(rec["text"]), t(rec["rec_off"]), torch.zeros((1, 4), dtype=torch.int32, device=dev), 0,
+                          torch.zeros(16, dtype=torch.uint8, device=dev), torch.zeros(1, dtype=torch.int64, device=dev), new_text, new_off)
+    assert ctx.sync() == 0
+    assert np.array_equal(new_text.cpu().numpy(), rec["text"]) and np.array_equal(new_off.cpu().numpy(), rec["rec_off"])
+    # capacity too small: latched, nothing written past the end
+    small = torch.full((want.size - 100,), 0xEE, dtype=torch.uint8, device=dev)
+    P.anon_splice_records(ctx, t(rec["text"]), t(rec["rec_off"]), t(np.asarray(spans, np.int32).reshape(-1, 4)), len(spans),
+                          t(ps["out_tokens"]), t(ps["out_offsets"]), small, new_off)
+    assert ctx.sync() == -3

@@ -113,3 +113,56 @@ def test_gather_spans():
     rec_off = np.array([0, 11, 27])
     data, off = decode.gather_spans(text, rec_off, [(0, 6, 11, 0), (1, 4, 12, 1), (1, 0, 0, 0)])
     assert bytes(data) == b"world10.0.0.1" and off.tolist() == [0, 5, 13, 13]
+
+
+def test_splice_records_hand_worked_and_library_replace():
+    """NEXT-1 pins: a hand-worked record pair; str.replace on records whose entity strings occur exactly once (an
+    independent library routine); zero spans = identity; total length = original + sum of (token - span) lengths;
+    splicing the originals back in place of the tokens recovers the input."""
+    text = np.frombuffer(b"ip 10.0.0.1 seen" + b"host a.b and 10.0.0.1", np.uint8)
+    rec_off = np.array([0, 16, 37], np.int64)
+    spans = [(0, 3, 11, 0), (1, 5, 8, 2), (1, 13, 21, 0)]
+    toks = [b"[IP_ADDRESS_aaaaaaaaaa]", b"[HOSTNAME_bbbbbbbbbb]", b"[IP_ADDRESS_aaaaaaaaaa]"]
+    tok = np.frombuffer(b"".join(toks), np.uint8)
+    toff = np.array([0] + list(np.cumsum([len(t) for t in toks])), np.int64)
+    out, ooff = decode.splice_records(text, rec_off, spans, tok, toff)
+    assert bytes(out[ooff[0]:ooff[1]]) == b"ip [IP_ADDRESS_aaaaaaaaaa] seen"
+    assert bytes(out[ooff[1]:ooff[2]]) == b"host [HOSTNAME_bbbbbbbbbb] and [IP_ADDRESS_aaaaaaaaaa]"
+    # identity with no spans
+    o2, f2 = decode.splice_records(text, rec_off, [], np.zeros(0, np.uint8), np.zeros(1, np.int64))
+    assert np.array_equal(o2, text) and np.array_equal(f2, rec_off)
+    # seeded records with unique entity strings: sequential str.replace gives the same bytes
+    rng = np.random.default_rng(4)
+    recs, sp, tk = [], [], []
+    for r in range(20):
+        words, pos, body = [], 0, b""
+        for k in range(int(rng.integers(0, 7))):
+            filler = bytes(rng.integers(97, 123, int(rng.integers(0, 9))).astype(np.uint8))
+            ent = b"<E%d_%d>" % (r, k)
+            body += filler + b" "
+            sp.append((r, len(body), len(body) + len(ent), k % 3))
+            tk.append(b"[T%d_%04x]" % (k % 3, int(rng.integers(0, 65536))) if k % 2 else b"[]")   # longer and shorter than the span
+            body += ent + b" "
+        recs.append(body + bytes(rng.integers(97, 123, int(rng.integers(0, 5))).astype(np.uint8)))
+    text2 = np.frombuffer(b"".join(recs), np.uint8)
+    roff = np.array([0] + list(np.cumsum([len(b) for b in recs])), np.int64)
+    tok2 = np.frombuffer(b"".join(tk), np.uint8)
+    toff2 = np.array([0] + list(np.cumsum([len(t) for t in tk])), np.int64)
+    out3, ooff3 = decode.splice_records(text2, roff, sp, tok2, toff2)
+    for r in range(20):
+        want = recs[r]
+        for (rr, cs, ce, _t), t in zip(sp, tk):
+            if rr == r:
+                want = want.replace(recs[r][cs:ce], t)
+        assert bytes(out3[ooff3[r]:ooff3[r + 1]]) == want
+    assert out3.size == text2.size + sum(len(t) - (ce - cs) for (_r, cs, ce, _t), t in zip(sp, tk))
+    # inverse splice: put the original strings back where the tokens now are
+    inv_spans, shift, last = [], 0, -1
+    for (r, cs, ce, t), tkn in zip(sp, tk):
+        if r != last:
+            shift, last = 0, r
+        inv_spans.append((r, cs + shift, cs + shift + len(tkn), t))
+        shift += len(tkn) - (ce - cs)
+    ent_bytes, ent_off = decode.gather_spans(text2, roff, sp)
+    back, boff = decode.splice_records(out3, ooff3, inv_spans, ent_bytes, ent_off)
+    assert np.array_equal(back, text2) and np.array_equal(boff, roff)

@@ -93,6 +93,38 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
 
 
+
+GEMM_CLASSES = {"gemm_qkv": "QKV projection, +bias (N = 3H, K = H)", "gemm_out": "out-projection, +bias +FP32 residual (N = K = H)",
+                "gemm_ffn1": "FFN up, +bias +erf-GELU (N = F, K = H)", "gemm_ffn2": "FFN down, +bias +FP32 residual (N = H, K = F)"}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of gemm_bf16_tcgen05_kernel at the DEFAULT workload (configs[1],
+# M = 1,005,578 tokens), from one `ncu --set full` capture (profiles/r01_summary.md, "r01d"); other workloads: null
+NCU_TRAFFIC_BASE = {}
+
+
+def gemm_rooflines(prof, peaks, traffic=None):
+    """Per-GEMM achieved TFLOP/s from the context's event timing, the class total, and the `roofline` object of the
+    dominant one (largest share of the timed region)."""
+    peak = peaks["bf16_tflops_sustained"]
+    per, tot_ms, tot_fl, tot_n = {}, 0.0, 0.0, 0
+    for k in GEMM_CLASSES:
+        ms, fl, n = prof[k]
+        tot_ms += ms; tot_fl += fl; tot_n += n
+        if ms > 0:
+            per[k] = {"ms": ms, "launches": n, "tflops": fl / (ms * 1e-3) / 1e12, "frac": fl / (ms * 1e-3) / 1e12 / peak}
+    top = max(per, key=lambda k: per[k]["ms"])
+    ms, fl, n = prof[top]
+    achieved = fl / (ms * 1e-3) / 1e12
+    roof = {"bound": "tensor", "kernel": "gemm_bf16_tcgen05_kernel: " + GEMM_CLASSES[top], "achieved": achieved, "peak": peak,
+            "unit": "TFLOP/s", "frac": achieved / peak,
+            "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (%s)" % peaks["source"],
+            "frac_of_burst_peak": achieved / peaks["bf16_tflops"], "frac_of_nominal_2250": achieved / 2250.0,
+            "launches": n, "avg_launch_ms": ms / max(n, 1), "flops_per_launch": fl / max(n, 1),
+            "traffic": (traffic or {}).get(top),
+            "all_gemms": {"ms": tot_ms, "launches": tot_n, "tflops": tot_fl / (tot_ms * 1e-3) / 1e12 if tot_ms > 0 else 0.0,
+                          "frac": tot_fl / (tot_ms * 1e-3) / 1e12 / peak if tot_ms > 0 else 0.0, "per_kernel": per}}
+    return roof, tot_ms
+
+
 # ---- workloads ---------------------------------------------------------------------------------------------
 def encoder_workload(name, rank, n_records=None):
     """Seeded synthetic record stream + windows for BASELINE.json configs[1] ("base") or configs[3] ("large");
@@ -343,11 +375,10 @@ def run_encoder(args):
 
     if rank != 0:
         return
-    g_ms, g_fl, g_n = prof["gemm"]
+    default_shape = args.workload == "base" and args.records is None
+    roof, g_ms = gemm_rooflines(prof, peaks, NCU_TRAFFIC_BASE if default_shape else None)
     a_ms, a_fl, a_n = prof["attention"]
     r_ms, r_by, r_n = prof["row"]
-    peak = peaks["bf16_tflops_sustained"]
-    achieved = g_fl / (g_ms * 1e-3) / 1e12 if g_ms > 0 else 0.0
     out = {
         "metric": "ner_tokens_per_s", "value": tokens_all / sec, "unit": "tokens/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps, "higher_is_better": True,
@@ -361,13 +392,8 @@ def run_encoder(args):
         "e2e": {"value": e2e_tokens / e2e_sec, "unit": "tokens/s", "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "steps": n_e2e, "ms_per_step": 1e3 * e2e_sec / n_e2e,
                 "records_per_s": R * n_e2e * world / e2e_sec},
-        "roofline": {"bound": "tensor", "kernel": "gemm_bf16_tcgen05_kernel (QKV, out, FFN1, FFN2)",
-                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                     "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (%s)" % peaks["source"],
-                     "frac_of_burst_peak": achieved / peaks["bf16_tflops"], "frac_of_nominal_2250": achieved / 2250.0,
-                     "launches": g_n, "avg_launch_ms": g_ms / max(g_n, 1), "flops_per_launch": g_fl / max(g_n, 1),
-                     "traffic": None},
-        "breakdown_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
+        "roofline": roof,
+        "breakdown_ms_per_step": dict({k: v[0] / args.steps for k, v in prof.items()}, gemm=g_ms / args.steps),
         "attention_tflops": a_fl / (a_ms * 1e-3) / 1e12 if a_ms > 0 else None,
         "row_kernels_gbs": r_by / (r_ms * 1e-3) / 1e9 if r_ms > 0 else None,
     }
@@ -501,9 +527,7 @@ def run_stream(args):
     if rank != 0:
         return
     nb = len(batches)
-    g_ms, g_fl, g_n = prof["gemm"]
-    peak = peaks["bf16_tflops_sustained"]
-    achieved = g_fl / (g_ms * 1e-3) / 1e12 if g_ms > 0 else 0.0
+    roof, g_ms = gemm_rooflines(prof, peaks)
     a_ms, a_fl, _ = prof["attention"]
     r_ms, r_by, _ = prof["row"]
     out = {
@@ -525,13 +549,8 @@ def run_stream(args):
                 "d2h_bytes_per_step": int(d2h // nb), "steps": nb, "seconds_whole_stream": e2e_sec,
                 "tokens_per_s": T_all * world / e2e_sec, "kb_per_s": rec["text"].size / 1024.0 * world / e2e_sec,
                 "cache_hit_rate": st2["n_hits"] / max(st2["n_lookups"], 1)},
-        "roofline": {"bound": "tensor", "kernel": "gemm_bf16_tcgen05_kernel (QKV, out, FFN1, FFN2)",
-                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                     "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (%s)" % peaks["source"],
-                     "frac_of_burst_peak": achieved / peaks["bf16_tflops"], "frac_of_nominal_2250": achieved / 2250.0,
-                     "launches": g_n, "avg_launch_ms": g_ms / max(g_n, 1), "flops_per_launch": g_fl / max(g_n, 1),
-                     "traffic": None},
-        "breakdown_ms_per_step": {k: v[0] / nb for k, v in prof.items()},
+        "roofline": roof,
+        "breakdown_ms_per_step": dict({k: v[0] / nb for k, v in prof.items()}, gemm=g_ms / nb),
         "attention_tflops": a_fl / (a_ms * 1e-3) / 1e12 if a_ms > 0 else None,
         "row_kernels_gbs": r_by / (r_ms * 1e-3) / 1e9 if r_ms > 0 else None,
     }

@@ -76,9 +76,9 @@ const char* anon_last_cuda_error(anon_ctx* ctx);
 /* Launch accounting and per-kernel-class CUDA-event timing (bench.py's roofline / gpu_launches keys).
  * anon_ctx_profile(ctx, 1) synchronises, zeroes the counters and starts bracketing every launch group
  * with events on the context stream; (ctx, 0) stops.  anon_ctx_profile_read synchronises and returns,
- * for class c (0 = GEMM, 1 = attention, 2 = row kernels embed/LN/head, 3 = decode+gather,
- * 4 = pseudonymize; arrays of 8): summed event time in ms, algorithmic work (FLOPs for classes 0-1,
- * bytes for 2-3, 0 for 4), launches; and the total number of kernels launched since the last
+ * for class c (0 = QKV GEMM, 1 = attention, 2 = row kernels embed/LN/head, 3 = decode+gather+splice,
+ * 4 = pseudonymize, 5 = out-projection GEMM, 6 = FFN1+GELU GEMM, 7 = FFN2 GEMM; arrays of 8): summed event time in ms, algorithmic work (FLOPs for classes 0-1
+ * and 5-7, bytes for 2-3, 0 for 4), launches; and the total number of kernels launched since the last
  * anon_ctx_profile call (counted whether or not timing is enabled).  Any pointer may be NULL. */
 int  anon_ctx_profile(anon_ctx* ctx, int enable);
 int  anon_ctx_profile_read(anon_ctx* ctx, double* class_ms, double* class_work, int64_t* class_launches,

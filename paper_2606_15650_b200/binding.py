@@ -133,7 +133,7 @@ class Context:
         ln, tot = np.zeros(8, np.int64), np.zeros(1, np.int64)
         self.check(lib().anon_ctx_profile_read(self._h, ms.ctypes.data, work.ctypes.data, ln.ctypes.data, tot.ctypes.data),
                    "anon_ctx_profile_read")
-        names = ["gemm", "attention", "row", "decode", "pseudonymize"]
+        names = ["gemm_qkv", "attention", "row", "decode", "pseudonymize", "gemm_out", "gemm_ffn1", "gemm_ffn2"]
         return {n: (float(ms[i]), float(work[i]), int(ln[i])) for i, n in enumerate(names)}, int(tot[0])
 
     def close(self):

@@ -13,7 +13,10 @@
 #include "../../include/anonshield.h"
 
 // per-kernel-class CUDA-event timing (anon_ctx_profile): classes index ctx->prof_* arrays
-enum ProfClass { PROF_GEMM = 0, PROF_ATTN = 1, PROF_ROW = 2, PROF_DECODE = 3, PROF_PSEUDO = 4, PROF_NCLASS = 8 };
+// PROF_GEMM = QKV projection (bias epilogue); the other three GEMMs have classes of their own so that bench.py can put
+// the single dominant kernel against its roofline
+enum ProfClass { PROF_GEMM = 0, PROF_ATTN = 1, PROF_ROW = 2, PROF_DECODE = 3, PROF_PSEUDO = 4, PROF_GEMM_OUT = 5,
+                 PROF_GEMM_FFN1 = 6, PROF_GEMM_FFN2 = 7, PROF_NCLASS = 8 };
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
 struct anon_ctx {

@@ -233,12 +233,12 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                 rc = attention_run(ctx, plan, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx); }
                 if (rc) return rc;
                 if (fused_ln) {       // out-projection + residual + LayerNorm in one kernel, x updated in place
-                    ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * H * H);
+                    ProfScope ps(ctx, PROF_GEMM_OUT, 2.0 * nt * H * H);
                     rc = gemm_bf16_ln_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, L.g_1, L.b_1,
                                            d.ln_eps, x, xb, nt, H, H);
                     if (rc) return rc;
                 } else {
-                    { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * H * H);
+                    { ProfScope ps(ctx, PROF_GEMM_OUT, 2.0 * nt * H * H);
                     if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, y, nt, H, H, 2);
                     else rc = sgemm<2>(ctx, (const float*)cx, (const float*)L.W_o, L.b_o, x, y, nt, H, H); }
                     if (rc) return rc;
@@ -246,17 +246,17 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                     launch_layer_norm(st, row_grid, y, nt, H, L.g_1, L.b_1, d.ln_eps, x, xb); }
                     CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
                 }
-                { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * F * H);
+                { ProfScope ps(ctx, PROF_GEMM_FFN1, 2.0 * nt * F * H);
                 if (bf) rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_1, L.b_1f, nullptr, f, nt, F, H, 1);
                 else rc = sgemm<1>(ctx, x, (const float*)L.W_1, L.b_1f, nullptr, (float*)f, nt, F, H); }
                 if (rc) return rc;
                 if (fused_ln && fused_ffn2) {
-                    ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * F * H);
+                    ProfScope ps(ctx, PROF_GEMM_FFN2, 2.0 * nt * F * H);
                     rc = gemm_bf16_ln_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, x, L.g_2, L.b_2,
                                            d.ln_eps, x, xb, nt, H, F);
                     if (rc) return rc;
                 } else {
-                    { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * F * H);
+                    { ProfScope ps(ctx, PROF_GEMM_FFN2, 2.0 * nt * F * H);
                     if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, x, y, nt, H, F, 2);
                     else rc = sgemm<2>(ctx, (const float*)f, (const float*)L.W_2, L.b_2f, x, y, nt, H, F); }
                     if (rc) return rc;

@@ -147,6 +147,11 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     // block (the LayerNorm needs whole rows); the other epilogues take tiles round-robin.
     auto get_tile = [&](int lt, int& m_blk, int& n_blk) -> bool {
         if (EPI == 3) { m_blk = cid + (lt / num_n) * ncl; n_blk = lt % num_n; return m_blk < num_m; }
+        if (EPI <= 1 && num_m >= 2 * ncl) {
+            // short-K GEMMs with many row blocks: a pair keeps its row block of A (256 x K, L2-resident across the
+            // pairs) for all n-tiles, starting at a different n so that the pairs do not ask for the same W tile at once
+            m_blk = cid + (lt / num_n) * ncl; n_blk = (lt + cid) % num_n; return m_blk < num_m;
+        }
         const int tile = cid + lt * ncl;
         m_blk = tile / num_n; n_blk = tile % num_n;
         return tile < num_tiles;

@@ -238,35 +238,77 @@ __global__ void __launch_bounds__(128) hmac_spans_kernel(
 // ------------------------------------------------------------------------------------------------
 // K11 write-back
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) emit_tokens_kernel(
+// Each warp assembles the tokens of 32 consecutive spans -- a contiguous byte range of the output, since out_off is a
+// prefix sum -- in shared memory (word-aligned with the global destination) and then copies the range with coalesced
+// 4-byte stores; only the ragged first / last word of the range goes out byte by byte.  The type-name table is staged
+// in shared memory once per CTA (lanes index it with different types).
+constexpr int kEmitWarps = 8;
+constexpr int kEmitMaxToken = 3 + 32 + 64;                 // '[' name '_' slug ']'
+constexpr int kEmitWarpBytes = 32 * kEmitMaxToken + 8;     // + alignment slack
+
+__global__ void __launch_bounds__(kEmitWarps * 32) emit_tokens_kernel(
     long long S, const int* __restrict__ slot_of, const u64* __restrict__ table, const uint8_t* __restrict__ type,
     const uint32_t* __restrict__ digests, const long long* __restrict__ out_off, uint8_t* out,
     long long* uid_out, uint8_t* dig_out, TypeTable tt, int slug_len, int* d_status)
 {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= S) return;
-    const int s = slot_of[i];
-    if (s < 0) return;
-    const long long e = slot_index(table[s]);
-    if (uid_out) uid_out[i] = e;
-    const uint4* dg = (const uint4*)(digests + e * 8);
-    const uint4 d0 = __ldg(dg), d1 = __ldg(dg + 1);
-    if (dig_out) { uint4* q = (uint4*)(dig_out + i * 32); q[0] = d0; q[1] = d1; }
-    int t = type ? type[i] : 0;
-    if (t >= tt.num) { t = tt.num - 1; latch_status(d_status, ANON_ERR_UNSUPPORTED); }
-    uint8_t* o = out + out_off[i];
-    *o++ = '[';
-    const int nl = tt.len[t];
-    for (int k = 0; k < nl; k++) *o++ = (uint8_t)tt.name[t][k];
-    *o++ = '_';
-    const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};   // little-endian words = digest bytes in order
-#pragma unroll 1
-    for (int c = 0; c < slug_len; c++) {
-        const uint32_t byte = (dw[c >> 3] >> (8 * ((c >> 1) & 3))) & 0xFFu;
-        const uint32_t nib = (c & 1) ? (byte & 15u) : (byte >> 4);
-        *o++ = (uint8_t)(nib < 10 ? '0' + nib : 'a' + (nib - 10));
+    __shared__ __align__(16) uint8_t s_tok[kEmitWarps][(kEmitWarpBytes + 15) / 16 * 16];
+    __shared__ uint8_t s_name[64][32];
+    __shared__ uint8_t s_len[64];
+    for (int k = threadIdx.x; k < 64 * 32; k += blockDim.x) s_name[k >> 5][k & 31] = (uint8_t)tt.name[k >> 5][k & 31];
+    if (threadIdx.x < 64) s_len[threadIdx.x] = tt.len[threadIdx.x];
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long i0 = ((long long)blockIdx.x * kEmitWarps + warp) * 32;
+    if (i0 >= S) return;
+    const long long i = i0 + lane;
+    const bool live = i < S;
+    const long long last = (i0 + 32 < S ? i0 + 32 : S);
+    const long long b0 = out_off[i0], b1 = out_off[last];   // this warp's byte range of the output
+    const long long base = b0 & ~3ll;                       // shared-memory offset 0 <-> global byte `base`
+    uint8_t* buf = s_tok[warp];
+    if (live) {
+        const int s = slot_of[i];
+        if (s >= 0) {
+            const long long e = slot_index(table[s]);
+            if (uid_out) uid_out[i] = e;
+            const uint4* dg = (const uint4*)(digests + e * 8);
+            const uint4 d0 = __ldg(dg), d1 = __ldg(dg + 1);
+            if (dig_out) { uint4* q = (uint4*)(dig_out + i * 32); q[0] = d0; q[1] = d1; }
+            int t = type ? type[i] : 0;
+            if (t >= tt.num) { t = tt.num - 1; latch_status(d_status, ANON_ERR_UNSUPPORTED); }
+            uint8_t* o = buf + (out_off[i] - base);
+            *o++ = '[';
+            const int nl = s_len[t];
+            for (int k = 0; k < nl; k++) *o++ = s_name[t][k];
+            *o++ = '_';
+            const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};   // little-endian words = digest bytes in order
+#pragma unroll
+            for (int k = 0; k < 8; k++) {                   // 8 hex characters per digest word, static register indexing
+                if (8 * k >= slug_len) break;
+#pragma unroll
+                for (int j = 0; j < 8; j++) {
+                    if (8 * k + j < slug_len) {
+                        const uint32_t byte = (dw[k] >> (8 * (j >> 1))) & 0xFFu;
+                        const uint32_t nib = (j & 1) ? (byte & 15u) : (byte >> 4);
+                        o[8 * k + j] = (uint8_t)(nib < 10 ? '0' + nib : 'a' + (nib - 10));
+                    }
+                }
+            }
+            o[slug_len] = ']';
+        }
     }
-    *o = ']';
+    __syncwarp();
+    // coalesced copy of [b0, b1): whole words in between, bytes at the two ragged ends
+    const long long w_lo = (b0 + 3) >> 2, w_hi = b1 >> 2;   // global word indices fully inside the range
+    const uint32_t* bw = reinterpret_cast<const uint32_t*>(buf);
+    uint32_t* ow = reinterpret_cast<uint32_t*>(out);
+    if (w_lo <= w_hi) {
+        for (long long w = w_lo + lane; w < w_hi; w += 32) ow[w] = bw[w - (base >> 2)];
+        if (lane < 3) { const long long p = b0 + lane; if (p < (w_lo << 2) && p < b1) out[p] = buf[p - base]; }
+        if (lane >= 29) { const long long p = (w_hi << 2) + (lane - 29); if (p < b1 && p >= (w_lo << 2)) out[p] = buf[p - base]; }
+    } else {
+        for (long long p = b0 + lane; p < b1; p += 32) out[p] = buf[p - base];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -458,7 +500,7 @@ int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t*
             c->d_entry_off, (uint32_t*)c->d_digests, ps);
         CU_LAUNCH_CHECK(ctx, "cache_insert_kernel");
     }
-    emit_tokens_kernel<<<nb256, 256, 0, st>>>(S, slot_of, c->d_table, d_type, (const uint32_t*)c->d_digests,
+    emit_tokens_kernel<<<nb256, kEmitWarps * 32, 0, st>>>(S, slot_of, c->d_table, d_type, (const uint32_t*)c->d_digests,
                                                (const long long*)d_out_off, d_out, (long long*)d_uid, d_digests,
                                                tt, slug_len, ctx->d_status);
     CU_LAUNCH_CHECK(ctx, "emit_tokens_kernel");

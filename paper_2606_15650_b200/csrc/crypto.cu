@@ -56,12 +56,52 @@ __device__ __forceinline__ uint32_t load_le_word(const uint8_t* p, int len, int 
     return w;
 }
 
+// A byte string at any alignment read as consecutive little-endian 32-bit words, four at a time, through ALIGNED
+// 16-byte loads (one LDG.128 per 16 bytes instead of up to eight 4-byte loads; a thread-per-span kernel pays one L1
+// sector per load instruction, whatever its width).  Touches only aligned 16-byte chunks that contain at least one
+// byte of the message.  Words past the end of the message are not defined: callers mask with tail_mask().
+struct Words16 {
+    const uint4* q; const uint8_t* end; uint4 prev; uint32_t wo, sh;
+    __device__ __forceinline__ void init(const uint8_t* p, int len) {
+        const uintptr_t addr = (uintptr_t)p;
+        q = reinterpret_cast<const uint4*>(addr & ~(uintptr_t)15);
+        end = p + len;
+        wo = (uint32_t)(addr & 15) >> 2;
+        sh = 8u * (uint32_t)(addr & 3);
+        prev = len > 0 ? __ldg(q) : make_uint4(0u, 0u, 0u, 0u);
+    }
+    __device__ __forceinline__ void next4(uint32_t (&o)[4]) {
+        q++;
+        const uint4 cur = (reinterpret_cast<const uint8_t*>(q) < end) ? __ldg(q) : make_uint4(0u, 0u, 0u, 0u);
+        // window of 8 words (prev, cur); wanted: words wo .. wo+4, then a byte funnel shift by sh
+        uint32_t w0 = prev.x, w1 = prev.y, w2 = prev.z, w3 = prev.w, w4 = cur.x, w5 = cur.y, w6 = cur.z, w7 = cur.w;
+        if (wo & 2u) { w0 = w2; w1 = w3; w2 = w4; w3 = w5; w4 = w6; w5 = w7; }
+        if (wo & 1u) { w0 = w1; w1 = w2; w2 = w3; w3 = w4; w4 = w5; }
+        o[0] = __funnelshift_r(w0, w1, sh); o[1] = __funnelshift_r(w1, w2, sh);
+        o[2] = __funnelshift_r(w2, w3, sh); o[3] = __funnelshift_r(w3, w4, sh);
+        prev = cur;
+    }
+};
+// mask of word j of a len-byte message: all ones inside, partial on the last word, zero beyond
+__device__ __forceinline__ uint32_t tail_mask(int len, int j) {
+    const int rem = len - 4 * j;
+    return rem >= 4 ? 0xFFFFFFFFu : (rem <= 0 ? 0u : (1u << (8 * rem)) - 1u);
+}
+
 __device__ __forceinline__ u64 hash_bytes(const uint8_t* p, int len) {
     u64 h = 0x9E3779B97F4A7C15ull ^ ((u64)(uint32_t)len * 0xFF51AFD7ED558CCDull);
     const int nw = (len + 3) >> 2;
-    for (int j = 0; j < nw; j++) {
-        h = (h ^ load_le_word(p, len, j)) * 0xD6E8FEB86659FD93ull;
-        h ^= h >> 32;
+    Words16 ws; ws.init(p, len);
+    for (int j = 0; j < nw; j += 4) {
+        uint32_t w[4];
+        ws.next4(w);
+#pragma unroll
+        for (int k = 0; k < 4; k++) {
+            if (j + k < nw) {
+                h = (h ^ (w[k] & tail_mask(len, j + k))) * 0xD6E8FEB86659FD93ull;
+                h ^= h >> 32;
+            }
+        }
     }
     h ^= h >> 33; h *= 0xFF51AFD7ED558CCDull; h ^= h >> 33; h *= 0xC4CEB9FE1A85EC53ull; h ^= h >> 33;
     return h;
@@ -69,8 +109,15 @@ __device__ __forceinline__ u64 hash_bytes(const uint8_t* p, int len) {
 
 __device__ __forceinline__ bool bytes_equal(const uint8_t* a, const uint8_t* b, int len) {
     const int nw = (len + 3) >> 2;
-    for (int j = 0; j < nw; j++)
-        if (load_le_word(a, len, j) != load_le_word(b, len, j)) return false;
+    Words16 wa, wb; wa.init(a, len); wb.init(b, len);
+    for (int j = 0; j < nw; j += 4) {
+        uint32_t x[4], y[4];
+        wa.next4(x); wb.next4(y);
+        uint32_t diff = 0;
+#pragma unroll
+        for (int k = 0; k < 4; k++) diff |= (x[k] ^ y[k]) & tail_mask(len, j + k);
+        if (diff) return false;
+    }
     return true;
 }
 

@@ -97,8 +97,8 @@ def measured_peaks():
 GEMM_CLASSES = {"gemm_qkv": "QKV projection, +bias (N = 3H, K = H)", "gemm_out": "out-projection, +bias +FP32 residual (N = K = H)",
                 "gemm_ffn1": "FFN up, +bias +erf-GELU (N = F, K = H)", "gemm_ffn2": "FFN down, +bias +FP32 residual (N = H, K = F)"}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of gemm_bf16_tcgen05_kernel at the DEFAULT workload (configs[1],
-# M = 1,005,578 tokens), from one `ncu --set full` capture (profiles/r01_summary.md, "r01d"); other workloads: null
-NCU_TRAFFIC_BASE = {}
+# M = 1,005,578 tokens), from one `ncu --set full` capture (profiles/r01d_top_ncu_full.txt, summarised in profiles/r01_summary.md "r01d"); other workloads: null
+NCU_TRAFFIC_BASE = {"gemm_qkv": 6.246e9, "gemm_out": 8.126e9, "gemm_ffn1": 7.730e9, "gemm_ffn2": 16.853e9}   # bytes
 
 
 def gemm_rooflines(prof, peaks, traffic=None):

@@ -506,20 +506,23 @@ def run_stream(args):
     bufs = dict(spans=torch.zeros((cap, 4), dtype=torch.int32).pin_memory().numpy(),
                 out=torch.zeros(out_cap, dtype=torch.uint8).pin_memory().numpy(),
                 off=torch.zeros(cap + 1, dtype=torch.int64).pin_memory().numpy(),
-                hit=torch.zeros(cap, dtype=torch.uint8).pin_memory().numpy())
+                hit=torch.zeros(cap, dtype=torch.uint8).pin_memory().numpy(),
+                new_text=torch.zeros(max_text + out_cap, dtype=torch.uint8).pin_memory().numpy(),
+                new_ro=torch.zeros(max(b["rec_off"].size for b in batches), dtype=torch.int64).pin_memory().numpy())
     cache2 = P.Cache(ctx, 1 << 20, 64 << 20)
     barrier(world)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     h2d = d2h = 0
-    hits = 0
+    hits = out_text_bytes = 0
     e0.record()
     for hb in hbat:
         res = P.anon_pipeline_host(ctx, W, cache2, hb["ids"], hb["cu"], hb["meta"], hb["text"], hb["ro"], KEY, SLUG_LEN,
-                                   names, cap, out_cap, want_hit=True, bufs=bufs)
+                                   names, cap, out_cap, want_hit=True, bufs=bufs, want_text=True)     # text in -> text out
         Sh = len(res["spans"])
         hits += int(res["hit"].sum())
+        out_text_bytes += int(res["new_text"].size)
         h2d += hb["ids"].nbytes + hb["cu"].nbytes + hb["meta"].nbytes + hb["text"].nbytes + hb["ro"].nbytes
-        d2h += Sh * 16 + int(res["out_tokens"].size) + (Sh + 1) * 8 + Sh + 8
+        d2h += Sh * 16 + int(res["out_tokens"].size) + (Sh + 1) * 8 + Sh + 8 + int(res["new_text"].size) + hb["ro"].nbytes
     e1.record()
     barrier(world)
     e2e_recs, e2e_sec = sharding.aggregate_throughput(n_records, e0.elapsed_time(e1) / 1e3, dev)
@@ -548,7 +551,8 @@ def run_stream(args):
         "e2e": {"value": e2e_recs / e2e_sec, "unit": "records/s", "h2d_bytes_per_step": int(h2d // nb),
                 "d2h_bytes_per_step": int(d2h // nb), "steps": nb, "seconds_whole_stream": e2e_sec,
                 "tokens_per_s": T_all * world / e2e_sec, "kb_per_s": rec["text"].size / 1024.0 * world / e2e_sec,
-                "cache_hit_rate": st2["n_hits"] / max(st2["n_lookups"], 1)},
+                "cache_hit_rate": st2["n_hits"] / max(st2["n_lookups"], 1),
+                "call": "anon_pipeline_host_text: records in, rewritten records out", "rewritten_text_bytes": out_text_bytes},
         "roofline": roof,
         "breakdown_ms_per_step": dict({k: v[0] / nb for k, v in prof.items()}, gemm=g_ms / nb),
         "attention_tflops": a_fl / (a_ms * 1e-3) / 1e12 if a_ms > 0 else None,

@@ -210,6 +210,21 @@ int  anon_pipeline_host(anon_ctx* ctx, const anon_weights* w, anon_cache* cache,
                         uint8_t* h_out_tokens, size_t out_capacity, int64_t* h_out_offsets,
                         uint8_t* h_hit);
 
+/* Same, and the records come back REWRITTEN (stage 5 of the paper's pipeline, restricted to record text): after
+ * anon_pseudonymize the device splices every token over its span (anon_splice_records) and copies the new text
+ * (h_new_record_offsets[R] bytes) and its int64[R+1] record offsets to the host.  new_text_capacity must be at least
+ * text_bytes + the total token bytes (text_bytes + out_capacity always suffices), else ANON_ERR_CAPACITY. */
+int  anon_pipeline_host_text(anon_ctx* ctx, const anon_weights* w, anon_cache* cache,
+                             const int32_t* h_token_ids, const int32_t* h_cu_seqlens, int32_t B, int32_t T,
+                             const anon_tok_meta* h_meta, const uint8_t* h_text, size_t text_bytes,
+                             const int64_t* h_record_offsets, int32_t R,
+                             const uint8_t* key, size_t key_len, int32_t slug_len,
+                             const char* const* type_names, int32_t num_types,
+                             anon_span* h_spans, int32_t span_capacity, int32_t* h_num_spans,
+                             uint8_t* h_out_tokens, size_t out_capacity, int64_t* h_out_offsets,
+                             uint8_t* h_hit,
+                             uint8_t* h_new_text, size_t new_text_capacity, int64_t* h_new_record_offsets);
+
 /* ---- building blocks exported for parity tests and per-kernel roofline measurement ----------- */
 /* C[M,N] = A[M,K] * W[N,K]^T + bias[N], BF16 operands, FP32 accumulate on the tcgen05
  * tensor cores (S8a A2/A4/A5/A6).  epilogue: 0 = bias -> BF16 out; 1 = bias, erf-GELU ->

@@ -61,6 +61,9 @@ _SIGNATURES = {
     "anon_hmac_spans": (ctypes.c_int, [_vp, _vp, _vp, _i64, _vp, _sz, _vp]),
     "anon_pipeline_host": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _vp, _sz, _vp, _i32, _vp, _sz, _i32,
                                           ctypes.POINTER(ctypes.c_char_p), _i32, _vp, _i32, _vp, _vp, _sz, _vp, _vp]),
+    "anon_pipeline_host_text": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _vp, _sz, _vp, _i32, _vp, _sz, _i32,
+                                               ctypes.POINTER(ctypes.c_char_p), _i32, _vp, _i32, _vp, _vp, _sz, _vp, _vp,
+                                               _vp, _sz, _vp]),
     "anon_ctx_profile": (ctypes.c_int, [_vp, ctypes.c_int]),
     "anon_ctx_profile_read": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "anon_gemm_bf16": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32]),
@@ -279,20 +282,33 @@ def anon_attention(ctx, qkv, cu_seqlens_dev, cu_seqlens_host, hidden, heads, dty
 
 
 def anon_pipeline_host(ctx, weights, cache, token_ids, cu_seqlens, meta, text, record_offsets, key, slug_len,
-                       type_names, span_capacity, out_capacity, want_hit=True, bufs=None):
-    """Whole hot path on HOST numpy buffers (pinned or pageable).  Returns dict(spans, out_tokens, out_offsets, hit)."""
+                       type_names, span_capacity, out_capacity, want_hit=True, bufs=None, want_text=False):
+    """Whole hot path on HOST numpy buffers (pinned or pageable).  Returns dict(spans, out_tokens, out_offsets, hit);
+    with want_text=True (anon_pipeline_host_text) also new_text and new_record_offsets, the rewritten records."""
     T, B, R = token_ids.size, cu_seqlens.size - 1, record_offsets.size - 1
     if bufs is None:
         bufs = dict(spans=np.zeros((span_capacity, 4), np.int32), out=np.zeros(out_capacity, np.uint8),
                     off=np.zeros(span_capacity + 1, np.int64), hit=np.zeros(span_capacity, np.uint8))
     n = _i32(0)
     k = np.frombuffer(bytes(key), np.uint8)
-    rc = lib().anon_pipeline_host(ctx._h, weights._h, cache._h, _ptr(token_ids), _ptr(cu_seqlens), B, T, _ptr(meta),
-                                  _ptr(text), text.size, _ptr(record_offsets), R, k.ctypes.data if k.size else None, k.size,
-                                  slug_len, _names(type_names), len(type_names), _ptr(bufs["spans"]), span_capacity,
-                                  ctypes.byref(n), _ptr(bufs["out"]), out_capacity, _ptr(bufs["off"]),
-                                  _ptr(bufs["hit"]) if want_hit else None)
-    ctx.check(rc, "anon_pipeline_host")
+    args = [ctx._h, weights._h, cache._h, _ptr(token_ids), _ptr(cu_seqlens), B, T, _ptr(meta),
+            _ptr(text), text.size, _ptr(record_offsets), R, k.ctypes.data if k.size else None, k.size,
+            slug_len, _names(type_names), len(type_names), _ptr(bufs["spans"]), span_capacity,
+            ctypes.byref(n), _ptr(bufs["out"]), out_capacity, _ptr(bufs["off"]),
+            _ptr(bufs["hit"]) if want_hit else None]
+    if want_text:
+        if "new_text" not in bufs:
+            bufs["new_text"] = np.zeros(text.size + out_capacity, np.uint8)
+            bufs["new_ro"] = np.zeros(R + 1, np.int64)
+        rc = lib().anon_pipeline_host_text(*args, _ptr(bufs["new_text"]), bufs["new_text"].size, _ptr(bufs["new_ro"]))
+        ctx.check(rc, "anon_pipeline_host_text")
+    else:
+        ctx.check(lib().anon_pipeline_host(*args), "anon_pipeline_host")
     S = n.value
     off = bufs["off"][:S + 1]
-    return {"spans": bufs["spans"][:S], "out_tokens": bufs["out"][:off[S]], "out_offsets": off, "hit": bufs["hit"][:S]}
+    res = {"spans": bufs["spans"][:S], "out_tokens": bufs["out"][:off[S]], "out_offsets": off, "hit": bufs["hit"][:S]}
+    if want_text:
+        ro = bufs["new_ro"][:R + 1]
+        res["new_record_offsets"] = ro
+        res["new_text"] = bufs["new_text"][:ro[R]]
+    return res

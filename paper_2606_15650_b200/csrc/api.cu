@@ -22,7 +22,7 @@ extern "C" const char* const* anon_exported_symbols(void) {
         "anon_last_cuda_error", "anon_workspace_bytes", "anon_weights_load", "anon_weights_free", "anon_ner_forward",
         "anon_decode_spans", "anon_gather_spans", "anon_cache_create", "anon_cache_destroy", "anon_cache_stats", "anon_cache_clear",
         "anon_cache_entry", "anon_pseudonymize", "anon_hmac_spans", "anon_pipeline_host", "anon_gemm_bf16",
-        "anon_attention", "anon_gemm_bf16_ln", "anon_splice_records", "anon_ctx_profile", "anon_ctx_profile_read", nullptr};
+        "anon_attention", "anon_gemm_bf16_ln", "anon_splice_records", "anon_pipeline_host_text", "anon_ctx_profile", "anon_ctx_profile_read", nullptr};
     return names;
 }
 
@@ -105,13 +105,19 @@ extern "C" int anon_ctx_profile_read(anon_ctx* ctx, double* class_ms, double* cl
 
 extern "C" const char* anon_last_cuda_error(anon_ctx* ctx) { return ctx ? ctx->cuda_err : ""; }
 
-extern "C" int anon_pipeline_host(anon_ctx* ctx, const anon_weights* w, anon_cache* cache,
-                                  const int32_t* h_ids, const int32_t* h_cu, int32_t B, int32_t T,
-                                  const anon_tok_meta* h_meta, const uint8_t* h_text, size_t text_bytes,
-                                  const int64_t* h_rec_off, int32_t R, const uint8_t* key, size_t key_len,
-                                  int32_t slug_len, const char* const* type_names, int32_t num_types,
-                                  anon_span* h_spans, int32_t span_capacity, int32_t* h_num_spans,
-                                  uint8_t* h_out_tokens, size_t out_capacity, int64_t* h_out_offsets, uint8_t* h_hit)
+int splice_records_impl(anon_ctx* ctx, WsCursor& ws, const uint8_t* d_text, size_t text_bytes, const int64_t* d_rec_off, int32_t R,
+                        const anon_span* d_spans, int32_t S, const uint8_t* d_tok, const int64_t* d_tok_off,
+                        uint8_t* d_new_text, size_t cap, int64_t* d_new_rec_off);
+
+// h_new_text != NULL: the records are also rewritten on the device (NEXT-1) and come back as text
+static int pipeline_host_impl(anon_ctx* ctx, const anon_weights* w, anon_cache* cache,
+                              const int32_t* h_ids, const int32_t* h_cu, int32_t B, int32_t T,
+                              const anon_tok_meta* h_meta, const uint8_t* h_text, size_t text_bytes,
+                              const int64_t* h_rec_off, int32_t R, const uint8_t* key, size_t key_len,
+                              int32_t slug_len, const char* const* type_names, int32_t num_types,
+                              anon_span* h_spans, int32_t span_capacity, int32_t* h_num_spans,
+                              uint8_t* h_out_tokens, size_t out_capacity, int64_t* h_out_offsets, uint8_t* h_hit,
+                              uint8_t* h_new_text, size_t new_text_capacity, int64_t* h_new_rec_off)
 {
     if (!ctx || !w || !cache || !h_ids || !h_cu || !h_meta || !h_text || !h_rec_off || !h_spans || !h_num_spans ||
         !h_out_tokens || !h_out_offsets || B < 0 || T < 0 || R < 0 || span_capacity < 0)
@@ -137,6 +143,9 @@ extern "C" int anon_pipeline_host(anon_ctx* ctx, const anon_weights* w, anon_cac
     // span bytes can never exceed the text that was scanned
     uint8_t* d_span_bytes = (uint8_t*)ws.take(text_bytes + 16);
     uint8_t* d_out = (uint8_t*)ws.take(out_capacity + 16);
+    uint8_t* d_new_text = h_new_text ? (uint8_t*)ws.take(new_text_capacity + 16) : nullptr;
+    int64_t* d_new_rec_off = h_new_text ? (int64_t*)ws.take(((size_t)R + 1) * 8) : nullptr;
+    if (h_new_text && (!d_new_text || !d_new_rec_off || !h_new_rec_off)) return d_new_text ? ANON_ERR_INVALID_ARG : ANON_ERR_OOM;
     if (!d_ids || !d_cu || !d_meta || !d_text || !d_rec_off || !d_labels || !d_spans || !d_num || !d_span_off ||
         !d_span_type || !d_out_off || !d_hit || !d_span_bytes || !d_out)
         return ANON_ERR_OOM;
@@ -179,6 +188,17 @@ extern "C" int anon_pipeline_host(anon_ctx* ctx, const anon_weights* w, anon_cac
                                num_types, d_out, out_capacity, d_out_off, h_hit ? d_hit : nullptr, nullptr, nullptr, &out_bytes);
         if (rc) return rc;
     }
+    if (h_new_text) {
+        if ((uint64_t)text_bytes + (uint64_t)out_bytes > new_text_capacity) return ANON_ERR_CAPACITY;     // safe upper bound
+        WsCursor c = ws;
+        rc = splice_records_impl(ctx, c, d_text, text_bytes, d_rec_off, R, d_spans, S, d_out, d_out_off, d_new_text,
+                                 new_text_capacity, d_new_rec_off);
+        if (rc) return rc;
+        CU_TRY(ctx, cudaMemcpyAsync(h_new_rec_off, d_new_rec_off, ((size_t)R + 1) * 8, cudaMemcpyDeviceToHost, st));
+        CU_TRY(ctx, cudaStreamSynchronize(st));
+        const int64_t new_bytes = h_new_rec_off[R];
+        if (new_bytes > 0) CU_TRY(ctx, cudaMemcpyAsync(h_new_text, d_new_text, (size_t)new_bytes, cudaMemcpyDeviceToHost, st));
+    }
     if (S > 0) {
         CU_TRY(ctx, cudaMemcpyAsync(h_spans, d_spans, (size_t)S * sizeof(anon_span), cudaMemcpyDeviceToHost, st));
         CU_TRY(ctx, cudaMemcpyAsync(h_out_tokens, d_out, (size_t)out_bytes, cudaMemcpyDeviceToHost, st));
@@ -186,4 +206,32 @@ extern "C" int anon_pipeline_host(anon_ctx* ctx, const anon_weights* w, anon_cac
     }
     CU_TRY(ctx, cudaMemcpyAsync(h_out_offsets, d_out_off, ((size_t)S + 1) * 8, cudaMemcpyDeviceToHost, st));
     return anon_ctx_sync(ctx);
+}
+
+extern "C" int anon_pipeline_host(anon_ctx* ctx, const anon_weights* w, anon_cache* cache,
+                                  const int32_t* h_ids, const int32_t* h_cu, int32_t B, int32_t T,
+                                  const anon_tok_meta* h_meta, const uint8_t* h_text, size_t text_bytes,
+                                  const int64_t* h_rec_off, int32_t R, const uint8_t* key, size_t key_len,
+                                  int32_t slug_len, const char* const* type_names, int32_t num_types,
+                                  anon_span* h_spans, int32_t span_capacity, int32_t* h_num_spans,
+                                  uint8_t* h_out_tokens, size_t out_capacity, int64_t* h_out_offsets, uint8_t* h_hit)
+{
+    return pipeline_host_impl(ctx, w, cache, h_ids, h_cu, B, T, h_meta, h_text, text_bytes, h_rec_off, R, key, key_len, slug_len,
+                              type_names, num_types, h_spans, span_capacity, h_num_spans, h_out_tokens, out_capacity,
+                              h_out_offsets, h_hit, nullptr, 0, nullptr);
+}
+
+extern "C" int anon_pipeline_host_text(anon_ctx* ctx, const anon_weights* w, anon_cache* cache,
+                                       const int32_t* h_ids, const int32_t* h_cu, int32_t B, int32_t T,
+                                       const anon_tok_meta* h_meta, const uint8_t* h_text, size_t text_bytes,
+                                       const int64_t* h_rec_off, int32_t R, const uint8_t* key, size_t key_len,
+                                       int32_t slug_len, const char* const* type_names, int32_t num_types,
+                                       anon_span* h_spans, int32_t span_capacity, int32_t* h_num_spans,
+                                       uint8_t* h_out_tokens, size_t out_capacity, int64_t* h_out_offsets, uint8_t* h_hit,
+                                       uint8_t* h_new_text, size_t new_text_capacity, int64_t* h_new_record_offsets)
+{
+    if (!h_new_text || !h_new_record_offsets) return ANON_ERR_INVALID_ARG;
+    return pipeline_host_impl(ctx, w, cache, h_ids, h_cu, B, T, h_meta, h_text, text_bytes, h_rec_off, R, key, key_len, slug_len,
+                              type_names, num_types, h_spans, span_capacity, h_num_spans, h_out_tokens, out_capacity,
+                              h_out_offsets, h_hit, h_new_text, new_text_capacity, h_new_record_offsets);
 }

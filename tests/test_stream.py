@@ -85,12 +85,14 @@ def test_stream_batches_match_oracle_on_gpu():
     ctx = P.Context(0, workspace_bytes=256 << 20)
     W = P.Weights(ctx, d, gen.pack_blob(w))
     cache = P.Cache(ctx, 4096, 1 << 20)
-    got_spans, got_tok, got_hit, got_len = [], [], [], []
+    got_spans, got_tok, got_hit, got_len, got_text, got_ro = [], [], [], [], [], []
     for a, b in plan:
         bt = stream.slice_batch(rec, win, a, b)
         T = bt["token_ids"].size
         res = P.anon_pipeline_host(ctx, W, cache, bt["token_ids"], bt["cu_seqlens"], bt["meta"], bt["text"], bt["rec_off"],
-                                   key, 10, names, span_capacity=T, out_capacity=T * 32)
+                                   key, 10, names, span_capacity=T, out_capacity=T * 32, want_text=True)
+        got_text.append(res["new_text"].copy())
+        got_ro.append(res["new_record_offsets"].copy())
         sp = res["spans"].copy()
         sp[:, 0] += bt["r0"]
         got_spans.append(sp)
@@ -104,3 +106,8 @@ def test_stream_batches_match_oracle_on_gpu():
     assert np.array_equal(np.concatenate(got_hit), want["hit"])
     assert np.array_equal(np.concatenate(got_len), np.diff(want["out_offsets"]))
     assert st["n_lookups"] == len(spans) and st["n_hits"] == int(want["hit"].sum())
+    # text in -> text out: the batches' rewritten records, concatenated, are the oracle's splice of the whole stream
+    want_text, want_ro = decode.splice_records(rec["text"], rec["rec_off"], spans, want["out_tokens"], want["out_offsets"])
+    assert np.array_equal(np.concatenate(got_text), want_text)
+    sizes = np.concatenate([np.diff(r) for r in got_ro])
+    assert np.array_equal(sizes, np.diff(want_ro))

@@ -106,8 +106,10 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
         // ===== TMA producer =====
         if (lane == 0) {
             uint32_t qi = 0, g = 0;
+            WorkItem wn = work[min((int)blockIdx.x, n_units - 1) / heads];     // next unit's item, loaded one unit ahead
             for (int u = blockIdx.x; u < n_units; u += gridDim.x, qi++) {
-                const WorkItem w = work[u / heads];
+                const WorkItem w = wn;
+                if (u + (int)gridDim.x < n_units) wn = work[(u + (int)gridDim.x) / heads];
                 const int head = u % heads;
                 const uint32_t qb = qi & 1u;
                 ptx::mbar_wait_backoff(q_empty(qb), ((qi >> 1) & 1u) ^ 1u);
@@ -129,11 +131,14 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
         if (lane == 0) {
             constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(kQT, kKC);          // both operands K-major
             constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(kQT, kD, 1);        // B = V is MN-major
-            struct Cur { int u, c, nc; uint32_t qi, g; };
-            auto load = [&](Cur& k) { k.c = 0; k.nc = k.u < n_units ? (work[k.u / heads].n + kKC - 1) / kKC : 0; };
-            auto advance = [&](Cur& k) { k.g++; if (++k.c == k.nc) { k.u += gridDim.x; k.qi++; load(k); } };
-            Cur a{(int)blockIdx.x, 0, 0, 0u, 0u}, b = a;
-            load(a); load(b);
+            // nc_next = chunk count of the unit after the cursor's, loaded one unit ahead so that no MMA waits on it
+            struct Cur { int u, c, nc, nc_next; uint32_t qi, g; };
+            auto chunks_of = [&](int u) { return u < n_units ? (work[u / heads].n + kKC - 1) / kKC : 0; };
+            auto advance = [&](Cur& k) {
+                k.g++;
+                if (++k.c == k.nc) { k.u += gridDim.x; k.qi++; k.c = 0; k.nc = k.nc_next; k.nc_next = chunks_of(k.u + (int)gridDim.x); }
+            };
+            Cur a{(int)blockIdx.x, 0, chunks_of((int)blockIdx.x), chunks_of((int)blockIdx.x + (int)gridDim.x), 0u, 0u}, b = a;
             auto issue_qk = [&]() {
                 const uint32_t qb = a.qi & 1u, st = a.g % kKVStages, sb = a.g & 1u;
                 if (a.c == 0) ptx::mbar_wait(q_full(qb), (a.qi >> 1) & 1u);
@@ -201,8 +206,10 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             }
             pend = false;
         };
+        WorkItem wn = work[min((int)blockIdx.x, n_units - 1) / heads];         // next unit's item, loaded one unit ahead
         for (int u = blockIdx.x; u < n_units; u += gridDim.x, qi++) {
-            const WorkItem w = work[u / heads];
+            const WorkItem w = wn;
+            if (u + (int)gridDim.x < n_units) wn = work[(u + (int)gridDim.x) / heads];
             const int head = u % heads;
             const int nc = (w.n + kKC - 1) / kKC;
             float m = -INFINITY, l = 0.f;                                // reference max (scaled, log2 domain), row sum

@@ -108,6 +108,8 @@ int pseudonymize_impl(anon_ctx*, WsCursor&, anon_cache*, const uint8_t* d_bytes,
                       int64_t* total_out_bytes);
 int gemm_bf16_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias,
                    const float* residual, void* C, int M, int N, int K, int epilogue);
+int gemm_bf16_res_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* res_y,
+                          const float2* res_stats, const float* gamma, const float* beta, float* C, int M, int N, int K);
 // x = LN(A W^T + bias + residual; gamma, beta) as FP32 (x_out may alias residual) plus its BF16 copy; N % 256 == 0
 int gemm_bf16_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
                       const float* gamma, const float* beta, float eps, float* x_out, __nv_bfloat16* xb_out, int M, int N, int K);

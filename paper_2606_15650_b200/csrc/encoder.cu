@@ -53,7 +53,7 @@ size_t desc_floats(const anon_model_desc& d) {
 
 size_t per_token_bytes(const anon_model_desc& d) {
     const size_t H = d.hidden, F = d.ffn;
-    if (d.dtype == 1) return 4 * H + 2 * H + 4 * H + 6 * H + 2 * H + 2 * F;
+    if (d.dtype == 1) return 4 * H + 2 * H + 4 * H + 6 * H + 2 * H + 2 * F + 8;
     return 4 * H + 4 * H + 12 * H + 4 * H + 4 * F;
 }
 
@@ -144,10 +144,10 @@ const anon_model_desc* weights_desc(const anon_weights* w) { return &w->d; }
 
 // K4 launcher: compile-time row length for the BF16 shapes (H = 768, 1024), generic kernel otherwise
 static void launch_layer_norm(cudaStream_t st, unsigned grid, const float* y, int nt, int H, const float* g, const float* b,
-                              float eps, float* x, __nv_bfloat16* xb)
+                              float eps, float* x, __nv_bfloat16* xb, float2* stats = nullptr)
 {
-    if (xb && H == 768) enc::layer_norm_fixed_kernel<6><<<grid, enc::kRowWarps * 32, 0, st>>>(y, nt, g, b, eps, x, xb);
-    else if (xb && H == 1024) enc::layer_norm_fixed_kernel<8><<<grid, enc::kRowWarps * 32, 0, st>>>(y, nt, g, b, eps, x, xb);
+    if (xb && H == 768) enc::layer_norm_fixed_kernel<6><<<grid, enc::kRowWarps * 32, 0, st>>>(y, nt, g, b, eps, x, xb, stats);
+    else if (xb && H == 1024) enc::layer_norm_fixed_kernel<8><<<grid, enc::kRowWarps * 32, 0, st>>>(y, nt, g, b, eps, x, xb, stats);
     else enc::layer_norm_kernel<<<grid, enc::kRowWarps * 32, 0, st>>>(y, nullptr, nt, H, g, b, eps, x, xb);
 }
 
@@ -222,7 +222,48 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                     d.ln_eps, H, d.vocab, d.max_pos, x, nullptr, ctx->d_status);
             }
             CU_LAUNCH_CHECK(ctx, "embed_ln_kernel");
-            for (int l = 0; l < d.layers; l++) {
+            // BF16 path with H = 768 / 1024: the residual stream is carried UN-normalised.  The LayerNorm kernel writes only
+            // the BF16 operand copy xb and the row statistics; the next residual GEMM normalises the residual on the fly in
+            // its epilogue and writes the new un-normalised rows (ping-pong between x and y: in-place updates measured 20 %
+            // slower).  Saves the FP32 write of x (4H bytes per token and LayerNorm).  Only the last LayerNorm writes the
+            // normalised FP32 rows (into y) for the classifier head.
+            const bool lazy_ln = bf && (H == 768 || H == 1024);
+            const float* head_in = x;
+            if (lazy_ln) {
+                float2* stats = (float2*)c.take((size_t)nt * 8);
+                if (!stats) return ANON_ERR_OOM;
+                const float2* pst = nullptr; const float* pg = nullptr; const float* pb = nullptr;   // embedding output: already normal
+                const double ln_bytes = (double)nt * (H * 4 + H * 2 + 8);
+                for (int l = 0; l < d.layers; l++) {
+                    const LayerW& L = w->layers[l];
+                    const bool last = l == d.layers - 1;
+                    int rc;
+                    { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * 3 * H * H);
+                    rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_qkv, L.b_qkv, nullptr, qkv, nt, 3 * H, H, 0); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_ATTN, attn_flops);
+                    rc = attention_run(ctx, plan, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_GEMM_OUT, 2.0 * nt * H * H);
+                    rc = gemm_bf16_res_ln_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, pst, pg, pb, y, nt, H, H); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_ROW, ln_bytes);
+                    launch_layer_norm(st, row_grid, y, nt, H, L.g_1, L.b_1, d.ln_eps, nullptr, xb, stats); }
+                    CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+                    { ProfScope ps(ctx, PROF_GEMM_FFN1, 2.0 * nt * F * H);
+                    rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_1, L.b_1f, nullptr, f, nt, F, H, 1); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_GEMM_FFN2, 2.0 * nt * F * H);
+                    rc = gemm_bf16_res_ln_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, y, stats, L.g_1, L.b_1, x, nt, H, F); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_ROW, ln_bytes + (last ? (double)nt * H * 4 : 0.0));
+                    launch_layer_norm(st, row_grid, x, nt, H, L.g_2, L.b_2, d.ln_eps, last ? y : nullptr, xb, stats); }
+                    CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+                    pst = stats; pg = L.g_2; pb = L.b_2;
+                    if (last) head_in = y;
+                }
+            }
+            for (int l = 0; l < (lazy_ln ? 0 : d.layers); l++) {
                 const LayerW& L = w->layers[l];
                 int rc;
                 { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * 3 * H * H);
@@ -267,7 +308,7 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
             }
             { ProfScope ps(ctx, PROF_ROW, (double)nt * (H * 4 + (d_logits ? NL * 4 : 0) + (d_labels ? 4 : 0)));
             enc::head_argmax_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(
-                x, nt, H, w->W_c, w->b_c, NL, d_logits ? d_logits + (size_t)tok0 * NL : nullptr,
+                head_in, nt, H, w->W_c, w->b_c, NL, d_logits ? d_logits + (size_t)tok0 * NL : nullptr,
                 d_labels ? d_labels + tok0 : nullptr); }
             CU_LAUNCH_CHECK(ctx, "head_argmax_kernel");
         }

@@ -112,8 +112,10 @@ static __global__ void __launch_bounds__(kRowWarps * 32) layer_norm_kernel(
 template <int N4>
 static __global__ void __launch_bounds__(kRowWarps * 32, (N4 <= 6) ? 5 : 4) layer_norm_fixed_kernel(
     const float* __restrict__ y, int ntok, const float* __restrict__ g, const float* __restrict__ b, float eps,
-    float* __restrict__ x, __nv_bfloat16* __restrict__ xb)
+    float* __restrict__ x, __nv_bfloat16* __restrict__ xb, float2* __restrict__ stats)
 {
+    // x == NULL: the FP32 row is not written; the consumer (the next residual GEMM's epilogue) recomputes it from y and
+    // stats[row] = (mean, rstd), which saves 4H bytes of HBM writes per token
     constexpr int H = 128 * N4;
     const int lane = threadIdx.x & 31;
     const int r = blockIdx.x * kRowWarps + (threadIdx.x >> 5);
@@ -133,6 +135,7 @@ static __global__ void __launch_bounds__(kRowWarps * 32, (N4 <= 6) ? 5 : 4) laye
         q += (v[k].x * v[k].x + v[k].y * v[k].y) + (v[k].z * v[k].z + v[k].w * v[k].w);
     }
     const float rstd = 1.0f / sqrtf(warp_sum(q) * (1.0f / (float)H) + eps);
+    if (stats && lane == 0) stats[r] = make_float2(mean, rstd);
     float4* xo = reinterpret_cast<float4*>(x + (size_t)r * H) + lane;
     uint2* xbo = reinterpret_cast<uint2*>(xb + (size_t)r * H) + lane;
 #pragma unroll
@@ -142,7 +145,7 @@ static __global__ void __launch_bounds__(kRowWarps * 32, (N4 <= 6) ? 5 : 4) laye
         float4 o;
         o.x = v[k].x * rstd * gg.x + bb.x; o.y = v[k].y * rstd * gg.y + bb.y;
         o.z = v[k].z * rstd * gg.z + bb.z; o.w = v[k].w * rstd * gg.w + bb.w;
-        xo[32 * k] = o;
+        if (x) xo[32 * k] = o;
         __nv_bfloat162 lo = __floats2bfloat162_rn(o.x, o.y), hi = __floats2bfloat162_rn(o.z, o.w);
         uint2 u;
         u.x = *reinterpret_cast<uint32_t*>(&lo); u.y = *reinterpret_cast<uint32_t*>(&hi);

@@ -40,10 +40,10 @@ template <int BN, int EPI, int NB, int CG> struct Cfg {
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
     static constexpr int EPI_WARPS = (EPI >= 2) ? 4 : 8;
     static constexpr int PAR_BYTES = 3 * 1024 * 4;                // EPI 3: bias, gamma, beta staged in shared memory (N <= 1024)
-    static constexpr int EPI_BYTES = (EPI == 3) ? 4 * (NB + 1) * 4096 + PAR_BYTES : (EPI == 2) ? 4 * NB * 4096 : 8 * 4096;   // 4 KB boxes
+    static constexpr int EPI_BYTES = (EPI == 3) ? 4 * (NB + 1) * 4096 + PAR_BYTES : (EPI == 2) ? 4 * NB * 4096 + 12288 /*bias, gamma, beta staged for the epilogue*/ : 8 * 4096;   // 4 KB boxes
     static constexpr int STAGES = (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES > 6 ? 6 : (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES;
     static constexpr int TMEM_COLS = 2 * BN;                      // two accumulator buffers
-    static constexpr int NUM_BARS = 2 * STAGES + 4 + 16;
+    static constexpr int NUM_BARS = 2 * STAGES + 4 + 32;
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + EPI_BYTES + 1024 /*align slack*/ + 512 /*barriers*/;
 };
 
@@ -121,7 +121,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                          const __grid_constant__ CUtensorMap tmap_c, const __grid_constant__ CUtensorMap tmap_r,
                          const __grid_constant__ CUtensorMap tmap_y, const __grid_constant__ CUtensorMap tmap_xb,
                          const float* __restrict__ bias, const float* __restrict__ ln_g, const float* __restrict__ ln_b,
-                         float ln_eps, int M, int N, int K)
+                         float ln_eps, const float2* __restrict__ res_stats, int M, int N, int K)
 {
     using C = Cfg<BN, EPI, NB, CG>;
     extern __shared__ uint8_t smem_raw[];
@@ -132,7 +132,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     auto empty_bar = [&](int s) { return bar_base + 8u * (C::STAGES + s); };
     auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * C::STAGES + a); };
     auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * C::STAGES + 2 + a); };
-    auto rfull_bar = [&](int q, int b) { return bar_base + 8u * (2 * C::STAGES + 4 + 4 * q + b); };
+    auto rfull_bar = [&](int q, int b) { return bar_base + 8u * (2 * C::STAGES + 4 + 8 * q + b); };      // up to 8 boxes per warp
     const uint32_t tmem_slot = bar_base + 8u * C::NUM_BARS;
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
@@ -167,13 +167,23 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < C::STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
         for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), CG * C::EPI_WARPS); }
-        for (int i = 0; i < 16; i++) ptx::mbar_init(rfull_bar(i >> 2, i & 3), 1);
+        for (int i = 0; i < 32; i++) ptx::mbar_init(rfull_bar(i >> 3, i & 7), 1);
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
     }
     if constexpr (EPI == 3) {             // bias / gamma / beta -> shared memory (every thread reads all N of them per row)
         float* par = reinterpret_cast<float*>(smem_raw + (epi_base + 4 * (NB + 1) * 4096 - ptx::smem_u32(smem_raw)));
         for (int i = threadIdx.x; i < N; i += kThreads) { par[i] = bias[i]; par[1024 + i] = ln_g[i]; par[2048 + i] = ln_b[i]; }
+    }
+    if constexpr (EPI == 2) {             // bias (and gamma / beta of the residual's LayerNorm) -> shared memory: every
+        if (N <= 1024) {                  // epilogue thread reads all N of them per row
+            float* par = reinterpret_cast<float*>(smem_raw + (epi_base + 4 * NB * 4096 - ptx::smem_u32(smem_raw)));
+            for (int i = threadIdx.x; i < N; i += kThreads) {
+                par[i] = bias[i];
+                par[1024 + i] = res_stats ? ln_g[i] : 1.f;
+                par[2048 + i] = res_stats ? ln_b[i] : 0.f;
+            }
+        }
     }
     if (warp == 2) {
         if (CG == 2) { ptx::tmem_alloc_cg2(tmem_slot, C::TMEM_COLS); ptx::tmem_relinquish_cg2(); }
@@ -405,6 +415,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         } else if constexpr (EPI == 2) {
             constexpr int BPT = BN / 32;              // 32x32 FP32 boxes per tile per warp
             const uint32_t stg = epi_base + (uint32_t)(q * NB * 4096);
+            const uint32_t par_base = epi_base + 4u * NB * 4096u;      // gamma | beta, 1024 floats each
             uint32_t rph = 0;                         // phase bit of each residual buffer's barrier
             auto issue_load = [&](uint32_t i) {       // lane 0: residual box i -> buffer i % NB
                 const int tile = cid + (int)(i / BPT) * ncl;
@@ -417,8 +428,22 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             };
             if (lane == 0) { for (uint32_t i = 0; i + 1 < NB; i++) issue_load(i); }
             int m_blk, n_blk;
+            float2 st_next = make_float2(0.f, 1.f);
+            if (res_stats && get_tile(0, m_blk, n_blk)) {
+                const int rn = m_blk * TM + rank * BM + q * 32 + lane;
+                if (rn < M) st_next = __ldg(res_stats + rn);
+            }
             for (int lt = 0; get_tile(lt, m_blk, n_blk); lt++) {
                 const int row0 = m_blk * TM + rank * BM + q * 32;
+                // (mean, rstd) of this thread's residual row: loaded one tile ahead so that no box waits for it
+                const float r_mu = st_next.x, r_rs = st_next.y;
+                {
+                    int mb2, nb2;
+                    if (res_stats && get_tile(lt + 1, mb2, nb2)) {
+                        const int rn = mb2 * TM + rank * BM + q * 32 + lane;
+                        if (rn < M) st_next = __ldg(res_stats + rn);
+                    }
+                }
                 ptx::mbar_wait(tfull_bar(acc), acc_ph);
                 ptx::tc_fence_after();
                 const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
@@ -439,16 +464,37 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                     if (valid) {
                         ptx::mbar_wait(rfull_bar(q, b), (rph >> b) & 1u);
                         rph ^= 1u << b;
+                        if (N <= 1024) {              // parameters from shared memory, packed FP32x2 arithmetic
+                            const uint64_t rs2 = pk2(r_rs, r_rs), nmr2 = pk2(-r_mu * r_rs, -r_mu * r_rs);
 #pragma unroll
-                        for (int v = 0; v < 8; v++) {
-                            const uint32_t addr = buf + row_off + (((uint32_t)v ^ sw) << 4);
-                            const float4 x = ld_shared_f4(addr);
-                            float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
-                            if (col + 4 * v < N) bb = __ldg(reinterpret_cast<const float4*>(bias + col + 4 * v));
-                            st_shared_v4(addr, __float_as_uint(__uint_as_float(r[4 * v + 0]) + bb.x + x.x),
-                                         __float_as_uint(__uint_as_float(r[4 * v + 1]) + bb.y + x.y),
-                                         __float_as_uint(__uint_as_float(r[4 * v + 2]) + bb.z + x.z),
-                                         __float_as_uint(__uint_as_float(r[4 * v + 3]) + bb.w + x.w));
+                            for (int v = 0; v < 8; v++) {
+                                const uint32_t addr = buf + row_off + (((uint32_t)v ^ sw) << 4);
+                                const uint32_t pc = par_base + (uint32_t)(col + 4 * v) * 4u;
+                                uint64_t x0, x1, b0, b1;
+                                ld_shared_2x2(addr, x0, x1);
+                                ld_shared_2x2(pc, b0, b1);
+                                if (res_stats) {          // the residual is stored un-normalised: x = LN(y) on the fly
+                                    uint64_t g0, g1, e0, e1;
+                                    ld_shared_2x2(pc + 4096u, g0, g1);
+                                    ld_shared_2x2(pc + 8192u, e0, e1);
+                                    x0 = fma2(fma2(x0, rs2, nmr2), g0, e0);
+                                    x1 = fma2(fma2(x1, rs2, nmr2), g1, e1);
+                                }
+                                st_shared_2x2(addr, add2(add2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), b0), x0),
+                                              add2(add2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), b1), x1));
+                            }
+                        } else {
+#pragma unroll
+                            for (int v = 0; v < 8; v++) {
+                                const uint32_t addr = buf + row_off + (((uint32_t)v ^ sw) << 4);
+                                const float4 x = ld_shared_f4(addr);
+                                float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
+                                if (col + 4 * v < N) bb = __ldg(reinterpret_cast<const float4*>(bias + col + 4 * v));
+                                st_shared_v4(addr, __float_as_uint(__uint_as_float(r[4 * v + 0]) + bb.x + x.x),
+                                             __float_as_uint(__uint_as_float(r[4 * v + 1]) + bb.y + x.y),
+                                             __float_as_uint(__uint_as_float(r[4 * v + 2]) + bb.z + x.z),
+                                             __float_as_uint(__uint_as_float(r[4 * v + 3]) + bb.w + x.w));
+                            }
                         }
                         ptx::fence_proxy_async();
                         __syncwarp();
@@ -561,7 +607,7 @@ int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_
 
 namespace {
 
-struct LnArgs { const float* gamma; const float* beta; float eps; void* xb_out; };
+struct LnArgs { const float* gamma; const float* beta; float eps; void* xb_out; const float2* res_stats; };
 
 template <int BN, int EPI, int NB, int CG>
 int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
@@ -621,7 +667,8 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
     const float* g = ln ? ln->gamma : nullptr;
     const float* be = ln ? ln->beta : nullptr;
     const float eps = ln ? ln->eps : 0.f;
-    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, ty, txb, bias, g, be, eps, M, N, K));
+    const float2* rs = ln ? ln->res_stats : nullptr;
+    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, ty, txb, bias, g, be, eps, rs, M, N, K));
     CU_LAUNCH_CHECK(ctx, "gemm_bf16_tcgen05_kernel");
     return ANON_OK;
 }
@@ -652,6 +699,20 @@ int gemm_bf16_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W
     }
 }
 
+// C = A W^T + bias + LN(res_y; stats, gamma, beta): the residual stream is kept UN-normalised (res_y, with per-row
+// (mean, rstd) in res_stats) and normalised on the fly in the epilogue; C may alias res_y.  N > 128 only.
+int gemm_bf16_res_ln_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* res_y,
+                          const float2* res_stats, const float* gamma, const float* beta, float* C, int M, int N, int K)
+{
+    if (!ctx || !A || !W || !bias || !res_y || !C || M < 0 || N <= 128 || K <= 0 || (res_stats && (!gamma || !beta)))
+        return ANON_ERR_INVALID_ARG;
+    if (K % BK != 0 || N % 8 != 0 || (res_stats && N > 1024)) return ANON_ERR_UNSUPPORTED;
+    if (M == 0) return ANON_OK;
+    LnArgs ln{gamma, beta, 0.f, nullptr, res_stats};
+    if (K >= 2048) return launch_gemm<256, 2, 2, 2>(ctx, A, W, bias, res_y, C, M, N, K, &ln);
+    return launch_gemm<256, 2, 5, 2>(ctx, A, W, bias, res_y, C, M, N, K, &ln);      // 5 boxes per warp + 4 mainloop stages
+}
+
 int gemm_bf16_ln_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias,
                       const float* residual, const float* gamma, const float* beta, float eps, float* x_out,
                       __nv_bfloat16* xb_out, int M, int N, int K)
@@ -660,7 +721,7 @@ int gemm_bf16_ln_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16
         return ANON_ERR_INVALID_ARG;
     if (K % BK != 0 || N % 256 != 0 || N > 1024) return ANON_ERR_UNSUPPORTED;
     if (M == 0) return ANON_OK;
-    LnArgs ln{gamma, beta, eps, xb_out};
+    LnArgs ln{gamma, beta, eps, xb_out, nullptr};
     return launch_gemm<256, 3, 4, 2>(ctx, A, W, bias, residual, x_out, M, N, K, &ln);
 }
 

@@ -103,8 +103,14 @@ def main():
     ms = timeit(lambda: P.anon_hmac_spans(ctx, d_bytes, d_off, kb, dig), n=5)
     lens = np.diff(off)
     comp = float(((lens + 9 + 63) // 64 + 1).sum())
+    # ALU-pipe instructions per SHA-256 compression counted in the SASS of hmac_spans_kernel (cuobjdump: 1,363 SHF + 774 LOP3
+    # + 531 IADD3 over the two inlined compressions = 1,334 each; another 190 IMAD go to the FMA pipe).  ALU-pipe peak
+    # (DESIGN.md section 6): 148 SMs x 64 lanes/clk x 1.965 GHz = 18.6 T lane-instructions/s.
+    alu_per_comp, alu_peak = 1334.0, 148 * 64 * 1.965e9
     res["hmac_sha256_no_dedup"] = {"spans": S, "ms": ms, "hmac_per_s": S / ms * 1e3, "compressions_per_s": comp / ms * 1e3,
-                                   "bytes_per_s_gb": (data.size + S * 40) / ms / 1e6}
+                                   "bytes_per_s_gb": (data.size + S * 40) / ms / 1e6,
+                                   "roofline": {"bound": "alu", "achieved": comp / ms * 1e3 * alu_per_comp / 1e12, "peak": alu_peak / 1e12,
+                                                "unit": "T ALU-pipe instr/s", "frac": comp / ms * 1e3 * alu_per_comp / alu_peak}}
     print(json.dumps(res, indent=1))
     ctx.close()
 

@@ -154,6 +154,16 @@ int  anon_cache_stats(anon_cache* c, uint64_t* n_unique, uint64_t* n_lookups, ui
 int64_t anon_cache_entry(anon_cache* c, uint64_t uid, uint8_t* h_bytes, size_t bytes_capacity,
                          uint8_t* h_digest);
 
+/* The whole mapping table at once, in uid (first-occurrence) order: entity bytes as CSR (h_bytes, h_offsets
+ * int64[n_unique + 1]) and the 32-byte digests -- the (original_name, full_hash) columns of the paper's SQLite
+ * mapping; slug_name is the first slug_len hex characters of the digest, entity_type travels with the spans.
+ * Any output pointer may be NULL; *n_unique / *n_bytes are always written, so a first call with NULL buffers sizes
+ * the second.  ANON_ERR_CAPACITY if bytes_capacity is too small.  Re-inserting the exported entities in this order
+ * into a fresh cache (anon_pseudonymize with the same key) reproduces the same uids and digests (resume).
+ * Synchronises. */
+int  anon_cache_export(anon_cache* c, uint8_t* h_bytes, size_t bytes_capacity, int64_t* h_offsets, uint8_t* h_digests,
+                       uint64_t* n_unique, uint64_t* n_bytes);
+
 /* For span i = 0..S-1 in order (e_i = d_span_bytes[off[i] .. off[i+1]), exact bytes):
  *   hit[i] = 1 if e_i is already in the cache (from an earlier call or an earlier i), else 0
  *            and (HMAC_SHA256(key, e_i), uid = number of entries before insertion) is inserted;

@@ -56,6 +56,7 @@ _SIGNATURES = {
     "anon_cache_clear": (ctypes.c_int, [_vp]),
     "anon_cache_stats": (ctypes.c_int, [_vp, ctypes.POINTER(_u64), ctypes.POINTER(_u64), ctypes.POINTER(_u64)]),
     "anon_cache_entry": (_i64, [_vp, _u64, _vp, _sz, _vp]),
+    "anon_cache_export": (ctypes.c_int, [_vp, _vp, _sz, _vp, _vp, ctypes.POINTER(_u64), ctypes.POINTER(_u64)]),
     "anon_pseudonymize": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i64, _vp, _sz, _i32,
                                          ctypes.POINTER(ctypes.c_char_p), _i32, _vp, _sz, _vp, _vp, _vp, _vp]),
     "anon_hmac_spans": (ctypes.c_int, [_vp, _vp, _vp, _i64, _vp, _sz, _vp]),
@@ -204,6 +205,16 @@ class Cache:
         buf = np.zeros(max(int(n), 1), np.uint8)
         lib().anon_cache_entry(self._h, uid, buf.ctypes.data, int(n), dig.ctypes.data)
         return buf[:n].tobytes(), dig.tobytes()
+
+    def export(self):
+        """The mapping table in uid order: (entity bytes uint8[], offsets int64[U+1], digests uint8[U,32])."""
+        n, nb = _u64(), _u64()
+        self.ctx.check(lib().anon_cache_export(self._h, None, 0, None, None, ctypes.byref(n), ctypes.byref(nb)), "anon_cache_export")
+        data, off = np.zeros(max(nb.value, 1), np.uint8), np.zeros(n.value + 1, np.int64)
+        dig = np.zeros((max(n.value, 1), 32), np.uint8)
+        self.ctx.check(lib().anon_cache_export(self._h, data.ctypes.data, data.size, off.ctypes.data, dig.ctypes.data,
+                                               ctypes.byref(n), ctypes.byref(nb)), "anon_cache_export")
+        return data[:nb.value], off, dig[:n.value]
 
     def close(self):
         if self._h:

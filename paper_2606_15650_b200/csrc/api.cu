@@ -21,7 +21,7 @@ extern "C" const char* const* anon_exported_symbols(void) {
         "anon_strerror", "anon_exported_symbols", "anon_ctx_create", "anon_ctx_destroy", "anon_ctx_sync",
         "anon_last_cuda_error", "anon_workspace_bytes", "anon_weights_load", "anon_weights_free", "anon_ner_forward",
         "anon_decode_spans", "anon_gather_spans", "anon_cache_create", "anon_cache_destroy", "anon_cache_stats", "anon_cache_clear",
-        "anon_cache_entry", "anon_pseudonymize", "anon_hmac_spans", "anon_pipeline_host", "anon_gemm_bf16",
+        "anon_cache_entry", "anon_cache_export", "anon_pseudonymize", "anon_hmac_spans", "anon_pipeline_host", "anon_gemm_bf16",
         "anon_attention", "anon_gemm_bf16_ln", "anon_splice_records", "anon_pipeline_host_text", "anon_ctx_profile", "anon_ctx_profile_read", nullptr};
     return names;
 }

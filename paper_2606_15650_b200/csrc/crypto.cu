@@ -480,6 +480,22 @@ extern "C" int64_t anon_cache_entry(anon_cache* c, uint64_t uid, uint8_t* h_byte
     return len;
 }
 
+extern "C" int anon_cache_export(anon_cache* c, uint8_t* h_bytes, size_t bytes_capacity, int64_t* h_offsets, uint8_t* h_digests,
+                                 uint64_t* n_unique, uint64_t* n_bytes)
+{
+    if (!c) return ANON_ERR_INVALID_ARG;
+    anon_ctx* ctx = c->ctx;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    if (n_unique) *n_unique = c->n_unique;
+    if (n_bytes) *n_bytes = c->arena_used;
+    if (h_bytes && bytes_capacity < c->arena_used) return ANON_ERR_CAPACITY;
+    if (h_offsets) CU_TRY(ctx, cudaMemcpy(h_offsets, c->d_entry_off, (c->n_unique + 1) * 8, cudaMemcpyDeviceToHost));
+    if (h_bytes && c->arena_used) CU_TRY(ctx, cudaMemcpy(h_bytes, c->d_arena, c->arena_used, cudaMemcpyDeviceToHost));
+    if (h_digests && c->n_unique) CU_TRY(ctx, cudaMemcpy(h_digests, c->d_digests, c->n_unique * 32, cudaMemcpyDeviceToHost));
+    return ANON_OK;
+}
+
 int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t* d_bytes, const int64_t* d_off,
                       const uint8_t* d_type, int64_t S, const uint8_t* key, size_t key_len, int32_t slug_len,
                       const char* const* type_names, int32_t num_types, uint8_t* d_out, size_t out_cap,

@@ -169,3 +169,31 @@ def test_zipf_stress_shape_bit_exact(env, n_unique, n_draws):
     _assert_same(got, want)
     assert gc.stats() == oc.stats()
     gc.close(); oc.close()
+
+
+def test_cache_export_is_the_mapping_table_and_resumes(env):
+    """P:L52 hand-off: the exported rows are (entity, HMAC-SHA256(key, entity)) in first-occurrence order -- checked
+    against Python's own hmac / dict, not the oracle -- and re-inserting them into a fresh cache reproduces uids and
+    digests, after which the original spans are all hits (checkpoint / resume)."""
+    P, torch, ctx = env
+    data, off, types, key = gen.spans_config1()
+    kb = key.tobytes()
+    gc = P.Cache(ctx, 4096, 1 << 20)
+    first = _run_gpu(P, torch, ctx, gc, data, off, types, kb, 10, gen.TYPE_NAMES_4)
+    ebytes, eoff, edig = gc.export()
+    seen = {}
+    for i in range(off.size - 1):
+        seen.setdefault(bytes(data[off[i]:off[i + 1]]), len(seen))
+    ents = sorted(seen, key=seen.get)
+    assert eoff.size - 1 == len(ents) == edig.shape[0]
+    for u, e in enumerate(ents):
+        assert bytes(ebytes[eoff[u]:eoff[u + 1]]) == e
+        assert bytes(edig[u]) == pyhmac.new(kb, e, hashlib.sha256).digest()
+    gc.close()
+    # resume: a fresh cache fed with the exported entities, then the original spans
+    g2 = P.Cache(ctx, 4096, 1 << 20)
+    r = _run_gpu(P, torch, ctx, g2, ebytes, eoff, None, kb, 10, gen.TYPE_NAMES_4)
+    assert not r["hit"].any() and np.array_equal(r["uid"], np.arange(len(ents))) and np.array_equal(r["digests"], edig)
+    again = _run_gpu(P, torch, ctx, g2, data, off, types, kb, 10, gen.TYPE_NAMES_4)
+    assert again["hit"].all() and np.array_equal(again["uid"], first["uid"]) and np.array_equal(again["out_tokens"], first["out_tokens"])
+    g2.close()

@@ -238,3 +238,19 @@ def test_config4_bf16_large_shape(env):
     w2 = gen.make_weights(d, gen.SEED_BASE + 4, planted=(2.0, 0.5, 4.0))
     e, a = _bf16_model_check(P, torch, ctx, d, w2, ids, cu, subset, require_agreement=True)
     print(f"\nconfig4 subsample: W2 max|dlogit|={e:.2e} agreement={a:.4%}")
+
+
+def test_bf16_small_hidden_generic_path(env):
+    """A BF16 model whose hidden size is neither 768 nor 1024 (2 layers, hidden 256, 4 heads, FFN 1024): exercises the
+    generic LayerNorm kernel with the normalised FP32 residual stream and the residual GEMM without the on-the-fly
+    LayerNorm, on every sequence of a small ragged batch (lengths 1 .. 512)."""
+    P, torch, ctx = env
+    d = dict(layers=2, hidden=256, heads=4, ffn=1024, vocab=4096, num_labels=9, max_pos=512, ln_eps=1e-5, dtype=1)
+    w = gen.make_weights(d, 77, planted=(2.0, 0.5, 4.0))
+    rng = np.random.default_rng(8)
+    lens = [1, 17, 64, 129, 512, 300, 2, 255]
+    cu = np.zeros(len(lens) + 1, np.int32); cu[1:] = np.cumsum(lens)
+    ids = rng.integers(5, d["vocab"], int(cu[-1])).astype(np.int32)
+    e, a = _bf16_model_check(P, torch, ctx, d, w, ids, cu, None, require_agreement=False)
+    assert a >= 0.995
+    print(f"\nhidden-256 BF16 model: max|dlogit|={e:.2e} agreement={a:.4%}")

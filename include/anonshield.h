@@ -41,6 +41,7 @@ extern "C" {
 typedef struct anon_ctx     anon_ctx;
 typedef struct anon_weights anon_weights;
 typedef struct anon_cache   anon_cache;
+typedef struct anon_regex   anon_regex;
 
 /* Encoder shape (BJ "embedding plus L encoder layers ... then the token-classification
  * head"; S8c O1).  dtype: 0 = FP32 parameters and arithmetic (BJ configs[0]);
@@ -201,6 +202,39 @@ int  anon_hmac_spans(anon_ctx* ctx, const uint8_t* d_span_bytes, const int64_t* 
 int  anon_splice_records(anon_ctx* ctx, const uint8_t* d_text, size_t text_bytes, const int64_t* d_record_offsets, int32_t R,
                          const anon_span* d_spans, int32_t S, const uint8_t* d_out_tokens, const int64_t* d_out_offsets,
                          uint8_t* d_new_text, size_t new_text_capacity, int64_t* d_new_record_offsets);
+
+/* ---- NEXT-4: regex detector and regex / NER span merge ("custom regex patterns"; S8f NEXT-4; D17-D19) ----- */
+/* Uploads a pattern automaton.  h_blob is the byte string regex_dfa.compile_patterns() returns (HOST pointer, layout in
+ * paper_2606_15650_b200/regex_dfa.py: header, class_of[256], is_word[256], type_of_pattern[256], accept[n_states],
+ * trans[n_states * n_classes]; state 0 dead, state 1 start).  The tables are validated here (sizes, every transition and
+ * accept label in range, at most 127 patterns, max_match <= 255) and must fit shared memory beside a text tile, else
+ * ANON_ERR_UNSUPPORTED.  The handle keeps its own device copy.  Synchronises.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA. */
+int  anon_regex_load(anon_ctx* ctx, const void* h_blob, size_t blob_bytes, anon_regex** out);
+void anon_regex_free(anon_regex* rx);
+/* Scans every record for the patterns, rule D18: matches are taken left to right inside a record, never overlap and never
+ * cross a record boundary; at a position the longest match wins (at most max_match bytes), ties go to the lowest pattern
+ * index; a match starts and ends at a word boundary (the byte before / after is not [0-9A-Za-z_], or it is the record's
+ * edge).  d_record_offsets int64[R+1] with [0] = 0 and [R] = text_bytes.  Spans are written in stream order
+ * (record, char_start) with type = type_of_pattern[pattern]; *d_num_spans (device) receives the TOTAL found, only the
+ * first span_capacity are written and ANON_ERR_CAPACITY is latched beyond.  Workspace: 2 * text_bytes + 12 * R + small.
+ * Asynchronous. */
+int  anon_regex_scan(anon_ctx* ctx, const anon_regex* rx, const uint8_t* d_text, size_t text_bytes,
+                     const int64_t* d_record_offsets, int32_t R, anon_span* d_spans, int32_t span_capacity,
+                     int32_t* d_num_spans);
+/* Rule D19: every regex span is kept; an NER span is kept iff it overlaps no regex span of its record; the result is
+ * ordered by (record_id, char_start), an NER span before a regex span on a tie.  Both inputs must be ordered by
+ * (record_id, char_start) and the regex spans non-overlapping (anon_decode_spans and anon_regex_scan write them so).
+ * The counts may live on the device: d_num_ner / d_num_regex (device int32, clamped to *_max) or NULL = *_max itself.
+ * *d_num_out (device) receives the merged count even when it exceeds `capacity` (then ANON_ERR_CAPACITY is latched).
+ * d_out_spans must not alias an input.  Asynchronous. */
+int  anon_merge_spans(anon_ctx* ctx, const anon_span* d_ner_spans, const int32_t* d_num_ner, int32_t ner_max,
+                      const anon_span* d_regex_spans, const int32_t* d_num_regex, int32_t regex_max,
+                      anon_span* d_out_spans, int32_t capacity, int32_t* d_num_out);
+/* Attaches a pattern automaton to the context (NULL detaches): anon_pipeline_host / anon_pipeline_host_text then run
+ * anon_regex_scan on the batch text and anon_merge_spans between the BIO decode and the span gather, so the spans they
+ * return, pseudonymize and splice are the merged list (the paper's hybrid strategy).  The handle must outlive its
+ * attachment.  The regex types index the same type_names array as the NER types. */
+int  anon_ctx_set_regex(anon_ctx* ctx, const anon_regex* rx);
 
 /* ---- whole hot path with HOST buffers (the call a user makes; bench.py's e2e leg) ------------- */
 /* Copies one batch host->device, runs A1-A13 and copies the results back, all on the

@@ -71,6 +71,11 @@ _SIGNATURES = {
     "anon_gemm_bf16_ln": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp, _vp, _i32, _i32, _i32]),
     "anon_splice_records": (ctypes.c_int, [_vp, _vp, _sz, _vp, _i32, _vp, _i32, _vp, _vp, _vp, _sz, _vp]),
     "anon_attention": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32, _i32, _vp]),
+    "anon_regex_load": (ctypes.c_int, [_vp, _vp, _sz, ctypes.POINTER(_vp)]),
+    "anon_regex_free": (None, [_vp]),
+    "anon_regex_scan": (ctypes.c_int, [_vp, _vp, _vp, _sz, _vp, _i32, _vp, _i32, _vp]),
+    "anon_merge_spans": (ctypes.c_int, [_vp, _vp, _vp, _i32, _vp, _vp, _i32, _vp, _i32, _vp]),
+    "anon_ctx_set_regex": (ctypes.c_int, [_vp, _vp]),
 }
 
 
@@ -228,6 +233,27 @@ class Cache:
             pass
 
 
+class Regex:
+    """anon_regex: a pattern automaton on the device.  `blob` comes from regex_dfa.compile_patterns (NEXT-4)."""
+
+    def __init__(self, ctx, blob):
+        self.ctx = ctx
+        self._h = _vp()
+        b = np.frombuffer(bytes(blob), np.uint8)
+        ctx.check(lib().anon_regex_load(ctx._h, b.ctypes.data, b.size, ctypes.byref(self._h)), "anon_regex_load")
+
+    def close(self):
+        if self._h:
+            lib().anon_regex_free(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
 # ---- the calls (same names as the C ABI) ---------------------------------------------------------------
 def anon_ner_forward(ctx, weights, token_ids, cu_seqlens, logits=None, labels=None):
     B, T = cu_seqlens.numel() - 1, token_ids.numel()
@@ -277,6 +303,26 @@ def anon_splice_records(ctx, text, record_offsets, spans, S, out_tokens, out_off
     ctx.check(lib().anon_splice_records(ctx._h, _ptr(text), text.numel(), _ptr(record_offsets), R, _ptr(spans), S,
                                         _ptr(out_tokens), _ptr(out_offsets), _ptr(new_text), new_text.numel(),
                                         _ptr(new_record_offsets)), "anon_splice_records")
+
+
+def anon_regex_scan(ctx, regex, text, record_offsets, spans, num_spans):
+    """text uint8[n], record_offsets int64[R+1], spans int32[cap,4], num_spans int32[1] -- device tensors (NEXT-4)."""
+    R = record_offsets.numel() - 1
+    ctx.check(lib().anon_regex_scan(ctx._h, regex._h, _ptr(text), text.numel(), _ptr(record_offsets), R, _ptr(spans),
+                                    spans.shape[0], _ptr(num_spans)), "anon_regex_scan")
+
+
+def anon_merge_spans(ctx, ner_spans, num_ner, regex_spans, num_regex, out_spans, num_out):
+    """Span lists int32[n,4] on the device; num_ner / num_regex: device int32[1] tensors or None (= the whole list)."""
+    ctx.check(lib().anon_merge_spans(ctx._h, _ptr(ner_spans), _ptr(num_ner), ner_spans.shape[0], _ptr(regex_spans),
+                                     _ptr(num_regex), regex_spans.shape[0], _ptr(out_spans), out_spans.shape[0],
+                                     _ptr(num_out)), "anon_merge_spans")
+
+
+def anon_ctx_set_regex(ctx, regex):
+    """Attach (or with None detach) a pattern automaton: anon_pipeline_host then merges regex spans into the NER spans."""
+    ctx.check(lib().anon_ctx_set_regex(ctx._h, regex._h if regex is not None else None), "anon_ctx_set_regex")
+    ctx._regex = regex            # keeps the handle alive while attached
 
 
 def anon_gemm_bf16_ln(ctx, A, W, bias, residual, gamma, beta, eps, x, xb):

@@ -22,7 +22,8 @@ extern "C" const char* const* anon_exported_symbols(void) {
         "anon_last_cuda_error", "anon_workspace_bytes", "anon_weights_load", "anon_weights_free", "anon_ner_forward",
         "anon_decode_spans", "anon_gather_spans", "anon_cache_create", "anon_cache_destroy", "anon_cache_stats", "anon_cache_clear",
         "anon_cache_entry", "anon_cache_export", "anon_pseudonymize", "anon_hmac_spans", "anon_pipeline_host", "anon_gemm_bf16",
-        "anon_attention", "anon_gemm_bf16_ln", "anon_splice_records", "anon_pipeline_host_text", "anon_ctx_profile", "anon_ctx_profile_read", nullptr};
+        "anon_attention", "anon_gemm_bf16_ln", "anon_splice_records", "anon_pipeline_host_text", "anon_ctx_profile", "anon_ctx_profile_read",
+        "anon_regex_load", "anon_regex_free", "anon_regex_scan", "anon_merge_spans", "anon_ctx_set_regex", nullptr};
     return names;
 }
 
@@ -103,6 +104,12 @@ extern "C" int anon_ctx_profile_read(anon_ctx* ctx, double* class_ms, double* cl
     return ANON_OK;
 }
 
+extern "C" int anon_ctx_set_regex(anon_ctx* ctx, const anon_regex* rx) {
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    ctx->regex = rx;
+    return ANON_OK;
+}
+
 extern "C" const char* anon_last_cuda_error(anon_ctx* ctx) { return ctx ? ctx->cuda_err : ""; }
 
 int splice_records_impl(anon_ctx* ctx, WsCursor& ws, const uint8_t* d_text, size_t text_bytes, const int64_t* d_rec_off, int32_t R,
@@ -145,6 +152,10 @@ static int pipeline_host_impl(anon_ctx* ctx, const anon_weights* w, anon_cache* 
     uint8_t* d_out = (uint8_t*)ws.take(out_capacity + 16);
     uint8_t* d_new_text = h_new_text ? (uint8_t*)ws.take(new_text_capacity + 16) : nullptr;
     int64_t* d_new_rec_off = h_new_text ? (int64_t*)ws.take(((size_t)R + 1) * 8) : nullptr;
+    // NEXT-4: regex spans and the merged list (only with an attached automaton)
+    anon_span* d_rx_spans = ctx->regex ? (anon_span*)ws.take((size_t)span_capacity * sizeof(anon_span) + 16) : nullptr;
+    anon_span* d_merged = ctx->regex ? (anon_span*)ws.take((size_t)span_capacity * sizeof(anon_span) + 16) : nullptr;
+    if (ctx->regex && (!d_rx_spans || !d_merged)) return ANON_ERR_OOM;
     if (h_new_text && (!d_new_text || !d_new_rec_off || !h_new_rec_off)) return d_new_text ? ANON_ERR_INVALID_ARG : ANON_ERR_OOM;
     if (!d_ids || !d_cu || !d_meta || !d_text || !d_rec_off || !d_labels || !d_spans || !d_num || !d_span_off ||
         !d_span_type || !d_out_off || !d_hit || !d_span_bytes || !d_out)
@@ -161,6 +172,20 @@ static int pipeline_host_impl(anon_ctx* ctx, const anon_weights* w, anon_cache* 
         WsCursor c = ws;
         rc = decode_spans_impl(ctx, c, d_labels, d_meta, T, NL, d_spans, span_capacity, d_num);
         if (rc) return rc;
+    }
+    if (ctx->regex) {
+        // d_num[0] = NER spans, [1] = regex spans, [2] = merged; a list that overflowed latches CAPACITY (checked below)
+        {
+            WsCursor c = ws;
+            rc = regex_scan_impl(ctx, c, ctx->regex, d_text, text_bytes, d_rec_off, R, d_rx_spans, span_capacity, d_num + 1);
+            if (rc) return rc;
+        }
+        WsCursor c = ws;
+        rc = merge_spans_impl(ctx, c, d_spans, d_num, span_capacity, d_rx_spans, d_num + 1, span_capacity, d_merged, span_capacity,
+                              d_num + 2);
+        if (rc) return rc;
+        d_spans = d_merged;
+        d_num += 2;
     }
     int* h_n = (int*)(ctx->h_pinned + 256);
     int* h_status = (int*)(ctx->h_pinned + 260);

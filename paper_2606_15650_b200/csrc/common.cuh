@@ -35,6 +35,8 @@ struct anon_ctx {
     // L2-resident scratch of the fused residual+LayerNorm GEMM epilogue (allocated on first use, grows only)
     void* ln_scratch = nullptr;
     size_t ln_scratch_bytes = 0;
+    // NEXT-4: pattern automaton the host pipeline merges into the NER spans (anon_ctx_set_regex; not owned)
+    const struct anon_regex* regex = nullptr;
     // launch accounting + optional event profiling
     long long n_launches = 0;
     bool prof_on = false;
@@ -106,6 +108,10 @@ int pseudonymize_impl(anon_ctx*, WsCursor&, anon_cache*, const uint8_t* d_bytes,
                       const char* const* type_names, int32_t num_types, uint8_t* d_out, size_t out_cap,
                       int64_t* d_out_off, uint8_t* d_hit, int64_t* d_uid, uint8_t* d_digests,
                       int64_t* total_out_bytes);
+int regex_scan_impl(anon_ctx*, WsCursor&, const anon_regex* rx, const uint8_t* d_text, size_t text_bytes, const int64_t* d_rec_off,
+                    int32_t R, anon_span* d_spans, int32_t cap, int32_t* d_num);
+int merge_spans_impl(anon_ctx*, WsCursor&, const anon_span* d_ner, const int32_t* d_num_ner, int32_t ner_max, const anon_span* d_rgx,
+                     const int32_t* d_num_rgx, int32_t rgx_max, anon_span* d_out, int32_t cap, int32_t* d_num_out);
 int gemm_bf16_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias,
                    const float* residual, void* C, int M, int N, int K, int epilogue);
 int gemm_bf16_res_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* res_y,

@@ -1,0 +1,395 @@
+// regex.cu -- NEXT-4: the regex detector as a table-driven DFA scan, and the regex / NER span merge.
+// P:L43 ("21 custom regex patterns" beside the transformer NER), P:L170 (overlap resolution); S8f NEXT-4; rules D17-D19 of
+// DESIGN.md.  Integer / byte work: bit-exact against oracle/regex_layer.py.
+//
+// The automaton comes from the host compiler (regex_dfa.py): one DFA for all patterns, over byte classes, anchored at the
+// candidate start.  Rule D18 (leftmost-longest, non-overlapping, word boundaries, lowest pattern index) in three passes:
+//   R1  regex_candidates_kernel   every byte position in parallel: the longest match that starts there (0 = none).  Tables
+//                                 and a text tile (+ max_match look-ahead) live in shared memory; most positions die on
+//                                 their first transition.  Writes one u16 per byte: len | pattern << 8.
+//   R2  regex_select_kernel       one warp per record walks the candidates left to right, 128 positions per step: the
+//                                 first candidate at or after the cursor is selected (bit 15), the cursor jumps to its end.
+//   R3  scan of the per-record counts, then regex_write_kernel compacts the selected candidates into the span list in
+//       stream order (ballot + popc ranks inside a warp).
+// Merge (D19): per NER span one binary search in the regex list (sorted, non-overlapping) decides keep / drop; a scan of
+// the keep flags plus cross ranks (binary searches) gives every surviving span its slot in the merged list.
+#include "common.cuh"
+#include "scan.cuh"
+
+#include <new>
+
+struct anon_regex {
+    anon_ctx* ctx = nullptr;
+    uint8_t* d_tab = nullptr;        // blob without its 32-byte header, padded to 16 bytes
+    uint32_t tab_bytes = 0;          // padded
+    int n_states = 0, n_classes = 0, n_patterns = 0, max_match = 0;
+    uint32_t off_accept = 0, off_trans = 0;   // byte offsets inside d_tab
+};
+
+namespace {
+
+constexpr uint32_t kMagic = 0x31585241u;     // 'ARX1'
+constexpr int kTile = 4096;                  // byte positions per tile of R1
+constexpr int kThreads = 256;
+constexpr int kTextSmem = kTile + 256 + 48;  // tile + look-ahead (max_match <= 255) + alignment slack
+
+// largest r in [lo, hi] with off[r] <= p  (off[lo] <= p is given)
+__device__ __forceinline__ int record_of(const long long* __restrict__ off, int lo, int hi, long long p) {
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (off[mid] <= p) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+__global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
+    const uint8_t* __restrict__ tab, uint32_t tab_bytes, uint32_t off_accept, uint32_t off_trans, int n_classes, int max_match,
+    const uint8_t* __restrict__ text, long long nbytes, const long long* __restrict__ rec_off, int R, long long n_tiles,
+    uint16_t* __restrict__ cand)
+{
+    extern __shared__ __align__(16) uint8_t smem[];
+    uint8_t* s_tab = smem;
+    uint8_t* s_text = smem + tab_bytes;
+    __shared__ int s_rec[2];
+    for (uint32_t i = threadIdx.x; i < tab_bytes / 16; i += kThreads)
+        reinterpret_cast<uint4*>(s_tab)[i] = reinterpret_cast<const uint4*>(tab)[i];
+    const uint8_t* class_of = s_tab;
+    const uint8_t* is_word = s_tab + 256;
+    const int16_t* accept = reinterpret_cast<const int16_t*>(s_tab + off_accept);
+    const uint16_t* trans = reinterpret_cast<const uint16_t*>(s_tab + off_trans);
+
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const long long tile0 = tile * kTile;
+        const long long lo = tile0 > 0 ? tile0 - 1 : 0;
+        long long hi = tile0 + kTile + max_match;
+        if (hi > nbytes) hi = nbytes;
+        // stage text[lo, hi) through aligned 16-byte loads (a chunk that holds one valid byte is readable as a whole)
+        const uintptr_t g0 = reinterpret_cast<uintptr_t>(text + lo) & ~(uintptr_t)15;
+        const int nchunk = (int)((reinterpret_cast<uintptr_t>(text + hi) - g0 + 15) >> 4);
+        __syncthreads();                               // previous tile fully consumed (and s_tab written, first time)
+        for (int i = threadIdx.x; i < nchunk; i += kThreads)
+            reinterpret_cast<uint4*>(s_text)[i] = __ldg(reinterpret_cast<const uint4*>(g0) + i);
+        if (threadIdx.x == 0) s_rec[0] = record_of(rec_off, 0, R - 1, tile0);
+        if (threadIdx.x == 32) s_rec[1] = record_of(rec_off, 0, R - 1, (tile0 + kTile <= nbytes ? tile0 + kTile : nbytes) - 1);
+        __syncthreads();
+        const int r_lo = s_rec[0], r_hi = s_rec[1];
+        const long long sbase = (long long)(reinterpret_cast<uintptr_t>(text) - g0);   // s_text index of text[0] (may be negative)
+#pragma unroll 1
+        for (int k = 0; k < kTile / kThreads; k++) {
+            const long long p = tile0 + k * kThreads + threadIdx.x;
+            if (p >= nbytes) break;
+            const uint8_t* b = s_text + (sbase + p);
+            uint32_t out = 0;
+            uint32_t st = trans[n_classes + class_of[b[0]]];           // from the start state (state 1)
+            if (st != 0) {
+                const int r = record_of(rec_off, r_lo, r_hi, p);
+                const long long rs = rec_off[r], re = rec_off[r + 1];
+                if (p == rs || !is_word[b[-1]]) {
+                    const int limit = (int)(re - p < (long long)max_match ? re - p : (long long)max_match);
+                    int i = 0;
+                    while (true) {
+                        const int a = accept[st];
+                        if (a >= 0 && (i + 1 == re - p || !is_word[b[i + 1]])) out = (uint32_t)(i + 1) | ((uint32_t)a << 8);
+                        if (++i >= limit) break;
+                        st = trans[st * n_classes + class_of[b[i]]];
+                        if (st == 0) break;
+                    }
+                }
+            }
+            cand[p] = (uint16_t)out;
+        }
+    }
+}
+
+// 4 candidates per lane, 128 positions per warp step; positions outside [s, re) read as "no candidate"
+__device__ __forceinline__ void load_cands(const uint16_t* __restrict__ cand, long long idx, long long s, long long re, uint32_t c[4]) {
+    uint2 v = make_uint2(0, 0);
+    if (idx < re) v = *reinterpret_cast<const uint2*>(cand + idx);     // cand is padded by 4 entries past nbytes
+    c[0] = v.x & 0xffffu; c[1] = v.x >> 16; c[2] = v.y & 0xffffu; c[3] = v.y >> 16;
+#pragma unroll
+    for (int j = 0; j < 4; j++)
+        if (idx + j < s || idx + j >= re) c[j] = 0;
+}
+
+__global__ void __launch_bounds__(kThreads) regex_select_kernel(uint16_t* __restrict__ cand, const long long* __restrict__ rec_off, int R,
+                                                                int* __restrict__ rec_count)
+{
+    const int r = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (r >= R) return;
+    long long s = rec_off[r];
+    const long long re = rec_off[r + 1];
+    int count = 0;
+    while (s < re) {
+        const long long wb = s & ~3LL, idx = wb + lane * 4;
+        uint32_t c[4];
+        load_cands(cand, idx, s, re, c);
+        int first = -1;
+#pragma unroll
+        for (int j = 3; j >= 0; j--)
+            if (c[j] & 0xffu) first = j;
+        const uint32_t any = __ballot_sync(0xffffffffu, first >= 0);
+        if (!any) { s = wb + 128; continue; }
+        const int f = __ffs(any) - 1;
+        const int fj = __shfl_sync(0xffffffffu, first, f);
+        const uint32_t cv = __shfl_sync(0xffffffffu, first >= 0 ? c[first] : 0u, f);
+        const long long pos = wb + f * 4 + fj;
+        if (lane == f) cand[pos] = (uint16_t)(cv | 0x8000u);
+        count++;
+        s = pos + (cv & 0xffu);
+    }
+    if (lane == 0) rec_count[r] = count;
+}
+
+struct CountIn {
+    const int* cnt;
+    __device__ __forceinline__ long long operator()(long long r) const { return cnt[r]; }
+};
+struct BaseOut {
+    long long* base;
+    __device__ __forceinline__ void operator()(long long r, long long ex, long long) const { base[r] = ex; }
+};
+
+__global__ void __launch_bounds__(kThreads) regex_write_kernel(const uint16_t* __restrict__ cand, const long long* __restrict__ rec_off, int R,
+                                                               const long long* __restrict__ rec_base, const uint8_t* __restrict__ type_of,
+                                                               anon_span* __restrict__ spans, long long cap)
+{
+    const int r = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (r >= R) return;
+    const long long rs = rec_off[r], re = rec_off[r + 1];
+    long long o = rec_base[r];
+    for (long long wb = rs & ~3LL; wb < re; wb += 128) {
+        const long long idx = wb + lane * 4;
+        uint32_t c[4];
+        load_cands(cand, idx, rs, re, c);
+        int n = 0;
+#pragma unroll
+        for (int j = 0; j < 4; j++) n += (c[j] >> 15) & 1;
+        int incl = n;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        long long k = o + incl - n;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            if (c[j] & 0x8000u) {
+                if (k < cap) {
+                    const int cs = (int)(idx + j - rs);
+                    spans[k] = anon_span{r, cs, cs + (int)(c[j] & 0xffu), (int)type_of[(c[j] >> 8) & 0x7fu]};
+                }
+                k++;
+            }
+        }
+        o += __shfl_sync(0xffffffffu, incl, 31);
+    }
+}
+
+__global__ void regex_finish_kernel(const long long* total, long long cap, int* d_num, int* d_status) {
+    const long long n = *total;
+    *d_num = (int)(n > 0x7fffffffLL ? 0x7fffffffLL : n);
+    if (n > cap) latch_status(d_status, ANON_ERR_CAPACITY);
+}
+
+// ---- merge (D19) ----
+__device__ __forceinline__ int dev_count(const int* d_n, int n_max) {
+    if (!d_n) return n_max;
+    const int n = *d_n;
+    return n < 0 ? 0 : (n < n_max ? n : n_max);
+}
+
+__global__ void __launch_bounds__(kThreads) merge_flag_kernel(const anon_span* __restrict__ ner, const int* d_n_ner, int ner_max,
+                                                              const anon_span* __restrict__ rgx, const int* d_n_rgx, int rgx_max,
+                                                              uint8_t* __restrict__ keep, int* __restrict__ rgx_before)
+{
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    const int n1 = dev_count(d_n_ner, ner_max), n2 = dev_count(d_n_rgx, rgx_max);
+    if (i >= n1) return;
+    const anon_span sp = ner[i];
+    // first regex span that ends after sp starts: (record, char_end) > (sp.record, sp.char_start)
+    int lo = 0, hi = n2;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        const anon_span q = rgx[mid];
+        if (q.record_id < sp.record_id || (q.record_id == sp.record_id && q.char_end <= sp.char_start)) lo = mid + 1; else hi = mid;
+    }
+    const bool clash = lo < n2 && rgx[lo].record_id == sp.record_id && rgx[lo].char_start < sp.char_end;
+    keep[i] = clash ? 0 : 1;
+    // regex spans ordered strictly before sp: (record, char_start) < (sp.record, sp.char_start)
+    int a = 0, b = n2;
+    while (a < b) {
+        const int mid = (a + b) >> 1;
+        const anon_span q = rgx[mid];
+        if (q.record_id < sp.record_id || (q.record_id == sp.record_id && q.char_start < sp.char_start)) a = mid + 1; else b = mid;
+    }
+    rgx_before[i] = a;
+}
+
+struct KeepIn {
+    const uint8_t* keep;
+    __device__ __forceinline__ long long operator()(long long i) const { return keep[i]; }
+};
+struct KeepOut {
+    long long* kpos;
+    __device__ __forceinline__ void operator()(long long i, long long ex, long long) const { kpos[i] = ex; }
+};
+
+__global__ void __launch_bounds__(kThreads) merge_write_kernel(const anon_span* __restrict__ ner, const int* d_n_ner, int ner_max,
+                                                               const anon_span* __restrict__ rgx, const int* d_n_rgx, int rgx_max,
+                                                               const uint8_t* __restrict__ keep, const int* __restrict__ rgx_before,
+                                                               const long long* __restrict__ kpos, const long long* __restrict__ kept_total,
+                                                               anon_span* __restrict__ out, long long cap, int* d_num, int* d_status)
+{
+    const long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
+    const int n1 = dev_count(d_n_ner, ner_max), n2 = dev_count(d_n_rgx, rgx_max);
+    const long long kept = n1 > 0 ? *kept_total : 0;
+    if (i == 0) {
+        *d_num = (int)(kept + n2);
+        if (kept + n2 > cap) latch_status(d_status, ANON_ERR_CAPACITY);
+    }
+    if (i < ner_max) {
+        if (i < n1 && keep[i]) {
+            const long long k = kpos[i] + rgx_before[i];
+            if (k < cap) out[k] = ner[i];
+        }
+        return;
+    }
+    const long long j = i - ner_max;
+    if (j >= n2) return;
+    const anon_span q = rgx[j];
+    int lo = 0, hi = n1;                                // NER spans ordered at or before q (ties: NER first)
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        const anon_span sp = ner[mid];
+        if (sp.record_id < q.record_id || (sp.record_id == q.record_id && sp.char_start <= q.char_start)) lo = mid + 1; else hi = mid;
+    }
+    const long long k = j + (lo < n1 ? kpos[lo] : kept);
+    if (k < cap) out[k] = q;
+}
+
+}  // namespace
+
+extern "C" int anon_regex_load(anon_ctx* ctx, const void* h_blob, size_t blob_bytes, anon_regex** out) {
+    if (!ctx || !h_blob || !out) return ANON_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (blob_bytes < 32 + 768) return ANON_ERR_INVALID_ARG;
+    uint32_t head[8];
+    memcpy(head, h_blob, 32);
+    const uint64_t ns = head[1], nc = head[2], np = head[3], mm = head[4];
+    if (head[0] != kMagic || ns < 2 || ns > 65535 || nc < 1 || nc > 256 || np < 1 || np > 127 || mm < 1 || mm > 255)
+        return ANON_ERR_INVALID_ARG;
+    const uint64_t off_accept = 768, off_trans = off_accept + (2 * ns + 3) / 4 * 4;
+    if (blob_bytes != 32 + off_trans + 2 * ns * nc) return ANON_ERR_INVALID_ARG;
+    const uint8_t* tab = (const uint8_t*)h_blob + 32;
+    const int16_t* accept = (const int16_t*)(tab + off_accept);
+    const uint16_t* trans = (const uint16_t*)(tab + off_trans);
+    for (uint64_t c = 0; c < 256; c++) if (tab[c] >= nc) return ANON_ERR_INVALID_ARG;
+    for (uint64_t s = 0; s < ns; s++) if (accept[s] < -1 || accept[s] >= (int)np) return ANON_ERR_INVALID_ARG;
+    for (uint64_t i = 0; i < ns * nc; i++) if (trans[i] >= ns || (i < nc && trans[i] != 0)) return ANON_ERR_INVALID_ARG;
+    if (accept[0] >= 0 || accept[1] >= 0) return ANON_ERR_INVALID_ARG;        // dead state / empty match
+    const uint64_t padded = (blob_bytes - 32 + 15) / 16 * 16;
+    if (padded + kTextSmem > (uint64_t)ctx->smem_optin) return ANON_ERR_UNSUPPORTED;   // tables must fit shared memory
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    anon_regex* rx = new (std::nothrow) anon_regex();
+    if (!rx) return ANON_ERR_OOM;
+    rx->ctx = ctx; rx->tab_bytes = (uint32_t)padded;
+    rx->n_states = (int)ns; rx->n_classes = (int)nc; rx->n_patterns = (int)np; rx->max_match = (int)mm;
+    rx->off_accept = (uint32_t)off_accept; rx->off_trans = (uint32_t)off_trans;
+    if (cudaMalloc(&rx->d_tab, padded) != cudaSuccess) { cudaGetLastError(); delete rx; return ANON_ERR_OOM; }
+    cudaError_t e = cudaMemsetAsync(rx->d_tab, 0, padded, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(rx->d_tab, tab, blob_bytes - 32, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(regex_candidates_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(padded + kTextSmem));
+    if (e != cudaSuccess) { cudaFree(rx->d_tab); delete rx; return cuda_fail(ctx, e, "anon_regex_load"); }
+    *out = rx;
+    return ANON_OK;
+}
+
+extern "C" void anon_regex_free(anon_regex* rx) {
+    if (!rx) return;
+    cudaSetDevice(rx->ctx->device);
+    cudaFree(rx->d_tab);
+    delete rx;
+}
+
+int regex_scan_impl(anon_ctx* ctx, WsCursor& ws, const anon_regex* rx, const uint8_t* d_text, size_t text_bytes,
+                    const int64_t* d_rec_off, int32_t R, anon_span* d_spans, int32_t cap, int32_t* d_num)
+{
+    if (!ctx || !rx || R < 0 || cap < 0 || !d_num || !d_rec_off || (text_bytes > 0 && !d_text) || (cap > 0 && !d_spans))
+        return ANON_ERR_INVALID_ARG;
+    cudaStream_t st = ctx->stream;
+    if (R == 0 || text_bytes == 0) { CU_TRY(ctx, cudaMemsetAsync(d_num, 0, 4, st)); return ANON_OK; }
+    const long long nbytes = (long long)text_bytes;
+    uint16_t* cand = (uint16_t*)ws.take(((size_t)nbytes + 8) * 2);
+    int* rec_count = (int*)ws.take((size_t)R * 4);
+    long long* rec_base = (long long*)ws.take((size_t)R * 8);
+    long long* agg = (long long*)ws.take(scan::agg_bytes<long long>(R));
+    if (!cand || !rec_count || !rec_base || !agg) return ANON_ERR_OOM;
+    ProfScope ps(ctx, PROF_DECODE, (double)nbytes * 7 + (double)R * 28, 7);
+    const long long n_tiles = (nbytes + kTile - 1) / kTile;
+    const unsigned grid = (unsigned)(n_tiles < (long long)ctx->sm_count * 4 ? n_tiles : (long long)ctx->sm_count * 4);
+    regex_candidates_kernel<<<grid, kThreads, rx->tab_bytes + kTextSmem, st>>>(
+        rx->d_tab, rx->tab_bytes, rx->off_accept, rx->off_trans, rx->n_classes, rx->max_match, d_text, nbytes,
+        (const long long*)d_rec_off, R, n_tiles, cand);
+    const unsigned rblocks = (unsigned)((R + kThreads / 32 - 1) / (kThreads / 32));
+    regex_select_kernel<<<rblocks, kThreads, 0, st>>>(cand, (const long long*)d_rec_off, R, rec_count);
+    CountIn cin{rec_count};
+    scan::reduce_and_scan<long long, scan::SumI64>(cin, R, nullptr, agg, st);
+    scan::apply<long long, scan::SumI64>(cin, BaseOut{rec_base}, R, nullptr, agg, st);
+    regex_write_kernel<<<rblocks, kThreads, 0, st>>>(cand, (const long long*)d_rec_off, R, rec_base, rx->d_tab + 512, d_spans, (long long)cap);
+    regex_finish_kernel<<<1, 1, 0, st>>>(agg + scan::num_tiles(R), (long long)cap, d_num, ctx->d_status);
+    CU_LAUNCH_CHECK(ctx, "regex_scan");
+    return ANON_OK;
+}
+
+int merge_spans_impl(anon_ctx* ctx, WsCursor& ws, const anon_span* d_ner, const int32_t* d_num_ner, int32_t ner_max,
+                     const anon_span* d_rgx, const int32_t* d_num_rgx, int32_t rgx_max, anon_span* d_out, int32_t cap, int32_t* d_num_out)
+{
+    if (!ctx || ner_max < 0 || rgx_max < 0 || cap < 0 || !d_num_out || (ner_max > 0 && !d_ner) || (rgx_max > 0 && !d_rgx) ||
+        (cap > 0 && !d_out))
+        return ANON_ERR_INVALID_ARG;
+    cudaStream_t st = ctx->stream;
+    if (ner_max + (long long)rgx_max == 0) { CU_TRY(ctx, cudaMemsetAsync(d_num_out, 0, 4, st)); return ANON_OK; }
+    const int n1 = ner_max > 0 ? ner_max : 1;
+    uint8_t* keep = (uint8_t*)ws.take((size_t)n1);
+    int* before = (int*)ws.take((size_t)n1 * 4);
+    long long* kpos = (long long*)ws.take((size_t)n1 * 8);
+    long long* agg = (long long*)ws.take(scan::agg_bytes<long long>(n1));
+    if (!keep || !before || !kpos || !agg) return ANON_ERR_OOM;
+    ProfScope ps(ctx, PROF_DECODE, ((double)ner_max + rgx_max) * 32, 5);
+    if (ner_max > 0) {
+        merge_flag_kernel<<<(unsigned)((ner_max + kThreads - 1) / kThreads), kThreads, 0, st>>>(d_ner, d_num_ner, ner_max, d_rgx, d_num_rgx,
+                                                                                              rgx_max, keep, before);
+        KeepIn kin{keep};
+        scan::reduce_and_scan<long long, scan::SumI64>(kin, ner_max, d_num_ner, agg, st);
+        scan::apply<long long, scan::SumI64>(kin, KeepOut{kpos}, ner_max, d_num_ner, agg, st);
+    }
+    const long long n = (long long)ner_max + rgx_max;
+    merge_write_kernel<<<(unsigned)((n + kThreads - 1) / kThreads), kThreads, 0, st>>>(
+        d_ner, d_num_ner, ner_max, d_rgx, d_num_rgx, rgx_max, keep, before, kpos, agg + scan::num_tiles(ner_max), d_out, (long long)cap,
+        d_num_out, ctx->d_status);
+    CU_LAUNCH_CHECK(ctx, "merge_spans");
+    return ANON_OK;
+}
+
+extern "C" int anon_regex_scan(anon_ctx* ctx, const anon_regex* rx, const uint8_t* d_text, size_t text_bytes,
+                               const int64_t* d_record_offsets, int32_t R, anon_span* d_spans, int32_t span_capacity,
+                               int32_t* d_num_spans)
+{
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    WsCursor ws = ws_begin(ctx);
+    return regex_scan_impl(ctx, ws, rx, d_text, text_bytes, d_record_offsets, R, d_spans, span_capacity, d_num_spans);
+}
+
+extern "C" int anon_merge_spans(anon_ctx* ctx, const anon_span* d_ner_spans, const int32_t* d_num_ner, int32_t ner_max,
+                                const anon_span* d_regex_spans, const int32_t* d_num_regex, int32_t regex_max,
+                                anon_span* d_out_spans, int32_t capacity, int32_t* d_num_out)
+{
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    WsCursor ws = ws_begin(ctx);
+    return merge_spans_impl(ctx, ws, d_ner_spans, d_num_ner, ner_max, d_regex_spans, d_num_regex, regex_max, d_out_spans, capacity,
+                            d_num_out);
+}

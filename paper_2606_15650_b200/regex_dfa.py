@@ -335,8 +335,8 @@ def compile_tables(patterns, max_states=60000):
 
 def compile_patterns(typed_patterns, max_match=80):
     """typed_patterns: [(type_id, pattern), ...] in priority order.  Returns the blob for anon_regex_load."""
-    if not 1 <= len(typed_patterns) <= 255:
-        raise ValueError("1..255 patterns")
+    if not 1 <= len(typed_patterns) <= 127:
+        raise ValueError("1..127 patterns")
     if not 1 <= max_match <= 255:
         raise ValueError("max_match must be in [1, 255]")
     class_of, accept, trans = compile_tables([p for _t, p in typed_patterns])

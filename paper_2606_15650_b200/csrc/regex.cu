@@ -20,10 +20,10 @@
 
 struct anon_regex {
     anon_ctx* ctx = nullptr;
-    uint8_t* d_tab = nullptr;        // blob without its 32-byte header, padded to 16 bytes
-    uint32_t tab_bytes = 0;          // padded
+    uint8_t* d_tab = nullptr;        // cw[256], type_of[256], tr[n_states * n_classes] (see regex_candidates_kernel)
+    uint32_t tab_bytes = 0;          // padded to 16 bytes
+    uint32_t smem_bytes = 0;         // dynamic shared memory of regex_candidates_kernel
     int n_states = 0, n_classes = 0, n_patterns = 0, max_match = 0;
-    uint32_t off_accept = 0, off_trans = 0;   // byte offsets inside d_tab
 };
 
 namespace {
@@ -32,6 +32,7 @@ constexpr uint32_t kMagic = 0x31585241u;     // 'ARX1'
 constexpr int kTile = 4096;                  // byte positions per tile of R1
 constexpr int kThreads = 256;
 constexpr int kTextSmem = kTile + 256 + 48;  // tile + look-ahead (max_match <= 255) + alignment slack
+constexpr int kStartWords = (kTile + 256) / 32 + 1;
 
 // largest r in [lo, hi] with off[r] <= p  (off[lo] <= p is given)
 __device__ __forceinline__ int record_of(const long long* __restrict__ off, int lo, int hi, long long p) {
@@ -42,21 +43,35 @@ __device__ __forceinline__ int record_of(const long long* __restrict__ off, int 
     return lo;
 }
 
+// tile_rec[t] = record that holds the first byte of tile t (t = 0 .. n_tiles; the last entry closes the last tile)
+__global__ void __launch_bounds__(kThreads) regex_tile_records_kernel(const long long* __restrict__ rec_off, int R, long long nbytes,
+                                                                      long long n_tiles, int* __restrict__ tile_rec)
+{
+    const long long t = (long long)blockIdx.x * kThreads + threadIdx.x;
+    if (t > n_tiles) return;
+    const long long p = t * kTile < nbytes ? t * kTile : nbytes - 1;
+    tile_rec[t] = record_of(rec_off, 0, R - 1, p);
+}
+
+// Device tables (built by anon_regex_load): cw[256] = class | is_word << 7, type_of[256], then tr[state * n_classes + class] =
+// next state | (accept(next state) + 1) << 16 -- one dependent shared-memory load per DFA step.
 __global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
-    const uint8_t* __restrict__ tab, uint32_t tab_bytes, uint32_t off_accept, uint32_t off_trans, int n_classes, int max_match,
-    const uint8_t* __restrict__ text, long long nbytes, const long long* __restrict__ rec_off, int R, long long n_tiles,
-    uint16_t* __restrict__ cand)
+    const uint8_t* __restrict__ tab, uint32_t tab_bytes, int n_classes, int max_match,
+    const uint8_t* __restrict__ text, long long nbytes, const long long* __restrict__ rec_off, int R, const int* __restrict__ tile_rec,
+    long long n_tiles, uint16_t* __restrict__ cand)
 {
     extern __shared__ __align__(16) uint8_t smem[];
     uint8_t* s_tab = smem;
     uint8_t* s_text = smem + tab_bytes;
-    __shared__ int s_rec[2];
+    uint16_t* s_cand = reinterpret_cast<uint16_t*>(s_text + kTextSmem);     // longest match per position of the tile
+    uint16_t* s_list = s_cand + kTile;                                      // positions that start a walk
+    __shared__ uint32_t s_startbits[kStartWords];                           // record starts inside the tile and its look-ahead
+    __shared__ int s_n, s_next;
     for (uint32_t i = threadIdx.x; i < tab_bytes / 16; i += kThreads)
         reinterpret_cast<uint4*>(s_tab)[i] = reinterpret_cast<const uint4*>(tab)[i];
-    const uint8_t* class_of = s_tab;
-    const uint8_t* is_word = s_tab + 256;
-    const int16_t* accept = reinterpret_cast<const int16_t*>(s_tab + off_accept);
-    const uint16_t* trans = reinterpret_cast<const uint16_t*>(s_tab + off_trans);
+    const uint8_t* cw = s_tab;
+    const uint32_t* tr = reinterpret_cast<const uint32_t*>(s_tab + 512);
+    const int lane = threadIdx.x & 31;
 
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const long long tile0 = tile * kTile;
@@ -69,35 +84,81 @@ __global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
         __syncthreads();                               // previous tile fully consumed (and s_tab written, first time)
         for (int i = threadIdx.x; i < nchunk; i += kThreads)
             reinterpret_cast<uint4*>(s_text)[i] = __ldg(reinterpret_cast<const uint4*>(g0) + i);
-        if (threadIdx.x == 0) s_rec[0] = record_of(rec_off, 0, R - 1, tile0);
-        if (threadIdx.x == 32) s_rec[1] = record_of(rec_off, 0, R - 1, (tile0 + kTile <= nbytes ? tile0 + kTile : nbytes) - 1);
+        if (threadIdx.x < kStartWords) s_startbits[threadIdx.x] = 0;
+        if (threadIdx.x == 0) { s_n = 0; s_next = 0; }
         __syncthreads();
-        const int r_lo = s_rec[0], r_hi = s_rec[1];
+        // record starts (and the end of the text, rec_off[R]) in [tile0, tile0 + kTile + 256): the left word boundary of rule D18
+        // and the distance from a start position to the end of its record both come from these bits
+        for (int r = tile_rec[tile] + threadIdx.x; r <= R; r += kThreads) {
+            const long long o = rec_off[r] - tile0;
+            if (o >= kTile + 256) break;
+            if (o >= 0) atomicOr(&s_startbits[o >> 5], 1u << (o & 31));
+        }
+        __syncthreads();
         const long long sbase = (long long)(reinterpret_cast<uintptr_t>(text) - g0);   // s_text index of text[0] (may be negative)
-#pragma unroll 1
+        // A: which positions can start a match (first transition alive, word boundary on the left)?
+#pragma unroll 4
         for (int k = 0; k < kTile / kThreads; k++) {
-            const long long p = tile0 + k * kThreads + threadIdx.x;
-            if (p >= nbytes) break;
-            const uint8_t* b = s_text + (sbase + p);
-            uint32_t out = 0;
-            uint32_t st = trans[n_classes + class_of[b[0]]];           // from the start state (state 1)
-            if (st != 0) {
-                const int r = record_of(rec_off, r_lo, r_hi, p);
-                const long long rs = rec_off[r], re = rec_off[r + 1];
-                if (p == rs || !is_word[b[-1]]) {
-                    const int limit = (int)(re - p < (long long)max_match ? re - p : (long long)max_match);
-                    int i = 0;
-                    while (true) {
-                        const int a = accept[st];
-                        if (a >= 0 && (i + 1 == re - p || !is_word[b[i + 1]])) out = (uint32_t)(i + 1) | ((uint32_t)a << 8);
-                        if (++i >= limit) break;
-                        st = trans[st * n_classes + class_of[b[i]]];
-                        if (st == 0) break;
-                    }
+            const int o = k * kThreads + threadIdx.x;
+            const long long p = tile0 + o;
+            bool start = false;
+            if (p < nbytes) {
+                const uint8_t* b = s_text + (sbase + p);
+                if ((tr[n_classes + (cw[b[0]] & 0x7f)] & 0xffffu) != 0)
+                    start = ((s_startbits[o >> 5] >> (o & 31)) & 1u) || !(cw[b[-1]] & 0x80);
+            }
+            const uint32_t m = __ballot_sync(0xffffffffu, start);
+            int base = 0;
+            if (lane == 0 && m) base = atomicAdd(&s_n, __popc(m));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (start) s_list[base + __popc(m & ((1u << lane) - 1))] = (uint16_t)o;
+            else s_cand[o] = 0;
+        }
+        __syncthreads();
+        // B: the walks, handed out one by one -- a lane that finishes takes the next start, so a warp pays the sum of its
+        // walks' steps / 32, not 32 x the longest
+        const int n = s_n;
+        int o = -1, i = 0, limit = 0;
+        int left = 0;                                  // bytes from the start position to the end of its record (capped)
+        uint32_t st = 1, out = 0, cwn = 0;
+        const uint8_t* b = s_text;
+        while (true) {
+            if (o == -1) {
+                const int j = atomicAdd(&s_next, 1);
+                if (j < n) {
+                    o = s_list[j];
+                    // bytes to the end of the record = distance to the next record start after o (max_match + 1 if none is near)
+                    int w = o >> 5;
+                    uint32_t bits = s_startbits[w] & ~((2u << (o & 31)) - 1u);
+                    const int w_last = (o + max_match) >> 5;
+                    while (!bits && w < w_last) bits = s_startbits[++w];
+                    left = bits ? (w << 5) + __ffs(bits) - 1 - o : max_match + 1;
+                    limit = left < max_match ? left : max_match;
+                    b = s_text + (sbase + tile0 + o);
+                    st = 1; i = 0; out = 0; cwn = cw[b[0]];
+                } else {
+                    o = -2;
                 }
             }
-            cand[p] = (uint16_t)out;
+            if (__all_sync(0xffffffffu, o == -2)) break;
+            if (o >= 0) {
+                const uint32_t cwi = cwn;
+                cwn = (i + 1 < left) ? cw[b[i + 1]] : 0u;                       // the record's edge counts as a non-word byte
+                const uint32_t t = tr[st * n_classes + (cwi & 0x7f)];
+                st = t & 0xffffu;
+                bool done = st == 0;
+                if (!done) {
+                    if ((t >> 16) && !(cwn & 0x80)) out = (uint32_t)(i + 1) | (((t >> 16) - 1) << 8);
+                    done = ++i >= limit;
+                }
+                if (done) { s_cand[o] = (uint16_t)out; o = -1; }
+            }
         }
+        __syncthreads();
+        // coalesced store of the tile's candidates (cand is padded, so the ragged last tile stores whole 16-byte words)
+        const long long n_here = nbytes - tile0 < kTile ? nbytes - tile0 : kTile;
+        for (int q = threadIdx.x; q * 8 < n_here; q += kThreads)
+            reinterpret_cast<uint4*>(cand + tile0)[q] = reinterpret_cast<const uint4*>(s_cand)[q];
     }
 }
 
@@ -287,20 +348,27 @@ extern "C" int anon_regex_load(anon_ctx* ctx, const void* h_blob, size_t blob_by
     for (uint64_t s = 0; s < ns; s++) if (accept[s] < -1 || accept[s] >= (int)np) return ANON_ERR_INVALID_ARG;
     for (uint64_t i = 0; i < ns * nc; i++) if (trans[i] >= ns || (i < nc && trans[i] != 0)) return ANON_ERR_INVALID_ARG;
     if (accept[0] >= 0 || accept[1] >= 0) return ANON_ERR_INVALID_ARG;        // dead state / empty match
-    const uint64_t padded = (blob_bytes - 32 + 15) / 16 * 16;
-    if (padded + kTextSmem > (uint64_t)ctx->smem_optin) return ANON_ERR_UNSUPPORTED;   // tables must fit shared memory
+    if (nc > 128) return ANON_ERR_UNSUPPORTED;                                 // the class shares a byte with the word flag
+    const uint64_t padded = (512 + 4 * ns * nc + 15) / 16 * 16;
+    const uint64_t smem_need = padded + kTextSmem + 2 * kTile * 2;
+    if (smem_need > (uint64_t)ctx->smem_optin) return ANON_ERR_UNSUPPORTED;    // tables must fit shared memory beside a tile
+    std::vector<uint8_t> dev_tab(padded, 0);
+    for (int c = 0; c < 256; c++) {
+        dev_tab[c] = (uint8_t)(tab[c] | (tab[256 + c] ? 0x80 : 0));
+        dev_tab[256 + c] = tab[512 + c];
+    }
+    uint32_t* tr = reinterpret_cast<uint32_t*>(dev_tab.data() + 512);
+    for (uint64_t i = 0; i < ns * nc; i++) tr[i] = (uint32_t)trans[i] | ((uint32_t)(accept[trans[i]] + 1) << 16);
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     anon_regex* rx = new (std::nothrow) anon_regex();
     if (!rx) return ANON_ERR_OOM;
-    rx->ctx = ctx; rx->tab_bytes = (uint32_t)padded;
+    rx->ctx = ctx; rx->tab_bytes = (uint32_t)padded; rx->smem_bytes = (uint32_t)smem_need;
     rx->n_states = (int)ns; rx->n_classes = (int)nc; rx->n_patterns = (int)np; rx->max_match = (int)mm;
-    rx->off_accept = (uint32_t)off_accept; rx->off_trans = (uint32_t)off_trans;
     if (cudaMalloc(&rx->d_tab, padded) != cudaSuccess) { cudaGetLastError(); delete rx; return ANON_ERR_OOM; }
-    cudaError_t e = cudaMemsetAsync(rx->d_tab, 0, padded, ctx->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(rx->d_tab, tab, blob_bytes - 32, cudaMemcpyHostToDevice, ctx->stream);
+    cudaError_t e = cudaMemcpyAsync(rx->d_tab, dev_tab.data(), padded, cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(regex_candidates_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(padded + kTextSmem));
+        e = cudaFuncSetAttribute(regex_candidates_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_need);
     if (e != cudaSuccess) { cudaFree(rx->d_tab); delete rx; return cuda_fail(ctx, e, "anon_regex_load"); }
     *out = rx;
     return ANON_OK;
@@ -321,23 +389,25 @@ int regex_scan_impl(anon_ctx* ctx, WsCursor& ws, const anon_regex* rx, const uin
     cudaStream_t st = ctx->stream;
     if (R == 0 || text_bytes == 0) { CU_TRY(ctx, cudaMemsetAsync(d_num, 0, 4, st)); return ANON_OK; }
     const long long nbytes = (long long)text_bytes;
-    uint16_t* cand = (uint16_t*)ws.take(((size_t)nbytes + 8) * 2);
+    const long long n_tiles = (nbytes + kTile - 1) / kTile;
+    uint16_t* cand = (uint16_t*)ws.take(((size_t)nbytes + 16) * 2);
+    int* tile_rec = (int*)ws.take(((size_t)n_tiles + 1) * 4);
     int* rec_count = (int*)ws.take((size_t)R * 4);
     long long* rec_base = (long long*)ws.take((size_t)R * 8);
     long long* agg = (long long*)ws.take(scan::agg_bytes<long long>(R));
-    if (!cand || !rec_count || !rec_base || !agg) return ANON_ERR_OOM;
-    ProfScope ps(ctx, PROF_DECODE, (double)nbytes * 7 + (double)R * 28, 7);
-    const long long n_tiles = (nbytes + kTile - 1) / kTile;
-    const unsigned grid = (unsigned)(n_tiles < (long long)ctx->sm_count * 4 ? n_tiles : (long long)ctx->sm_count * 4);
-    regex_candidates_kernel<<<grid, kThreads, rx->tab_bytes + kTextSmem, st>>>(
-        rx->d_tab, rx->tab_bytes, rx->off_accept, rx->off_trans, rx->n_classes, rx->max_match, d_text, nbytes,
-        (const long long*)d_rec_off, R, n_tiles, cand);
+    if (!cand || !tile_rec || !rec_count || !rec_base || !agg) return ANON_ERR_OOM;
+    ProfScope ps(ctx, PROF_DECODE, (double)nbytes * 7 + (double)R * 28, 8);
+    const unsigned grid = (unsigned)(n_tiles < (long long)ctx->sm_count * 6 ? n_tiles : (long long)ctx->sm_count * 6);
+    regex_tile_records_kernel<<<(unsigned)((n_tiles + 1 + kThreads - 1) / kThreads), kThreads, 0, st>>>((const long long*)d_rec_off, R, nbytes,
+                                                                                                      n_tiles, tile_rec);
+    regex_candidates_kernel<<<grid, kThreads, rx->smem_bytes, st>>>(rx->d_tab, rx->tab_bytes, rx->n_classes, rx->max_match, d_text, nbytes,
+                                                                    (const long long*)d_rec_off, R, tile_rec, n_tiles, cand);
     const unsigned rblocks = (unsigned)((R + kThreads / 32 - 1) / (kThreads / 32));
     regex_select_kernel<<<rblocks, kThreads, 0, st>>>(cand, (const long long*)d_rec_off, R, rec_count);
     CountIn cin{rec_count};
     scan::reduce_and_scan<long long, scan::SumI64>(cin, R, nullptr, agg, st);
     scan::apply<long long, scan::SumI64>(cin, BaseOut{rec_base}, R, nullptr, agg, st);
-    regex_write_kernel<<<rblocks, kThreads, 0, st>>>(cand, (const long long*)d_rec_off, R, rec_base, rx->d_tab + 512, d_spans, (long long)cap);
+    regex_write_kernel<<<rblocks, kThreads, 0, st>>>(cand, (const long long*)d_rec_off, R, rec_base, rx->d_tab + 256, d_spans, (long long)cap);
     regex_finish_kernel<<<1, 1, 0, st>>>(agg + scan::num_tiles(R), (long long)cap, d_num, ctx->d_status);
     CU_LAUNCH_CHECK(ctx, "regex_scan");
     return ANON_OK;

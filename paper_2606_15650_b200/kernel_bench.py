@@ -4,8 +4,8 @@
 
 Times, with CUDA events on the context's stream after warm-up: the four encoder GEMM shapes (QKV, out-proj+residual,
 FFN1+GELU, FFN2+residual) against cuBLAS (torch.matmul, no epilogue -- context, not the product), the varlen
-attention kernel on a lognormal length mix and at n = 512, and the HMAC-SHA256 kernel with dedup disabled
-(anon_hmac_spans; SURVEY.md §8(d) c5 "HMAC-only run").  Prints one JSON object; inputs are seeded and larger than
+attention kernel on a lognormal length mix and at n = 512, the HMAC-SHA256 kernel with dedup disabled
+(anon_hmac_spans; SURVEY.md §8(d) c5 "HMAC-only run"), and the DFA regex scan (NEXT-4) over 400 MB of record text.  Prints one JSON object; inputs are seeded and larger than
 L2 where the kernel is memory-bound.  Peaks: MEASURED_PEAKS.json (else the B200_PROFILING.md fallback).
 """
 import argparse
@@ -18,6 +18,12 @@ import numpy as np
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
+
+
+# rule D17's pattern set: one pattern per synthetic entity kind, in type order
+REGEX_PATTERNS = [r"(?:[0-9]{1,3}\.){3}[0-9]{1,3}", r"(?:[0-9a-f]{1,4}:){7}[0-9a-f]{1,4}",
+                  r"(?:[a-z0-9]+\.)+(?:example|internal|corp|lan|test|invalid)", r"CVE-[0-9]{4}-[0-9]{4,7}",
+                  r"(?:[0-9a-f]{2}:){5}[0-9a-f]{2}", r"[0-9a-f]{16,32}"]
 
 
 def _peaks():
@@ -38,6 +44,8 @@ def main():
     ap.add_argument("--hidden", type=int, default=768)
     ap.add_argument("--spans", type=int, default=8_000_000)
     ap.add_argument("--iters", type=int, default=10)
+    ap.add_argument("--regex-records", type=int, default=2000)
+    ap.add_argument("--regex-mb", type=float, default=400.0)
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("kernel_bench: no CUDA device (the hot path has no CPU fallback)")
@@ -111,6 +119,30 @@ def main():
                                    "bytes_per_s_gb": (data.size + S * 40) / ms / 1e6,
                                    "roofline": {"bound": "alu", "achieved": comp / ms * 1e3 * alu_per_comp / 1e12, "peak": alu_peak / 1e12,
                                                 "unit": "T ALU-pipe instr/s", "frac": comp / ms * 1e3 * alu_per_comp / alu_peak}}
+
+    # NEXT-4: DFA regex scan over record text (HBM-bound; algorithmic traffic = 1 B per text byte read + 16 B per span written)
+    from paper_2606_15650_b200 import regex_dfa
+    rec = gen.workload_stream(n_records=args.regex_records, n_pool=50000)
+    reps = max(1, int(args.regex_mb * 1e6 / rec["text"].size))
+    text = np.tile(rec["text"], reps)
+    sizes = np.tile(np.diff(rec["rec_off"]), reps)
+    roff = np.zeros(sizes.size + 1, np.int64)
+    roff[1:] = np.cumsum(sizes)
+    blob = regex_dfa.compile_patterns(list(enumerate(REGEX_PATTERNS)), 80)
+    d_text, d_roff = torch.from_numpy(text).to(dev), torch.from_numpy(roff).to(dev)
+    cap = text.size // 40
+    spans = torch.empty((cap, 4), dtype=torch.int32, device=dev)
+    num = torch.zeros(1, dtype=torch.int32, device=dev)
+    ctx2 = P.Context(0, workspace_bytes=int(text.size * 2.2) + (64 << 20))
+    rx2 = P.Regex(ctx2, blob)
+    ms = timeit(lambda: P.anon_regex_scan(ctx2, rx2, d_text, d_roff, spans, num), n=5)
+    assert ctx2.sync() == 0
+    nsp = int(num.item())
+    byts = text.size + 16.0 * nsp + 8.0 * roff.size
+    res["regex_scan"] = {"text_bytes": int(text.size), "records": int(sizes.size), "spans": nsp, "ms": ms,
+                         "text_gb_per_s": text.size / ms / 1e6,
+                         "roofline": {"bound": "hbm", "achieved": byts / ms / 1e6, "peak": hbm, "unit": "GB/s", "frac": byts / ms / 1e6 / hbm}}
+    rx2.close(); ctx2.close()
     print(json.dumps(res, indent=1))
     ctx.close()
 

@@ -23,6 +23,7 @@ struct anon_regex {
     uint8_t* d_tab = nullptr;        // cw[256], type_of[256], tr[n_states * n_classes] (see regex_candidates_kernel)
     uint32_t tab_bytes = 0;          // padded to 16 bytes
     uint32_t smem_bytes = 0;         // dynamic shared memory of regex_candidates_kernel
+    int ctas_per_sm = 1;             // resident CTAs of regex_candidates_kernel per SM (sizes its persistent grid)
     int n_states = 0, n_classes = 0, n_patterns = 0, max_match = 0;
 };
 
@@ -33,6 +34,7 @@ constexpr int kTile = 4096;                  // byte positions per tile of R1
 constexpr int kThreads = 256;
 constexpr int kTextSmem = kTile + 256 + 48;  // tile + look-ahead (max_match <= 255) + alignment slack
 constexpr int kStartWords = (kTile + 256) / 32 + 1;
+constexpr int kShortWalk = 8;                // steps of the first walking pass of R1
 
 // largest r in [lo, hi] with off[r] <= p  (off[lo] <= p is given)
 __device__ __forceinline__ int record_of(const long long* __restrict__ off, int lo, int hi, long long p) {
@@ -53,6 +55,27 @@ __global__ void __launch_bounds__(kThreads) regex_tile_records_kernel(const long
     tile_rec[t] = record_of(rec_off, 0, R - 1, p);
 }
 
+// One DFA walk from a start position: the longest accepting prefix that ends on a word boundary, as len | pattern << 8.
+// `left` = bytes to the end of the record (capped), `lim` = steps allowed in this call.  Returns true if the automaton is
+// still alive after `lim` steps (the caller may walk on with a larger `lim`).
+__device__ __forceinline__ bool dfa_walk(const uint8_t* __restrict__ b, int left, int lim, const uint8_t* __restrict__ cw,
+                                         const uint32_t* __restrict__ tr, int n_classes, uint32_t& out)
+{
+    uint32_t st = 1, cwn = cw[b[0]];
+    out = 0;
+    int i = 0;
+    while (i < lim) {
+        const uint32_t cwi = cwn;
+        cwn = (i + 1 < left) ? cw[b[i + 1]] : 0u;                               // the record's edge counts as a non-word byte
+        const uint32_t t = tr[st * n_classes + (cwi & 0x7f)];
+        st = t & 0xffffu;
+        if (st == 0) return false;
+        ++i;
+        if ((t >> 16) && !(cwn & 0x80)) out = (uint32_t)i | (((t >> 16) - 1) << 8);
+    }
+    return true;
+}
+
 // Device tables (built by anon_regex_load): cw[256] = class | is_word << 7, type_of[256], then tr[state * n_classes + class] =
 // next state | (accept(next state) + 1) << 16 -- one dependent shared-memory load per DFA step.
 __global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
@@ -65,13 +88,16 @@ __global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
     uint8_t* s_text = smem + tab_bytes;
     uint16_t* s_cand = reinterpret_cast<uint16_t*>(s_text + kTextSmem);     // longest match per position of the tile
     uint16_t* s_list = s_cand + kTile;                                      // positions that start a walk
-    __shared__ uint32_t s_startbits[kStartWords];                           // record starts inside the tile and its look-ahead
-    __shared__ int s_n, s_next;
+    uint16_t* s_surv = s_list + kTile;                                      // starts whose walk outlives the short first pass
+    __shared__ uint32_t s_recbits[kStartWords];                             // record starts inside the tile and its look-ahead
+    __shared__ uint32_t s_startbits[kTile / 32];                            // positions that can start a match
+    __shared__ int s_wtot[kThreads / 32];
+    __shared__ int s_nsurv;
     for (uint32_t i = threadIdx.x; i < tab_bytes / 16; i += kThreads)
         reinterpret_cast<uint4*>(s_tab)[i] = reinterpret_cast<const uint4*>(tab)[i];
     const uint8_t* cw = s_tab;
     const uint32_t* tr = reinterpret_cast<const uint32_t*>(s_tab + 512);
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const long long tile0 = tile * kTile;
@@ -84,79 +110,94 @@ __global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
         __syncthreads();                               // previous tile fully consumed (and s_tab written, first time)
         for (int i = threadIdx.x; i < nchunk; i += kThreads)
             reinterpret_cast<uint4*>(s_text)[i] = __ldg(reinterpret_cast<const uint4*>(g0) + i);
-        if (threadIdx.x < kStartWords) s_startbits[threadIdx.x] = 0;
-        if (threadIdx.x == 0) { s_n = 0; s_next = 0; }
+        for (int i = threadIdx.x; i < kTile / 8; i += kThreads) reinterpret_cast<uint4*>(s_cand)[i] = make_uint4(0, 0, 0, 0);
+        if (threadIdx.x < kStartWords) s_recbits[threadIdx.x] = 0;
+        if (threadIdx.x == 0) s_nsurv = 0;
         __syncthreads();
         // record starts (and the end of the text, rec_off[R]) in [tile0, tile0 + kTile + 256): the left word boundary of rule D18
         // and the distance from a start position to the end of its record both come from these bits
         for (int r = tile_rec[tile] + threadIdx.x; r <= R; r += kThreads) {
             const long long o = rec_off[r] - tile0;
             if (o >= kTile + 256) break;
-            if (o >= 0) atomicOr(&s_startbits[o >> 5], 1u << (o & 31));
+            if (o >= 0) atomicOr(&s_recbits[o >> 5], 1u << (o & 31));
         }
         __syncthreads();
-        const long long sbase = (long long)(reinterpret_cast<uintptr_t>(text) - g0);   // s_text index of text[0] (may be negative)
-        // A: which positions can start a match (first transition alive, word boundary on the left)?
-#pragma unroll 4
-        for (int k = 0; k < kTile / kThreads; k++) {
-            const int o = k * kThreads + threadIdx.x;
-            const long long p = tile0 + o;
-            bool start = false;
-            if (p < nbytes) {
-                const uint8_t* b = s_text + (sbase + p);
-                if ((tr[n_classes + (cw[b[0]] & 0x7f)] & 0xffffu) != 0)
-                    start = ((s_startbits[o >> 5] >> (o & 31)) & 1u) || !(cw[b[-1]] & 0x80);
+        const uint8_t* tbase = s_text + ((long long)(reinterpret_cast<uintptr_t>(text) - g0) + tile0);   // tile position 0
+        const int n_here = (int)(nbytes - tile0 < kTile ? nbytes - tile0 : kTile);
+        // A: which positions can start a match (first transition alive, word boundary on the left)?  Four per thread.
+#pragma unroll
+        for (int k = 0; k < kTile / 4 / kThreads; k++) {
+            const int q = k * kThreads + threadIdx.x, o = q * 4;
+            uint32_t nib = 0;
+            if (o < n_here) {
+                const uint32_t rb = (s_recbits[q >> 3] >> ((q & 7) * 4)) & 0xfu;
+                uint32_t prev_word = (o > 0 || tile0 > 0) ? (cw[tbase[o - 1]] & 0x80u) : 0u;
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    const uint32_t c = cw[tbase[o + j]];
+                    const bool alive = (tr[n_classes + (c & 0x7f)] & 0xffffu) != 0;
+                    if (alive && o + j < n_here && (!prev_word || ((rb >> j) & 1u))) nib |= 1u << j;
+                    prev_word = c & 0x80u;
+                }
             }
-            const uint32_t m = __ballot_sync(0xffffffffu, start);
-            int base = 0;
-            if (lane == 0 && m) base = atomicAdd(&s_n, __popc(m));
-            base = __shfl_sync(0xffffffffu, base, 0);
-            if (start) s_list[base + __popc(m & ((1u << lane) - 1))] = (uint16_t)o;
-            else s_cand[o] = 0;
+            uint32_t v = nib << ((lane & 7) * 4);
+            v |= __shfl_xor_sync(0xffffffffu, v, 1);
+            v |= __shfl_xor_sync(0xffffffffu, v, 2);
+            v |= __shfl_xor_sync(0xffffffffu, v, 4);
+            if ((lane & 7) == 0) s_startbits[q >> 3] = v;
         }
         __syncthreads();
-        // B: the walks, handed out one by one -- a lane that finishes takes the next start, so a warp pays the sum of its
-        // walks' steps / 32, not 32 x the longest
-        const int n = s_n;
-        int o = -1, i = 0, limit = 0;
-        int left = 0;                                  // bytes from the start position to the end of its record (capped)
-        uint32_t st = 1, out = 0, cwn = 0;
-        const uint8_t* b = s_text;
-        while (true) {
-            if (o == -1) {
-                const int j = atomicAdd(&s_next, 1);
-                if (j < n) {
-                    o = s_list[j];
-                    // bytes to the end of the record = distance to the next record start after o (max_match + 1 if none is near)
-                    int w = o >> 5;
-                    uint32_t bits = s_startbits[w] & ~((2u << (o & 31)) - 1u);
-                    const int w_last = (o + max_match) >> 5;
-                    while (!bits && w < w_last) bits = s_startbits[++w];
-                    left = bits ? (w << 5) + __ffs(bits) - 1 - o : max_match + 1;
-                    limit = left < max_match ? left : max_match;
-                    b = s_text + (sbase + tile0 + o);
-                    st = 1; i = 0; out = 0; cwn = cw[b[0]];
-                } else {
-                    o = -2;
-                }
-            }
-            if (__all_sync(0xffffffffu, o == -2)) break;
-            if (o >= 0) {
-                const uint32_t cwi = cwn;
-                cwn = (i + 1 < left) ? cw[b[i + 1]] : 0u;                       // the record's edge counts as a non-word byte
-                const uint32_t t = tr[st * n_classes + (cwi & 0x7f)];
-                st = t & 0xffffu;
-                bool done = st == 0;
-                if (!done) {
-                    if ((t >> 16) && !(cwn & 0x80)) out = (uint32_t)(i + 1) | (((t >> 16) - 1) << 8);
-                    done = ++i >= limit;
-                }
-                if (done) { s_cand[o] = (uint16_t)out; o = -1; }
-            }
+        // compaction of the start bits into a position list: warp w owns 16 words, lanes 0..15 one word each
+        uint32_t word = lane < 16 ? s_startbits[warp * 16 + lane] : 0u;
+        int incl = __popc(word);
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        if (lane == 31) s_wtot[warp] = incl;
+        __syncthreads();
+        int pos = incl - __popc(word), n = 0;
+#pragma unroll
+        for (int w = 0; w < kThreads / 32; w++) {
+            if (w < warp) pos += s_wtot[w];
+            n += s_wtot[w];
+        }
+        while (word) {
+            s_list[pos++] = (uint16_t)((warp * 16 + lane) * 32 + __ffs(word) - 1);
+            word &= word - 1;
+        }
+        __syncthreads();
+        // B: the walks.  First pass: every start, at most kShortWalk steps (most die on the next separator); the few that
+        // are still alive are walked to the end in a second pass, so a warp never waits 80 steps for one long entity per round.
+        for (int idx = threadIdx.x; idx < n; idx += kThreads) {
+            const int o = s_list[idx];
+            int w = o >> 5;                            // bytes to the end of the record = distance to the next record start
+            uint32_t bits = s_recbits[w] & ~((2u << (o & 31)) - 1u);
+            const int w_last = (o + max_match) >> 5;
+            while (!bits && w < w_last) bits = s_recbits[++w];
+            const int left = bits ? (w << 5) + __ffs(bits) - 1 - o : max_match + 1;
+            const int limit = left < max_match ? left : max_match;
+            uint32_t out;
+            const bool alive = dfa_walk(tbase + o, left, limit < kShortWalk ? limit : kShortWalk, cw, tr, n_classes, out);
+            if (alive && limit > kShortWalk) s_surv[atomicAdd(&s_nsurv, 1)] = (uint16_t)o;
+            else s_cand[o] = (uint16_t)out;
+        }
+        __syncthreads();
+        const int nsurv = s_nsurv;
+        for (int idx = threadIdx.x; idx < nsurv; idx += kThreads) {
+            const int o = s_surv[idx];
+            int w = o >> 5;
+            uint32_t bits = s_recbits[w] & ~((2u << (o & 31)) - 1u);
+            const int w_last = (o + max_match) >> 5;
+            while (!bits && w < w_last) bits = s_recbits[++w];
+            const int left = bits ? (w << 5) + __ffs(bits) - 1 - o : max_match + 1;
+            uint32_t out;
+            dfa_walk(tbase + o, left, left < max_match ? left : max_match, cw, tr, n_classes, out);
+            s_cand[o] = (uint16_t)out;
         }
         __syncthreads();
         // coalesced store of the tile's candidates (cand is padded, so the ragged last tile stores whole 16-byte words)
-        const long long n_here = nbytes - tile0 < kTile ? nbytes - tile0 : kTile;
         for (int q = threadIdx.x; q * 8 < n_here; q += kThreads)
             reinterpret_cast<uint4*>(cand + tile0)[q] = reinterpret_cast<const uint4*>(s_cand)[q];
     }
@@ -350,7 +391,7 @@ extern "C" int anon_regex_load(anon_ctx* ctx, const void* h_blob, size_t blob_by
     if (accept[0] >= 0 || accept[1] >= 0) return ANON_ERR_INVALID_ARG;        // dead state / empty match
     if (nc > 128) return ANON_ERR_UNSUPPORTED;                                 // the class shares a byte with the word flag
     const uint64_t padded = (512 + 4 * ns * nc + 15) / 16 * 16;
-    const uint64_t smem_need = padded + kTextSmem + 2 * kTile * 2;
+    const uint64_t smem_need = padded + kTextSmem + 3 * kTile * 2;
     if (smem_need > (uint64_t)ctx->smem_optin) return ANON_ERR_UNSUPPORTED;    // tables must fit shared memory beside a tile
     std::vector<uint8_t> dev_tab(padded, 0);
     for (int c = 0; c < 256; c++) {
@@ -369,7 +410,10 @@ extern "C" int anon_regex_load(anon_ctx* ctx, const void* h_blob, size_t blob_by
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(regex_candidates_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_need);
+    if (e == cudaSuccess)
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&rx->ctas_per_sm, regex_candidates_kernel, kThreads, smem_need);
     if (e != cudaSuccess) { cudaFree(rx->d_tab); delete rx; return cuda_fail(ctx, e, "anon_regex_load"); }
+    if (rx->ctas_per_sm < 1) rx->ctas_per_sm = 1;
     *out = rx;
     return ANON_OK;
 }
@@ -397,7 +441,8 @@ int regex_scan_impl(anon_ctx* ctx, WsCursor& ws, const anon_regex* rx, const uin
     long long* agg = (long long*)ws.take(scan::agg_bytes<long long>(R));
     if (!cand || !tile_rec || !rec_count || !rec_base || !agg) return ANON_ERR_OOM;
     ProfScope ps(ctx, PROF_DECODE, (double)nbytes * 7 + (double)R * 28, 8);
-    const unsigned grid = (unsigned)(n_tiles < (long long)ctx->sm_count * 6 ? n_tiles : (long long)ctx->sm_count * 6);
+    const long long resident = (long long)ctx->sm_count * rx->ctas_per_sm;
+    const unsigned grid = (unsigned)(n_tiles < resident ? n_tiles : resident);
     regex_tile_records_kernel<<<(unsigned)((n_tiles + 1 + kThreads - 1) / kThreads), kThreads, 0, st>>>((const long long*)d_rec_off, R, nbytes,
                                                                                                       n_tiles, tile_rec);
     regex_candidates_kernel<<<grid, kThreads, rx->smem_bytes, st>>>(rx->d_tab, rx->tab_bytes, rx->n_classes, rx->max_match, d_text, nbytes,

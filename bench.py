@@ -434,8 +434,14 @@ def run_stream(args):
     cap = maxT // 4 + 4096
     out_cap = cap * 32
     ws = P.anon_workspace_bytes(desc, maxT, maxB) + 96 * maxT + 2 * max_text + out_cap + 40 * cap + (128 << 20)
+    if args.regex:
+        ws += 2 * max_text + 48 * cap + (16 << 20)
     ctx = P.Context(local, workspace_bytes=ws)
     W = P.Weights(ctx, desc, gen.pack_blob(w))
+    rx = None
+    if args.regex:      # NEXT-4: the hybrid strategy -- regex spans merged into the NER spans before the gather
+        from paper_2606_15650_b200 import kernel_bench, regex_dfa
+        rx = P.Regex(ctx, regex_dfa.compile_patterns(list(enumerate(kernel_bench.REGEX_PATTERNS)), 80))
     log(f"[rank {rank}] setup {time.time() - t_setup:.0f}s: {len(batches)} batches, {T_all} window-tokens, "
         f"{len(win['cu_seqlens']) - 1} windows, max batch {maxT} tokens, ws={ws / 2**30:.1f} GiB")
 
@@ -452,12 +458,20 @@ def run_stream(args):
     out_off = torch.zeros(cap + 1, dtype=torch.int64, device=dev)
     hit = torch.zeros(cap, dtype=torch.uint8, device=dev)
     nsp_host = torch.zeros(1, dtype=torch.int32).pin_memory()
+    if rx is not None:
+        ner_spans, rx_spans = torch.zeros_like(spans), torch.zeros_like(spans)
+        n_ner, n_rx = torch.zeros(1, dtype=torch.int32, device=dev), torch.zeros(1, dtype=torch.int32, device=dev)
 
     def step(cache, k):
         b = dbat[k]
         T = b["ids"].numel()
         P.anon_ner_forward(ctx, W, b["ids"], b["cu"], None, labels[:T])
-        P.anon_decode_spans(ctx, labels[:T], b["meta"], desc["num_labels"], spans, nsp)
+        if rx is None:
+            P.anon_decode_spans(ctx, labels[:T], b["meta"], desc["num_labels"], spans, nsp)
+        else:           # counts stay on the device between decode, scan and merge
+            P.anon_decode_spans(ctx, labels[:T], b["meta"], desc["num_labels"], ner_spans, n_ner)
+            P.anon_regex_scan(ctx, rx, b["text"], b["ro"], rx_spans, n_rx)
+            P.anon_merge_spans(ctx, ner_spans, n_ner, rx_spans, n_rx, spans, nsp)
         nsp_host.copy_(nsp, non_blocking=True)
         rc = ctx.sync()
         if rc:
@@ -510,6 +524,8 @@ def run_stream(args):
                 new_text=torch.zeros(max_text + out_cap, dtype=torch.uint8).pin_memory().numpy(),
                 new_ro=torch.zeros(max(b["rec_off"].size for b in batches), dtype=torch.int64).pin_memory().numpy())
     cache2 = P.Cache(ctx, 1 << 20, 64 << 20)
+    if rx is not None:
+        P.anon_ctx_set_regex(ctx, rx)
     barrier(world)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     h2d = d2h = 0
@@ -542,6 +558,8 @@ def run_stream(args):
                                % (n_records, rec["text"].size / 2**20, len(win["cu_seqlens"]) - 1, T_all, args.batch_tokens),
                    "batches": nb, "weights": "W2 planted-detector, seeded random-init", "slug_len": SLUG_LEN,
                    "splice": "records rewritten on the device (anon_splice_records) inside the timed region",
+                   "regex": ("hybrid detection: DFA scan of %d patterns over the batch text + regex/NER span merge inside the "
+                             "timed region (NEXT-4)" % len(kernel_bench.REGEX_PATTERNS)) if rx is not None else "off (--regex enables NEXT-4)",
                    "spans": S_all, "planted_entities": int(rec["n_entities"]), "unique_entities": st["n_unique"],
                    "cache_hit_rate": st["n_hits"] / max(st["n_lookups"], 1),
                    "l2": "inputs larger than L2 (each batch streams ~20 GB of activations through HBM)"},
@@ -642,6 +660,7 @@ def main():
     ap.add_argument("--records", type=int, default=None, help="override the number of records / sequences / strings")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--batch-tokens", type=int, default=1 << 20, help="stream workload: token budget per batch")
+    ap.add_argument("--regex", action="store_true", help="stream workload: also run the regex detector and merge its spans (NEXT-4)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         log("note: timing rules ask for >= 3 warm-up steps")

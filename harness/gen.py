@@ -23,6 +23,13 @@ DESCS = {
     "large": dict(layers=24, hidden=1024, heads=16, ffn=4096, vocab=250002, num_labels=13,
                   max_pos=512, ln_eps=1e-5, dtype=1),
 }
+# NEXT-3: ModernBERT-shaped variants (reading D20): arch 1 = pre-LN, RoPE, GeGLU (W_i is [2 ffn, hidden]), local window 128
+# in every layer that is not a multiple of global_every, no biases.  "base_modern" has ModernBERT-base's published sizes.
+_MODERN = dict(arch=1, local_window=128, global_every=3, rope_theta_global=160000.0, rope_theta_local=10000.0)
+DESCS["tiny_modern"] = dict(layers=4, hidden=128, heads=2, ffn=192, vocab=8192, num_labels=9, max_pos=512, ln_eps=1e-5,
+                            dtype=0, **_MODERN)
+DESCS["base_modern"] = dict(layers=22, hidden=768, heads=12, ffn=1152, vocab=50368, num_labels=13, max_pos=512, ln_eps=1e-5,
+                            dtype=1, **_MODERN)
 TYPE_NAMES_6 = ["IP_ADDRESS", "IPV6_ADDRESS", "HOSTNAME", "CVE_ID", "MAC_ADDRESS", "SERIAL_NUMBER"]
 TYPE_NAMES_4 = ["TYPE0", "TYPE1", "TYPE2", "TYPE3"]
 PAD, CLS, SEP, UNK, MASK = 0, 1, 2, 3, 4
@@ -78,6 +85,48 @@ def make_weights(desc, seed, planted=None):
             for k in ("W_qkv", "W_o", "W_1", "W_2"):
                 lw[k] = bf16_round(lw[k])
     return w
+
+
+MODERN_LAYER_ORDER = ["g_a", "W_qkv", "W_o", "g_m", "W_i", "W_2"]
+
+
+def make_weights_modern(desc, seed, planted=None):
+    """Parameters of the arch-1 encoder (names of oracle/encoder_modern.py); W1 or planted-detector W2 like make_weights."""
+    g = rng(seed)
+    H, F, V, NL, L = (desc[k] for k in ("hidden", "ffn", "vocab", "num_labels", "layers"))
+    n = lambda *s: (0.02 * g.standard_normal(s)).astype(np.float32)
+    gam = lambda: (1.0 + 0.02 * g.standard_normal(H)).astype(np.float32)
+    w = {"E_w": n(V, H), "g_e": gam(), "layers": []}
+    for _ in range(L):
+        w["layers"].append({"g_a": gam(), "W_qkv": n(3 * H, H), "W_o": n(H, H), "g_m": gam(), "W_i": n(2 * F, H), "W_2": n(H, F)})
+    w["g_f"] = gam()
+    w["W_c"] = n(NL, H)
+    w["b_c"] = n(NL)
+    if planted is not None:
+        alpha, beta, gamma = planted
+        q, _ = np.linalg.qr(g.standard_normal((H, NL - 1)))
+        for c in range(1, NL):
+            u = q[:, c - 1].astype(np.float32)
+            lo = FIRST_ID + (c - 1) * BAND
+            w["E_w"][lo:lo + BAND] += alpha * u
+            w["W_c"][c] += beta * u
+        w["b_c"][0] += gamma
+    if desc["dtype"] == 1:
+        for k in ("E_w", "W_c"):
+            w[k] = bf16_round(w[k])
+        for lw in w["layers"]:
+            for k in ("W_qkv", "W_o", "W_i", "W_2"):
+                lw[k] = bf16_round(lw[k])
+    return w
+
+
+def pack_blob_modern(w):
+    """Flat fp32 blob of the arch-1 parameters in the ABI's order: E_w, g_e, {g_a, W_qkv, W_o, g_m, W_i, W_2} x L, g_f, W_c, b_c."""
+    parts = [w["E_w"], w["g_e"]]
+    for lw in w["layers"]:
+        parts += [lw[k] for k in MODERN_LAYER_ORDER]
+    parts += [w["g_f"], w["W_c"], w["b_c"]]
+    return np.concatenate([np.ascontiguousarray(p, np.float32).ravel() for p in parts])
 
 
 def pack_blob(w):

@@ -51,6 +51,13 @@ typedef struct {
     int32_t layers, hidden, heads, ffn, vocab, num_labels, max_pos;
     float   ln_eps;
     int32_t dtype;
+    /* S8f NEXT-3, reading D20.  arch 0 (all further fields ignored) = the post-LN BERT-style block above; arch 1 = the
+     * ModernBERT-shaped block: pre-LN without bias terms, rotary position embedding on q and k (rotate-half pairing,
+     * angle = pos * theta^(-2i/64)), GeGLU feed-forward (W_i is [2 ffn, hidden]: gelu(first half) * second half), no
+     * biases except b_c; layer l attends globally (rope_theta_global) iff l % global_every == 0, else only to keys with
+     * |i - j| <= local_window / 2 (rope_theta_local).  dtype 1 supports local_window = 128 (or no local layer). */
+    int32_t arch, local_window, global_every;
+    float   rope_theta_global, rope_theta_local;
 } anon_model_desc;
 
 /* Per-token metadata for span decoding (S8c O3).  flags bit0 = keep. */
@@ -96,7 +103,8 @@ size_t anon_workspace_bytes(const anon_model_desc* desc, int64_t max_tokens, int
  *   { W_qkv[3H,H], b_qkv[3H], W_o[H,H], b_o[H], g_1[H], b_1[H],
  *     W_1[F,H], b_1f[F], W_2[H,F], b_2f[H], g_2[H], b_2[H] } x layers,
  *   W_c[NL,H], b_c[NL]
- * (all matrices row-major [out,in]: y = W x + b; S8d W0).  For dtype 1 the matrices and
+ * (all matrices row-major [out,in]: y = W x + b; S8d W0).  For arch 1 the order is
+ *   E_w[V,H], g_e[H], { g_a[H], W_qkv[3H,H], W_o[H,H], g_m[H], W_i[2F,H], W_2[H,F] } x layers, g_f[H], W_c[NL,H], b_c[NL].  For dtype 1 the matrices and
  * embedding tables are converted to BF16 (round-to-nearest-even; exact when the caller
  * pre-rounded them).  Synchronises.  Errors: INVALID_ARG (size mismatch), UNSUPPORTED
  * (hidden/heads != 64, hidden % 64, ffn % 64, even num_labels, num_labels > 64,
@@ -289,6 +297,11 @@ int  anon_gemm_bf16_ln(anon_ctx* ctx, const void* d_A, const void* d_W, const fl
 int  anon_attention(anon_ctx* ctx, const void* d_qkv, const int32_t* d_cu_seqlens,
                     const int32_t* h_cu_seqlens, int32_t B, int32_t T, int32_t hidden, int32_t heads,
                     int32_t dtype, void* d_ctx);
+/* Same with a local window (NEXT-3, D20): query i sees the keys j of its sequence with |i - j| <= window / 2; window 0 =
+ * anon_attention.  dtype 1 supports window 128 only (ANON_ERR_UNSUPPORTED otherwise).  Asynchronous. */
+int  anon_attention_local(anon_ctx* ctx, const void* d_qkv, const int32_t* d_cu_seqlens,
+                          const int32_t* h_cu_seqlens, int32_t B, int32_t T, int32_t hidden, int32_t heads,
+                          int32_t dtype, int32_t window, void* d_ctx);
 
 #ifdef __cplusplus
 }

@@ -18,12 +18,15 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CAPACITY, ERR_KEY_MISMATCH, ERR_CUDA, 
 class ModelDesc(ctypes.Structure):
     _fields_ = [("layers", ctypes.c_int32), ("hidden", ctypes.c_int32), ("heads", ctypes.c_int32),
                 ("ffn", ctypes.c_int32), ("vocab", ctypes.c_int32), ("num_labels", ctypes.c_int32),
-                ("max_pos", ctypes.c_int32), ("ln_eps", ctypes.c_float), ("dtype", ctypes.c_int32)]
+                ("max_pos", ctypes.c_int32), ("ln_eps", ctypes.c_float), ("dtype", ctypes.c_int32),
+                ("arch", ctypes.c_int32), ("local_window", ctypes.c_int32), ("global_every", ctypes.c_int32),
+                ("rope_theta_global", ctypes.c_float), ("rope_theta_local", ctypes.c_float)]
 
     @classmethod
     def from_dict(cls, d):
         return cls(d["layers"], d["hidden"], d["heads"], d["ffn"], d["vocab"], d["num_labels"], d["max_pos"],
-                   d["ln_eps"], d["dtype"])
+                   d["ln_eps"], d["dtype"], d.get("arch", 0), d.get("local_window", 0), d.get("global_every", 1),
+                   d.get("rope_theta_global", 0.0), d.get("rope_theta_local", 0.0))
 
 
 class AnonError(RuntimeError):
@@ -71,6 +74,7 @@ _SIGNATURES = {
     "anon_gemm_bf16_ln": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp, _vp, _i32, _i32, _i32]),
     "anon_splice_records": (ctypes.c_int, [_vp, _vp, _sz, _vp, _i32, _vp, _i32, _vp, _vp, _vp, _sz, _vp]),
     "anon_attention": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32, _i32, _vp]),
+    "anon_attention_local": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32, _i32, _i32, _vp]),
     "anon_regex_load": (ctypes.c_int, [_vp, _vp, _sz, ctypes.POINTER(_vp)]),
     "anon_regex_free": (None, [_vp]),
     "anon_regex_scan": (ctypes.c_int, [_vp, _vp, _vp, _sz, _vp, _i32, _vp, _i32, _vp]),
@@ -336,6 +340,12 @@ def anon_attention(ctx, qkv, cu_seqlens_dev, cu_seqlens_host, hidden, heads, dty
     h = np.ascontiguousarray(cu_seqlens_host, np.int32)
     ctx.check(lib().anon_attention(ctx._h, _ptr(qkv), _ptr(cu_seqlens_dev), h.ctypes.data, h.size - 1, qkv.shape[0],
                                    hidden, heads, dtype, _ptr(out)), "anon_attention")
+
+
+def anon_attention_local(ctx, qkv, cu_seqlens_dev, cu_seqlens_host, hidden, heads, dtype, window, out):
+    h = np.ascontiguousarray(cu_seqlens_host, np.int32)
+    ctx.check(lib().anon_attention_local(ctx._h, _ptr(qkv), _ptr(cu_seqlens_dev), h.ctypes.data, h.size - 1, qkv.shape[0],
+                                         hidden, heads, dtype, window, _ptr(out)), "anon_attention_local")
 
 
 def anon_pipeline_host(ctx, weights, cache, token_ids, cu_seqlens, meta, text, record_offsets, key, slug_len,

@@ -36,7 +36,11 @@ constexpr int kKVBytes = kKC * kD * 2;         // 8 KB (K and V each)
 constexpr int kAttSmem = 2 * kQBytes + kKVStages * 2 * kKVBytes + 1024 /*align slack*/ + 256 /*barriers*/;
 constexpr int kAttTmemCols = 256;              // S/P buffers 2 x 64, O buffers 2 x 64
 
-struct WorkItem { int q_row0; int kv_row0; int n; int q_valid; };   // rows relative to the chunk
+// rows relative to the chunk.  Global attention: kv_row0 = the sequence's first row, n = its length.  Local (band) attention
+// (NEXT-3, D20): kv_row0 = first key row any query of the tile may see, n = keys from there, and q_valid carries
+// (q_row0 - kv_row0) << 8 in its upper bits: query row r sees key kk (relative to kv_row0) iff |kk - (delta + r)| <= band.
+struct WorkItem { int q_row0; int kv_row0; int n; int q_valid; };
+constexpr int kBand = 64;   // half width of the local window the tcgen05 kernel supports (window 128)
 
 __device__ __forceinline__ float ex2f(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float max3(float a, float b, float c) {
@@ -55,6 +59,7 @@ __device__ __forceinline__ uint32_t pack2(float a, float b) {
     return *reinterpret_cast<uint32_t*>(&v);
 }
 
+template <bool BAND>
 __global__ void __launch_bounds__(kAttThreads, 2)
 attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_kv,
                          const WorkItem* __restrict__ work, int n_units, int heads, int H, __nv_bfloat16* __restrict__ ctx)
@@ -218,7 +223,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 const uint32_t t_s = tmem_base + lane_base + sb * 64u;
                 ptx::mbar_wait(s_full(sb), (g >> 1) & 1u);
                 ptx::tc_fence_after();
-                if ((int)quarter * 32 >= w.q_valid) {                    // no query of this warp is real: P rows are don't-care
+                if ((int)quarter * 32 >= (w.q_valid & 0xff)) {           // no query of this warp is real: P rows are don't-care
                     ptx::tc_fence_before();
                     __syncwarp();
                     if (lane == 0) ptx::mbar_arrive(p_full(sb));
@@ -233,6 +238,14 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 if (valid < kKC) {
 #pragma unroll
                     for (int j = 0; j < kKC; j++) if (j >= valid) r[j] = 0xff800000u;      // -inf
+                }
+                if (BAND) {                                              // keys outside |key - query| <= kBand: -inf
+                    const int qq = (w.q_valid >> 8) + row - c * kKC;     // the query's own column in this chunk
+                    const int jlo = qq - kBand, jhi = qq + kBand;
+                    if (jlo > 0 || jhi < kKC - 1) {
+#pragma unroll
+                        for (int j = 0; j < kKC; j++) if (j < jlo || j > jhi) r[j] = 0xff800000u;
+                    }
                 }
                 float cmx[4];                                            // four independent chains, then a tree
 #pragma unroll
@@ -266,7 +279,9 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 }
                 uint32_t pk[32];
                 uint64_t sum_a = pk2(0.f, 0.f), sum_b = sum_a;           // packed FP32x2 partial row sums
-                const uint64_t sc2 = pk2(sc, sc), nm2 = pk2(-m, -m);
+                // BAND: a row may not have seen any key yet (m = -inf): exponentiate against 0, every p is then 0
+                const float mref = (BAND && m == -INFINITY) ? 0.f : m;
+                const uint64_t sc2 = pk2(sc, sc), nm2 = pk2(-mref, -mref);
 #pragma unroll
                 for (int hh = 0; hh < 2; hh++) {
                     if (hh == 1 && valid <= 32) {                        // second half of a short last chunk: all masked
@@ -298,7 +313,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             // the O / l write-back of this unit is deferred until after the first chunk of the next one, so that the
             // wait for the last PV overlaps useful work
             pend = true; pend_ob = qi & 1u; pend_par = (qi >> 1) & 1u; pend_l = l;
-            pend_row0 = w.q_row0; pend_valid = w.q_valid; pend_head = head;
+            pend_row0 = w.q_row0; pend_valid = w.q_valid & 0xff; pend_head = head;
         }
         if (pend) finalize();
     }
@@ -316,8 +331,10 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
 // enc::attention_f32_kernel lives in encoder_kernels.cuh (FP32 path); declared here for the dtype-0 branch
 #include "encoder_kernels.cuh"
 
-int attention_plan(anon_ctx* ctx, WsCursor& ws, const int32_t* h_cu, int B, int dtype, AttnPlan* plan)
+int attention_plan(anon_ctx* ctx, WsCursor& ws, const int32_t* h_cu, int B, int dtype, AttnPlan* plan, int window)
 {
+    plan->window = window;
+    if (window != 0 && dtype == 1 && window != 2 * kBand) return ANON_ERR_UNSUPPORTED;
     // h_cu points at this chunk's first sequence boundary; rows are relative to token h_cu[0]
     plan->d_work = nullptr; plan->n_items = 0; plan->n_rows = 0;
     if (!ctx || !h_cu || B < 0) return ANON_ERR_INVALID_ARG;
@@ -330,7 +347,11 @@ int attention_plan(anon_ctx* ctx, WsCursor& ws, const int32_t* h_cu, int B, int 
     items.reserve((size_t)(h_cu[B] - tok0) / kQT + B);
     for (int s = 0; s < B; s++) {
         const int a = h_cu[s] - tok0, n = h_cu[s + 1] - h_cu[s];
-        for (int q0 = 0; q0 < n; q0 += kQT) items.push_back(WorkItem{a + q0, a, n, std::min(kQT, n - q0)});
+        for (int q0 = 0; q0 < n; q0 += kQT) {
+            if (window == 0) { items.push_back(WorkItem{a + q0, a, n, std::min(kQT, n - q0)}); continue; }
+            const int k0 = std::max(0, q0 - kBand), k1 = std::min(n, q0 + kQT + kBand);
+            items.push_back(WorkItem{a + q0, a + k0, k1 - k0, std::min(kQT, n - q0) | ((q0 - k0) << 8)});
+        }
     }
     if (items.empty()) return ANON_OK;
     std::stable_sort(items.begin(), items.end(), [](const WorkItem& x, const WorkItem& y) { return x.n > y.n; });
@@ -351,7 +372,8 @@ int attention_run(anon_ctx* ctx, const AttnPlan& plan, const void* d_qkv, const 
     if (heads <= 0 || hidden != heads * 64) return ANON_ERR_UNSUPPORTED;
     if (B == 0) return ANON_OK;
     if (dtype == 0) {
-        enc::attention_f32_kernel<<<dim3(B, heads), 128, 0, ctx->stream>>>((const float*)d_qkv, d_cu, 0, tok0, hidden, (float*)d_ctx);
+        enc::attention_f32_kernel<<<dim3(B, heads), 128, 0, ctx->stream>>>((const float*)d_qkv, d_cu, 0, tok0, hidden, (float*)d_ctx,
+                                                                           plan.window ? plan.window / 2 : -1);
         CU_LAUNCH_CHECK(ctx, "attention_f32_kernel");
         return ANON_OK;
     }
@@ -364,13 +386,18 @@ int attention_run(anon_ctx* ctx, const AttnPlan& plan, const void* d_qkv, const 
     if (rc) return rc;
     static bool attr_set = false;
     if (!attr_set) {
-        CU_TRY(ctx, cudaFuncSetAttribute(attention_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kAttSmem));
+        CU_TRY(ctx, cudaFuncSetAttribute(attention_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kAttSmem));
+        CU_TRY(ctx, cudaFuncSetAttribute(attention_tcgen05_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kAttSmem));
         attr_set = true;
     }
     const long long units = (long long)plan.n_items * heads;
     const int grid = (int)std::min<long long>(units, 2LL * ctx->sm_count);
-    attention_tcgen05_kernel<<<grid, kAttThreads, kAttSmem, ctx->stream>>>(tq, tkv, (const WorkItem*)plan.d_work, (int)units,
-                                                                            heads, hidden, (__nv_bfloat16*)d_ctx);
+    if (plan.window)
+        attention_tcgen05_kernel<true><<<grid, kAttThreads, kAttSmem, ctx->stream>>>(tq, tkv, (const WorkItem*)plan.d_work, (int)units,
+                                                                                      heads, hidden, (__nv_bfloat16*)d_ctx);
+    else
+        attention_tcgen05_kernel<false><<<grid, kAttThreads, kAttSmem, ctx->stream>>>(tq, tkv, (const WorkItem*)plan.d_work, (int)units,
+                                                                                       heads, hidden, (__nv_bfloat16*)d_ctx);
     CU_LAUNCH_CHECK(ctx, "attention_tcgen05_kernel");
     return ANON_OK;
 }
@@ -384,6 +411,19 @@ extern "C" int anon_attention(anon_ctx* ctx, const void* d_qkv, const int32_t* d
     WsCursor ws = ws_begin(ctx);
     AttnPlan plan;
     int rc = attention_plan(ctx, ws, h_cu_seqlens, B, dtype, &plan);
+    if (rc) return rc;
+    return attention_run(ctx, plan, d_qkv, d_cu_seqlens, h_cu_seqlens[0], B, hidden, heads, dtype, d_ctx);
+}
+
+extern "C" int anon_attention_local(anon_ctx* ctx, const void* d_qkv, const int32_t* d_cu_seqlens, const int32_t* h_cu_seqlens,
+                                    int32_t B, int32_t T, int32_t hidden, int32_t heads, int32_t dtype, int32_t window, void* d_ctx)
+{
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    if (!h_cu_seqlens || B < 0 || T < 0 || window < 0 || (window & 1)) return ANON_ERR_INVALID_ARG;
+    WsCursor ws = ws_begin(ctx);
+    AttnPlan plan;
+    int rc = attention_plan(ctx, ws, h_cu_seqlens, B, dtype, &plan, window);
     if (rc) return rc;
     return attention_run(ctx, plan, d_qkv, d_cu_seqlens, h_cu_seqlens[0], B, hidden, heads, dtype, d_ctx);
 }

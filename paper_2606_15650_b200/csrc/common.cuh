@@ -123,8 +123,9 @@ int gemm_bf16_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W,
 // 128-byte swizzle (gemm_tcgen05.cu).
 int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_t esize, const void* base, uint64_t rows,
                  uint64_t cols, uint32_t box_cols, uint32_t box_rows);
-struct AttnPlan { void* d_work; int n_items; int n_rows; };
-int attention_plan(anon_ctx*, WsCursor&, const int32_t* h_cu, int B, int dtype, AttnPlan* plan);
+struct AttnPlan { void* d_work; int n_items; int n_rows; int window; };
+// window = 0: every query sees its whole sequence; else keys with |i - j| <= window / 2 (NEXT-3 local layers)
+int attention_plan(anon_ctx*, WsCursor&, const int32_t* h_cu, int B, int dtype, AttnPlan* plan, int window = 0);
 int attention_run(anon_ctx*, const AttnPlan&, const void* d_qkv, const int32_t* d_cu, int tok0, int B, int hidden,
                   int heads, int dtype, void* d_ctx);
 const anon_model_desc* weights_desc(const anon_weights* w);

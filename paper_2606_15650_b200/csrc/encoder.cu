@@ -12,6 +12,8 @@
 #include <new>
 #include <vector>
 #include <stdlib.h>
+#include <math.h>
+#include <algorithm>
 
 struct LayerW {
     void *W_qkv, *W_o, *W_1, *W_2;                     // BF16 or FP32 matrices
@@ -23,6 +25,9 @@ struct anon_weights {
     uint8_t* store = nullptr;
     void *E_w = nullptr, *E_p = nullptr;
     float *E_t = nullptr, *g_e = nullptr, *b_e = nullptr, *W_c = nullptr, *b_c = nullptr;
+    // arch 1 (NEXT-3): LayerW reuses g_1 = g_a, g_2 = g_m, W_1 = W_i [2F, H]; every bias / beta / E_p / E_t points at `zeros`
+    float* g_f = nullptr;
+    void* zeros = nullptr;
     std::vector<LayerW> layers;
 };
 
@@ -42,17 +47,28 @@ int check_desc(const anon_model_desc* d) {
     if (d->hidden != d->heads * 64 || d->hidden % 128 != 0 || d->hidden > 1024 || d->ffn % 64 != 0 ||
         (d->num_labels & 1) == 0 || d->num_labels > 64 || d->max_pos > 512)
         return ANON_ERR_UNSUPPORTED;
+    if (d->arch != 0 && d->arch != 1) return ANON_ERR_INVALID_ARG;
+    if (d->arch == 1) {
+        if (d->local_window < 0 || (d->local_window & 1) || d->global_every < 1 || !(d->rope_theta_global > 0.f) ||
+            !(d->rope_theta_local > 0.f))
+            return ANON_ERR_INVALID_ARG;
+        const bool has_local = d->global_every > 1 && d->layers > 1;
+        if (d->dtype == 1 && has_local && d->local_window != 128) return ANON_ERR_UNSUPPORTED;
+    }
     return ANON_OK;
 }
 
 size_t desc_floats(const anon_model_desc& d) {
     const size_t H = d.hidden, F = d.ffn, V = d.vocab, NL = d.num_labels, P = d.max_pos, L = d.layers;
+    if (d.arch == 1) return V * H + H + L * (H + 3 * H * H + H * H + H + 2 * F * H + H * F) + H + NL * H + NL;
     const size_t per_layer = 3 * H * H + 3 * H + H * H + H + 2 * H + F * H + F + H * F + H + 2 * H;
     return V * H + P * H + 3 * H + L * per_layer + NL * H + NL;
 }
 
 size_t per_token_bytes(const anon_model_desc& d) {
     const size_t H = d.hidden, F = d.ffn;
+    if (d.arch == 1)      // x, y, h FP32; xb; qkv; ctx; u [2F]; f [F]; position id
+        return d.dtype == 1 ? 12 * H + 2 * H + 6 * H + 2 * H + 4 * F + 2 * F + 4 : 12 * H + 12 * H + 4 * H + 8 * F + 4 * F + 4;
     if (d.dtype == 1) return 4 * H + 2 * H + 4 * H + 6 * H + 2 * H + 2 * F + 8;
     return 4 * H + 4 * H + 12 * H + 4 * H + 4 * F;
 }
@@ -83,6 +99,19 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
     struct Item { void** dst; size_t n; bool matrix; };
     std::vector<Item> items;
     w->layers.resize(d.layers);
+    size_t zero_bytes = 0;
+    if (d.arch == 1) {
+        items.push_back({&w->E_w, V * H, true});
+        items.push_back({(void**)&w->g_e, H, false});
+        for (int l = 0; l < d.layers; l++) {
+            LayerW& L = w->layers[l];
+            items.push_back({(void**)&L.g_1, H, false});    items.push_back({&L.W_qkv, 3 * H * H, true});
+            items.push_back({&L.W_o, H * H, true});         items.push_back({(void**)&L.g_2, H, false});
+            items.push_back({&L.W_1, 2 * F * H, true});     items.push_back({&L.W_2, H * F, true});
+        }
+        items.push_back({(void**)&w->g_f, H, false});
+        zero_bytes = std::max(P * H * msz, 4 * std::max(3 * H, 2 * F));
+    } else {
     items.push_back({&w->E_w, V * H, true});
     items.push_back({&w->E_p, P * H, true});
     items.push_back({(void**)&w->E_t, H, false});
@@ -97,6 +126,7 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
         items.push_back({&L.W_2, H * F, true});         items.push_back({(void**)&L.b_2f, H, false});
         items.push_back({(void**)&L.g_2, H, false});    items.push_back({(void**)&L.b_2, H, false});
     }
+    }
     items.push_back({(void**)&w->W_c, NL * H, false});   // head stays FP32 (values are BF16-representable)
     items.push_back({(void**)&w->b_c, NL, false});
     size_t total = 0, max_matrix = 0;
@@ -105,6 +135,8 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
         if (it.matrix && bf && it.n > max_matrix) max_matrix = it.n;
     }
     float* stage = nullptr;
+    const size_t zero_off = (total + 255) / 256 * 256;
+    total = zero_off + zero_bytes;
     cudaError_t e = cudaMalloc(&w->store, total + 256);
     if (e == cudaSuccess && max_matrix) e = cudaMalloc(&stage, max_matrix * 4);
     if (e != cudaSuccess) { cudaFree(w->store); delete w; cuda_fail(ctx, e, "cudaMalloc(weights)"); return ANON_ERR_OOM; }
@@ -126,6 +158,12 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
         if (e != cudaSuccess) break;
         off += it.n * (it.matrix ? msz : 4);
         src += it.n;
+    }
+    if (e == cudaSuccess && zero_bytes) {
+        e = cudaMemsetAsync(w->store + zero_off, 0, zero_bytes, ctx->stream);
+        w->zeros = w->store + zero_off;
+        w->E_p = w->zeros; w->E_t = (float*)w->zeros; w->b_e = (float*)w->zeros;
+        for (auto& L : w->layers) L.b_qkv = L.b_o = L.b_1 = L.b_1f = L.b_2f = L.b_2 = (float*)w->zeros;
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     cudaFree(stage);
@@ -157,6 +195,107 @@ static int sgemm(anon_ctx* ctx, const float* A, const float* W, const float* bia
     dim3 grid((N + 63) / 64, (M + 63) / 64);
     enc::sgemm_tn_kernel<EPI><<<grid, 256, 0, ctx->stream>>>(A, W, bias, res, C, M, N, K);
     CU_LAUNCH_CHECK(ctx, "sgemm_tn_kernel");
+    return ANON_OK;
+}
+
+// ---- NEXT-3: one chunk of the ModernBERT-shaped forward (reading D20; oracle/encoder_modern.py) ---------------------
+// x is the FP32 residual stream (never normalised in place): h / xb = LN(x) feed the GEMMs, the residual GEMM epilogue
+// writes x + (...) into the other buffer of the x / y pair.
+static int modern_chunk(anon_ctx* ctx, WsCursor c, const anon_weights* w, const int32_t* d_ids, const int32_t* d_cu, const int32_t* h_cu,
+                        int B, int s0, int s1, float* d_logits, int32_t* d_labels)
+{
+    const anon_model_desc& d = w->d;
+    const int H = d.hidden, F = d.ffn, NL = d.num_labels;
+    const bool bf = d.dtype == 1;
+    const int tok0 = h_cu[s0], nt = h_cu[s1] - tok0, nb = s1 - s0;
+    cudaStream_t st = ctx->stream;
+    const size_t es = bf ? 2 : 4;
+    float* x = (float*)c.take((size_t)nt * H * 4);
+    float* y = (float*)c.take((size_t)nt * H * 4);
+    float* h = (float*)c.take((size_t)nt * H * 4);
+    __nv_bfloat16* xb = bf ? (__nv_bfloat16*)c.take((size_t)nt * H * 2) : nullptr;
+    void* qkv = c.take((size_t)nt * 3 * H * es);
+    void* cx = c.take((size_t)nt * H * es);
+    void* u = c.take((size_t)nt * 2 * F * es);
+    void* f = c.take((size_t)nt * F * es);
+    int* pos = (int*)c.take((size_t)nt * 4);
+    if (!x || !y || !h || (bf && !xb) || !qkv || !cx || !u || !f || !pos) return ANON_ERR_OOM;
+    const bool has_local = d.global_every > 1 && d.layers > 1;
+    AttnPlan plan_g, plan_l;
+    int rc = attention_plan(ctx, c, h_cu + s0, nb, d.dtype, &plan_g, 0);
+    if (rc) return rc;
+    plan_l = plan_g;
+    if (has_local) { rc = attention_plan(ctx, c, h_cu + s0, nb, d.dtype, &plan_l, d.local_window); if (rc) return rc; }
+    double fl_g = 0, fl_l = 0;                       // 4 n k d per (sequence, head), k = keys a query sees
+    for (int s = s0; s < s1; s++) {
+        const double n = h_cu[s + 1] - h_cu[s];
+        fl_g += 4.0 * n * n * H;
+        fl_l += 4.0 * n * std::min(n, (double)d.local_window + 1.0) * H;
+    }
+    enc::RopeFreq fr_g, fr_l;
+    for (int i = 0; i < 32; i++) {
+        fr_g.inv_freq[i] = (float)pow((double)d.rope_theta_global, -2.0 * i / 64.0);
+        fr_l.inv_freq[i] = (float)pow((double)d.rope_theta_local, -2.0 * i / 64.0);
+    }
+    const unsigned row_grid = (unsigned)((nt + enc::kRowWarps - 1) / enc::kRowWarps);
+    const bool fixed_ln = bf && (H == 768 || H == 1024);
+    const float* zf = (const float*)w->zeros;
+    auto norm = [&](const float* in, const float* g, float* out32) {      // (out32, xb) = LN(in; g)
+        ProfScope ps(ctx, PROF_ROW, (double)nt * H * (4 + (out32 ? 4 : 0) + (bf ? 2 : 0)));
+        launch_layer_norm(st, row_grid, in, nt, H, g, zf, d.ln_eps, out32, xb);
+    };
+    auto gemm = [&](int cls, const void* A, const void* W, const float* res, void* C, int N, int K, int epi) -> int {
+        ProfScope ps(ctx, cls, 2.0 * nt * N * K);
+        if (bf) return gemm_bf16_impl(ctx, (const __nv_bfloat16*)A, (const __nv_bfloat16*)W, zf, res, C, nt, N, K, epi);
+        return epi == 2 ? sgemm<2>(ctx, (const float*)A, (const float*)W, zf, res, (float*)C, nt, N, K)
+                        : sgemm<0>(ctx, (const float*)A, (const float*)W, zf, res, (float*)C, nt, N, K);
+    };
+    { ProfScope ps(ctx, PROF_ROW, (double)nt * (4 + H * es + H * 4 + 4), 2);
+    if (bf)
+        enc::embed_ln_kernel<__nv_bfloat16><<<row_grid, enc::kRowWarps * 32, 0, st>>>(
+            d_ids, d_cu, B, tok0, nt, (const __nv_bfloat16*)w->E_w, (const __nv_bfloat16*)w->E_p, w->E_t, w->g_e, w->b_e, d.ln_eps, H,
+            d.vocab, d.max_pos, x, xb, ctx->d_status);
+    else
+        enc::embed_ln_kernel<float><<<row_grid, enc::kRowWarps * 32, 0, st>>>(
+            d_ids, d_cu, B, tok0, nt, (const float*)w->E_w, (const float*)w->E_p, w->E_t, w->g_e, w->b_e, d.ln_eps, H, d.vocab,
+            d.max_pos, x, nullptr, ctx->d_status);
+    enc::token_pos_kernel<<<(unsigned)((nt + 255) / 256), 256, 0, st>>>(d_cu + s0, nb, tok0, nt, pos); }
+    CU_LAUNCH_CHECK(ctx, "embed_ln_kernel");
+    const void* gin = bf ? (const void*)xb : (const void*)h;             // the GEMM operand copy of LN(x)
+    const long long rope_threads = (long long)nt * 2 * (H / 64) * 32;
+    for (int l = 0; l < d.layers; l++) {
+        const LayerW& L = w->layers[l];
+        const bool glob = !has_local || l % d.global_every == 0;
+        norm(x, L.g_1, fixed_ln ? nullptr : h);
+        CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+        if ((rc = gemm(PROF_GEMM, gin, L.W_qkv, nullptr, qkv, 3 * H, H, 0))) return rc;
+        { ProfScope ps(ctx, PROF_ROW, (double)nt * 2 * H * es * 2);
+        if (bf) enc::rope_kernel<__nv_bfloat16><<<(unsigned)((rope_threads + 255) / 256), 256, 0, st>>>((__nv_bfloat16*)qkv, pos, nt, H, glob ? fr_g : fr_l);
+        else enc::rope_kernel<float><<<(unsigned)((rope_threads + 255) / 256), 256, 0, st>>>((float*)qkv, pos, nt, H, glob ? fr_g : fr_l); }
+        CU_LAUNCH_CHECK(ctx, "rope_kernel");
+        { ProfScope ps(ctx, PROF_ATTN, glob ? fl_g : fl_l);
+        rc = attention_run(ctx, glob ? plan_g : plan_l, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx); }
+        if (rc) return rc;
+        if ((rc = gemm(PROF_GEMM_OUT, cx, L.W_o, x, y, H, H, 2))) return rc;
+        std::swap(x, y);
+        norm(x, L.g_2, fixed_ln ? nullptr : h);
+        CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+        if ((rc = gemm(PROF_GEMM_FFN1, gin, L.W_1, nullptr, u, 2 * F, H, 0))) return rc;
+        { ProfScope ps(ctx, PROF_ROW, (double)nt * 3 * F * es);
+        const long long pairs = (long long)nt * F / 2;
+        if (bf) enc::geglu_kernel<__nv_bfloat16><<<(unsigned)((pairs + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)u, (__nv_bfloat16*)f, nt, F);
+        else enc::geglu_kernel<float><<<(unsigned)((pairs + 255) / 256), 256, 0, st>>>((const float*)u, (float*)f, nt, F); }
+        CU_LAUNCH_CHECK(ctx, "geglu_kernel");
+        if ((rc = gemm(PROF_GEMM_FFN2, f, L.W_2, x, y, H, F, 2))) return rc;
+        std::swap(x, y);
+    }
+    norm(x, w->g_f, y);                                                  // final norm: FP32 rows for the head
+    CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+    { ProfScope ps(ctx, PROF_ROW, (double)nt * (H * 4 + (d_logits ? NL * 4 : 0) + (d_labels ? 4 : 0)));
+    enc::head_argmax_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nt, H, w->W_c, w->b_c, NL,
+                                                                        d_logits ? d_logits + (size_t)tok0 * NL : nullptr,
+                                                                        d_labels ? d_labels + tok0 : nullptr); }
+    CU_LAUNCH_CHECK(ctx, "head_argmax_kernel");
     return ANON_OK;
 }
 
@@ -195,7 +334,10 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
         while (s1 < B && (long long)(h_cu[s1 + 1] - h_cu[s0]) <= cap) s1++;
         if (s1 == s0) return ANON_ERR_OOM;
         const int tok0 = h_cu[s0], nt = h_cu[s1] - tok0, nb = s1 - s0;
-        if (nt > 0) {
+        if (nt > 0 && d.arch == 1) {
+            const int rc = modern_chunk(ctx, ws, w, d_ids, d_cu, h_cu, B, s0, s1, d_logits, d_labels);
+            if (rc) return rc;
+        } else if (nt > 0) {
             WsCursor c = ws;          // chunk-local carve (same region reused by every chunk; stream-ordered)
             float* x = (float*)c.take((size_t)nt * H * 4);
             float* y = (float*)c.take((size_t)nt * H * 4);

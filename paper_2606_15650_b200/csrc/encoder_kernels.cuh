@@ -230,8 +230,9 @@ static __global__ void __launch_bounds__(256) sgemm_tn_kernel(const float* __res
 
 // FP32 varlen attention: one CTA per (sequence, head); each warp owns one query at a time; scores in shared
 // memory; exact two-pass softmax in FP32.  qkv [T,3H] with q | k | v column blocks; d_head = 64.
+// half >= 0 (NEXT-3 local layers): query i sees keys m with |i - m| <= half only.
 static __global__ void __launch_bounds__(128) attention_f32_kernel(const float* __restrict__ qkv, const int* __restrict__ cu,
-                                                            int seq0, int tok0, int H, float* __restrict__ ctx)
+                                                            int seq0, int tok0, int H, float* __restrict__ ctx, int half = -1)
 {
     __shared__ float sc[4][512];
     __shared__ float qs[4][64];
@@ -246,8 +247,10 @@ static __global__ void __launch_bounds__(128) attention_f32_kernel(const float* 
         qs[warp][lane] = Q[(size_t)i * ld + lane];
         qs[warp][lane + 32] = Q[(size_t)i * ld + lane + 32];
         __syncwarp();
+        const int m_lo = half >= 0 && i - half > 0 ? i - half : 0;
+        const int m_hi = half >= 0 && i + half + 1 < n ? i + half + 1 : n;       // exclusive
         float mx = -INFINITY;
-        for (int m = lane; m < n; m += 32) {
+        for (int m = m_lo + lane; m < m_hi; m += 32) {
             const float4* kr = reinterpret_cast<const float4*>(Kp + (size_t)m * ld);
             float s = 0.f;
 #pragma unroll
@@ -262,11 +265,11 @@ static __global__ void __launch_bounds__(128) attention_f32_kernel(const float* 
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, d));
         float sum = 0.f;
-        for (int m = lane; m < n; m += 32) { const float e = expf(sc[warp][m] - mx); sc[warp][m] = e; sum += e; }
+        for (int m = m_lo + lane; m < m_hi; m += 32) { const float e = expf(sc[warp][m] - mx); sc[warp][m] = e; sum += e; }
         sum = warp_sum(sum);
         __syncwarp();
         float o0 = 0.f, o1 = 0.f;
-        for (int m = 0; m < n; m++) {
+        for (int m = m_lo; m < m_hi; m++) {
             const float p = sc[warp][m];
             o0 = fmaf(p, __ldg(Vp + (size_t)m * ld + lane), o0);
             o1 = fmaf(p, __ldg(Vp + (size_t)m * ld + lane + 32), o1);
@@ -275,6 +278,61 @@ static __global__ void __launch_bounds__(128) attention_f32_kernel(const float* 
         ctx[(size_t)(a + i) * H + head * 64 + lane] = o0 * inv;
         ctx[(size_t)(a + i) * H + head * 64 + lane + 32] = o1 * inv;
         __syncwarp();
+    }
+}
+
+
+// ---- NEXT-3 (ModernBERT-shaped variant, reading D20): position ids, RoPE, GeGLU ---------------------------------------
+// pos[t] = index of token t inside its sequence (chunk-local rows; cu points at the chunk's first boundary)
+static __global__ void __launch_bounds__(256) token_pos_kernel(const int* __restrict__ cu, int B, int tok0, int ntok, int* __restrict__ pos)
+{
+    const int t = blockIdx.x * 256 + threadIdx.x;
+    if (t >= ntok) return;
+    int lo = 0, hi = B;                                   // largest s with cu[s] - tok0 <= t
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (cu[mid] - tok0 <= t) lo = mid; else hi = mid; }
+    pos[t] = t - (cu[lo] - tok0);
+}
+
+struct RopeFreq { float inv_freq[32]; };                 // theta^(-2i/64), i = 0..31, computed in double on the host
+
+__device__ __forceinline__ float to_f32(float v) { return v; }
+__device__ __forceinline__ float to_f32(__nv_bfloat16 v) { return __bfloat162float(v); }
+__device__ __forceinline__ void from_f32(float& d, float v) { d = v; }
+__device__ __forceinline__ void from_f32(__nv_bfloat16& d, float v) { d = __float2bfloat16_rn(v); }
+
+// In place on the q and k column blocks of qkv [ntok, 3H]: pair (i, i + 32) of every head turns by pos * inv_freq[i].
+// One thread per (token, q|k, head, i): lanes of a warp are the 32 pairs of one head, so both accesses are coalesced.
+template <class T>
+static __global__ void __launch_bounds__(256) rope_kernel(T* __restrict__ qkv, const int* __restrict__ pos, int ntok, int H, RopeFreq fr)
+{
+    const int heads2 = 2 * (H >> 6);                      // q heads then k heads: columns [0, 2H) in blocks of 64
+    const long long gid = (long long)blockIdx.x * 256 + threadIdx.x;
+    const int i = (int)(gid & 31);
+    const long long hw = gid >> 5;
+    const int hh = (int)(hw % heads2);
+    const long long t = hw / heads2;
+    if (t >= ntok) return;
+    T* p = qkv + (size_t)t * 3 * H + hh * 64 + i;
+    float s, c;
+    sincosf((float)pos[t] * fr.inv_freq[i], &s, &c);
+    const float x1 = to_f32(p[0]), x2 = to_f32(p[32]);
+    from_f32(p[0], x1 * c - x2 * s);
+    from_f32(p[32], x2 * c + x1 * s);
+}
+
+// f[t, j] = gelu(u[t, j]) * u[t, F + j] (erf GELU), u [ntok, 2F]; two elements per thread
+template <class T>
+static __global__ void __launch_bounds__(256) geglu_kernel(const T* __restrict__ u, T* __restrict__ f, long long ntok, int F)
+{
+    const long long gid = ((long long)blockIdx.x * 256 + threadIdx.x) * 2;
+    if (gid >= ntok * F) return;
+    const long long t = gid / F;
+    const int j = (int)(gid - t * F);                     // F is even: both elements are in the same row
+    const T* a = u + (size_t)t * 2 * F + j;
+#pragma unroll
+    for (int e = 0; e < 2; e++) {
+        const float z = to_f32(a[e]), gt = to_f32(a[F + e]);
+        from_f32(f[(size_t)t * F + j + e], 0.5f * z * (1.0f + erff(z * 0.70710678118654752f)) * gt);
     }
 }
 

@@ -1,0 +1,183 @@
+"""GPU parity (through the C ABI) of NEXT-3, the ModernBERT-shaped encoder (reading D20): banded attention alone,
+then the whole forward in FP32 (tolerance D13) and BF16 (max-abs <= 3e-2 + the label rule) against
+oracle/encoder_modern.py, and the host pipeline on arch-1 weights."""
+import numpy as np
+import pytest
+
+from harness import gen
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    import paper_2606_15650_b200 as P
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device")
+    ctx = P.Context(0, workspace_bytes=3 << 30)
+    yield P, torch, ctx
+    ctx.close()
+
+
+def _bf16(a):
+    return gen.bf16_round(np.asarray(a, np.float32))
+
+
+def _forward(P, torch, ctx, W, ids, cu):
+    dev = "cuda:0"
+    NL = W.desc["num_labels"]
+    d_ids = torch.from_numpy(np.ascontiguousarray(ids, np.int32)).to(dev)
+    d_cu = torch.from_numpy(np.ascontiguousarray(cu, np.int32)).to(dev)
+    logits = torch.full((ids.size, NL), float("nan"), dtype=torch.float32, device=dev)
+    labels = torch.full((ids.size,), -1, dtype=torch.int32, device=dev)
+    P.anon_ner_forward(ctx, W, d_ids, d_cu, logits, labels)
+    assert ctx.sync() == 0
+    return logits.cpu().numpy().astype(np.float64), labels.cpu().numpy()
+
+
+@pytest.mark.parametrize("dtype,window", [(1, 128), (0, 128), (0, 16), (0, 0)])
+def test_local_attention_against_oracle(env, dtype, window):
+    """K3 with a band: lengths below, at and above the band and tile sizes (64 / 65 / 128 / 129 / 193 / 512), a 1-token and an
+    empty sequence.  window 0 through this entry point is global attention."""
+    P, torch, ctx = env
+    from oracle import encoder_modern as em
+    H, A = 256, 4
+    lens = [1, 5, 63, 64, 65, 0, 128, 129, 193, 512, 300, 2, 257]
+    cu = np.zeros(len(lens) + 1, np.int32); cu[1:] = np.cumsum(lens)
+    T = int(cu[-1])
+    rng = np.random.default_rng(21)
+    qkv = rng.standard_normal((T, 3 * H)).astype(np.float32) * 1.5
+    if dtype == 1:
+        qkv = _bf16(qkv)
+    q64 = qkv.astype(np.float64)
+    want = np.zeros((T, H))
+    for s in range(len(lens)):
+        a, b = int(cu[s]), int(cu[s + 1])
+        for h in range(A):
+            sl = lambda blk: slice(blk * H + h * 64, blk * H + (h + 1) * 64)
+            if b > a:
+                want[a:b, h * 64:(h + 1) * 64] = em.attention_head(q64[a:b, sl(0)], q64[a:b, sl(1)], q64[a:b, sl(2)],
+                                                                   window if window else None)
+    dev = "cuda:0"
+    tq = torch.from_numpy(qkv).to(dev)
+    if dtype == 1:
+        tq = tq.to(torch.bfloat16)
+    out = torch.full((T, H), float("nan"), dtype=tq.dtype, device=dev)
+    P.anon_attention_local(ctx, tq, torch.from_numpy(cu).to(dev), cu, H, A, dtype, window, out)
+    assert ctx.sync() == 0
+    got = out.float().cpu().numpy().astype(np.float64)
+    assert not np.isnan(got).any()
+    if dtype == 1:
+        assert np.abs(got - want).max() <= 2e-2 * np.abs(want).max()
+        assert np.sqrt(((got - want) ** 2).mean()) <= 3e-3 * np.sqrt((want ** 2).mean())
+    else:
+        assert np.abs(got - want).max() <= 2e-5 * np.abs(want).max()
+    if dtype == 1:       # a window the tcgen05 kernel does not support is refused, not approximated
+        with pytest.raises(P.AnonError) as ei:
+            P.anon_attention_local(ctx, tq, torch.from_numpy(cu).to(dev), cu, H, A, 1, 64, out)
+        assert ei.value.code == -2
+
+
+def test_tiny_modern_fp32_logits_and_labels(env):
+    """FP32 path of arch 1 (4 layers: global, local, local, global): ragged batch incl. sequences longer than the window."""
+    P, torch, ctx = env
+    from oracle import encoder, encoder_modern as em
+    d = gen.DESCS["tiny_modern"]
+    w = gen.make_weights_modern(d, gen.SEED_BASE + 6, planted=(2.0, 0.5, 4.0))
+    rng = np.random.default_rng(5)
+    lens = [1, 0, 512, 33, 64, 65, 129, 200, 300, 7]
+    cu = np.zeros(len(lens) + 1, np.int32); cu[1:] = np.cumsum(lens)
+    ids = rng.integers(5, d["vocab"], int(cu[-1])).astype(np.int32)
+    want = em.forward_packed(w, d, ids, cu)
+    W = P.Weights(ctx, d, gen.pack_blob_modern(w))
+    got, labels = _forward(P, torch, ctx, W, ids, cu)
+    W.close()
+    rms = np.sqrt((want ** 2).mean())
+    tol = 1e-4 * np.maximum(np.abs(want), rms)
+    assert (np.abs(got - want) <= tol).all(), float((np.abs(got - want) / tol).max())
+    mism = np.nonzero(labels != encoder.argmax_labels(want))[0]
+    assert (encoder.top2_margin(want)[mism] < 1e-4).all()
+    assert np.array_equal(labels, encoder.argmax_labels(got.astype(np.float32)))
+    # chunked execution gives bit-identical results
+    small = P.Context(0, workspace_bytes=6 << 20)
+    W2 = P.Weights(small, d, gen.pack_blob_modern(w))
+    got2, labels2 = _forward(P, torch, small, W2, ids, cu)
+    assert np.array_equal(got2, got) and np.array_equal(labels2, labels)
+    W2.close(); small.close()
+    # a blob of the wrong size (the arch-0 layout) is refused
+    with pytest.raises(P.AnonError):
+        P.Weights(ctx, d, gen.pack_blob_modern(w)[:-1])
+
+
+def _bf16_check(P, torch, ctx, d, w, ids, cu, subset):
+    from oracle import encoder, encoder_modern as em
+    W = P.Weights(ctx, d, gen.pack_blob_modern(w))
+    got, labels = _forward(P, torch, ctx, W, ids, cu)
+    W.close()
+    want = em.forward_packed(w, d, ids, cu, seq_subset=subset)
+    rows = ~np.isnan(want[:, 0])
+    err = np.abs(got[rows] - want[rows])
+    assert err.max() <= 3e-2, err.max()
+    mism = labels[rows] != encoder.argmax_labels(want[rows])
+    assert (encoder.top2_margin(want[rows])[mism] < 3e-2).all()
+    return err.max(), 1.0 - mism.mean()
+
+
+def test_bf16_modern_generic_hidden(env):
+    """BF16 arch 1 with hidden 256 (generic LayerNorm kernel), 4 layers, every sequence checked."""
+    P, torch, ctx = env
+    d = dict(gen.DESCS["tiny_modern"], hidden=256, heads=4, ffn=320, vocab=4096, dtype=1)
+    w = gen.make_weights_modern(d, 31, planted=(2.0, 0.5, 4.0))
+    rng = np.random.default_rng(9)
+    lens = [1, 17, 64, 129, 512, 300, 2, 255]
+    cu = np.zeros(len(lens) + 1, np.int32); cu[1:] = np.cumsum(lens)
+    ids = rng.integers(5, d["vocab"], int(cu[-1])).astype(np.int32)
+    e, a = _bf16_check(P, torch, ctx, d, w, ids, cu, None)
+    assert a >= 0.995
+    print(f"\nmodern hidden-256 BF16: max|dlogit|={e:.2e} agreement={a:.4%}")
+
+
+def test_bf16_base_modern_shape(env):
+    """ModernBERT-base sizes (22 layers, hidden 768, GeGLU width 1152, vocab 50,368) on a stratified subsample of the
+    configs[1]-shaped workload, planted-detector weights: logit bound and >= 99.9 % label agreement."""
+    P, torch, ctx = env
+    d = gen.DESCS["base_modern"]
+    rec, win = gen.workload_base(n_records=64, desc=d)
+    ids, cu = win["token_ids"], win["cu_seqlens"]
+    order = np.argsort(np.diff(cu))
+    subset = sorted(set(order[:2].tolist() + order[-2:].tolist() + order[30:32].tolist()))
+    w = gen.make_weights_modern(d, gen.SEED_BASE + 7, planted=(2.0, 0.5, 4.0))
+    e, a = _bf16_check(P, torch, ctx, d, w, ids, cu, subset)
+    assert a >= 0.999, a
+    print(f"\nbase_modern subsample: max|dlogit|={e:.2e} agreement={a:.4%}")
+
+
+def test_pipeline_on_modern_weights(env):
+    """anon_pipeline_host with an arch-1 model: spans and pseudonyms equal the oracle composition."""
+    P, torch, ctx = env
+    from oracle import crypto, decode, encoder, encoder_modern as em
+    d = dict(gen.DESCS["tiny_modern"])
+    pool, poff, ptype = gen.entity_pool(48, 3)
+    g = gen.rng(4)
+    n_tok = np.minimum(g.lognormal(np.log(200), 0.8, 20), 1500).astype(np.int64) + 8
+    rec = gen.make_records(20, n_tok, d, pool, poff, ptype % 4, 5, zipf_s=1.1)
+    win = gen.window_records(rec)
+    w = gen.make_weights_modern(d, gen.SEED_BASE + 8, planted=(2.0, 0.5, 4.0))
+    key, names = bytes(range(1, 33)), gen.TYPE_NAMES_4
+    logits = em.forward_packed(w, d, win["token_ids"], win["cu_seqlens"])
+    assert encoder.top2_margin(logits).min() > 1e-3
+    spans = decode.decode_spans(encoder.argmax_labels(logits), win["meta"])
+    sb, so = decode.gather_spans(rec["text"], rec["rec_off"], spans)
+    oc = crypto.Cache()
+    want = oc.pseudonymize(sb, so, np.asarray([s[3] for s in spans], np.uint8), key, 10, names)
+    oc.close()
+    assert len(spans) > 30
+    W = P.Weights(ctx, d, gen.pack_blob_modern(w))
+    cache = P.Cache(ctx, 4096, 1 << 20)
+    T = win["token_ids"].size
+    res = P.anon_pipeline_host(ctx, W, cache, win["token_ids"], win["cu_seqlens"], win["meta"], rec["text"], rec["rec_off"],
+                               key, 10, names, span_capacity=T, out_capacity=T * 32)
+    cache.close(); W.close()
+    assert np.array_equal(res["spans"], np.asarray(spans, np.int32).reshape(-1, 4))
+    assert np.array_equal(res["out_tokens"], want["out_tokens"]) and np.array_equal(res["hit"], want["hit"])

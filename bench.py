@@ -134,6 +134,12 @@ def encoder_workload(name, rank, n_records=None):
         rec, win = gen.workload_base(n_records=n_records or 4096, seed=gen.SEED_BASE + 2 + 1000 * rank)
         wseed = gen.SEED_BASE + 2
         label = "BASELINE.json configs[1]: BERT-base shape BF16, %d packed sequences, lognormal(median 200, cap 512)"
+    elif name == "modern":       # NEXT-3: the configs[1] input recipe through the ModernBERT-base-shaped encoder (reading D20)
+        desc = gen.DESCS["base_modern"]
+        rec, win = gen.workload_base(n_records=n_records or 4096, seed=gen.SEED_BASE + 2 + 1000 * rank, desc=desc)
+        wseed = gen.SEED_BASE + 7
+        label = ("S8f NEXT-3: ModernBERT-base shape BF16 (22 layers, hidden 768, GeGLU 1152, RoPE, local window 128 in 2 of 3 "
+                 "layers), %d packed sequences, lognormal(median 200, cap 512)")
     else:
         desc = gen.DESCS["large"]
         rec, win = gen.workload_large(n_seqs=n_records or 16384, seed=gen.SEED_BASE + 4 + 1000 * rank)
@@ -142,15 +148,23 @@ def encoder_workload(name, rank, n_records=None):
     return desc, rec, win, wseed, label % (len(win["cu_seqlens"]) - 1)
 
 
+def make_weights_for(desc, seed):
+    return (gen.make_weights_modern if desc.get("arch") == 1 else gen.make_weights)(desc, seed, planted=PLANTED)
+
+
+def pack_for(desc, w):
+    return gen.pack_blob_modern(w) if desc.get("arch") == 1 else gen.pack_blob(w)
+
+
 def oracle_sample_pass(w, desc, rec, win, n_seqs, names):
     """The oracle, as it stands, over the first n_seqs sequences of the workload: encoder + argmax + BIO decode +
     gather + dedup/HMAC/write-back.  Returns (tokens, spans, seconds)."""
-    from oracle import crypto, decode, encoder
+    from oracle import crypto, decode, encoder, encoder_modern
     cu = win["cu_seqlens"]
     T = int(cu[n_seqs])
     ids, meta = win["token_ids"][:T], win["meta"][:T]
     t0 = time.perf_counter()
-    logits = encoder.forward_packed(w, desc, ids, cu[:n_seqs + 1])
+    logits = (encoder_modern if desc.get("arch") == 1 else encoder).forward_packed(w, desc, ids, cu[:n_seqs + 1])
     labels = encoder.argmax_labels(logits)
     spans = decode.decode_spans(labels, meta)
     sb, so = decode.gather_spans(rec["text"], rec["rec_off"], spans)
@@ -189,7 +203,7 @@ def run_reference(args):
         label = "BASELINE.json configs[2]: synthetic record stream, 510+2-token windows (first 64 records generated)"
     else:
         desc, rec, win, wseed, label = encoder_workload(args.workload, 0, n_records=64)
-    w = gen.make_weights(desc, wseed, planted=PLANTED)
+    w = make_weights_for(desc, wseed)
     names = gen.TYPE_NAMES_6
     n = seqs_for_tokens(win["cu_seqlens"], 250 if args.workload == "large" else 600)
     tot_t = tot_s = 0
@@ -285,7 +299,7 @@ def run_encoder(args):
     t_setup = time.time()
     desc, rec, win, wseed, label = encoder_workload(args.workload, rank, args.records)
     names = gen.TYPE_NAMES_6
-    w = gen.make_weights(desc, wseed, planted=PLANTED)
+    w = make_weights_for(desc, wseed)
     ids, cu, meta = win["token_ids"], win["cu_seqlens"], np.ascontiguousarray(win["meta"])
     text, rec_off = rec["text"], rec["rec_off"]
     T, B, R = int(ids.size), int(cu.size - 1), int(rec_off.size - 1)
@@ -293,7 +307,7 @@ def run_encoder(args):
     out_cap = cap * 32
     ws = P.anon_workspace_bytes(desc, T, B) + 96 * T + 2 * text.size + out_cap + 40 * cap + (128 << 20)
     ctx = P.Context(local, workspace_bytes=ws)
-    W = P.Weights(ctx, desc, gen.pack_blob(w))
+    W = P.Weights(ctx, desc, pack_for(desc, w))
     cache = P.Cache(ctx, 1 << 20, 64 << 20)
     log(f"[rank {rank}] setup {time.time() - t_setup:.1f}s: T={T} B={B} R={R} text={text.size} ws={ws / 2**30:.1f} GiB")
 
@@ -656,7 +670,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="base", choices=["base", "large", "stream", "pseudonym"])
+    ap.add_argument("--workload", default="base", choices=["base", "large", "stream", "pseudonym", "modern"])
     ap.add_argument("--records", type=int, default=None, help="override the number of records / sequences / strings")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--batch-tokens", type=int, default=1 << 20, help="stream workload: token budget per batch")

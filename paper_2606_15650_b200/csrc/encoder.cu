@@ -28,6 +28,7 @@ struct anon_weights {
     // arch 1 (NEXT-3): LayerW reuses g_1 = g_a, g_2 = g_m, W_1 = W_i [2F, H]; every bias / beta / E_p / E_t points at `zeros`
     float* g_f = nullptr;
     void* zeros = nullptr;
+    float2 *rope_g = nullptr, *rope_l = nullptr;       // (cos, sin) of pos * theta^(-2i/64), [max_pos][32]
     std::vector<LayerW> layers;
 };
 
@@ -111,6 +112,7 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
         }
         items.push_back({(void**)&w->g_f, H, false});
         zero_bytes = std::max(P * H * msz, 4 * std::max(3 * H, 2 * F));
+        if (F % 8) { delete w; return ANON_ERR_UNSUPPORTED; }
     } else {
     items.push_back({&w->E_w, V * H, true});
     items.push_back({&w->E_p, P * H, true});
@@ -136,7 +138,8 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
     }
     float* stage = nullptr;
     const size_t zero_off = (total + 255) / 256 * 256;
-    total = zero_off + zero_bytes;
+    const size_t rope_off = (zero_off + zero_bytes + 255) / 256 * 256, rope_bytes = d.arch == 1 ? P * 32 * sizeof(float2) : 0;
+    total = rope_off + 2 * rope_bytes;
     cudaError_t e = cudaMalloc(&w->store, total + 256);
     if (e == cudaSuccess && max_matrix) e = cudaMalloc(&stage, max_matrix * 4);
     if (e != cudaSuccess) { cudaFree(w->store); delete w; cuda_fail(ctx, e, "cudaMalloc(weights)"); return ANON_ERR_OOM; }
@@ -164,6 +167,21 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
         w->zeros = w->store + zero_off;
         w->E_p = w->zeros; w->E_t = (float*)w->zeros; w->b_e = (float*)w->zeros;
         for (auto& L : w->layers) L.b_qkv = L.b_o = L.b_1 = L.b_1f = L.b_2f = L.b_2 = (float*)w->zeros;
+    }
+    if (e == cudaSuccess && rope_bytes) {
+        std::vector<float2> tab(2 * P * 32);
+        for (int which = 0; which < 2; which++) {
+            const double theta = which ? d.rope_theta_local : d.rope_theta_global;
+            for (size_t p = 0; p < P; p++)
+                for (int i = 0; i < 32; i++) {
+                    const double ang = (double)p * pow(theta, -2.0 * i / 64.0);
+                    tab[(which * P + p) * 32 + i] = make_float2((float)cos(ang), (float)sin(ang));
+                }
+        }
+        w->rope_g = (float2*)(w->store + rope_off);
+        w->rope_l = w->rope_g + P * 32;
+        e = cudaMemcpyAsync(w->rope_g, tab.data(), 2 * rope_bytes, cudaMemcpyHostToDevice, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);          // tab dies at the end of this block
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     cudaFree(stage);
@@ -232,11 +250,6 @@ static int modern_chunk(anon_ctx* ctx, WsCursor c, const anon_weights* w, const 
         fl_g += 4.0 * n * n * H;
         fl_l += 4.0 * n * std::min(n, (double)d.local_window + 1.0) * H;
     }
-    enc::RopeFreq fr_g, fr_l;
-    for (int i = 0; i < 32; i++) {
-        fr_g.inv_freq[i] = (float)pow((double)d.rope_theta_global, -2.0 * i / 64.0);
-        fr_l.inv_freq[i] = (float)pow((double)d.rope_theta_local, -2.0 * i / 64.0);
-    }
     const unsigned row_grid = (unsigned)((nt + enc::kRowWarps - 1) / enc::kRowWarps);
     const bool fixed_ln = bf && (H == 768 || H == 1024);
     const float* zf = (const float*)w->zeros;
@@ -262,7 +275,7 @@ static int modern_chunk(anon_ctx* ctx, WsCursor c, const anon_weights* w, const 
     enc::token_pos_kernel<<<(unsigned)((nt + 255) / 256), 256, 0, st>>>(d_cu + s0, nb, tok0, nt, pos); }
     CU_LAUNCH_CHECK(ctx, "embed_ln_kernel");
     const void* gin = bf ? (const void*)xb : (const void*)h;             // the GEMM operand copy of LN(x)
-    const long long rope_threads = (long long)nt * 2 * (H / 64) * 32;
+    const long long rope_threads = (long long)nt * 2 * (H / 64) * (bf ? 4 : 8);
     for (int l = 0; l < d.layers; l++) {
         const LayerW& L = w->layers[l];
         const bool glob = !has_local || l % d.global_every == 0;
@@ -270,8 +283,9 @@ static int modern_chunk(anon_ctx* ctx, WsCursor c, const anon_weights* w, const 
         CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
         if ((rc = gemm(PROF_GEMM, gin, L.W_qkv, nullptr, qkv, 3 * H, H, 0))) return rc;
         { ProfScope ps(ctx, PROF_ROW, (double)nt * 2 * H * es * 2);
-        if (bf) enc::rope_kernel<__nv_bfloat16><<<(unsigned)((rope_threads + 255) / 256), 256, 0, st>>>((__nv_bfloat16*)qkv, pos, nt, H, glob ? fr_g : fr_l);
-        else enc::rope_kernel<float><<<(unsigned)((rope_threads + 255) / 256), 256, 0, st>>>((float*)qkv, pos, nt, H, glob ? fr_g : fr_l); }
+        const float2* tab = glob ? w->rope_g : w->rope_l;
+        if (bf) enc::rope_kernel<__nv_bfloat16><<<(unsigned)((rope_threads + 255) / 256), 256, 0, st>>>((__nv_bfloat16*)qkv, pos, nt, H, tab);
+        else enc::rope_kernel<float><<<(unsigned)((rope_threads + 255) / 256), 256, 0, st>>>((float*)qkv, pos, nt, H, tab); }
         CU_LAUNCH_CHECK(ctx, "rope_kernel");
         { ProfScope ps(ctx, PROF_ATTN, glob ? fl_g : fl_l);
         rc = attention_run(ctx, glob ? plan_g : plan_l, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx); }
@@ -282,9 +296,9 @@ static int modern_chunk(anon_ctx* ctx, WsCursor c, const anon_weights* w, const 
         CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
         if ((rc = gemm(PROF_GEMM_FFN1, gin, L.W_1, nullptr, u, 2 * F, H, 0))) return rc;
         { ProfScope ps(ctx, PROF_ROW, (double)nt * 3 * F * es);
-        const long long pairs = (long long)nt * F / 2;
-        if (bf) enc::geglu_kernel<__nv_bfloat16><<<(unsigned)((pairs + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)u, (__nv_bfloat16*)f, nt, F);
-        else enc::geglu_kernel<float><<<(unsigned)((pairs + 255) / 256), 256, 0, st>>>((const float*)u, (float*)f, nt, F); }
+        const long long vecs = (long long)nt * F / (bf ? 8 : 4);
+        if (bf) enc::geglu_kernel<__nv_bfloat16><<<(unsigned)((vecs + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)u, (__nv_bfloat16*)f, nt, F);
+        else enc::geglu_kernel<float><<<(unsigned)((vecs + 255) / 256), 256, 0, st>>>((const float*)u, (float*)f, nt, F); }
         CU_LAUNCH_CHECK(ctx, "geglu_kernel");
         if ((rc = gemm(PROF_GEMM_FFN2, f, L.W_2, x, y, H, F, 2))) return rc;
         std::swap(x, y);

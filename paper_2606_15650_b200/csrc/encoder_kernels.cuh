@@ -293,47 +293,65 @@ static __global__ void __launch_bounds__(256) token_pos_kernel(const int* __rest
     pos[t] = t - (cu[lo] - tok0);
 }
 
-struct RopeFreq { float inv_freq[32]; };                 // theta^(-2i/64), i = 0..31, computed in double on the host
-
 __device__ __forceinline__ float to_f32(float v) { return v; }
 __device__ __forceinline__ float to_f32(__nv_bfloat16 v) { return __bfloat162float(v); }
 __device__ __forceinline__ void from_f32(float& d, float v) { d = v; }
 __device__ __forceinline__ void from_f32(__nv_bfloat16& d, float v) { d = __float2bfloat16_rn(v); }
 
-// In place on the q and k column blocks of qkv [ntok, 3H]: pair (i, i + 32) of every head turns by pos * inv_freq[i].
-// One thread per (token, q|k, head, i): lanes of a warp are the 32 pairs of one head, so both accesses are coalesced.
+// 16 bytes of T (4 floats or 8 bf16) moved as one vector
+template <class T> struct Vec16 {
+    static constexpr int N = 16 / (int)sizeof(T);
+    T v[N];
+    __device__ __forceinline__ void load(const T* p) { *reinterpret_cast<uint4*>(v) = *reinterpret_cast<const uint4*>(p); }
+    __device__ __forceinline__ void store(T* p) const { *reinterpret_cast<uint4*>(p) = *reinterpret_cast<const uint4*>(v); }
+};
+
+// In place on the q and k column blocks of qkv [ntok, 3H]: pair (i, i + 32) of every head turns by the angle whose
+// (cos, sin) sits in table[pos][i] (float2 [max_pos][32], built in double at weights load).  A thread owns N consecutive
+// pairs of one head (N = 4 FP32 / 8 BF16): two 16-byte loads, two 16-byte stores, all coalesced.
 template <class T>
-static __global__ void __launch_bounds__(256) rope_kernel(T* __restrict__ qkv, const int* __restrict__ pos, int ntok, int H, RopeFreq fr)
+static __global__ void __launch_bounds__(256) rope_kernel(T* __restrict__ qkv, const int* __restrict__ pos, int ntok, int H,
+                                                           const float2* __restrict__ table)
 {
-    const int heads2 = 2 * (H >> 6);                      // q heads then k heads: columns [0, 2H) in blocks of 64
+    constexpr int N = Vec16<T>::N;
+    const int per_head = 32 / N, per_tok = 2 * (H >> 6) * per_head;       // q heads then k heads: columns [0, 2H)
     const long long gid = (long long)blockIdx.x * 256 + threadIdx.x;
-    const int i = (int)(gid & 31);
-    const long long hw = gid >> 5;
-    const int hh = (int)(hw % heads2);
-    const long long t = hw / heads2;
+    const int t = (int)(gid / per_tok);
     if (t >= ntok) return;
-    T* p = qkv + (size_t)t * 3 * H + hh * 64 + i;
-    float s, c;
-    sincosf((float)pos[t] * fr.inv_freq[i], &s, &c);
-    const float x1 = to_f32(p[0]), x2 = to_f32(p[32]);
-    from_f32(p[0], x1 * c - x2 * s);
-    from_f32(p[32], x2 * c + x1 * s);
+    const int slot = (int)(gid - (long long)t * per_tok);
+    const int hh = slot / per_head, i0 = (slot - hh * per_head) * N;
+    T* p = qkv + (size_t)t * 3 * H + hh * 64 + i0;
+    const float2* cs = table + (size_t)pos[t] * 32 + i0;
+    Vec16<T> x1, x2;
+    x1.load(p); x2.load(p + 32);
+#pragma unroll
+    for (int e = 0; e < N; e++) {
+        const float2 r = __ldg(cs + e);
+        const float a = to_f32(x1.v[e]), b = to_f32(x2.v[e]);
+        from_f32(x1.v[e], a * r.x - b * r.y);
+        from_f32(x2.v[e], b * r.x + a * r.y);
+    }
+    x1.store(p); x2.store(p + 32);
 }
 
-// f[t, j] = gelu(u[t, j]) * u[t, F + j] (erf GELU), u [ntok, 2F]; two elements per thread
+// f[t, j] = gelu(u[t, j]) * u[t, F + j] (erf GELU), u [ntok, 2F]; 16 bytes of the activation per thread (F % 8 == 0)
 template <class T>
-static __global__ void __launch_bounds__(256) geglu_kernel(const T* __restrict__ u, T* __restrict__ f, long long ntok, int F)
+static __global__ void __launch_bounds__(256) geglu_kernel(const T* __restrict__ u, T* __restrict__ f, int ntok, int F)
 {
-    const long long gid = ((long long)blockIdx.x * 256 + threadIdx.x) * 2;
-    if (gid >= ntok * F) return;
-    const long long t = gid / F;
-    const int j = (int)(gid - t * F);                     // F is even: both elements are in the same row
-    const T* a = u + (size_t)t * 2 * F + j;
+    constexpr int N = Vec16<T>::N;
+    const int per_tok = F / N;
+    const long long gid = (long long)blockIdx.x * 256 + threadIdx.x;
+    const int t = (int)(gid / per_tok);
+    if (t >= ntok) return;
+    const int j = (int)(gid - (long long)t * per_tok) * N;
+    Vec16<T> a, g;
+    a.load(u + (size_t)t * 2 * F + j); g.load(u + (size_t)t * 2 * F + F + j);
 #pragma unroll
-    for (int e = 0; e < 2; e++) {
-        const float z = to_f32(a[e]), gt = to_f32(a[F + e]);
-        from_f32(f[(size_t)t * F + j + e], 0.5f * z * (1.0f + erff(z * 0.70710678118654752f)) * gt);
+    for (int e = 0; e < N; e++) {
+        const float z = to_f32(a.v[e]);
+        from_f32(a.v[e], 0.5f * z * (1.0f + erff(z * 0.70710678118654752f)) * to_f32(g.v[e]));
     }
+    a.store(f + (size_t)t * F + j);
 }
 
 }  // namespace enc

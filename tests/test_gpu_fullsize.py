@@ -134,3 +134,88 @@ def test_configs4_full_size_50m_spans():
         want_tok = ("[" + gen.TYPE_NAMES_6[types[i]] + "_" + bytes(dig[k]).hex()[:10] + "]").encode()
         assert bytes(got_tok[got_off[i]:got_off[i + 1]]) == want_tok, int(i)
     cache.close(); ctx.close()
+
+
+def test_modern_shape_full_size_in_bench_configuration():
+    """NEXT-3 at the size `bench.py --workload modern` times: 4096 records, ~1 M tokens in one chunk through the 22-layer
+    ModernBERT-base-shaped encoder; oracle logits / labels on sampled sequences (shortest, longest, first, last, seeded picks)."""
+    import torch
+    import paper_2606_15650_b200 as P
+    from oracle import encoder, encoder_modern
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device")
+    dev = "cuda:0"
+    d = gen.DESCS["base_modern"]
+    rec, win = gen.workload_base(n_records=4096, seed=gen.SEED_BASE + 2, desc=d)    # bench.py's "modern" workload
+    w = gen.make_weights_modern(d, gen.SEED_BASE + 7, planted=(2.0, 0.5, 4.0))
+    ids, cu = win["token_ids"], win["cu_seqlens"]
+    T, B = ids.size, cu.size - 1
+    assert T > 900_000
+    ctx = P.Context(0, workspace_bytes=P.anon_workspace_bytes(d, T, B) + (256 << 20))
+    W = P.Weights(ctx, d, gen.pack_blob_modern(w))
+    logits = torch.zeros((T, d["num_labels"]), dtype=torch.float32, device=dev)
+    labels = torch.zeros(T, dtype=torch.int32, device=dev)
+    P.anon_ner_forward(ctx, W, torch.from_numpy(ids).to(dev), torch.from_numpy(cu).to(dev), logits, labels)
+    assert ctx.sync() == 0
+    got_logits, got_labels = logits.cpu().numpy(), labels.cpu().numpy()
+    W.close(); ctx.close()
+    assert np.array_equal(got_labels, encoder.argmax_labels(got_logits))
+    lens = np.diff(cu)
+    picks = {int(np.argmin(lens)), int(np.argmax(lens)), 0, B - 1} | set(np.random.default_rng(6).integers(0, B, 3).tolist())
+    want = encoder_modern.forward_packed(w, d, ids, cu, seq_subset=sorted(picks))
+    rows = ~np.isnan(want[:, 0])
+    assert rows.sum() >= 512
+    err = np.abs(got_logits[rows] - want[rows])
+    assert err.max() <= 3e-2, err.max()
+    mism = got_labels[rows] != encoder.argmax_labels(want[rows])
+    assert (encoder.top2_margin(want[rows])[mism] < 3e-2).all()
+    assert 1.0 - mism.mean() >= 0.999
+
+
+def test_regex_scan_full_size():
+    """NEXT-4 at the size kernel_bench times (~400 MB of configs[2]-shaped text, one call): the oracle's brute-force scan on
+    sampled records (first, last, longest, seeded picks) equals the GPU's spans for those records; over ALL spans: ordered,
+    inside their record, non-overlapping, word-bounded, and `re.fullmatch` of the reported pattern on a seeded sample."""
+    import re
+    import torch
+    import paper_2606_15650_b200 as P
+    from oracle import regex_layer as rx
+    from paper_2606_15650_b200 import regex_dfa
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device")
+    dev = "cuda:0"
+    rec = gen.workload_stream(n_records=2000, n_pool=50000)
+    reps = int(400e6 / rec["text"].size)
+    text = np.tile(rec["text"], reps)
+    sizes = np.tile(np.diff(rec["rec_off"]), reps)
+    roff = np.zeros(sizes.size + 1, np.int64)
+    roff[1:] = np.cumsum(sizes)
+    R = sizes.size
+    ctx = P.Context(0, workspace_bytes=int(text.size * 2.2) + (64 << 20))
+    rgx = P.Regex(ctx, regex_dfa.compile_patterns([(k, p) for k, (_n, p) in enumerate(rx.PATTERNS)], rx.MAX_MATCH))
+    cap = text.size // 40
+    spans = torch.zeros((cap, 4), dtype=torch.int32, device=dev)
+    num = torch.zeros(1, dtype=torch.int32, device=dev)
+    P.anon_regex_scan(ctx, rgx, torch.from_numpy(text).to(dev), torch.from_numpy(roff).to(dev), spans, num)
+    assert ctx.sync() == 0
+    n = int(num.item())
+    got = spans[:n].cpu().numpy()
+    rgx.close(); ctx.close()
+    assert 1_000_000 < n <= cap
+    r, cs, ce, k = got[:, 0].astype(np.int64), got[:, 1].astype(np.int64), got[:, 2].astype(np.int64), got[:, 3]
+    assert (np.diff(r) >= 0).all() and (cs < ce).all() and (ce - cs <= rx.MAX_MATCH).all() and (ce <= sizes[r]).all()
+    same = np.diff(r) == 0
+    assert (cs[1:][same] >= ce[:-1][same]).all()                                   # non-overlapping, ordered inside a record
+    word = np.zeros(256, bool); word[list(rx._WORD)] = True
+    a, b = roff[r] + cs, roff[r] + ce
+    inner = cs > 0
+    assert not word[text[a[inner] - 1]].any()                                      # left word boundary
+    inner = ce < sizes[r]
+    assert not word[text[b[inner]]].any()                                          # right word boundary
+    for i in np.random.default_rng(8).integers(0, n, 3000):
+        assert re.fullmatch(rx.PATTERNS[k[i]][1].encode(), text[a[i]:b[i]].tobytes())
+    picks = {0, R - 1, int(np.argmax(sizes))} | set(np.random.default_rng(9).integers(0, R, 40).tolist())
+    for q in sorted(picks):
+        want = rx.scan_record(text[roff[q]:roff[q + 1]].tobytes())
+        lo, hi = np.searchsorted(r, q), np.searchsorted(r, q, side="right")
+        assert [tuple(x) for x in got[lo:hi, 1:].tolist()] == want, q

@@ -280,7 +280,9 @@ int  anon_pipeline_host_text(anon_ctx* ctx, const anon_weights* w, anon_cache* c
 /* ---- building blocks exported for parity tests and per-kernel roofline measurement ----------- */
 /* C[M,N] = A[M,K] * W[N,K]^T + bias[N], BF16 operands, FP32 accumulate on the tcgen05
  * tensor cores (S8a A2/A4/A5/A6).  epilogue: 0 = bias -> BF16 out; 1 = bias, erf-GELU ->
- * BF16 out; 2 = bias + FP32 residual[M,N] -> FP32 out.  K % 64 == 0, N % 8 == 0 required.
+ * BF16 out; 2 = bias + FP32 residual[M,N] -> FP32 out; 4 = GeGLU (NEXT-3): C is BF16 [M, N/2] with
+ * C[:, 128t + j] = gelu(acc[:, 256t + j]) * acc[:, 256t + 128 + j], i.e. W holds, per 256-row tile, 128 "input" rows followed
+ * by their 128 gate rows; no bias is added; N % 256 == 0.  K % 64 == 0, N % 8 == 0 required.
  * d_A, d_W BF16 (uint16 bit patterns) row-major, 16-byte aligned.  Asynchronous. */
 int  anon_gemm_bf16(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,
                     const float* d_residual, void* d_C, int32_t M, int32_t N, int32_t K, int32_t epilogue);

@@ -29,6 +29,9 @@ struct anon_weights {
     float* g_f = nullptr;
     void* zeros = nullptr;
     float2 *rope_g = nullptr, *rope_l = nullptr;       // (cos, sin) of pos * theta^(-2i/64), [max_pos][32]
+    // W_i stored with its rows interleaved per 256-row tile (128 a-rows, then their 128 gate rows) so that the FFN1 GEMM's
+    // GeGLU epilogue (gemm_tcgen05.cu EPI 4) finds a and gate in the same accumulator tile
+    bool geglu_fused = false;
     std::vector<LayerW> layers;
 };
 
@@ -97,18 +100,19 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
     const size_t H = d.hidden, F = d.ffn, V = d.vocab, NL = d.num_labels, P = d.max_pos;
     const bool bf = d.dtype == 1;
     const size_t msz = bf ? 2 : 4;
-    struct Item { void** dst; size_t n; bool matrix; };
+    struct Item { void** dst; size_t n; bool matrix; bool geglu_rows = false; };
     std::vector<Item> items;
     w->layers.resize(d.layers);
     size_t zero_bytes = 0;
     if (d.arch == 1) {
+        w->geglu_fused = bf && F % 128 == 0;
         items.push_back({&w->E_w, V * H, true});
         items.push_back({(void**)&w->g_e, H, false});
         for (int l = 0; l < d.layers; l++) {
             LayerW& L = w->layers[l];
             items.push_back({(void**)&L.g_1, H, false});    items.push_back({&L.W_qkv, 3 * H * H, true});
             items.push_back({&L.W_o, H * H, true});         items.push_back({(void**)&L.g_2, H, false});
-            items.push_back({&L.W_1, 2 * F * H, true});     items.push_back({&L.W_2, H * F, true});
+            items.push_back({&L.W_1, 2 * F * H, true, w->geglu_fused});     items.push_back({&L.W_2, H * F, true});
         }
         items.push_back({(void**)&w->g_f, H, false});
         zero_bytes = std::max(P * H * msz, 4 * std::max(3 * H, 2 * F));
@@ -149,8 +153,19 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
         off = (off + 255) / 256 * 256;
         void* dst = w->store + off;
         *it.dst = dst;
+        std::vector<float> perm;
+        const float* from = src;
+        if (it.geglu_rows) {                         // tile k: a-rows [128k, 128k + 128), then gate rows F + [128k, 128k + 128)
+            perm.resize(it.n);
+            for (size_t k = 0; k < F / 128; k++)
+                for (size_t r = 0; r < 128; r++) {
+                    memcpy(&perm[((2 * k) * 128 + r) * H], src + (k * 128 + r) * H, H * 4);
+                    memcpy(&perm[((2 * k + 1) * 128 + r) * H], src + (F + k * 128 + r) * H, H * 4);
+                }
+            from = perm.data();
+        }
         if (it.matrix && bf) {
-            e = cudaMemcpyAsync(stage, src, it.n * 4, cudaMemcpyHostToDevice, ctx->stream);
+            e = cudaMemcpyAsync(stage, from, it.n * 4, cudaMemcpyHostToDevice, ctx->stream);
             if (e == cudaSuccess) {
                 f32_to_bf16_kernel<<<1024, 256, 0, ctx->stream>>>(stage, (__nv_bfloat16*)dst, it.n);
                 e = cudaStreamSynchronize(ctx->stream);      // stage is reused by the next matrix
@@ -294,12 +309,16 @@ static int modern_chunk(anon_ctx* ctx, WsCursor c, const anon_weights* w, const 
         std::swap(x, y);
         norm(x, L.g_2, fixed_ln ? nullptr : h);
         CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+        if (w->geglu_fused) {
+            if ((rc = gemm(PROF_GEMM_FFN1, gin, L.W_1, nullptr, f, 2 * F, H, 4))) return rc;
+        } else {
         if ((rc = gemm(PROF_GEMM_FFN1, gin, L.W_1, nullptr, u, 2 * F, H, 0))) return rc;
         { ProfScope ps(ctx, PROF_ROW, (double)nt * 3 * F * es);
         const long long vecs = (long long)nt * F / (bf ? 8 : 4);
         if (bf) enc::geglu_kernel<__nv_bfloat16><<<(unsigned)((vecs + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)u, (__nv_bfloat16*)f, nt, F);
         else enc::geglu_kernel<float><<<(unsigned)((vecs + 255) / 256), 256, 0, st>>>((const float*)u, (float*)f, nt, F); }
         CU_LAUNCH_CHECK(ctx, "geglu_kernel");
+        }
         if ((rc = gemm(PROF_GEMM_FFN2, f, L.W_2, x, y, H, F, 2))) return rc;
         std::swap(x, y);
     }

@@ -38,7 +38,7 @@ constexpr int A_STAGE_BYTES = BM * BK * 2;
 template <int BN, int EPI, int NB, int CG> struct Cfg {
     static constexpr int B_STAGE_BYTES = (BN / CG) * BK * 2;
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
-    static constexpr int EPI_WARPS = (EPI >= 2) ? 4 : 8;
+    static constexpr int EPI_WARPS = (EPI == 2 || EPI == 3) ? 4 : 8;
     static constexpr int PAR_BYTES = 3 * 1024 * 4;                // EPI 3: bias, gamma, beta staged in shared memory (N <= 1024)
     static constexpr int EPI_BYTES = (EPI == 3) ? 4 * (NB + 1) * 4096 + PAR_BYTES : (EPI == 2) ? 4 * NB * 4096 + 12288 /*bias, gamma, beta staged for the epilogue*/ : 8 * 4096;   // 4 KB boxes
     static constexpr int STAGES = (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES > 6 ? 6 : (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES;
@@ -70,7 +70,7 @@ __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.
 // every z (the leading coefficient is positive, so the form saturates correctly and needs no clamp).  That is
 // ~1e3 below the BF16 rounding of the stored activation.  The coefficients below carry the factor -log2(e) so that
 // sigma(u) = 1 / (1 + 2^(u')).  Cost per pair: 8 packed FMA-pipe ops + 4 MUFU (ex2, rcp) + 1 convert.
-__device__ __forceinline__ uint32_t gelu2_bf16(uint64_t z) {
+__device__ __forceinline__ uint64_t gelu2_f32(uint64_t z) {
     constexpr float kL = -1.4426950408889634f;
     const uint64_t c1 = pk2(kL * 1.5956562720997576f, kL * 1.5956562720997576f);
     const uint64_t c3 = pk2(kL * 0.07293758090262617f, kL * 0.07293758090262617f);
@@ -88,9 +88,11 @@ __device__ __forceinline__ uint32_t gelu2_bf16(uint64_t z) {
     const uint64_t d = add2(pk2(ex2_approx(u0), ex2_approx(u1)), pk2(1.0f, 1.0f));
     float d0, d1;
     upk2(d, d0, d1);
-    const uint64_t g = mul2(z, pk2(rcp_approx(d0), rcp_approx(d1)));
+    return mul2(z, pk2(rcp_approx(d0), rcp_approx(d1)));
+}
+__device__ __forceinline__ uint32_t gelu2_bf16(uint64_t z) {
     float g0, g1;
-    upk2(g, g0, g1);
+    upk2(gelu2_f32(z), g0, g1);
     return pack_bf16(g0, g1);
 }
 
@@ -115,6 +117,8 @@ __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
 
 // EPI: 0 = +bias -> BF16;  1 = +bias, GELU -> BF16;  2 = +bias +residual(FP32) -> FP32;
 //      3 = LayerNorm(+bias +residual) -> FP32 x and BF16 xb (whole rows per CTA pair, see the EPI 3 branch)
+//      4 = GeGLU (NEXT-3): the tile's first BN/2 accumulator columns are a, the last BN/2 their gates (W's rows are
+//          interleaved per tile by the caller); writes gelu(a) * gate as BF16 [M, N/2]; no bias
 template <int BN, int EPI, int NB, int CG>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
@@ -147,7 +151,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     // block (the LayerNorm needs whole rows); the other epilogues take tiles round-robin.
     auto get_tile = [&](int lt, int& m_blk, int& n_blk) -> bool {
         if (EPI == 3) { m_blk = cid + (lt / num_n) * ncl; n_blk = lt % num_n; return m_blk < num_m; }
-        if (EPI <= 1 && num_m >= 2 * ncl) {
+        if ((EPI <= 1 || EPI == 4) && num_m >= 2 * ncl) {
             // short-K GEMMs with many row blocks: a pair keeps its row block of A (256 x K, L2-resident across the
             // pairs) for all n-tiles, starting at a different n so that the pairs do not ask for the same W tile at once
             m_blk = cid + (lt / num_n) * ncl; n_blk = (lt + cid) % num_n; return m_blk < num_m;
@@ -519,6 +523,44 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                 ptx::mbar_wait(tfull_bar(acc), acc_ph);
                 ptx::tc_fence_after();
                 const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
+                if constexpr (EPI == 4) {
+                    // this warp's 64 output columns: a = accumulator columns [half*64, +64), gates = [BN/2 + half*64, +64)
+                    static_assert(EPI != 4 || BN == 256, "GeGLU epilogue: 256-column tiles");
+                    const int col = n_blk * (BN / 2) + half * 64;
+                    uint32_t o[32];
+#pragma unroll
+                    for (int hh = 0; hh < 2; hh++) {
+                        uint32_t ra[32], rg[32];
+                        ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)(half * 64 + hh * 32), ra);
+                        ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)(BN / 2 + half * 64 + hh * 32), rg);
+                        ptx::tmem_ld_wait();
+                        if (hh == 1) {                             // this warp's share of the accumulator is read
+                            ptx::tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) arrive_tempty(acc);
+                        }
+#pragma unroll
+                        for (int v = 0; v < 8; v++) {
+                            float a0, a1, a2, a3;
+                            upk2(mul2(gelu2_f32(pk2(__uint_as_float(ra[4 * v]), __uint_as_float(ra[4 * v + 1]))),
+                                      pk2(__uint_as_float(rg[4 * v]), __uint_as_float(rg[4 * v + 1]))), a0, a1);
+                            upk2(mul2(gelu2_f32(pk2(__uint_as_float(ra[4 * v + 2]), __uint_as_float(ra[4 * v + 3]))),
+                                      pk2(__uint_as_float(rg[4 * v + 2]), __uint_as_float(rg[4 * v + 3]))), a2, a3);
+                            o[hh * 16 + 2 * v] = pack_bf16(a0, a1);
+                            o[hh * 16 + 2 * v + 1] = pack_bf16(a2, a3);
+                        }
+                    }
+                    if (row0 < M && col < N / 2) {                 // warp-uniform
+                        if (lane == 0) ptx::bulk_wait_read<0>();   // the previous store has read the staging box
+                        __syncwarp();
+#pragma unroll
+                        for (int v = 0; v < 8; v++)
+                            st_shared_v4(buf + row_off + (((uint32_t)v ^ sw) << 4), o[4 * v], o[4 * v + 1], o[4 * v + 2], o[4 * v + 3]);
+                        ptx::fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) { ptx::tma_store_2d(&tmap_c, buf, col, row0); ptx::bulk_commit(); }
+                    }
+                } else {
 #pragma unroll 1
                 for (int c0 = half * (BN / 2); c0 < (half + 1) * (BN / 2); c0 += 64) {   // 32-row x 64-column BF16 boxes
                     const int col = n_blk * BN + c0;
@@ -558,6 +600,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                         __syncwarp();
                         if (lane == 0) { ptx::tma_store_2d(&tmap_c, buf, col, row0); ptx::bulk_commit(); }
                     }
+                }
                 }
                 if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
             }
@@ -626,13 +669,13 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
     if (rc) return rc;
     rc = make_tmap_2d(ctx, &tb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, W, (uint64_t)N, (uint64_t)K, BK, BN / CG);
     if (rc) return rc;
-    if (EPI >= 2) {
+    if (EPI == 2 || EPI == 3) {
         rc = make_tmap_2d(ctx, &tc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Cout, (uint64_t)M, (uint64_t)N, 32, 32);
         if (rc) return rc;
         rc = make_tmap_2d(ctx, &tr, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, residual, (uint64_t)M, (uint64_t)N, 32, 32);
         if (rc) return rc;
     } else {
-        rc = make_tmap_2d(ctx, &tc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, Cout, (uint64_t)M, (uint64_t)N, 64, 32);
+        rc = make_tmap_2d(ctx, &tc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, Cout, (uint64_t)M, (uint64_t)(EPI == 4 ? N / 2 : N), 64, 32);
         if (rc) return rc;
         tr = tc;
     }
@@ -678,11 +721,13 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
 int gemm_bf16_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias,
                    const float* residual, void* Cout, int M, int N, int K, int epilogue)
 {
-    if (!ctx || !A || !W || !bias || !Cout || M < 0 || N <= 0 || K <= 0 || epilogue < 0 || epilogue > 2 ||
+    if (!ctx || !A || !W || !bias || !Cout || M < 0 || N <= 0 || K <= 0 || epilogue < 0 || epilogue == 3 || epilogue > 4 ||
         (epilogue == 2 && !residual))
         return ANON_ERR_INVALID_ARG;
     if (K % BK != 0 || N % 8 != 0) return ANON_ERR_UNSUPPORTED;
+    if (epilogue == 4 && N % 256 != 0) return ANON_ERR_UNSUPPORTED;       // whole (a | gate) tiles only
     if (M == 0) return ANON_OK;
+    if (epilogue == 4) return launch_gemm<256, 4, 2, 2>(ctx, A, W, bias, residual, Cout, M, N, K);
     const bool long_k = K >= 2048;
     if (N > 128) {                 // CTA pairs: 256 x 256 tiles
         switch (epilogue) {

@@ -181,3 +181,29 @@ def test_pipeline_on_modern_weights(env):
     cache.close(); W.close()
     assert np.array_equal(res["spans"], np.asarray(spans, np.int32).reshape(-1, 4))
     assert np.array_equal(res["out_tokens"], want["out_tokens"]) and np.array_equal(res["hit"], want["hit"])
+
+
+@pytest.mark.parametrize("M,F,K", [(300, 128, 128), (1000, 1152, 768), (4096 + 77, 256, 64)])
+def test_geglu_gemm_epilogue_against_fp64(env, M, F, K):
+    """K2 with the GeGLU epilogue (anon_gemm_bf16 epilogue 4): W_i's rows interleaved per 256-row tile exactly as
+    anon_weights_load does for arch 1; several M tiles + a ragged tail, one and many column tiles."""
+    P, torch, ctx = env
+    from oracle import encoder_modern as em
+    rng = np.random.default_rng(M + F + K)
+    A = _bf16(rng.standard_normal((M, K)))
+    Wi = _bf16(rng.standard_normal((2 * F, K)) * 0.08)
+    u = A.astype(np.float64) @ Wi.astype(np.float64).T
+    want = em.gelu(u[:, :F]) * u[:, F:]
+    perm = np.concatenate([np.concatenate([np.arange(128 * k, 128 * k + 128), F + np.arange(128 * k, 128 * k + 128)])
+                           for k in range(F // 128)])
+    dev = "cuda:0"
+    dA = torch.from_numpy(A).to(dev).to(torch.bfloat16)
+    dW = torch.from_numpy(np.ascontiguousarray(Wi[perm])).to(dev).to(torch.bfloat16)
+    dC = torch.full((M, F), float("nan"), dtype=torch.bfloat16, device=dev)
+    P.anon_gemm_bf16(ctx, dA, dW, torch.zeros(2 * F, device=dev), None, dC, 4)
+    assert ctx.sync() == 0
+    got = dC.float().cpu().numpy().astype(np.float64)
+    assert (np.abs(got - want) <= 2.0 ** -8 * np.abs(want) + 1e-4 * np.abs(want).max()).all()
+    with pytest.raises(P.AnonError) as ei:          # N must be whole (a | gate) tiles
+        P.anon_gemm_bf16(ctx, dA, dW[:192], torch.zeros(192, device=dev), None, dC, 4)
+    assert ei.value.code == -2

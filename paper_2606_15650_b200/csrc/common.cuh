@@ -116,6 +116,9 @@ int gemm_bf16_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, co
                    const float* residual, void* C, int M, int N, int K, int epilogue);
 int gemm_bf16_res_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* res_y,
                           const float2* res_stats, const float* gamma, const float* beta, float* C, int M, int N, int K);
+// qkv = A W^T, RoPE on the q / k heads in the epilogue; table float2 [32][512] pair-major (cos, sin), pos int [M]
+int gemm_bf16_rope_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const int* pos, const float2* table, void* C,
+                        int M, int N, int K);
 // x = LN(A W^T + bias + residual; gamma, beta) as FP32 (x_out may alias residual) plus its BF16 copy; N % 256 == 0
 int gemm_bf16_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
                       const float* gamma, const float* beta, float eps, float* x_out, __nv_bfloat16* xb_out, int M, int N, int K);

@@ -29,6 +29,7 @@ struct anon_weights {
     float* g_f = nullptr;
     void* zeros = nullptr;
     float2 *rope_g = nullptr, *rope_l = nullptr;       // (cos, sin) of pos * theta^(-2i/64), [max_pos][32]
+    float2 *rope_gt = nullptr, *rope_lt = nullptr;     // the same, pair-major [32][512], for the QKV GEMM's RoPE epilogue
     // W_i stored with its rows interleaved per 256-row tile (128 a-rows, then their 128 gate rows) so that the FFN1 GEMM's
     // GeGLU epilogue (gemm_tcgen05.cu EPI 4) finds a and gate in the same accumulator tile
     bool geglu_fused = false;
@@ -143,7 +144,8 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
     float* stage = nullptr;
     const size_t zero_off = (total + 255) / 256 * 256;
     const size_t rope_off = (zero_off + zero_bytes + 255) / 256 * 256, rope_bytes = d.arch == 1 ? P * 32 * sizeof(float2) : 0;
-    total = rope_off + 2 * rope_bytes;
+    const size_t ropet_off = (rope_off + 2 * rope_bytes + 255) / 256 * 256, ropet_bytes = d.arch == 1 ? 32 * 512 * sizeof(float2) : 0;
+    total = ropet_off + 2 * ropet_bytes;
     cudaError_t e = cudaMalloc(&w->store, total + 256);
     if (e == cudaSuccess && max_matrix) e = cudaMalloc(&stage, max_matrix * 4);
     if (e != cudaSuccess) { cudaFree(w->store); delete w; cuda_fail(ctx, e, "cudaMalloc(weights)"); return ANON_ERR_OOM; }
@@ -196,7 +198,14 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
         w->rope_g = (float2*)(w->store + rope_off);
         w->rope_l = w->rope_g + P * 32;
         e = cudaMemcpyAsync(w->rope_g, tab.data(), 2 * rope_bytes, cudaMemcpyHostToDevice, ctx->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);          // tab dies at the end of this block
+        std::vector<float2> tabt(2 * 32 * 512, make_float2(1.f, 0.f));
+        for (int which = 0; which < 2; which++)
+            for (size_t p = 0; p < P; p++)
+                for (int i = 0; i < 32; i++) tabt[(which * 32 + i) * 512 + p] = tab[(which * P + p) * 32 + i];
+        w->rope_gt = (float2*)(w->store + ropet_off);
+        w->rope_lt = w->rope_gt + 32 * 512;
+        if (e == cudaSuccess) e = cudaMemcpyAsync(w->rope_gt, tabt.data(), 2 * ropet_bytes, cudaMemcpyHostToDevice, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);          // the tables die at the end of this block
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     cudaFree(stage);
@@ -296,12 +305,18 @@ static int modern_chunk(anon_ctx* ctx, WsCursor c, const anon_weights* w, const 
         const bool glob = !has_local || l % d.global_every == 0;
         norm(x, L.g_1, fixed_ln ? nullptr : h);
         CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+        if (bf && H % 64 == 0 && 3 * H > 128) {          // RoPE in the QKV GEMM's epilogue
+            ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * 3 * H * H);
+            rc = gemm_bf16_rope_impl(ctx, xb, (const __nv_bfloat16*)L.W_qkv, pos, glob ? w->rope_gt : w->rope_lt, qkv, nt, 3 * H, H);
+            if (rc) return rc;
+        } else {
         if ((rc = gemm(PROF_GEMM, gin, L.W_qkv, nullptr, qkv, 3 * H, H, 0))) return rc;
         { ProfScope ps(ctx, PROF_ROW, (double)nt * 2 * H * es * 2);
         const float2* tab = glob ? w->rope_g : w->rope_l;
         if (bf) enc::rope_kernel<__nv_bfloat16><<<(unsigned)((rope_threads + 255) / 256), 256, 0, st>>>((__nv_bfloat16*)qkv, pos, nt, H, tab);
         else enc::rope_kernel<float><<<(unsigned)((rope_threads + 255) / 256), 256, 0, st>>>((float*)qkv, pos, nt, H, tab); }
         CU_LAUNCH_CHECK(ctx, "rope_kernel");
+        }
         { ProfScope ps(ctx, PROF_ATTN, glob ? fl_g : fl_l);
         rc = attention_run(ctx, glob ? plan_g : plan_l, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx); }
         if (rc) return rc;

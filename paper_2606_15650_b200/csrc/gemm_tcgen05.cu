@@ -35,6 +35,8 @@ constexpr int A_STAGE_BYTES = BM * BK * 2;
 // paces the kernel), 2 for long K (a fourth mainloop stage is worth more).
 // CG = CTAs per MMA (tcgen05 cta_group): 1 = 128 x BN tile per CTA; 2 = a CTA pair computes 256 x BN, each CTA owning
 // 128 rows of the accumulator and staging only half of the B tile (halves shared-memory fill and operand traffic).
+constexpr int kRopeStride = 512;   // positions per pair row of the EPI 5 (cos, sin) table (max_pos <= 512)
+
 template <int BN, int EPI, int NB, int CG> struct Cfg {
     static constexpr int B_STAGE_BYTES = (BN / CG) * BK * 2;
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
@@ -119,6 +121,10 @@ __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
 //      3 = LayerNorm(+bias +residual) -> FP32 x and BF16 xb (whole rows per CTA pair, see the EPI 3 branch)
 //      4 = GeGLU (NEXT-3): the tile's first BN/2 accumulator columns are a, the last BN/2 their gates (W's rows are
 //          interleaved per tile by the caller); writes gelu(a) * gate as BF16 [M, N/2]; no bias
+//      5 = QKV projection with rotary position embedding (NEXT-3): like 0 without bias; in the q and k column blocks
+//          (columns < 2N/3) every 64-column box is one head and its pairs (j, j + 32) turn by the angle of the row's
+//          position.  Parameter reuse: ln_g = (cos, sin) table float2 [32][kRopeStride] (pair-major, so that the rows
+//          of a warp -- consecutive positions -- read consecutive entries), res_stats = int position id per row
 template <int BN, int EPI, int NB, int CG>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
@@ -151,7 +157,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     // block (the LayerNorm needs whole rows); the other epilogues take tiles round-robin.
     auto get_tile = [&](int lt, int& m_blk, int& n_blk) -> bool {
         if (EPI == 3) { m_blk = cid + (lt / num_n) * ncl; n_blk = lt % num_n; return m_blk < num_m; }
-        if ((EPI <= 1 || EPI == 4) && num_m >= 2 * ncl) {
+        if ((EPI <= 1 || EPI >= 4) && num_m >= 2 * ncl) {
             // short-K GEMMs with many row blocks: a pair keeps its row block of A (256 x K, L2-resident across the
             // pairs) for all n-tiles, starting at a different n so that the pairs do not ask for the same W tile at once
             m_blk = cid + (lt / num_n) * ncl; n_blk = (lt + cid) % num_n; return m_blk < num_m;
@@ -573,12 +579,24 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                         __syncwarp();
                         if (lane == 0) arrive_tempty(acc);
                     }
+                    if (EPI == 5 && row0 < M && col < 2 * (N / 3)) {   // warp-uniform: a q or k head
+                        const int row = row0 + lane;
+                        const int p = row < M ? reinterpret_cast<const int*>(res_stats)[row] : 0;
+                        const float2* tab = reinterpret_cast<const float2*>(ln_g) + p;
+#pragma unroll
+                        for (int j = 0; j < 32; j++) {
+                            const float2 cs = __ldg(tab + j * kRopeStride);
+                            const float a = __uint_as_float(r[j]), b = __uint_as_float(r[j + 32]);
+                            r[j] = __float_as_uint(a * cs.x - b * cs.y);
+                            r[j + 32] = __float_as_uint(b * cs.x + a * cs.y);
+                        }
+                    }
                     if (row0 < M && col < N) {                     // warp-uniform
                         uint32_t o[32];
 #pragma unroll
                         for (int v = 0; v < 16; v++) {             // 4 columns per step; N % 8 == 0
                             float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
-                            if (col + 4 * v < N) bb = __ldg(reinterpret_cast<const float4*>(bias + col + 4 * v));
+                            if (EPI != 5 && col + 4 * v < N) bb = __ldg(reinterpret_cast<const float4*>(bias + col + 4 * v));
                             const uint64_t z0 = add2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), pk2(bb.x, bb.y));
                             const uint64_t z1 = add2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), pk2(bb.z, bb.w));
                             if (EPI == 1) {
@@ -742,6 +760,18 @@ int gemm_bf16_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W
         case 1: return launch_gemm<128, 1, 2, 1>(ctx, A, W, bias, residual, Cout, M, N, K);
         default: return launch_gemm<128, 2, 4, 1>(ctx, A, W, bias, residual, Cout, M, N, K);
     }
+}
+
+// qkv = A W^T with RoPE applied to the q and k heads in the epilogue (EPI 5); N = 3H, H % 64 == 0, N % 256 == 0 not needed
+// (boxes are 64 columns = one head).  table: float2 [32][512] pair-major (cos, sin); pos: int [M].
+int gemm_bf16_rope_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const int* pos, const float2* table,
+                        void* Cout, int M, int N, int K)
+{
+    if (!ctx || !A || !W || !pos || !table || !Cout || M < 0 || N <= 128 || K <= 0) return ANON_ERR_INVALID_ARG;
+    if (K % BK != 0 || N % 192 != 0) return ANON_ERR_UNSUPPORTED;
+    if (M == 0) return ANON_OK;
+    LnArgs ln{reinterpret_cast<const float*>(table), nullptr, 0.f, nullptr, reinterpret_cast<const float2*>(pos)};
+    return launch_gemm<256, 5, 2, 2>(ctx, A, W, reinterpret_cast<const float*>(table), nullptr, Cout, M, N, K, &ln);
 }
 
 // C = A W^T + bias + LN(res_y; stats, gamma, beta): the residual stream is kept UN-normalised (res_y, with per-row

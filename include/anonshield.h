@@ -173,6 +173,20 @@ int64_t anon_cache_entry(anon_cache* c, uint64_t uid, uint8_t* h_bytes, size_t b
 int  anon_cache_export(anon_cache* c, uint8_t* h_bytes, size_t bytes_capacity, int64_t* h_offsets, uint8_t* h_digests,
                        uint64_t* n_unique, uint64_t* n_bytes);
 
+/* ---- NEXT-5: bounded cache, call-granular LRU eviction ("LRU cache"; S8f NEXT-5; reading D21) ------------------------ */
+/* Enables (or with 0 disables and forgets) recency tracking: from now on every anon_pseudonymize call stamps each entry it
+ * looks up -- hit or newly inserted -- with the call's sequence number (4 bytes of device memory per max_unique; entries that
+ * predate tracking count as oldest).  Synchronises.  Errors: OOM, CUDA. */
+int  anon_cache_track_use(anon_cache* c, int enable);
+/* Shrinks the cache to its `keep` most recently used entries: the entries with the largest stamps stay, inside the cut-off
+ * stamp the lowest uids stay; everything else is forgotten (a later lookup of such a string is a miss and recomputes the
+ * same HMAC -- no pseudonym ever changes).  Survivors are renumbered 0..keep-1 in their old uid order and keep their
+ * bytes, digests and stamps; the lookup / hit counters and the key binding are untouched.  Export the mapping
+ * (anon_cache_export) BEFORE evicting if it must stay complete (the paper's persistent mapping).  keep >= n_unique is
+ * a no-op.  *n_evicted (may be NULL) receives the number of entries dropped.  Needs workspace for the surviving bytes plus
+ * 45 bytes per entry.  Synchronises.  Errors: UNSUPPORTED (tracking not enabled), OOM, CUDA. */
+int  anon_cache_evict(anon_cache* c, uint64_t keep, uint64_t* n_evicted);
+
 /* For span i = 0..S-1 in order (e_i = d_span_bytes[off[i] .. off[i+1]), exact bytes):
  *   hit[i] = 1 if e_i is already in the cache (from an earlier call or an earlier i), else 0
  *            and (HMAC_SHA256(key, e_i), uid = number of entries before insertion) is inserted;

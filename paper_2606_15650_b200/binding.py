@@ -60,6 +60,8 @@ _SIGNATURES = {
     "anon_cache_stats": (ctypes.c_int, [_vp, ctypes.POINTER(_u64), ctypes.POINTER(_u64), ctypes.POINTER(_u64)]),
     "anon_cache_entry": (_i64, [_vp, _u64, _vp, _sz, _vp]),
     "anon_cache_export": (ctypes.c_int, [_vp, _vp, _sz, _vp, _vp, ctypes.POINTER(_u64), ctypes.POINTER(_u64)]),
+    "anon_cache_track_use": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "anon_cache_evict": (ctypes.c_int, [_vp, _u64, ctypes.POINTER(_u64)]),
     "anon_pseudonymize": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i64, _vp, _sz, _i32,
                                          ctypes.POINTER(ctypes.c_char_p), _i32, _vp, _sz, _vp, _vp, _vp, _vp]),
     "anon_hmac_spans": (ctypes.c_int, [_vp, _vp, _vp, _i64, _vp, _sz, _vp]),
@@ -214,6 +216,16 @@ class Cache:
         buf = np.zeros(max(int(n), 1), np.uint8)
         lib().anon_cache_entry(self._h, uid, buf.ctypes.data, int(n), dig.ctypes.data)
         return buf[:n].tobytes(), dig.tobytes()
+
+    def track_use(self, enable=True):
+        """NEXT-5: stamp every entry with the sequence number of the last anon_pseudonymize call that looked it up."""
+        self.ctx.check(lib().anon_cache_track_use(self._h, 1 if enable else 0), "anon_cache_track_use")
+
+    def evict(self, keep):
+        """Keep the `keep` most recently used entries (call-granular LRU, reading D21); returns the number evicted."""
+        n = _u64()
+        self.ctx.check(lib().anon_cache_evict(self._h, keep, ctypes.byref(n)), "anon_cache_evict")
+        return n.value
 
     def export(self):
         """The mapping table in uid order: (entity bytes uint8[], offsets int64[U+1], digests uint8[U,32])."""

@@ -16,6 +16,9 @@
 //   emit     every span reads its slot -> uid -> digest and writes its token.
 #include "common.cuh"
 #include "scan.cuh"
+
+#include <algorithm>
+#include <vector>
 #include "sha256.cuh"
 
 #include <new>
@@ -30,6 +33,10 @@ struct anon_cache {
     long long* d_entry_off = nullptr;   // [max_unique + 1]
     uint8_t* d_digests = nullptr;       // [max_unique, 32]
     uint64_t n_unique = 0, arena_used = 0, n_lookups = 0, n_hits = 0;
+    // NEXT-5 (D21): call-granular recency.  epoch = number of anon_pseudonymize calls so far; d_last_use[uid] = epoch of the
+    // last call that looked the entry up (allocated by anon_cache_track_use, NULL = not tracked)
+    uint32_t* d_last_use = nullptr;
+    uint32_t epoch = 0;
     bool key_bound = false;
     uint32_t ipad[8], opad[8];
 };
@@ -296,7 +303,7 @@ constexpr int kEmitWarpBytes = 32 * kEmitMaxToken + 8;     // + alignment slack
 __global__ void __launch_bounds__(kEmitWarps * 32) emit_tokens_kernel(
     long long S, const int* __restrict__ slot_of, const u64* __restrict__ table, const uint8_t* __restrict__ type,
     const uint32_t* __restrict__ digests, const long long* __restrict__ out_off, uint8_t* out,
-    long long* uid_out, uint8_t* dig_out, TypeTable tt, int slug_len, int* d_status)
+    long long* uid_out, uint8_t* dig_out, TypeTable tt, int slug_len, int* d_status, uint32_t* last_use, uint32_t epoch)
 {
     __shared__ __align__(16) uint8_t s_tok[kEmitWarps][(kEmitWarpBytes + 15) / 16 * 16];
     __shared__ uint8_t s_name[64][32];
@@ -318,6 +325,7 @@ __global__ void __launch_bounds__(kEmitWarps * 32) emit_tokens_kernel(
         if (s >= 0) {
             const long long e = slot_index(table[s]);
             if (uid_out) uid_out[i] = e;
+            if (last_use) last_use[e] = epoch;              // every writer of one call stores the same value
             const uint4* dg = (const uint4*)(digests + e * 8);
             const uint4 d0 = __ldg(dg), d1 = __ldg(dg + 1);
             if (dig_out) { uint4* q = (uint4*)(dig_out + i * 32); q[0] = d0; q[1] = d1; }
@@ -443,7 +451,7 @@ extern "C" int anon_cache_create(anon_ctx* ctx, uint64_t max_unique, uint64_t ke
 
 extern "C" void anon_cache_destroy(anon_cache* c) {
     if (!c) return;
-    cudaFree(c->d_table); cudaFree(c->d_arena); cudaFree(c->d_entry_off); cudaFree(c->d_digests);
+    cudaFree(c->d_table); cudaFree(c->d_arena); cudaFree(c->d_entry_off); cudaFree(c->d_digests); cudaFree(c->d_last_use);
     delete c;
 }
 
@@ -453,7 +461,129 @@ extern "C" int anon_cache_clear(anon_cache* c) {
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     CU_TRY(ctx, cudaMemsetAsync(c->d_table, 0, c->n_slots * 8, ctx->stream));
     c->n_unique = c->arena_used = c->n_lookups = c->n_hits = 0;
+    c->epoch = 0;
     c->key_bound = false;
+    return ANON_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-5: bounded cache -- call-granular LRU eviction ("LRU cache"; reading D21)
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+struct EvictIn {
+    const uint8_t* keep; const long long* entry_off;
+    __device__ __forceinline__ scan::I64x3 operator()(long long e) const {
+        const long long k = keep[e];
+        return scan::I64x3{k, k ? entry_off[e + 1] - entry_off[e] : 0, 0};
+    }
+};
+// survivors move to (new uid, new arena offset) in temporary arrays; one thread per old entry
+struct EvictOut {
+    const uint8_t* keep; const long long* entry_off; const uint8_t* arena; const uint32_t* digests; const uint32_t* last_use;
+    long long* new_off; uint8_t* new_arena; uint32_t* new_digests; uint32_t* new_last_use; long long n;
+    __device__ __forceinline__ void operator()(long long e, const scan::I64x3& ex, const scan::I64x3& v) const {
+        if (v.a) {
+            new_off[ex.a] = ex.b;
+            const uint8_t* src = arena + entry_off[e];
+            for (long long k = 0; k < v.b; k++) new_arena[ex.b + k] = src[k];
+#pragma unroll
+            for (int k = 0; k < 8; k++) new_digests[ex.a * 8 + k] = digests[e * 8 + k];
+            new_last_use[ex.a] = last_use[e];
+        }
+        if (e == n - 1) new_off[ex.a + v.a] = ex.b + v.b;
+    }
+};
+
+// rebuilds the table from the compacted entries: all strings are distinct, so the first empty slot of the probe sequence is it
+__global__ void __launch_bounds__(256) cache_reinsert_kernel(const uint8_t* __restrict__ arena, const long long* __restrict__ entry_off,
+                                                             long long n, u64* table, u64 mask)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const long long o = entry_off[e];
+    const u64 h = hash_bytes(arena + o, (int)(entry_off[e + 1] - o));
+    const u64 mine = make_slot(slot_tag(h), 0u, (uint32_t)e);
+    u64 slot = h & mask;
+    while (atomicCAS(&table[slot], 0ull, mine) != 0ull) slot = (slot + 1) & mask;
+}
+
+}  // namespace
+
+extern "C" int anon_cache_track_use(anon_cache* c, int enable) {
+    if (!c) return ANON_ERR_INVALID_ARG;
+    anon_ctx* ctx = c->ctx;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    if (!enable) { cudaFree(c->d_last_use); c->d_last_use = nullptr; return ANON_OK; }
+    if (c->d_last_use) return ANON_OK;
+    if (cudaMalloc(&c->d_last_use, c->max_unique * 4) != cudaSuccess) { cudaGetLastError(); return ANON_ERR_OOM; }
+    CU_TRY(ctx, cudaMemset(c->d_last_use, 0, c->max_unique * 4));     // entries that predate tracking: oldest
+    return ANON_OK;
+}
+
+extern "C" int anon_cache_evict(anon_cache* c, uint64_t keep, uint64_t* n_evicted) {
+    if (!c) return ANON_ERR_INVALID_ARG;
+    anon_ctx* ctx = c->ctx;
+    if (n_evicted) *n_evicted = 0;
+    if (!c->d_last_use) return ANON_ERR_UNSUPPORTED;                   // anon_cache_track_use first
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    CU_TRY(ctx, cudaStreamSynchronize(st));
+    const uint64_t n = c->n_unique;
+    if (keep >= n) return ANON_OK;
+    // which entries stay: the `keep` largest stamps, the lowest uids inside the cut-off stamp (host: n stamps, once per eviction)
+    std::vector<uint32_t> stamp(n);
+    CU_TRY(ctx, cudaMemcpy(stamp.data(), c->d_last_use, n * 4, cudaMemcpyDeviceToHost));
+    std::vector<uint8_t> flag(n, 0);
+    if (keep > 0) {
+        std::vector<uint32_t> sorted(stamp);
+        std::nth_element(sorted.begin(), sorted.begin() + (n - keep), sorted.end());
+        const uint32_t cut = sorted[n - keep];                         // the keep-th largest stamp
+        uint64_t above = 0;
+        for (uint64_t e = 0; e < n; e++) above += stamp[e] > cut;
+        uint64_t quota = keep - above;
+        for (uint64_t e = 0; e < n; e++) {
+            if (stamp[e] > cut) flag[e] = 1;
+            else if (stamp[e] == cut && quota) { flag[e] = 1; quota--; }
+        }
+    }
+    WsCursor ws = ws_begin(ctx);
+    uint8_t* d_keep = (uint8_t*)ws.take(n);
+    long long* new_off = (long long*)ws.take((keep + 1) * 8);
+    uint8_t* new_arena = (uint8_t*)ws.take(c->arena_used + 16);
+    uint32_t* new_dig = (uint32_t*)ws.take(keep * 32 + 32);
+    uint32_t* new_use = (uint32_t*)ws.take(keep * 4 + 4);
+    scan::I64x3* agg = (scan::I64x3*)ws.take(scan::agg_bytes<scan::I64x3>((long long)n));
+    if (!d_keep || !new_off || !new_arena || !new_dig || !new_use || !agg) return ANON_ERR_OOM;
+    CU_TRY(ctx, cudaMemcpyAsync(d_keep, flag.data(), n, cudaMemcpyHostToDevice, st));
+    CU_TRY(ctx, cudaMemsetAsync(new_off, 0, 8, st));
+    ProfScope prof(ctx, PROF_PSEUDO, 0.0, 4);
+    EvictIn in{d_keep, c->d_entry_off};
+    scan::reduce_and_scan<scan::I64x3, scan::SumI64x3>(in, (long long)n, nullptr, agg, st);
+    scan::apply<scan::I64x3, scan::SumI64x3>(in, EvictOut{d_keep, c->d_entry_off, c->d_arena, (const uint32_t*)c->d_digests, c->d_last_use,
+                                                          new_off, new_arena, new_dig, new_use, (long long)n},
+                                             (long long)n, nullptr, agg, st);
+    CU_LAUNCH_CHECK(ctx, "evict compaction");
+    long long kept_bytes = 0;
+    CU_TRY(ctx, cudaMemcpyAsync(&kept_bytes, new_off + keep, 8, cudaMemcpyDeviceToHost, st));
+    CU_TRY(ctx, cudaStreamSynchronize(st));                            // also: flag[] has been consumed
+    CU_TRY(ctx, cudaMemcpyAsync(c->d_entry_off, new_off, (keep + 1) * 8, cudaMemcpyDeviceToDevice, st));
+    if (kept_bytes) CU_TRY(ctx, cudaMemcpyAsync(c->d_arena, new_arena, (size_t)kept_bytes, cudaMemcpyDeviceToDevice, st));
+    if (keep) {
+        CU_TRY(ctx, cudaMemcpyAsync(c->d_digests, new_dig, keep * 32, cudaMemcpyDeviceToDevice, st));
+        CU_TRY(ctx, cudaMemcpyAsync(c->d_last_use, new_use, keep * 4, cudaMemcpyDeviceToDevice, st));
+    }
+    CU_TRY(ctx, cudaMemsetAsync(c->d_table, 0, c->n_slots * 8, st));
+    if (keep) {
+        cache_reinsert_kernel<<<(unsigned)((keep + 255) / 256), 256, 0, st>>>(c->d_arena, c->d_entry_off, (long long)keep, c->d_table,
+                                                                             c->n_slots - 1);
+        CU_LAUNCH_CHECK(ctx, "cache_reinsert_kernel");
+    }
+    CU_TRY(ctx, cudaStreamSynchronize(st));
+    c->n_unique = keep;
+    c->arena_used = (uint64_t)kept_bytes;
+    if (n_evicted) *n_evicted = n - keep;
     return ANON_OK;
 }
 
@@ -565,8 +695,9 @@ int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t*
     }
     emit_tokens_kernel<<<nb256, kEmitWarps * 32, 0, st>>>(S, slot_of, c->d_table, d_type, (const uint32_t*)c->d_digests,
                                                (const long long*)d_out_off, d_out, (long long*)d_uid, d_digests,
-                                               tt, slug_len, ctx->d_status);
+                                               tt, slug_len, ctx->d_status, c->d_last_use, c->epoch + 1);
     CU_LAUNCH_CHECK(ctx, "emit_tokens_kernel");
+    c->epoch++;
     if (!c->key_bound) { memcpy(c->ipad, ps.ipad, 32); memcpy(c->opad, ps.opad, 32); c->key_bound = true; }
     c->n_unique += (uint64_t)n_new;
     c->arena_used += (uint64_t)new_bytes;

@@ -123,15 +123,16 @@ __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
 //          interleaved per tile by the caller); writes gelu(a) * gate as BF16 [M, N/2]; no bias
 //      5 = QKV projection with rotary position embedding (NEXT-3): like 0 without bias; in the q and k column blocks
 //          (columns < 2N/3) every 64-column box is one head and its pairs (j, j + 32) turn by the angle of the row's
-//          position.  Parameter reuse: ln_g = (cos, sin) table float2 [32][kRopeStride] (pair-major, so that the rows
-//          of a warp -- consecutive positions -- read consecutive entries), res_stats = int position id per row
+//          position.  rope_tab = (cos, sin) table float2 [32][kRopeStride] (pair-major, so that the rows of a warp --
+//          consecutive positions -- read consecutive entries), rope_pos = int position id per row
 template <int BN, int EPI, int NB, int CG>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                          const __grid_constant__ CUtensorMap tmap_c, const __grid_constant__ CUtensorMap tmap_r,
                          const __grid_constant__ CUtensorMap tmap_y, const __grid_constant__ CUtensorMap tmap_xb,
                          const float* __restrict__ bias, const float* __restrict__ ln_g, const float* __restrict__ ln_b,
-                         float ln_eps, const float2* __restrict__ res_stats, int M, int N, int K)
+                         float ln_eps, const float2* __restrict__ res_stats, const float2* __restrict__ rope_tab,
+                         const int* __restrict__ rope_pos, int M, int N, int K)
 {
     using C = Cfg<BN, EPI, NB, CG>;
     extern __shared__ uint8_t smem_raw[];
@@ -581,8 +582,8 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                     }
                     if (EPI == 5 && row0 < M && col < 2 * (N / 3)) {   // warp-uniform: a q or k head
                         const int row = row0 + lane;
-                        const int p = row < M ? reinterpret_cast<const int*>(res_stats)[row] : 0;
-                        const float2* tab = reinterpret_cast<const float2*>(ln_g) + p;
+                        const int p = row < M ? rope_pos[row] : 0;
+                        const float2* tab = rope_tab + p;
 #pragma unroll
                         for (int j = 0; j < 32; j++) {
                             const float2 cs = __ldg(tab + j * kRopeStride);
@@ -668,7 +669,8 @@ int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_
 
 namespace {
 
-struct LnArgs { const float* gamma; const float* beta; float eps; void* xb_out; const float2* res_stats; };
+struct LnArgs { const float* gamma; const float* beta; float eps; void* xb_out; const float2* res_stats;
+                const float2* rope_tab = nullptr; const int* rope_pos = nullptr; };
 
 template <int BN, int EPI, int NB, int CG>
 int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
@@ -729,7 +731,9 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
     const float* be = ln ? ln->beta : nullptr;
     const float eps = ln ? ln->eps : 0.f;
     const float2* rs = ln ? ln->res_stats : nullptr;
-    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, ty, txb, bias, g, be, eps, rs, M, N, K));
+    const float2* rtab = ln ? ln->rope_tab : nullptr;
+    const int* rpos = ln ? ln->rope_pos : nullptr;
+    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, ty, txb, bias, g, be, eps, rs, rtab, rpos, M, N, K));
     CU_LAUNCH_CHECK(ctx, "gemm_bf16_tcgen05_kernel");
     return ANON_OK;
 }
@@ -770,8 +774,8 @@ int gemm_bf16_rope_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat
     if (!ctx || !A || !W || !pos || !table || !Cout || M < 0 || N <= 128 || K <= 0) return ANON_ERR_INVALID_ARG;
     if (K % BK != 0 || N % 192 != 0) return ANON_ERR_UNSUPPORTED;
     if (M == 0) return ANON_OK;
-    LnArgs ln{reinterpret_cast<const float*>(table), nullptr, 0.f, nullptr, reinterpret_cast<const float2*>(pos)};
-    return launch_gemm<256, 5, 2, 2>(ctx, A, W, reinterpret_cast<const float*>(table), nullptr, Cout, M, N, K, &ln);
+    LnArgs ln{nullptr, nullptr, 0.f, nullptr, nullptr, table, pos};
+    return launch_gemm<256, 5, 2, 2>(ctx, A, W, nullptr, nullptr, Cout, M, N, K, &ln);
 }
 
 // C = A W^T + bias + LN(res_y; stats, gamma, beta): the residual stream is kept UN-normalised (res_y, with per-row

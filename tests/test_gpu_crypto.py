@@ -197,3 +197,41 @@ def test_cache_export_is_the_mapping_table_and_resumes(env):
     again = _run_gpu(P, torch, ctx, g2, data, off, types, kb, 10, gen.TYPE_NAMES_4)
     assert again["hit"].all() and np.array_equal(again["uid"], first["uid"]) and np.array_equal(again["out_tokens"], first["out_tokens"])
     g2.close()
+
+
+def test_bounded_cache_eviction_matches_oracle(env):
+    """NEXT-5 (reading D21): a Zipf span stream in 12 calls with an eviction after most of them; hit flags, uids and digests
+    of every call, the surviving entries in uid order and the counters equal oracle/cache_lru.py."""
+    P, torch, ctx = env
+    from oracle import cache_lru
+    key = bytes(range(40, 72))
+    pool, poff, _t = gen.entity_pool(3000, 17)
+    ents = [pool[poff[i]:poff[i + 1]].tobytes() for i in range(3000)]
+    rng = np.random.default_rng(12)
+    oc = cache_lru.LruCache(key)
+    gc = P.Cache(ctx, 4096, 1 << 20)
+    with pytest.raises(P.AnonError) as ei:                      # eviction needs recency tracking
+        gc.evict(10)
+    assert ei.value.code == -2
+    gc.track_use()
+    keeps = [None, 900, 900, None, 300, 300, 2000, 1, 50, 0, None, 40]
+    for step, keep in enumerate(keeps):
+        draws = np.minimum(rng.zipf(1.15, 4000) - 1, 2999) if step != 7 else np.arange(5)
+        spans = [ents[int(v)] for v in draws]
+        data = np.frombuffer(b"".join(spans), np.uint8).copy()
+        off = np.zeros(len(spans) + 1, np.int64); off[1:] = np.cumsum([len(s) for s in spans])
+        got = _run_gpu(P, torch, ctx, gc, data, off, None, key, 10, gen.TYPE_NAMES_4)
+        hit, uid, dig = oc.pseudonymize(spans)
+        assert np.array_equal(got["hit"], np.asarray(hit, np.uint8)), step
+        assert np.array_equal(got["uid"], np.asarray(uid, np.int64)), step
+        assert np.array_equal(got["digests"], np.frombuffer(b"".join(dig), np.uint8).reshape(-1, 32)), step
+        if keep is not None:
+            assert gc.evict(keep) == oc.evict(keep), step
+        bytes_, offs, digs = gc.export()
+        want = oc.export()
+        assert offs.size - 1 == len(want), step
+        assert [bytes_[offs[i]:offs[i + 1]].tobytes() for i in range(len(want))] == [e for e, _d in want], step
+        assert digs.tobytes() == b"".join(d for _e, d in want), step
+        st = gc.stats()
+        assert (st["n_unique"], st["n_lookups"], st["n_hits"]) == (len(want), oc.n_lookups, oc.n_hits), step
+    gc.close()

@@ -147,7 +147,7 @@ int  anon_gather_spans(anon_ctx* ctx, const uint8_t* d_text, const int64_t* d_re
 /* ---- A11-A13: hash-cache dedup, HMAC-SHA256, pseudonym write-back (S8c O4) */
 /* An open-addressing table with room for max_unique distinct entity strings (slots =
  * next power of two >= 2*max_unique) plus an arena of key_arena_bytes for their bytes and
- * 32 bytes of digest each.  No eviction (reading S18).  Synchronises. */
+ * 32 bytes of digest each.  Nothing is evicted implicitly (reading S18); anon_cache_evict shrinks it on request.  Synchronises. */
 int  anon_cache_create(anon_ctx* ctx, uint64_t max_unique, uint64_t key_arena_bytes, anon_cache** out);
 void anon_cache_destroy(anon_cache* c);
 /* Forgets every entry, the counters and the key binding (table memset on the context stream;

@@ -100,6 +100,12 @@ def main():
         n2 = float((lens[:B].astype(np.float64) ** 2).sum())
         res[name] = {"tokens": T, "sequences": B, "ms": ms, "tflops": 4.0 * n2 * H / ms / 1e9,
                      "exp_per_s": n2 * (H // 64) / ms * 1e3, "algorithmic_gbs": T * H * 2 * 4 / ms / 1e6}
+        # NEXT-3: the same inputs through the banded kernel (window 128): a query sees at most 129 keys
+        ms = timeit(lambda: P.anon_attention_local(ctx, qkv, d_cu, cu, H, H // 64, 1, 128, out))
+        ln = lens[:B].astype(np.float64)
+        vis = float(sum(np.minimum(np.arange(n) + 64, n - 1).sum() - np.maximum(np.arange(n) - 64, 0).sum() + n for n in lens[:B]))
+        res[name + "_window128"] = {"tokens": T, "sequences": B, "ms": ms, "visible_pairs": vis, "tflops": 4.0 * vis * H / ms / 1e9,
+                                    "exp_per_s": vis * (H // 64) / ms * 1e3, "algorithmic_gbs": T * H * 2 * 4 / ms / 1e6}
         del qkv, out
 
     # HMAC-SHA256 with dedup disabled: integer-ALU bound (K10)

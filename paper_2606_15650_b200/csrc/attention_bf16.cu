@@ -289,6 +289,14 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                         for (int j = 16; j < 32; j++) pk[j] = 0u;
                         break;
                     }
+                    if (BAND) {                                          // a half-chunk none of this warp's 32 rows can see
+                        const int wq = (w.q_valid >> 8) + (int)quarter * 32 - c * kKC;    // column of the warp's first row
+                        if (32 * hh + 31 < wq - kBand || 32 * hh > wq + 31 + kBand) {
+#pragma unroll
+                            for (int j = 16 * hh; j < 16 * hh + 16; j++) pk[j] = 0u;
+                            continue;
+                        }
+                    }
 #pragma unroll
                     for (int j = 16 * hh; j < 16 * hh + 16; j++) {
                         float t0, t1;

@@ -409,7 +409,13 @@ extern "C" int anon_regex_load(anon_ctx* ctx, const void* h_blob, size_t blob_by
     cudaError_t e = cudaMemcpyAsync(rx->d_tab, dev_tab.data(), padded, cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(regex_candidates_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_need);
+    {   // the device's maximum, not this automaton's need: handles with different table sizes share the kernel
+        cudaFuncAttributes fa;
+        e = cudaFuncGetAttributes(&fa, regex_candidates_kernel);
+        const long long max_dyn = (long long)ctx->smem_optin - (long long)fa.sharedSizeBytes;
+        if (e == cudaSuccess && (long long)smem_need > max_dyn) { cudaFree(rx->d_tab); delete rx; return ANON_ERR_UNSUPPORTED; }
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(regex_candidates_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_dyn);
+    }
     if (e == cudaSuccess)
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&rx->ctas_per_sm, regex_candidates_kernel, kThreads, smem_need);
     if (e != cudaSuccess) { cudaFree(rx->d_tab); delete rx; return cuda_fail(ctx, e, "anon_regex_load"); }

@@ -221,3 +221,24 @@ def test_pipeline_with_regex_matches_oracle_composition():
                                key, 10, names, span_capacity=T, out_capacity=T * 32)
     assert np.array_equal(res["spans"], np.asarray(ner, np.int32).reshape(-1, 4))
     R.close(); cache.close(); W.close(); ctx.close()
+
+
+def test_two_automata_of_different_size_side_by_side():
+    """A small automaton loaded after a large one must not shrink what the large one may launch with (both share one kernel)."""
+    from oracle import regex_layer as rx
+    from paper_2606_15650_b200 import regex_dfa
+    torch, P = _env()
+    d, rec, _pool = _records(30, 71)
+    text, off = rec["text"], rec["rec_off"]
+    one = [("CVE_ID", rx.PATTERNS[3][1])]
+    ctx = P.Context(0, workspace_bytes=64 << 20)
+    big = P.Regex(ctx, _blob())
+    small = P.Regex(ctx, regex_dfa.compile_patterns([(3, one[0][1])], rx.MAX_MATCH))
+    for R, pats in ((big, rx.PATTERNS), (small, one), (big, rx.PATTERNS)):
+        want = rx.scan_records(text, off, pats)
+        if pats is one:
+            want = [(r, a, b, 3) for r, a, b, _k in want]            # the automaton reports the type id given at compile time
+        rc, n, got = _scan_gpu(torch, P, ctx, R, text, off, len(want) + 4)
+        assert rc == 0 and n == len(want) and n > 5
+        assert np.array_equal(got, np.asarray(want, np.int32).reshape(-1, 4))
+    small.close(); big.close(); ctx.close()

@@ -101,3 +101,56 @@ def test_minimisation_merges_equivalent_states():
     c1, a1, t1 = regex_dfa.compile_tables([r"(?:a|b)c"])
     c2, a2, t2 = regex_dfa.compile_tables([r"[ab]c"])
     assert t1.shape[0] == 4 and np.array_equal(a1, a2) and np.array_equal(t1[:, c1[list(b"abc ")]], t2[:, c2[list(b"abc ")]])
+
+
+def _random_pattern(rng, depth=0):
+    """A random pattern of the restricted grammar.  Unbounded repeats are put on single atoms only: the ORACLE is a
+    backtracking `re.fullmatch` per (start, end) pair, and nested or ambiguous stars make it exponential -- the compiler has no
+    such problem, but the test has to finish."""
+    atoms = ["a", "b", "c", "0", "1", r"\.", "-", "[ab]", "[0-9]", "[^a ]", r"\d", "[a-c0]", "."]
+    r = rng.random()
+    if depth >= 3 or r < 0.35:
+        node = atoms[int(rng.integers(0, len(atoms)))]
+        q = rng.random()
+        if q < 0.15:
+            node += "+"
+        elif q < 0.25:
+            node += "*"
+        elif q < 0.32:
+            node += "{2,}"
+        return node
+    if r < 0.6:
+        node = "".join(_random_pattern(rng, depth + 1) for _ in range(int(rng.integers(2, 4))))
+    elif r < 0.85:
+        node = "(?:" + "|".join(_random_pattern(rng, depth + 1) for _ in range(int(rng.integers(2, 4)))) + ")"
+    else:
+        node = "(?:" + _random_pattern(rng, depth + 1) + ")"
+    q = rng.random()
+    if q < 0.15:
+        node = "(?:" + node + ")?"
+    elif q < 0.3:
+        lo = int(rng.integers(0, 3))
+        node = "(?:" + node + "){%d,%d}" % (lo, lo + int(rng.integers(0, 2)))
+    return node
+
+
+def test_random_patterns_against_oracle():
+    """Fuzz: random pattern sets from the restricted grammar, random bodies; the table walk must equal the oracle's
+    brute-force `re.fullmatch` scan (rule D18) for every set the compiler accepts."""
+    import re
+    rng = np.random.default_rng(2026)
+    alphabet = np.frombuffer(b"abc01.- x", np.uint8)
+    done = 0
+    for trial in range(400):
+        pats = [_random_pattern(rng) for _ in range(int(rng.integers(1, 4)))]
+        if any(re.fullmatch(p, "") for p in pats):
+            with pytest.raises(ValueError):
+                regex_dfa.compile_patterns(list(enumerate(pats)), 24)
+            continue
+        t = parse_blob(regex_dfa.compile_patterns(list(enumerate(pats)), 24))
+        named = [("P%d" % k, p) for k, p in enumerate(pats)]
+        for _ in range(6):
+            body = bytes(rng.choice(alphabet, 60).astype(np.uint8))
+            assert walk(t, body) == rx.scan_record(body, named, 24), (pats, body)
+        done += 1
+    assert done > 150

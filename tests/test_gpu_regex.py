@@ -242,3 +242,33 @@ def test_two_automata_of_different_size_side_by_side():
         assert rc == 0 and n == len(want) and n > 5
         assert np.array_equal(got, np.asarray(want, np.int32).reshape(-1, 4))
     small.close(); big.close(); ctx.close()
+
+
+def test_random_pattern_sets_match_oracle():
+    """Fuzz on the device: 40 random pattern sets of the restricted grammar (different automaton sizes, class counts, type
+    maps and max_match), random text over a small alphabet cut into ragged records; spans bit-exact against the oracle."""
+    import re
+    from oracle import regex_layer as rx
+    from paper_2606_15650_b200 import regex_dfa
+    from test_regex_dfa import _random_pattern
+    torch, P = _env()
+    rng = np.random.default_rng(77)
+    alphabet = np.frombuffer(b"abc01.- x", np.uint8)
+    ctx = P.Context(0, workspace_bytes=64 << 20)
+    done = 0
+    while done < 40:
+        pats = [_random_pattern(rng) for _ in range(int(rng.integers(1, 5)))]
+        if any(re.fullmatch(p, "") for p in pats):
+            continue
+        mm = int(rng.integers(3, 40))
+        types = [int(rng.integers(0, 9)) for _ in pats]
+        R = P.Regex(ctx, regex_dfa.compile_patterns(list(zip(types, pats)), mm))
+        text = alphabet[rng.integers(0, alphabet.size, 9000)].copy()
+        cuts = np.unique(np.concatenate([[0, text.size], rng.integers(0, text.size, 25)]))
+        want = [(r, a, b, types[k]) for r, a, b, k in rx.scan_records(text, cuts, [("P", p) for p in pats], mm)]
+        rc, n, got = _scan_gpu(torch, P, ctx, R, text, cuts, len(want) + 2)
+        assert rc == 0 and n == len(want), (pats, mm)
+        assert np.array_equal(got, np.asarray(want, np.int32).reshape(-1, 4)), (pats, mm)
+        R.close()
+        done += 1
+    ctx.close()

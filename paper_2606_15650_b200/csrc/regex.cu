@@ -7,8 +7,9 @@
 //   R1  regex_candidates_kernel   every byte position in parallel: the longest match that starts there (0 = none).  Tables
 //                                 and a text tile (+ max_match look-ahead) live in shared memory; most positions die on
 //                                 their first transition.  Writes one u16 per byte: len | pattern << 8.
-//   R2  regex_select_kernel       one warp per record walks the candidates left to right, 128 positions per step: the
-//                                 first candidate at or after the cursor is selected (bit 15), the cursor jumps to its end.
+//   R2  regex_select_kernel       one warp per record walks the candidates left to right, 128 positions per step, from
+//                                 2048-position chunks staged in shared memory: the first candidate at or after the cursor
+//                                 is selected (bit 15), the cursor jumps to its end.
 //   R3  scan of the per-record counts, then regex_write_kernel compacts the selected candidates into the span list in
 //       stream order (ballot + popc ranks inside a warp).
 // Merge (D19): per NER span one binary search in the regex list (sorted, non-overlapping) decides keep / drop; a scan of
@@ -203,41 +204,53 @@ __global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
     }
 }
 
-// 4 candidates per lane, 128 positions per warp step; positions outside [s, re) read as "no candidate"
-__device__ __forceinline__ void load_cands(const uint16_t* __restrict__ cand, long long idx, long long s, long long re, uint32_t c[4]) {
-    uint2 v = make_uint2(0, 0);
-    if (idx < re) v = *reinterpret_cast<const uint2*>(cand + idx);     // cand is padded by 4 entries past nbytes
-    c[0] = v.x & 0xffffu; c[1] = v.x >> 16; c[2] = v.y & 0xffffu; c[3] = v.y >> 16;
-#pragma unroll
-    for (int j = 0; j < 4; j++)
-        if (idx + j < s || idx + j >= re) c[j] = 0;
-}
+// One warp per record.  The record's candidate words are staged through shared memory in chunks of kSelChunk positions
+// (coalesced 16-byte loads), so that the walk itself -- find the first candidate at or after the cursor, select it, jump to
+// its end -- runs at shared-memory latency: a 64 KB record costs 32 global round trips instead of one per selected span.
+constexpr int kSelWarps = 4;
+constexpr int kSelChunk = 2048;
 
-__global__ void __launch_bounds__(kThreads) regex_select_kernel(uint16_t* __restrict__ cand, const long long* __restrict__ rec_off, int R,
-                                                                int* __restrict__ rec_count)
+__global__ void __launch_bounds__(kSelWarps * 32) regex_select_kernel(uint16_t* __restrict__ cand, const long long* __restrict__ rec_off, int R,
+                                                                      int* __restrict__ rec_count)
 {
-    const int r = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    __shared__ __align__(16) uint16_t s_c[kSelWarps][kSelChunk];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int r = blockIdx.x * kSelWarps + warp;
     if (r >= R) return;
     long long s = rec_off[r];
     const long long re = rec_off[r + 1];
+    uint16_t* sc = s_c[warp];
     int count = 0;
     while (s < re) {
-        const long long wb = s & ~3LL, idx = wb + lane * 4;
-        uint32_t c[4];
-        load_cands(cand, idx, s, re, c);
-        int first = -1;
+        const long long cbase = s & ~7LL;                                       // 16-byte aligned entry
+        long long nent = ((re - cbase) + 7) & ~7LL;                            // cand is padded: whole 16-byte words may be read
+        if (nent > kSelChunk) nent = kSelChunk;
+        for (int i = lane; i * 8 < nent; i += 32)
+            reinterpret_cast<uint4*>(sc)[i] = reinterpret_cast<const uint4*>(cand + cbase)[i];
+        __syncwarp();
+        const long long cend = cbase + nent < re ? cbase + nent : re;          // positions of this chunk that belong to the record
+        while (s < cend) {
+            const long long wb = s & ~3LL, idx = wb + lane * 4;
+            uint32_t c[4] = {0u, 0u, 0u, 0u};
+            if (idx < cend) {
+                const uint2 v = *reinterpret_cast<const uint2*>(sc + (idx - cbase));
+                c[0] = v.x & 0xffffu; c[1] = v.x >> 16; c[2] = v.y & 0xffffu; c[3] = v.y >> 16;
+            }
+            int first = -1;
 #pragma unroll
-        for (int j = 3; j >= 0; j--)
-            if (c[j] & 0xffu) first = j;
-        const uint32_t any = __ballot_sync(0xffffffffu, first >= 0);
-        if (!any) { s = wb + 128; continue; }
-        const int f = __ffs(any) - 1;
-        const int fj = __shfl_sync(0xffffffffu, first, f);
-        const uint32_t cv = __shfl_sync(0xffffffffu, first >= 0 ? c[first] : 0u, f);
-        const long long pos = wb + f * 4 + fj;
-        if (lane == f) cand[pos] = (uint16_t)(cv | 0x8000u);
-        count++;
-        s = pos + (cv & 0xffu);
+            for (int j = 3; j >= 0; j--)
+                if ((c[j] & 0xffu) && idx + j >= s && idx + j < cend) first = j;
+            const uint32_t any = __ballot_sync(0xffffffffu, first >= 0);
+            if (!any) { s = wb + 128 < cend ? wb + 128 : cend; continue; }
+            const int f = __ffs(any) - 1;
+            const int fj = __shfl_sync(0xffffffffu, first, f);
+            const uint32_t cv = __shfl_sync(0xffffffffu, first >= 0 ? c[first] : 0u, f);
+            const long long pos = wb + f * 4 + fj;
+            if (lane == f) cand[pos] = (uint16_t)(cv | 0x8000u);
+            count++;
+            s = pos + (cv & 0xffu);
+        }
+        __syncwarp();                                                          // the chunk is consumed: it may be overwritten
     }
     if (lane == 0) rec_count[r] = count;
 }
@@ -259,31 +272,42 @@ __global__ void __launch_bounds__(kThreads) regex_write_kernel(const uint16_t* _
     if (r >= R) return;
     const long long rs = rec_off[r], re = rec_off[r + 1];
     long long o = rec_base[r];
-    for (long long wb = rs & ~3LL; wb < re; wb += 128) {
-        const long long idx = wb + lane * 4;
-        uint32_t c[4];
-        load_cands(cand, idx, rs, re, c);
-        int n = 0;
+    for (long long wb0 = rs & ~3LL; wb0 < re; wb0 += 512) {                     // four independent window loads in flight
+        uint2 v[4];
 #pragma unroll
-        for (int j = 0; j < 4; j++) n += (c[j] >> 15) & 1;
-        int incl = n;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += t;
+        for (int u = 0; u < 4; u++) {
+            const long long idx = wb0 + u * 128 + lane * 4;
+            v[u] = idx < re ? *reinterpret_cast<const uint2*>(cand + idx) : make_uint2(0u, 0u);
         }
-        long long k = o + incl - n;
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
-            if (c[j] & 0x8000u) {
-                if (k < cap) {
-                    const int cs = (int)(idx + j - rs);
-                    spans[k] = anon_span{r, cs, cs + (int)(c[j] & 0xffu), (int)type_of[(c[j] >> 8) & 0x7fu]};
-                }
-                k++;
+        for (int u = 0; u < 4; u++) {
+            const long long idx = wb0 + u * 128 + lane * 4;
+            uint32_t c[4] = {v[u].x & 0xffffu, v[u].x >> 16, v[u].y & 0xffffu, v[u].y >> 16};
+#pragma unroll
+            for (int j = 0; j < 4; j++)
+                if (idx + j < rs || idx + j >= re) c[j] = 0;
+            int n = 0;
+#pragma unroll
+            for (int j = 0; j < 4; j++) n += (c[j] >> 15) & 1;
+            int incl = n;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
             }
+            long long k = o + incl - n;
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                if (c[j] & 0x8000u) {
+                    if (k < cap) {
+                        const int cs = (int)(idx + j - rs);
+                        spans[k] = anon_span{r, cs, cs + (int)(c[j] & 0xffu), (int)type_of[(c[j] >> 8) & 0x7fu]};
+                    }
+                    k++;
+                }
+            }
+            o += __shfl_sync(0xffffffffu, incl, 31);
         }
-        o += __shfl_sync(0xffffffffu, incl, 31);
     }
 }
 
@@ -454,7 +478,7 @@ int regex_scan_impl(anon_ctx* ctx, WsCursor& ws, const anon_regex* rx, const uin
     regex_candidates_kernel<<<grid, kThreads, rx->smem_bytes, st>>>(rx->d_tab, rx->tab_bytes, rx->n_classes, rx->max_match, d_text, nbytes,
                                                                     (const long long*)d_rec_off, R, tile_rec, n_tiles, cand);
     const unsigned rblocks = (unsigned)((R + kThreads / 32 - 1) / (kThreads / 32));
-    regex_select_kernel<<<rblocks, kThreads, 0, st>>>(cand, (const long long*)d_rec_off, R, rec_count);
+    regex_select_kernel<<<(unsigned)((R + kSelWarps - 1) / kSelWarps), kSelWarps * 32, 0, st>>>(cand, (const long long*)d_rec_off, R, rec_count);
     CountIn cin{rec_count};
     scan::reduce_and_scan<long long, scan::SumI64>(cin, R, nullptr, agg, st);
     scan::apply<long long, scan::SumI64>(cin, BaseOut{rec_base}, R, nullptr, agg, st);

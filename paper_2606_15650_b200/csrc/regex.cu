@@ -56,19 +56,23 @@ __global__ void __launch_bounds__(kThreads) regex_tile_records_kernel(const long
     tile_rec[t] = record_of(rec_off, 0, R - 1, p);
 }
 
+__device__ __forceinline__ uint32_t lds_u8(uint32_t addr) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr)); return v; }
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr)); return v; }
+
 // One DFA walk from a start position: the longest accepting prefix that ends on a word boundary, as len | pattern << 8.
 // `left` = bytes to the end of the record (capped), `lim` = steps allowed in this call.  Returns true if the automaton is
-// still alive after `lim` steps (the caller may walk on with a larger `lim`).
-__device__ __forceinline__ bool dfa_walk(const uint8_t* __restrict__ b, int left, int lim, const uint8_t* __restrict__ cw,
-                                         const uint32_t* __restrict__ tr, int n_classes, uint32_t& out)
+// still alive after `lim` steps (the caller may walk on with a larger `lim`).  All operands are 32-bit shared-memory
+// addresses (text byte, cw table, transition table): ~14 instructions and one dependent load per step.
+__device__ __forceinline__ bool dfa_walk(uint32_t b, int left, int lim, uint32_t cw, uint32_t tr, int n_classes, uint32_t& out)
 {
-    uint32_t st = 1, cwn = cw[b[0]];
+    uint32_t st = 1, cwn = lds_u8(cw + lds_u8(b));
     out = 0;
     int i = 0;
     while (i < lim) {
         const uint32_t cwi = cwn;
-        cwn = (i + 1 < left) ? cw[b[i + 1]] : 0u;                               // the record's edge counts as a non-word byte
-        const uint32_t t = tr[st * n_classes + (cwi & 0x7f)];
+        cwn = lds_u8(cw + lds_u8(b + i + 1));                                   // inside the staged look-ahead for every i < lim
+        if (i + 1 >= left) cwn = 0u;                                            // the record's edge counts as a non-word byte
+        const uint32_t t = lds_u32(tr + ((st * n_classes + (cwi & 0x7f)) << 2));
         st = t & 0xffffu;
         if (st == 0) return false;
         ++i;
@@ -125,6 +129,8 @@ __global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
         __syncthreads();
         const uint8_t* tbase = s_text + ((long long)(reinterpret_cast<uintptr_t>(text) - g0) + tile0);   // tile position 0
         const int n_here = (int)(nbytes - tile0 < kTile ? nbytes - tile0 : kTile);
+        const uint32_t tbase_s = (uint32_t)__cvta_generic_to_shared(tbase);
+        const uint32_t cw_s = (uint32_t)__cvta_generic_to_shared(cw), tr_s = (uint32_t)__cvta_generic_to_shared(tr);
         // A: which positions can start a match (first transition alive, word boundary on the left)?  Four per thread.
 #pragma unroll
         for (int k = 0; k < kTile / 4 / kThreads; k++) {
@@ -180,7 +186,7 @@ __global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
             const int left = bits ? (w << 5) + __ffs(bits) - 1 - o : max_match + 1;
             const int limit = left < max_match ? left : max_match;
             uint32_t out;
-            const bool alive = dfa_walk(tbase + o, left, limit < kShortWalk ? limit : kShortWalk, cw, tr, n_classes, out);
+            const bool alive = dfa_walk(tbase_s + o, left, limit < kShortWalk ? limit : kShortWalk, cw_s, tr_s, n_classes, out);
             if (alive && limit > kShortWalk) s_surv[atomicAdd(&s_nsurv, 1)] = (uint16_t)o;
             else s_cand[o] = (uint16_t)out;
         }
@@ -194,7 +200,7 @@ __global__ void __launch_bounds__(kThreads) regex_candidates_kernel(
             while (!bits && w < w_last) bits = s_recbits[++w];
             const int left = bits ? (w << 5) + __ffs(bits) - 1 - o : max_match + 1;
             uint32_t out;
-            dfa_walk(tbase + o, left, left < max_match ? left : max_match, cw, tr, n_classes, out);
+            dfa_walk(tbase_s + o, left, left < max_match ? left : max_match, cw_s, tr_s, n_classes, out);
             s_cand[o] = (uint16_t)out;
         }
         __syncthreads();

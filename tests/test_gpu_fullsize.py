@@ -136,6 +136,54 @@ def test_configs4_full_size_50m_spans():
     cache.close(); ctx.close()
 
 
+def test_configs3_full_size_in_bench_configuration():
+    """BASELINE.json configs[3] at the size `bench.py --workload large` times: 16,384 packed sequences U[32, 512]
+    (~4.45 M tokens) through the 24 x 1024 encoder with the 250,002-row embedding table, in one `anon_ner_forward`
+    call.  Oracle logits / labels on sampled sequences (shortest, longest, last, one seeded pick); labels == argmax of
+    the GPU's own logits on every token; decode bit-exact against the oracle fed with the GPU's labels."""
+    import torch
+    import paper_2606_15650_b200 as P
+    from oracle import decode, encoder
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device")
+    dev = "cuda:0"
+    d = gen.DESCS["large"]
+    rec, win = gen.workload_large(n_seqs=16384, seed=gen.SEED_BASE + 4)             # exactly bench.py's "large" workload
+    w = gen.make_weights(d, gen.SEED_BASE + 4, planted=(2.0, 0.5, 4.0))
+    ids, cu, meta = win["token_ids"], win["cu_seqlens"], np.ascontiguousarray(win["meta"])
+    T, B = ids.size, cu.size - 1
+    assert B == 16384 and T > 4_000_000
+    ctx = P.Context(0, workspace_bytes=P.anon_workspace_bytes(d, T, B) + (256 << 20))
+    W = P.Weights(ctx, d, gen.pack_blob(w))
+    logits = torch.zeros((T, d["num_labels"]), dtype=torch.float32, device=dev)
+    labels = torch.zeros(T, dtype=torch.int32, device=dev)
+    P.anon_ner_forward(ctx, W, torch.from_numpy(ids).to(dev), torch.from_numpy(cu).to(dev), logits, labels)
+    assert ctx.sync() == 0
+    got_logits, got_labels = logits.cpu().numpy(), labels.cpu().numpy()
+    assert np.array_equal(got_labels, encoder.argmax_labels(got_logits))
+    cap = T // 2
+    spans = torch.zeros((cap, 4), dtype=torch.int32, device=dev)
+    nsp = torch.zeros(1, dtype=torch.int32, device=dev)
+    P.anon_decode_spans(ctx, labels, torch.from_numpy(meta).to(dev), d["num_labels"], spans, nsp)
+    assert ctx.sync() == 0
+    S = int(nsp.item())
+    got_spans = spans.cpu().numpy()[:S]
+    W.close(); ctx.close()
+    want_spans = decode.decode_spans(got_labels, meta)
+    assert S == len(want_spans)                 # the planted detector fades over 24 layers: few or no spans here
+    assert np.array_equal(got_spans, np.asarray(want_spans, np.int32).reshape(-1, 4))
+    lens = np.diff(cu)
+    picks = {int(np.argmin(lens)), int(np.argmax(lens)), B - 1} | set(np.random.default_rng(7).integers(0, B, 1).tolist())
+    want = encoder.forward_packed(w, d, ids, cu, seq_subset=sorted(picks))
+    rows = ~np.isnan(want[:, 0])
+    assert rows.sum() >= 512
+    err = np.abs(got_logits[rows] - want[rows])
+    assert err.max() <= 3e-2, err.max()
+    mism = got_labels[rows] != encoder.argmax_labels(want[rows])
+    assert (encoder.top2_margin(want[rows])[mism] < 3e-2).all()
+    assert 1.0 - mism.mean() >= 0.999
+
+
 def test_modern_shape_full_size_in_bench_configuration():
     """NEXT-3 at the size `bench.py --workload modern` times: 4096 records, ~1 M tokens in one chunk through the 22-layer
     ModernBERT-base-shaped encoder; oracle logits / labels on sampled sequences (shortest, longest, first, last, seeded picks)."""

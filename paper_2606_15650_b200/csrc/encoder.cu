@@ -340,9 +340,8 @@ static int modern_chunk(anon_ctx* ctx, WsCursor c, const anon_weights* w, const 
     norm(x, w->g_f, y);                                                  // final norm: FP32 rows for the head
     CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
     { ProfScope ps(ctx, PROF_ROW, (double)nt * (H * 4 + (d_logits ? NL * 4 : 0) + (d_labels ? 4 : 0)));
-    enc::head_argmax_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(y, nt, H, w->W_c, w->b_c, NL,
-                                                                        d_logits ? d_logits + (size_t)tok0 * NL : nullptr,
-                                                                        d_labels ? d_labels + tok0 : nullptr); }
+    enc::launch_head_argmax(st, y, nt, H, w->W_c, w->b_c, NL, d_logits ? d_logits + (size_t)tok0 * NL : nullptr,
+                            d_labels ? d_labels + tok0 : nullptr); }
     CU_LAUNCH_CHECK(ctx, "head_argmax_kernel");
     return ANON_OK;
 }
@@ -497,9 +496,8 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                 }
             }
             { ProfScope ps(ctx, PROF_ROW, (double)nt * (H * 4 + (d_logits ? NL * 4 : 0) + (d_labels ? 4 : 0)));
-            enc::head_argmax_kernel<<<row_grid, enc::kRowWarps * 32, 0, st>>>(
-                head_in, nt, H, w->W_c, w->b_c, NL, d_logits ? d_logits + (size_t)tok0 * NL : nullptr,
-                d_labels ? d_labels + tok0 : nullptr); }
+            enc::launch_head_argmax(st, head_in, nt, H, w->W_c, w->b_c, NL, d_logits ? d_logits + (size_t)tok0 * NL : nullptr,
+                                    d_labels ? d_labels + tok0 : nullptr); }
             CU_LAUNCH_CHECK(ctx, "head_argmax_kernel");
         }
         s0 = s1;

@@ -180,6 +180,83 @@ static __global__ void __launch_bounds__(kRowWarps * 32) head_argmax_kernel(
     if (labels && lane == 0) labels[r] = best_c;
 }
 
+// K6 for NL <= 16 (the paper's 9 / 13 BIO labels): two token rows per warp, all class sums kept per lane as FMA chains (hidden
+// loop outside, class loop inside, so a W_c vector serves both rows), then ONE transposed butterfly per row -- at every step a
+// lane keeps half of its class sums and trades the other half -- 16 shuffles instead of 5 per class.  Lanes 2c and 2c + 1 end up
+// with the logit of class c; the argmax (ties -> lowest index) runs across lanes on those same values.  ncu on the kernel
+// above: L1 data pipe 95 % and issue slots 75 % busy at 1,450 instructions per token; this one issues about a third of that.
+constexpr int kHeadRows = 2;
+static __global__ void __launch_bounds__(kRowWarps * 32, 2) head_argmax16_kernel(
+    const float* __restrict__ x, int ntok, int H, const float* __restrict__ W_c, const float* __restrict__ b_c, int NL,
+    float* __restrict__ logits, int* __restrict__ labels)
+{
+    const int lane = threadIdx.x & 31;
+    const int r0 = (blockIdx.x * kRowWarps + (threadIdx.x >> 5)) * kHeadRows;
+    if (r0 >= ntok) return;
+    const int n4 = H >> 7;
+    float4 v[kHeadRows][kMaxVec];
+#pragma unroll
+    for (int i = 0; i < kHeadRows; i++) {
+        const int r = min(r0 + i, ntok - 1);          // a row past the end repeats the last one; nothing is stored for it
+#pragma unroll
+        for (int k = 0; k < kMaxVec; k++) if (k < n4) v[i][k] = load4(x + (size_t)r * H + 4 * (lane + 32 * k));
+    }
+    float s[kHeadRows][16];
+#pragma unroll
+    for (int i = 0; i < kHeadRows; i++)
+#pragma unroll
+        for (int c = 0; c < 16; c++) s[i][c] = 0.f;
+#pragma unroll
+    for (int k = 0; k < kMaxVec; k++) if (k < n4) {
+#pragma unroll
+        for (int c = 0; c < 16; c++) if (c < NL) {
+            const float4 w = load4(W_c + (size_t)c * H + 4 * (lane + 32 * k));
+#pragma unroll
+            for (int i = 0; i < kHeadRows; i++)
+                s[i][c] = fmaf(v[i][k].w, w.w, fmaf(v[i][k].z, w.z, fmaf(v[i][k].y, w.y, fmaf(v[i][k].x, w.x, s[i][c]))));
+        }
+    }
+    const int cls = lane >> 1;
+    const float bias = cls < NL ? __ldg(b_c + cls) : 0.f;
+#pragma unroll
+    for (int i = 0; i < kHeadRows; i++) {
+        float* a = s[i];
+#pragma unroll
+        for (int half = 8; half >= 1; half >>= 1) {     // lane bit (2 * half) set: keep the upper half of the class sums
+            const bool up = (lane & (2 * half)) != 0;
+#pragma unroll
+            for (int j = 0; j < half; j++) {
+                const float keep = up ? a[j + half] : a[j], send = up ? a[j] : a[j + half];
+                a[j] = keep + __shfl_xor_sync(0xffffffffu, send, 2 * half);
+            }
+        }
+        float t = a[0] + __shfl_xor_sync(0xffffffffu, a[0], 1) + bias;      // class lane >> 1, summed over all 32 lanes
+        const int r = r0 + i;
+        if (logits && r < ntok && cls < NL && !(lane & 1)) logits[(size_t)r * NL + cls] = t;
+        if (cls >= NL) t = -INFINITY;
+        int best_c = cls;
+#pragma unroll
+        for (int off = 2; off < 32; off <<= 1) {
+            const float ot = __shfl_xor_sync(0xffffffffu, t, off);
+            const int oc = __shfl_xor_sync(0xffffffffu, best_c, off);
+            if (ot > t || (ot == t && oc < best_c)) { t = ot; best_c = oc; }
+        }
+        if (labels && lane == 0 && r < ntok) labels[r] = best_c;
+    }
+}
+
+static inline void launch_head_argmax(cudaStream_t st, const float* x, int ntok, int H, const float* W_c, const float* b_c,
+                                      int NL, float* logits, int* labels)
+{
+    if (NL <= 16) {
+        const unsigned grid = (unsigned)((ntok + kRowWarps * kHeadRows - 1) / (kRowWarps * kHeadRows));
+        head_argmax16_kernel<<<grid, kRowWarps * 32, 0, st>>>(x, ntok, H, W_c, b_c, NL, logits, labels);
+    } else {
+        const unsigned grid = (unsigned)((ntok + kRowWarps - 1) / kRowWarps);
+        head_argmax_kernel<<<grid, kRowWarps * 32, 0, st>>>(x, ntok, H, W_c, b_c, NL, logits, labels);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // FP32 SIMT path (BJ configs[0]; TF32 would miss the 1e-4 bound, S7 H5): 64x64x16 tiles, 4x4 per thread
 // ---------------------------------------------------------------------------------------------------------

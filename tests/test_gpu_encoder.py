@@ -88,6 +88,31 @@ def test_fp32_path_edge_cases(env):
     W.close()
 
 
+@pytest.mark.parametrize("num_labels", [3, 15, 17, 33])
+def test_head_label_counts_and_ties(env, num_labels):
+    """K6 on both sides of its 16-label dispatch (transposed-butterfly kernel up to 16 labels, warp-per-token kernel above),
+    odd token counts (the two-rows-per-warp tail) included: FP32 logits within 1e-4 of the oracle, the label is the argmax of
+    the GPU's own logits with ties going to the lowest index (two identical classifier rows force ties on every token)."""
+    P, torch, ctx = env
+    from oracle import encoder
+    d = dict(gen.DESCS["tiny"]); d["num_labels"] = num_labels
+    w = gen.make_weights(d, 11)
+    w["W_c"][num_labels - 1] = w["W_c"][1]; w["b_c"][num_labels - 1] = w["b_c"][1]       # classes 1 and NL-1 always tie
+    W = P.Weights(ctx, d, gen.pack_blob(w))
+    rng = np.random.default_rng(num_labels)
+    lens = [1, 2, 37, 128, 3]                        # 171 tokens: odd
+    cu = np.zeros(len(lens) + 1, np.int32); cu[1:] = np.cumsum(lens)
+    ids = rng.integers(5, d["vocab"], int(cu[-1])).astype(np.int32)
+    want = encoder.forward_packed(w, d, ids, cu)
+    got, labels = _forward(P, torch, ctx, W, ids, cu)
+    rms = np.sqrt((want ** 2).mean())
+    assert (np.abs(got - want) <= 1e-4 * np.maximum(np.abs(want), rms)).all()
+    assert np.array_equal(got[:, 1], got[:, num_labels - 1])
+    assert np.array_equal(labels, encoder.argmax_labels(got))
+    assert not (labels == num_labels - 1).any()
+    W.close()
+
+
 @pytest.mark.parametrize("M,N,K,epi", [(300, 768, 768, 0), (128, 2304, 768, 0), (1000, 3072, 768, 1), (257, 768, 3072, 2),
                                        (4096 + 77, 1024, 1024, 2), (64, 128, 128, 0), (200, 136, 64, 1)])
 def test_tcgen05_gemm_against_fp64(env, M, N, K, epi):

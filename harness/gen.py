@@ -33,6 +33,11 @@ DESCS["base_modern"] = dict(layers=22, hidden=768, heads=12, ffn=1152, vocab=503
 TYPE_NAMES_6 = ["IP_ADDRESS", "IPV6_ADDRESS", "HOSTNAME", "CVE_ID", "MAC_ADDRESS", "SERIAL_NUMBER"]
 TYPE_NAMES_4 = ["TYPE0", "TYPE1", "TYPE2", "TYPE3"]
 PAD, CLS, SEP, UNK, MASK = 0, 1, 2, 3, 4
+# W2 planted-detector strengths: (alpha, beta, gamma) plants the embedding bands and the
+# head only; the 6-tuple adds (kappa, theta, lam), one re-amplifying FFN unit per class in every layer (make_weights), which a
+# 24-layer stack needs -- with the 3-tuple the oracle itself labels no entity token at L = 24 and only 79 % of them at L = 12.
+PLANTED = (2.0, 0.5, 4.0)
+PLANTED_DEEP = (2.0, 0.5, 4.0, 1.0, 8.0, 1.0)
 FIRST_ID = 5
 BAND = 256
 
@@ -70,7 +75,7 @@ def make_weights(desc, seed, planted=None):
     w["W_c"] = n(NL, H)
     w["b_c"] = n(NL)
     if planted is not None:
-        alpha, beta, gamma = planted
+        alpha, beta, gamma = planted[:3]
         q, _ = np.linalg.qr(g.standard_normal((H, NL - 1)))
         for c in range(1, NL):
             u = q[:, c - 1].astype(np.float32)
@@ -78,6 +83,17 @@ def make_weights(desc, seed, planted=None):
             w["E_w"][lo:lo + BAND] += alpha * u
             w["W_c"][c] += beta * u
         w["b_c"][0] += gamma
+        if len(planted) == 6:
+            # W2 "deep" variant: every layer also carries one FFN unit per class that re-amplifies the planted direction when
+            # it is clearly present (unit c-1: pre-activation kappa * (x . u_c) - theta, output lam * u_c), so that the detector
+            # survives the LayerNorm rescaling of a deep stack (24 layers fade the embedding-only plant to nothing)
+            kappa, theta, lam = planted[3:]
+            for lw in w["layers"]:
+                for c in range(1, NL):
+                    u = q[:, c - 1].astype(np.float32)
+                    lw["W_1"][c - 1] += kappa * u
+                    lw["b_1f"][c - 1] -= theta
+                    lw["W_2"][:, c - 1] += lam * u
     if desc["dtype"] == 1:
         for k in ("E_w", "E_p", "W_c"):
             w[k] = bf16_round(w[k])

@@ -198,6 +198,9 @@ int  anon_cache_evict(anon_cache* c, uint64_t keep, uint64_t* n_evicted);
  * [0,64].  type_names: HOST array of num_types NUL-terminated ASCII names (<= 32 bytes
  * each, num_types <= 64); a type >= num_types is clamped to num_types-1 and latches
  * ANON_ERR_UNSUPPORTED in the sticky status.  d_hit / d_uid / d_digests may be NULL.
+ * Alignment: d_span_offsets / d_out_offsets / d_uid are int64 arrays (8-byte aligned); d_digests, when given, must be
+ * 16-byte aligned (ANON_ERR_INVALID_ARG otherwise); d_span_bytes, d_out_tokens, d_span_type and d_hit may sit at ANY byte
+ * address (e.g. a sub-buffer of a larger allocation).  S > 0 needs d_span_bytes and d_out_tokens (INVALID_ARG if NULL).
  * Synchronises once (to learn how many entities are new, so that capacity errors are
  * returned, not latched): on ANON_ERR_CAPACITY (max_unique, arena or out_capacity
  * exceeded) the cache is left exactly as before the call.  S must be < 2^31. */
@@ -210,7 +213,8 @@ int  anon_pseudonymize(anon_ctx* ctx, anon_cache* cache,
                        uint8_t* d_hit, int64_t* d_uid, uint8_t* d_digests);
 
 /* A12 alone, dedup disabled: digests[i] = HMAC_SHA256(key, e_i) for every span (used to
- * measure the SHA-256 kernel's integer issue rate, S8d c5).  Asynchronous. */
+ * measure the SHA-256 kernel's integer issue rate, S8d c5).  Asynchronous.  d_digests must be
+ * 16-byte aligned (ANON_ERR_INVALID_ARG otherwise); d_span_bytes may sit at any byte address. */
 int  anon_hmac_spans(anon_ctx* ctx, const uint8_t* d_span_bytes, const int64_t* d_span_offsets, int64_t S,
                      const uint8_t* key, size_t key_len, uint8_t* d_digests /* [S,32] */);
 

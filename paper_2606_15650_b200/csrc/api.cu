@@ -2,6 +2,7 @@
 #include "common.cuh"
 
 #include <new>
+#include <stdlib.h>
 
 extern "C" const char* anon_strerror(int code) {
     switch (code) {
@@ -36,6 +37,7 @@ extern "C" int anon_ctx_create(anon_ctx** out, int device, void* cuda_stream, si
     if (!c) return ANON_ERR_OOM;
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
+    { const char* e = getenv("ANON_CHUNK_TOKENS"); c->chunk_tokens_cap = e ? atoll(e) : 0; }
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
@@ -206,6 +208,16 @@ static int pipeline_host_impl(anon_ctx* ctx, const anon_weights* w, anon_cache* 
         rc = gather_spans_impl(ctx, c, d_text, d_rec_off, d_spans, nullptr, S, d_span_bytes, text_bytes, d_span_off, d_span_type);
         if (rc) return rc;
     }
+    {   // a gather overflow (span bytes past their buffer) must stop the pipeline before the probe reads them
+        CU_TRY(ctx, cudaMemcpyAsync(h_status, ctx->d_status, 4, cudaMemcpyDeviceToHost, st));
+        CU_TRY(ctx, cudaStreamSynchronize(st));
+        if (*h_status != 0) {
+            const int s = *h_status;
+            CU_TRY(ctx, cudaMemsetAsync(ctx->d_status, 0, 4, st));
+            CU_TRY(ctx, cudaStreamSynchronize(st));
+            return s;
+        }
+    }
     int64_t out_bytes = 0;
     {
         WsCursor c = ws;
@@ -214,7 +226,8 @@ static int pipeline_host_impl(anon_ctx* ctx, const anon_weights* w, anon_cache* 
         if (rc) return rc;
     }
     if (h_new_text) {
-        if ((uint64_t)text_bytes + (uint64_t)out_bytes > new_text_capacity) return ANON_ERR_CAPACITY;     // safe upper bound
+        // the splice kernels bound-check every write against the capacity and latch CAPACITY; the exact new size
+        // (text - span bytes + token bytes) comes back with the new record offsets
         WsCursor c = ws;
         rc = splice_records_impl(ctx, c, d_text, text_bytes, d_rec_off, R, d_spans, S, d_out, d_out_off, d_new_text,
                                  new_text_capacity, d_new_rec_off);
@@ -222,6 +235,11 @@ static int pipeline_host_impl(anon_ctx* ctx, const anon_weights* w, anon_cache* 
         CU_TRY(ctx, cudaMemcpyAsync(h_new_rec_off, d_new_rec_off, ((size_t)R + 1) * 8, cudaMemcpyDeviceToHost, st));
         CU_TRY(ctx, cudaStreamSynchronize(st));
         const int64_t new_bytes = h_new_rec_off[R];
+        if (new_bytes < 0 || (uint64_t)new_bytes > new_text_capacity) {
+            CU_TRY(ctx, cudaMemsetAsync(ctx->d_status, 0, 4, st));
+            CU_TRY(ctx, cudaStreamSynchronize(st));
+            return ANON_ERR_CAPACITY;
+        }
         if (new_bytes > 0) CU_TRY(ctx, cudaMemcpyAsync(h_new_text, d_new_text, (size_t)new_bytes, cudaMemcpyDeviceToHost, st));
     }
     if (S > 0) {

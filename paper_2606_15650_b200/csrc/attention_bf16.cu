@@ -392,12 +392,10 @@ int attention_run(anon_ctx* ctx, const AttnPlan& plan, const void* d_qkv, const 
     if (rc) return rc;
     rc = make_tmap_2d(ctx, &tkv, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, d_qkv, (uint64_t)plan.n_rows, (uint64_t)3 * hidden, kD, kKC);
     if (rc) return rc;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CU_TRY(ctx, cudaFuncSetAttribute(attention_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kAttSmem));
-        CU_TRY(ctx, cudaFuncSetAttribute(attention_tcgen05_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kAttSmem));
-        attr_set = true;
-    }
+    rc = ensure_smem_attr(ctx, (const void*)attention_tcgen05_kernel<false>, kAttSmem);
+    if (rc) return rc;
+    rc = ensure_smem_attr(ctx, (const void*)attention_tcgen05_kernel<true>, kAttSmem);
+    if (rc) return rc;
     const long long units = (long long)plan.n_items * heads;
     const int grid = (int)std::min<long long>(units, 2LL * ctx->sm_count);
     if (plan.window)

@@ -24,7 +24,8 @@ struct anon_ctx {
     cudaStream_t stream = nullptr;
     uint8_t* ws = nullptr;          // device scratch
     size_t ws_bytes = 0;
-    int* d_status = nullptr;        // sticky device-side status word (0 = ok, else first ANON_ERR_*)
+    int* d_status = nullptr;        // sticky device-side status word (0 = ok, else first ANON_ERR_*); 256-byte allocation:
+                                    // word 16 = the cache probe's own "table full" flag (zeroed by every anon_pseudonymize)
     uint8_t* h_pinned = nullptr;    // small pinned host buffer for read-backs
     size_t h_pinned_bytes = 0;
     int sm_count = 148;
@@ -32,6 +33,10 @@ struct anon_ctx {
     // cached driver entry point for cuTensorMapEncodeTiled (resolved lazily, see gemm_tcgen05.cu)
     void* encode_tiled = nullptr;
     int smem_optin = 0;
+    // kernels whose MaxDynamicSharedMemorySize opt-in has been set on THIS context's device (the attribute is per device)
+    const void* smem_attr_done[48] = {nullptr};
+    int n_smem_attr_done = 0;
+    long long chunk_tokens_cap = 0;     // ANON_CHUNK_TOKENS read once at context creation (0 = workspace-limited only)
     // L2-resident scratch of the fused residual+LayerNorm GEMM epilogue (allocated on first use, grows only)
     void* ln_scratch = nullptr;
     size_t ln_scratch_bytes = 0;
@@ -89,6 +94,15 @@ static inline int cuda_fail(anon_ctx* c, cudaError_t e, const char* what) {
     do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return cuda_fail((ctx), e__, #expr); } while (0)
 #define CU_LAUNCH_CHECK(ctx, name)                                                   \
     do { cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return cuda_fail((ctx), e__, name); } while (0)
+
+// Opt a kernel in to `bytes` of dynamic shared memory on the context's device, once per (context, kernel).
+static inline int ensure_smem_attr(anon_ctx* c, const void* func, int bytes) {
+    for (int i = 0; i < c->n_smem_attr_done; i++) if (c->smem_attr_done[i] == func) return ANON_OK;
+    cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
+    if (c->n_smem_attr_done < 48) c->smem_attr_done[c->n_smem_attr_done++] = func;
+    return ANON_OK;
+}
 
 __device__ __forceinline__ void latch_status(int* d_status, int code) { atomicCAS(d_status, 0, code); }
 

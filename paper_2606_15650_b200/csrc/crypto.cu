@@ -141,7 +141,7 @@ __device__ __forceinline__ uint32_t slot_index(u64 v) { return (uint32_t)(v & 0x
 __global__ void __launch_bounds__(256) cache_probe_kernel(
     const uint8_t* __restrict__ bytes, const long long* __restrict__ off, long long S,
     u64* table, u64 mask, const uint8_t* __restrict__ arena, const long long* __restrict__ entry_off,
-    int* __restrict__ slot_of, int* d_status)
+    int* __restrict__ slot_of, int* d_full)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= S) return;
@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(256) cache_probe_kernel(
         slot = (slot + 1) & mask;
     }
     slot_of[i] = -1;
-    latch_status(d_status, ANON_ERR_CAPACITY);
+    *d_full = 1;               // the probe's own flag (not the sticky status word: an earlier stage's CAPACITY is not "table full")
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -317,7 +317,11 @@ __global__ void __launch_bounds__(kEmitWarps * 32) emit_tokens_kernel(
     const long long i = i0 + lane;
     const bool live = i < S;
     const long long last = (i0 + 32 < S ? i0 + 32 : S);
-    const long long b0 = out_off[i0], b1 = out_off[last];   // this warp's byte range of the output
+    // `out` may sit at any byte address (a caller's sub-buffer): work in offsets relative to the 4-byte aligned address
+    // just below it, so that "word-aligned" below means aligned in memory, not merely in the offset
+    const long long mis = (long long)(reinterpret_cast<uintptr_t>(out) & 3);
+    out -= mis;
+    const long long b0 = out_off[i0] + mis, b1 = out_off[last] + mis;   // this warp's byte range of the output
     const long long base = b0 & ~3ll;                       // shared-memory offset 0 <-> global byte `base`
     uint8_t* buf = s_tok[warp];
     if (live) {
@@ -331,7 +335,7 @@ __global__ void __launch_bounds__(kEmitWarps * 32) emit_tokens_kernel(
             if (dig_out) { uint4* q = (uint4*)(dig_out + i * 32); q[0] = d0; q[1] = d1; }
             int t = type ? type[i] : 0;
             if (t >= tt.num) { t = tt.num - 1; latch_status(d_status, ANON_ERR_UNSUPPORTED); }
-            uint8_t* o = buf + (out_off[i] - base);
+            uint8_t* o = buf + (out_off[i] + mis - base);
             *o++ = '[';
             const int nl = s_len[t];
             for (int k = 0; k < nl; k++) *o++ = s_name[t][k];
@@ -634,10 +638,9 @@ int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t*
 {
     if (!ctx || !c || c->ctx != ctx || S < 0 || !d_off || !d_out_off || (!key && key_len) || slug_len < 0 || slug_len > 64)
         return ANON_ERR_INVALID_ARG;
-    if (S > 0 && (!d_bytes || !d_out)) {
-        // d_bytes may legitimately be NULL only when every span is empty; we cannot know: require it
-        if (!d_out) return ANON_ERR_INVALID_ARG;
-    }
+    if (S > 0 && (!d_bytes || !d_out)) return ANON_ERR_INVALID_ARG;
+    // uint4 stores of the per-span digests: 16-byte alignment is part of the ABI (include/anonshield.h)
+    if (d_digests && (reinterpret_cast<uintptr_t>(d_digests) & 15)) return ANON_ERR_INVALID_ARG;
     if (S >= (1ll << 31)) return ANON_ERR_UNSUPPORTED;
     TypeTable tt;
     int rc = fill_type_table(type_names, num_types, &tt);
@@ -662,8 +665,10 @@ int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t*
     const unsigned nb256 = (unsigned)((S + 255) / 256);
     ProfScope prof(ctx, PROF_PSEUDO, 0.0, 6);
 
+    int* d_full = ctx->d_status + 16;
+    CU_TRY(ctx, cudaMemsetAsync(d_full, 0, 4, st));
     cache_probe_kernel<<<nb256, 256, 0, st>>>(d_bytes, off, S, c->d_table, c->n_slots - 1, c->d_arena,
-                                               c->d_entry_off, slot_of, ctx->d_status);
+                                               c->d_entry_off, slot_of, d_full);
     CU_LAUNCH_CHECK(ctx, "cache_probe_kernel");
     ClassifyIn in{off, d_type, slot_of, c->d_table, tt, slug_len};
     scan::reduce_and_scan<scan::I64x3, scan::SumI64x3>(in, S, nullptr, agg, st);
@@ -671,15 +676,14 @@ int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t*
     scan::I64x3* h_tot = (scan::I64x3*)ctx->h_pinned;
     int* h_status = (int*)(ctx->h_pinned + 64);
     CU_TRY(ctx, cudaMemcpyAsync(h_tot, agg + scan::num_tiles(S), sizeof(scan::I64x3), cudaMemcpyDeviceToHost, st));
-    CU_TRY(ctx, cudaMemcpyAsync(h_status, ctx->d_status, 4, cudaMemcpyDeviceToHost, st));
+    CU_TRY(ctx, cudaMemcpyAsync(h_status, d_full, 4, cudaMemcpyDeviceToHost, st));
     CU_TRY(ctx, cudaStreamSynchronize(st));
     const long long n_new = h_tot->a, new_bytes = h_tot->b, out_bytes = h_tot->c;
     if (total_out_bytes) *total_out_bytes = out_bytes;
-    const bool table_full = (*h_status == ANON_ERR_CAPACITY);
+    const bool table_full = (*h_status != 0);
     if (table_full || c->n_unique + (uint64_t)n_new > c->max_unique ||
         c->arena_used + (uint64_t)new_bytes > c->arena_bytes || (uint64_t)out_bytes > out_cap) {
         cache_rollback_kernel<<<nb256, 256, 0, st>>>(S, slot_of, c->d_table);
-        if (table_full) cudaMemsetAsync(ctx->d_status, 0, 4, st);
         CU_TRY(ctx, cudaStreamSynchronize(st));
         return ANON_ERR_CAPACITY;
     }
@@ -724,7 +728,8 @@ extern "C" int anon_pseudonymize(anon_ctx* ctx, anon_cache* cache, const uint8_t
 extern "C" int anon_hmac_spans(anon_ctx* ctx, const uint8_t* d_span_bytes, const int64_t* d_span_offsets, int64_t S,
                                const uint8_t* key, size_t key_len, uint8_t* d_digests)
 {
-    if (!ctx || S < 0 || !d_span_offsets || (S > 0 && !d_digests) || (!key && key_len)) return ANON_ERR_INVALID_ARG;
+    if (!ctx || S < 0 || !d_span_offsets || (S > 0 && (!d_digests || !d_span_bytes)) || (!key && key_len)) return ANON_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(d_digests) & 15) return ANON_ERR_INVALID_ARG;      // uint4 stores
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     if (S == 0) return ANON_OK;
     PadStates ps;

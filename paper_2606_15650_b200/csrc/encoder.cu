@@ -370,9 +370,7 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
     const size_t per_tok = per_token_bytes(d);
     const size_t avail = ws.left() > ((size_t)2 << 20) ? ws.left() - ((size_t)2 << 20) : 0;
     long long cap = (long long)(avail / per_tok);
-    static long long env_cap = -1;
-    if (env_cap < 0) { const char* e = getenv("ANON_CHUNK_TOKENS"); env_cap = e ? atoll(e) : 0; }
-    if (env_cap > 0 && cap > env_cap) cap = env_cap;
+    if (ctx->chunk_tokens_cap > 0 && cap > ctx->chunk_tokens_cap) cap = ctx->chunk_tokens_cap;
     if (cap < d.max_pos && cap < T) return ANON_ERR_OOM;
 
     int s0 = 0;

@@ -716,11 +716,8 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
         if (rc) return rc;
     }
     auto kern = gemm_bf16_tcgen05_kernel<BN, EPI, NB, CG>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CU_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-        attr_set = true;
-    }
+    rc = ensure_smem_attr(ctx, (const void*)kern, C::SMEM_BYTES);
+    if (rc) return rc;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];

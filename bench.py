@@ -1,19 +1,32 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the AnonShield hot path (A1-A13) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload base|large|stream|pseudonym] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload base|large|stream|pseudonym|fields|modern]
+                    [--headline-only] [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of seeded synthetic input: anon_ner_forward ->
 anon_decode_spans -> anon_gather_spans -> anon_pseudonymize (cache cleared first, so every step inserts and
-HMACs the same entities).  Default workload = BASELINE.json configs[1] (BERT-base shape, BF16, 4,096 packed
-sequences, lognormal lengths); `value` = tokens/s with inputs resident in HBM; `e2e` = the same metric through
-anon_pipeline_host with pinned HOST buffers (H2D + D2H inside the timed region).  One JSON line on stdout.
-Under torchrun (N > 1) every rank runs its own shard of the same size (weak scaling, no data-path collective);
-time = max over ranks, value = sum of tokens / that time.
+HMACs the same entities).  The timed workload of the ONE JSON line is BASELINE.json configs[1] (BERT-base shape, BF16,
+4,096 packed sequences, lognormal lengths): `value` = tokens/s with inputs resident in HBM; `e2e` = the same metric through
+anon_pipeline_host with pinned HOST buffers (H2D + D2H inside the timed region).
+
+At N = 1 with the default workload the same process then also measures, each in its own timed region, and embeds as extra
+keys of the same line (skipped with --headline-only or when the time budget --extra-budget-s runs out):
+  "stream"    BASELINE.json configs[2]: the full 70,951-record stream (records/s, seconds, e2e text in -> text out)
+  "pseudonym" configs[4]: 50 M spans through the hash cache + HMAC-SHA256 + write-back (spans/s, e2e with host span buffers,
+              the C oracle on the full 50 M spans as cpu_baseline)
+  "large"     configs[3]: 24 x 1024 encoder, vocab 250,002 (tokens/s)
+  "fields"    S8f NEXT-2: field spans -> gather -> pseudonymize -> splice over the stream's text, no encoder (KB/s, spans/s)
+Each carries its own `roofline` (and `cpu_baseline` / `e2e` where the metric has one).  `--workload X` runs one of them alone
+as the main line.  Under torchrun (N > 1) every rank runs its own shard of the same size (weak scaling, no data-path
+collective); time = max over ranks, value = sum of tokens / that time.  `--gpus N` without torchrun re-executes itself under
+`python -m torch.distributed.run --nproc-per-node N`.
 """
 import argparse
+import hashlib
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -29,7 +42,8 @@ from harness import gen  # noqa: E402  (seeded input generators: no arithmetic o
 
 KEY = bytes((7 * i + 3) & 255 for i in range(32))
 SLUG_LEN = 10
-PLANTED = (2.0, 0.5, 4.0)        # W2 planted-detector weights (DESIGN.md input recipe)
+PLANTED = gen.PLANTED_DEEP       # W2 planted-detector weights (DESIGN.md input recipe): survives 12 and 24 layers
+T_START = time.time()
 
 
 def log(*a):
@@ -96,9 +110,18 @@ def measured_peaks():
 
 GEMM_CLASSES = {"gemm_qkv": "QKV projection, +bias (N = 3H, K = H)", "gemm_out": "out-projection, +bias +FP32 residual (N = K = H)",
                 "gemm_ffn1": "FFN up, +bias +erf-GELU (N = F, K = H)", "gemm_ffn2": "FFN down, +bias +FP32 residual (N = H, K = F)"}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of gemm_bf16_tcgen05_kernel at the DEFAULT workload (configs[1],
-# M = 1,005,578 tokens), from one `ncu --set full` capture (profiles/r01d_top_ncu_full.txt, summarised in profiles/r01_summary.md "r01d"); other workloads: null
-NCU_TRAFFIC_BASE = {"gemm_qkv": 6.246e9, "gemm_out": 8.126e9, "gemm_ffn1": 7.730e9, "gemm_ffn2": 16.853e9}   # bytes
+def ncu_traffic_base():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the four GEMMs at the DEFAULT workload, from the `ncu --set
+    full` capture recorded in profiles/traffic_base.json.txt.  The file names the commit and the SHA-256 of the kernel source it
+    was taken from; if csrc/gemm_tcgen05.cu has changed since, the numbers are stale and `traffic` is null."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic_base.json.txt")) as f:
+            rec = json.load(f)
+        with open(os.path.join(ROOT, "paper_2606_15650_b200", "csrc", "gemm_tcgen05.cu"), "rb") as f:
+            sha = hashlib.sha256(f.read()).hexdigest()
+        return rec["traffic_bytes_per_launch"] if rec.get("gemm_tcgen05_cu_sha256") == sha else None
+    except (OSError, ValueError, KeyError):
+        return None
 
 
 def gemm_rooflines(prof, peaks, traffic=None):
@@ -190,68 +213,99 @@ def seqs_for_tokens(cu, budget):
 
 
 # ---- reference arm: the oracle on the host cores --------------------------------------------------------------
-def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
-        return
-    if args.workload == "pseudonym":
-        return run_reference_pseudonym(args)
-    if args.workload == "stream":
+def reference_line(args, workload, steps, warmup):
+    """The oracle, as it stands, on the host cores over a bounded sample of `workload`; returns the JSON object."""
+    if workload == "pseudonym":
+        return reference_pseudonym(args, steps, warmup)
+    if workload == "fields":
+        return reference_fields(args, steps, warmup)
+    if workload == "stream":
         desc, wseed = gen.DESCS["base"], gen.SEED_BASE + 2
-        rec = gen.workload_stream(n_records=64, seed=gen.SEED_BASE + 3, n_pool=20000)
+        rec = gen.workload_stream(n_records=64, seed=gen.SEED_BASE + 3, n_pool=300000)
         win = gen.window_records(rec)
         label = "BASELINE.json configs[2]: synthetic record stream, 510+2-token windows (first 64 records generated)"
     else:
-        desc, rec, win, wseed, label = encoder_workload(args.workload, 0, n_records=64)
+        desc, rec, win, wseed, label = encoder_workload(workload, 0, n_records=64)
     w = make_weights_for(desc, wseed)
     names = gen.TYPE_NAMES_6
-    n = seqs_for_tokens(win["cu_seqlens"], 250 if args.workload == "large" else 600)
+    n = seqs_for_tokens(win["cu_seqlens"], 250 if workload == "large" else 600)
     tot_t = tot_s = 0
     times = []
-    for i in range(args.warmup + args.steps):
+    for i in range(warmup + steps):
         T, S, dt = oracle_sample_pass(w, desc, rec, win, n, names)
-        if i >= args.warmup:
+        if i >= warmup:
             tot_t += T; tot_s += S; times.append(dt)
     sec = sum(times)
     v = tot_t / sec
     sample = "first %d sequences (%d tokens) of the workload per step" % (n, int(win["cu_seqlens"][n]))
     metric, unit = "ner_tokens_per_s", "tokens/s"
-    if args.workload == "stream":     # records/s = tokens/s over the stream's window-tokens per record
+    if workload == "stream":     # records/s = tokens/s over the stream's window-tokens per record
         v = v * (len(rec["rec_off"]) - 1) / float(win["cu_seqlens"][-1])
         metric, unit = "records_per_s", "records/s"
         sample += "; tokens/s scaled by the sample's window-tokens per record"
-    out = {"impl": "reference", "metric": metric, "value": v, "unit": unit, "n_gpus": args.gpus,
-           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps, "higher_is_better": True,
-           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": label, "sample": sample},
-           "cpu_baseline": {"value": v, "unit": unit, "cores": blas_threads(), "kind": "oracle", "sample": sample},
-           "e2e": {"value": v, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-           "spans_per_s": tot_s / sec}
-    print(json.dumps(out), flush=True)
+    return {"impl": "reference", "metric": metric, "value": v, "unit": unit, "n_gpus": args.gpus,
+            "steps": steps, "warmup": warmup, "ms_per_step": 1e3 * sec / steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": label, "sample": sample},
+            "cpu_baseline": {"value": v, "unit": unit, "cores": blas_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "spans_per_s": tot_s / sec}
 
 
-def run_reference_pseudonym(args):
+def reference_pseudonym(args, steps, warmup):
     from oracle import crypto
     n_draws = 2_000_000
     data, off, types, key, _ = gen.spans_zipf(200_000, n_draws, 7, 128, 6, gen.SEED_BASE + 5)
     times = []
-    for i in range(args.warmup + args.steps):
+    for i in range(warmup + steps):
         oc = crypto.Cache(1 << 20)
         t0 = time.perf_counter()
         oc.pseudonymize(data, off, types, key.tobytes(), SLUG_LEN, gen.TYPE_NAMES_6)
         dt = time.perf_counter() - t0
         oc.close()
-        if i >= args.warmup:
+        if i >= warmup:
             times.append(dt)
     sec = sum(times)
-    v = n_draws * args.steps / sec
+    v = n_draws * steps / sec
     sample = "2,000,000 spans Zipf(1.1) over 200,000 strings (1/25 of configs[4]) per step"
-    out = {"impl": "reference", "metric": "pseudonym_spans_per_s", "value": v, "unit": "spans/s", "n_gpus": args.gpus,
-           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps, "higher_is_better": True,
-           "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-           "config": {"workload": "BASELINE.json configs[4] pseudonym-stage stress", "sample": sample},
-           "cpu_baseline": {"value": v, "unit": "spans/s", "cores": 1, "kind": "oracle", "sample": sample},
-           "e2e": {"value": v, "unit": "spans/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    return {"impl": "reference", "metric": "pseudonym_spans_per_s", "value": v, "unit": "spans/s", "n_gpus": args.gpus,
+            "steps": steps, "warmup": warmup, "ms_per_step": 1e3 * sec / steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[4] pseudonym-stage stress", "sample": sample},
+            "cpu_baseline": {"value": v, "unit": "spans/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "spans/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+
+
+def reference_fields(args, steps, warmup):
+    rec = gen.workload_stream(n_records=1500, seed=gen.SEED_BASE + 3, n_pool=300000)
+    times, nb, ns = [], 0, 0
+    for i in range(warmup + steps):
+        nb, ns, dt = oracle_fields_pass(rec, 1500)
+        if i >= warmup:
+            times.append(dt)
+    sec = sum(times)
+    v = nb / 1024.0 * steps / sec
+    sample = "first 1500 records of the configs[2] stream (%.1f MiB, %d field spans) per step" % (nb / 2**20, ns)
+    return {"impl": "reference", "metric": "field_path_kb_per_s", "value": v, "unit": "KB/s", "n_gpus": args.gpus,
+            "steps": steps, "warmup": warmup, "ms_per_step": 1e3 * sec / steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+            "config": {"workload": "S8f NEXT-2 field path on the configs[2] records", "sample": sample},
+            "cpu_baseline": {"value": v, "unit": "KB/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "KB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "spans_per_s": ns * steps / sec}
+
+
+def run_reference(args):
+    """--impl reference: rank 0 alone; the main line on args.workload, and (default workload, not --headline-only) the
+    same extra keys as our arm, each on its own bounded sample with one timed step."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    out = reference_line(args, args.workload, args.steps, args.warmup)
+    if args.workload == "base" and not args.headline_only:
+        for name in ("stream", "pseudonym", "large", "fields"):
+            t0 = time.time()
+            out[name] = reference_line(args, name, 1, 0)
+            log(f"[reference] {name}: {time.time() - t0:.0f}s")
     print(json.dumps(out), flush=True)
 
 
@@ -289,15 +343,19 @@ def gpu_id_for_smi(local):
         return vis.split(",")[local] if vis else local
 
 
-def run_encoder(args):
+def run_encoder(args, workload=None, steps=None, warmup=None, e2e_steps=5, records=None):
+    """One encoder workload (configs[1] "base", configs[3] "large", NEXT-3 "modern"); returns the JSON object (rank 0) or None."""
     import torch
     import paper_2606_15650_b200 as P
     from paper_2606_15650_b200 import sharding
+    workload = workload or args.workload
+    steps = steps or args.steps
+    warmup = args.warmup if warmup is None else warmup
     world, rank, local = dist_setup(args)
     dev = torch.device("cuda", local)
     peaks = measured_peaks()
     t_setup = time.time()
-    desc, rec, win, wseed, label = encoder_workload(args.workload, rank, args.records)
+    desc, rec, win, wseed, label = encoder_workload(workload, rank, records)
     names = gen.TYPE_NAMES_6
     w = make_weights_for(desc, wseed)
     ids, cu, meta = win["token_ids"], win["cu_seqlens"], np.ascontiguousarray(win["meta"])
@@ -339,7 +397,7 @@ def run_encoder(args):
                             out_off[:S + 1], hit)
         state["S"] = S
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     assert ctx.sync() == 0
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -347,7 +405,7 @@ def run_encoder(args):
     sampler = ClockSampler(gpu_id_for_smi(local)) if rank == 0 else None
     ctx.profile(True)
     ev0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     ev1.record()
     barrier(world)
@@ -356,9 +414,9 @@ def run_encoder(args):
     clocks = sampler.stop() if sampler else None
     sec_local = ev0.elapsed_time(ev1) / 1e3
     S = state["S"]
-    tokens_all, sec = sharding.aggregate_throughput(T * args.steps, sec_local, dev)
-    spans_all, _ = sharding.aggregate_throughput(S * args.steps, sec_local, dev)
-    recs_all, _ = sharding.aggregate_throughput(R * args.steps, sec_local, dev)
+    tokens_all, sec = sharding.aggregate_throughput(T * steps, sec_local, dev)
+    spans_all, _ = sharding.aggregate_throughput(S * steps, sec_local, dev)
+    recs_all, _ = sharding.aggregate_throughput(R * steps, sec_local, dev)
 
     # ---- e2e: the same pass through anon_pipeline_host with pinned HOST buffers ----
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
@@ -372,11 +430,11 @@ def run_encoder(args):
         cache.clear()
         return P.anon_pipeline_host(ctx, W, cache, h_ids, h_cu, h_meta, h_text, h_rec_off, KEY, SLUG_LEN, names, cap,
                                     out_cap, want_hit=True, bufs=bufs)
-    for _ in range(min(args.warmup, 2)):
+    for _ in range(min(warmup, 2, e2e_steps)):
         res = step_host()
     barrier(world)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    n_e2e = max(1, min(args.steps, 5))
+    n_e2e = max(1, min(steps, e2e_steps))
     e0.record()
     for _ in range(n_e2e):
         res = step_host()
@@ -387,18 +445,21 @@ def run_encoder(args):
     Sh = len(res["spans"])
     d2h = Sh * 16 + int(res["out_tokens"].size) + (Sh + 1) * 8 + Sh + 8
 
+    cache.close(); W.close(); ctx.close()
+    del d_ids, d_cu, d_meta, d_text, d_rec_off, labels, spans, span_bytes, span_off, span_type, out_tokens, out_off, hit, bufs
+    torch.cuda.empty_cache()
     if rank != 0:
-        return
-    default_shape = args.workload == "base" and args.records is None
-    roof, g_ms = gemm_rooflines(prof, peaks, NCU_TRAFFIC_BASE if default_shape else None)
+        return None
+    default_shape = workload == "base" and records is None
+    roof, g_ms = gemm_rooflines(prof, peaks, ncu_traffic_base() if default_shape else None)
     a_ms, a_fl, a_n = prof["attention"]
     r_ms, r_by, r_n = prof["row"]
     out = {
         "metric": "ner_tokens_per_s", "value": tokens_all / sec, "unit": "tokens/s", "n_gpus": world,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps, "higher_is_better": True,
+        "steps": steps, "warmup": warmup, "ms_per_step": 1e3 * sec / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": label, "tokens_per_step_per_gpu": T, "records_per_step_per_gpu": R,
-                   "spans_per_step_per_gpu": S, "weights": "W2 planted-detector, seeded random-init",
+                   "spans_per_step_per_gpu": S, "weights": "W2 planted-detector (deep variant), seeded random-init",
                    "l2": "inputs larger than L2 (activations %.1f GB per step stream through HBM)" % (T * 19968 / 1e9),
                    "slug_len": SLUG_LEN},
         "records_per_s": recs_all / sec, "spans_per_s": spans_all / sec,
@@ -407,19 +468,19 @@ def run_encoder(args):
                 "d2h_bytes_per_step": int(d2h), "steps": n_e2e, "ms_per_step": 1e3 * e2e_sec / n_e2e,
                 "records_per_s": R * n_e2e * world / e2e_sec},
         "roofline": roof,
-        "breakdown_ms_per_step": dict({k: v[0] / args.steps for k, v in prof.items()}, gemm=g_ms / args.steps),
+        "breakdown_ms_per_step": dict({k: v[0] / steps for k, v in prof.items()}, gemm=g_ms / steps),
         "attention_tflops": a_fl / (a_ms * 1e-3) / 1e12 if a_ms > 0 else None,
         "row_kernels_gbs": r_by / (r_ms * 1e-3) / 1e9 if r_ms > 0 else None,
     }
     if world == 1 and not args.no_cpu_baseline:
-        n = seqs_for_tokens(cu, 4000 if args.workload == "base" else 1500)
+        n = seqs_for_tokens(cu, 4000 if workload == "base" else 1500)
         Tc, Sc, dt = oracle_sample_pass(w, desc, rec, win, n, names)
         out["cpu_baseline"] = {"value": Tc / dt, "unit": "tokens/s", "cores": blas_threads(), "kind": "oracle",
                                "sample": "first %d sequences (%d tokens, %d spans) of the workload, %.1f s" % (n, Tc, Sc, dt)}
-    print(json.dumps(out), flush=True)
+    return out
 
 
-def run_stream(args):
+def run_stream(args, records=None):
     """BASELINE.json configs[2]: the full synthetic record stream (70,951 records, ~550 MB) in token-budgeted
     batches of whole records; the entity cache persists across batches.  A "step" is one batch (~1 M tokens);
     the timed region is ALL batches of the stream, after 3 warm-up batches run on a scratch cache."""
@@ -431,7 +492,7 @@ def run_stream(args):
     peaks = measured_peaks()
     t_setup = time.time()
     desc = gen.DESCS["base"]
-    n_records = args.records or 70951
+    n_records = records or 70951
     rec = gen.workload_stream(n_records=n_records, seed=gen.SEED_BASE + 3 + 1000 * rank,
                               n_pool=300000 if n_records >= 20000 else 20000)
     log(f"[rank {rank}] records generated in {time.time() - t_setup:.0f}s: {rec['text'].size / 2**20:.1f} MiB, "
@@ -454,8 +515,8 @@ def run_stream(args):
     W = P.Weights(ctx, desc, gen.pack_blob(w))
     rx = None
     if args.regex:      # NEXT-4: the hybrid strategy -- regex spans merged into the NER spans before the gather
-        from paper_2606_15650_b200 import kernel_bench, regex_dfa
-        rx = P.Regex(ctx, regex_dfa.compile_patterns(list(enumerate(kernel_bench.REGEX_PATTERNS)), 80))
+        from paper_2606_15650_b200 import regex_dfa
+        rx = P.Regex(ctx, regex_dfa.compile_patterns(list(enumerate(gen.REGEX_PATTERNS)), 80))
     log(f"[rank {rank}] setup {time.time() - t_setup:.0f}s: {len(batches)} batches, {T_all} window-tokens, "
         f"{len(win['cu_seqlens']) - 1} windows, max batch {maxT} tokens, ws={ws / 2**30:.1f} GiB")
 
@@ -557,8 +618,15 @@ def run_stream(args):
     barrier(world)
     e2e_recs, e2e_sec = sharding.aggregate_throughput(n_records, e0.elapsed_time(e1) / 1e3, dev)
     st2 = cache2.stats()
+    cache2.close(); W.close()
+    if rx is not None:
+        P.anon_ctx_set_regex(ctx, None)
+        rx.close()
+    ctx.close()
+    del hbat, bufs, labels, spans, span_bytes, span_off, span_type, out_tokens, out_off, hit, new_text, new_ro
+    torch.cuda.empty_cache()
     if rank != 0:
-        return
+        return None, rec
     nb = len(batches)
     roof, g_ms = gemm_rooflines(prof, peaks)
     a_ms, a_fl, _ = prof["attention"]
@@ -570,10 +638,10 @@ def run_stream(args):
         "config": {"workload": "BASELINE.json configs[2]: %d synthetic records, %.1f MiB of text, %d windows (510+2, overlap 128), "
                                "%d window-tokens, Zipf(1.1) entities; batches of whole records, <= %d tokens"
                                % (n_records, rec["text"].size / 2**20, len(win["cu_seqlens"]) - 1, T_all, args.batch_tokens),
-                   "batches": nb, "weights": "W2 planted-detector, seeded random-init", "slug_len": SLUG_LEN,
+                   "batches": nb, "weights": "W2 planted-detector (deep variant), seeded random-init", "slug_len": SLUG_LEN,
                    "splice": "records rewritten on the device (anon_splice_records) inside the timed region",
                    "regex": ("hybrid detection: DFA scan of %d patterns over the batch text + regex/NER span merge inside the "
-                             "timed region (NEXT-4)" % len(kernel_bench.REGEX_PATTERNS)) if rx is not None else "off (--regex enables NEXT-4)",
+                             "timed region (NEXT-4)" % len(gen.REGEX_PATTERNS)) if rx is not None else "off (--regex enables NEXT-4)",
                    "spans": S_all, "planted_entities": int(rec["n_entities"]), "unique_entities": st["n_unique"],
                    "cache_hit_rate": st["n_hits"] / max(st["n_lookups"], 1),
                    "l2": "inputs larger than L2 (each batch streams ~20 GB of activations through HBM)"},
@@ -597,18 +665,26 @@ def run_stream(args):
                                "kind": "oracle",
                                "sample": "first %d windows (%d tokens, %d spans) of the stream in %.1f s = %.0f tokens/s, "
                                          "scaled by tokens per record" % (n, Tc, Sc, dt, Tc / dt)}
-    print(json.dumps(out), flush=True)
+    return out, rec
 
 
-def run_pseudonym(args):
+def pseudonym_alg_bytes(span_bytes, S, out_bytes):
+    """Algorithmic bytes of anon_pseudonymize: span bytes once for the hash + once for the compare against the
+    stored key, 16 B of offsets, one 32 B slot sector, hit / uid / type (10 B), the token written and its 8 B offset."""
+    return 2 * span_bytes + 16 * S + 32 * S + 10 * S + out_bytes + 8 * S
+
+
+def run_pseudonym(args, records=None, steps=None, warmup=None):
     """BASELINE.json configs[4]: 50 M spans Zipf(1.1) over 2 M strings -> dedup + HMAC + write-back."""
     import torch
     import paper_2606_15650_b200 as P
     from paper_2606_15650_b200 import sharding
+    steps = steps or args.steps
+    warmup = args.warmup if warmup is None else warmup
     world, rank, local = dist_setup(args)
     dev = torch.device("cuda", local)
     peaks = measured_peaks()
-    n_unique, n_draws = (args.records or 2_000_000), (args.records or 2_000_000) * 25
+    n_unique, n_draws = (records or 2_000_000), (records or 2_000_000) * 25
     t0 = time.time()
     data, off, types, key, _ = gen.spans_zipf(n_unique, n_draws, 7, 128, 6, gen.SEED_BASE + 5 + 1000 * rank)
     log(f"[rank {rank}] generated {n_draws} spans, {data.size / 1e9:.2f} GB in {time.time() - t0:.0f}s")
@@ -626,7 +702,7 @@ def run_pseudonym(args):
     def step():
         cache.clear()
         P.anon_pseudonymize(ctx, cache, d_bytes, d_off, d_type, kb, SLUG_LEN, gen.TYPE_NAMES_6, out, out_off, hit, uid)
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     assert ctx.sync() == 0
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -634,34 +710,216 @@ def run_pseudonym(args):
     sampler = ClockSampler(gpu_id_for_smi(local)) if rank == 0 else None
     ctx.profile(True)
     ev0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     ev1.record()
     barrier(world)
     prof, launches = ctx.profile_read()
     ctx.profile(False)
     clocks = sampler.stop() if sampler else None
-    spans_all, sec = sharding.aggregate_throughput(S * args.steps, ev0.elapsed_time(ev1) / 1e3, dev)
+    spans_all, sec = sharding.aggregate_throughput(S * steps, ev0.elapsed_time(ev1) / 1e3, dev)
     st = cache.stats()
-    # algorithmic bytes per span: span bytes + 16 B offsets + 32 B slot + stored-key compare + hit/uid/type
-    # + token written + out offset; the dominant kernel is the probe.
     out_bytes = int(out_off[S].item())
-    alg = 2 * data.size + 16 * S + 32 * S + 10 * S + out_bytes + 8 * S
+    alg = pseudonym_alg_bytes(data.size, S, out_bytes)
+
+    # ---- e2e: span bytes / offsets / types in pinned HOST buffers -> H2D -> anon_pseudonymize -> D2H of tokens, offsets, hit ----
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_bytes, h_off, h_type = pin(data), pin(off), pin(types)
+    h_out = torch.zeros(out_bytes, dtype=torch.uint8).pin_memory()
+    h_out_off = torch.zeros(S + 1, dtype=torch.int64).pin_memory()
+    h_hit = torch.zeros(S, dtype=torch.uint8).pin_memory()
+
+    def step_host():
+        cache.clear()
+        d_bytes.copy_(h_bytes, non_blocking=True); d_off.copy_(h_off, non_blocking=True); d_type.copy_(h_type, non_blocking=True)
+        P.anon_pseudonymize(ctx, cache, d_bytes, d_off, d_type, kb, SLUG_LEN, gen.TYPE_NAMES_6, out, out_off, hit, None)
+        h_out.copy_(out[:out_bytes], non_blocking=True); h_out_off.copy_(out_off, non_blocking=True); h_hit.copy_(hit, non_blocking=True)
+    step_host()
+    barrier(world)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n_e2e = max(1, min(steps, 3))
+    e0.record()
+    for _ in range(n_e2e):
+        step_host()
+    e1.record()
+    barrier(world)
+    e2e_spans, e2e_sec = sharding.aggregate_throughput(S * n_e2e, e0.elapsed_time(e1) / 1e3, dev)
+    assert ctx.sync() == 0
+    h2d, d2h = data.nbytes + off.nbytes + types.nbytes, out_bytes + (S + 1) * 8 + S
+    cache.close(); ctx.close()
+    del d_bytes, d_off, d_type, out, out_off, hit, uid, h_bytes, h_off, h_type, h_out, h_out_off, h_hit
+    torch.cuda.empty_cache()
     if rank != 0:
-        return
-    ms = prof["pseudonymize"][0] / args.steps
+        return None
+    ms = prof["pseudonymize"][0] / steps
     res = {"metric": "pseudonym_spans_per_s", "value": spans_all / sec, "unit": "spans/s", "n_gpus": world,
-           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps, "higher_is_better": True,
+           "steps": steps, "warmup": warmup, "ms_per_step": 1e3 * sec / steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
            "config": {"workload": "BASELINE.json configs[4]: %d spans of 7-128 B, Zipf(1.1) over %d strings" % (S, n_unique),
                       "unique_found": st["n_unique"], "hit_rate": st["n_hits"] / max(st["n_lookups"], 1),
                       "l2": "inputs larger than L2 (%.1f GB of span bytes)" % (data.size / 1e9)},
            "clocks": clocks, "gpu_launches": launches,
+           "e2e": {"value": e2e_spans / e2e_sec, "unit": "spans/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                   "steps": n_e2e, "ms_per_step": 1e3 * e2e_sec / n_e2e,
+                   "call": "pinned host span CSR -> H2D -> anon_pseudonymize -> D2H of tokens, offsets, hit flags"},
            "roofline": {"bound": "hbm", "kernel": "anon_pseudonymize (probe + classify scan + insert/HMAC + emit)",
                         "achieved": alg / (ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": alg / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None,
+                        "algorithmic_bytes_per_step": int(alg), "avg_launch_ms": ms,
                         "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"]}}
-    print(json.dumps(res), flush=True)
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import crypto
+        oc = crypto.Cache(1 << 22)
+        t0 = time.perf_counter()
+        oc.pseudonymize(data, off, types, kb, SLUG_LEN, gen.TYPE_NAMES_6)
+        dt = time.perf_counter() - t0
+        oc.close()
+        res["cpu_baseline"] = {"value": S / dt, "unit": "spans/s", "cores": 1, "kind": "oracle",
+                               "sample": "the FULL workload (%d spans, %d unique) through oracle/anon_oracle.c, one thread, %.1f s" % (S, st["n_unique"], dt)}
+    return res
+
+
+FIELD_TYPE = 2          # NEXT-2: every field span carries one fixed type (the schema names the field)
+
+
+def oracle_fields_pass(rec, n_records):
+    """The oracle over the first n_records records of the field workload: gather + dedup / HMAC / write-back + splice."""
+    from oracle import crypto, decode
+    ro = rec["rec_off"][:n_records + 1]
+    text = rec["text"][:int(ro[-1])]
+    spans = gen.field_spans(rec, FIELD_TYPE)
+    spans = spans[spans[:, 0] < n_records]
+    sp = [tuple(int(v) for v in s) for s in spans]
+    t0 = time.perf_counter()
+    sb, so = decode.gather_spans(text, ro, sp)
+    oc = crypto.Cache(1 << 20)
+    w = oc.pseudonymize(sb, so, spans[:, 3].astype(np.uint8), KEY, SLUG_LEN, gen.TYPE_NAMES_6)
+    decode.splice_records(text, ro, sp, w["out_tokens"], w["out_offsets"])
+    dt = time.perf_counter() - t0
+    oc.close()
+    return text.size, len(sp), dt
+
+
+def run_fields(args, rec=None, records=None, steps=None, warmup=None):
+    """S8f NEXT-2: caller-supplied field spans with a fixed type over the configs[2] record text ->
+    anon_gather_spans -> anon_pseudonymize -> anon_splice_records.  No encoder kernel runs.  Unit: KB of record text per second
+    (the paper's unit for this path: 34,341 KB/s for D2-CSV on its machine -- context, not the target)."""
+    import torch
+    import paper_2606_15650_b200 as P
+    from paper_2606_15650_b200 import sharding
+    steps = steps or args.steps
+    warmup = args.warmup if warmup is None else warmup
+    world, rank, local = dist_setup(args)
+    dev = torch.device("cuda", local)
+    peaks = measured_peaks()
+    if rec is None:
+        n_records = records or 70951
+        rec = gen.workload_stream(n_records=n_records, seed=gen.SEED_BASE + 3 + 1000 * rank, n_pool=300000 if n_records >= 20000 else 20000)
+    text, ro = rec["text"], rec["rec_off"]
+    spans = gen.field_spans(rec, FIELD_TYPE)
+    S, R = int(spans.shape[0]), int(ro.size - 1)
+    sb_total = int((spans[:, 2] - spans[:, 1]).sum())
+    ctx = P.Context(local, workspace_bytes=(64 << 20) + 64 * S)
+    cache = P.Cache(ctx, 1 << 20, 64 << 20)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    d_text, d_ro, d_spans = d(text), d(ro), d(spans)
+    span_bytes = torch.zeros(sb_total + 16, dtype=torch.uint8, device=dev)
+    span_off = torch.zeros(S + 1, dtype=torch.int64, device=dev)
+    span_type = torch.zeros(S, dtype=torch.uint8, device=dev)
+    out_cap = S * (3 + 13 + SLUG_LEN)
+    out = torch.zeros(out_cap, dtype=torch.uint8, device=dev)
+    out_off = torch.zeros(S + 1, dtype=torch.int64, device=dev)
+    hit = torch.zeros(S, dtype=torch.uint8, device=dev)
+    new_text = torch.zeros(text.size + out_cap, dtype=torch.uint8, device=dev)
+    new_ro = torch.zeros(R + 1, dtype=torch.int64, device=dev)
+
+    def step():
+        cache.clear()
+        P.anon_gather_spans(ctx, d_text, d_ro, d_spans, S, span_bytes, span_off, span_type)
+        P.anon_pseudonymize(ctx, cache, span_bytes, span_off, span_type, KEY, SLUG_LEN, gen.TYPE_NAMES_6, out, out_off, hit)
+        P.anon_splice_records(ctx, d_text, d_ro, d_spans, S, out, out_off, new_text, new_ro)
+    for _ in range(warmup):
+        step()
+    assert ctx.sync() == 0
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier(world)
+    sampler = ClockSampler(gpu_id_for_smi(local)) if rank == 0 else None
+    ctx.profile(True)
+    ev0.record()
+    for _ in range(steps):
+        step()
+    ev1.record()
+    barrier(world)
+    prof, launches = ctx.profile_read()
+    ctx.profile(False)
+    clocks = sampler.stop() if sampler else None
+    bytes_all, sec = sharding.aggregate_throughput(text.size * steps, ev0.elapsed_time(ev1) / 1e3, dev)
+    st = cache.stats()
+    out_bytes = int(out_off[S].item())
+    new_bytes = int(new_ro[R].item())
+    alg = (16 * S + 2 * sb_total + 8 * S) + pseudonym_alg_bytes(sb_total, S, out_bytes) + (text.size + new_bytes + out_bytes + 24 * S)
+
+    # ---- e2e: text, record offsets and field spans in pinned HOST buffers; the rewritten text comes back to the host ----
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_text, h_ro, h_spans = pin(text), pin(ro), pin(spans)
+    h_new_text = torch.zeros(text.size + out_cap, dtype=torch.uint8).pin_memory()
+    h_new_ro = torch.zeros(R + 1, dtype=torch.int64).pin_memory()
+
+    def step_host():
+        d_text.copy_(h_text, non_blocking=True); d_ro.copy_(h_ro, non_blocking=True); d_spans.copy_(h_spans, non_blocking=True)
+        step()
+        h_new_ro.copy_(new_ro, non_blocking=True)
+        if ctx.sync():
+            raise RuntimeError("device status")
+        n = int(h_new_ro[R])
+        h_new_text[:n].copy_(new_text[:n], non_blocking=True)
+        return n
+    step_host()
+    barrier(world)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n_e2e = max(1, min(steps, 3))
+    e0.record()
+    for _ in range(n_e2e):
+        n_out = step_host()
+    e1.record()
+    barrier(world)
+    e2e_bytes, e2e_sec = sharding.aggregate_throughput(text.size * n_e2e, e0.elapsed_time(e1) / 1e3, dev)
+    h2d, d2h = text.nbytes + ro.nbytes + spans.nbytes, n_out + (R + 1) * 8
+    cache.close(); ctx.close()
+    del d_text, d_ro, d_spans, span_bytes, span_off, span_type, out, out_off, hit, new_text, new_ro, h_text, h_new_text
+    torch.cuda.empty_cache()
+    if rank != 0:
+        return None
+    ms = 1e3 * sec / steps
+    res = {"metric": "field_path_kb_per_s", "value": bytes_all / 1024.0 / sec, "unit": "KB/s", "n_gpus": world,
+           "steps": steps, "warmup": warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "u32", "data": "synthetic",
+           "config": {"workload": "S8f NEXT-2 on the BASELINE.json configs[2] records: %d records, %.1f MiB of text, %d field spans of one "
+                                  "fixed type (%s), no NER" % (R, text.size / 2**20, S, gen.TYPE_NAMES_6[FIELD_TYPE]),
+                      "unique_entities": st["n_unique"], "cache_hit_rate": st["n_hits"] / max(st["n_lookups"], 1),
+                      "l2": "inputs larger than L2 (%.0f MB of text per step)" % (text.size / 1e6),
+                      "calls": "anon_gather_spans -> anon_pseudonymize -> anon_splice_records"},
+           "spans_per_s": S * steps * world / sec, "records_per_s": R * steps * world / sec,
+           "clocks": clocks, "gpu_launches": launches,
+           "e2e": {"value": e2e_bytes / 1024.0 / e2e_sec, "unit": "KB/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                   "steps": n_e2e, "ms_per_step": 1e3 * e2e_sec / n_e2e, "records_per_s": R * n_e2e * world / e2e_sec,
+                   "call": "pinned host text + field spans -> H2D -> gather / pseudonymize / splice -> D2H of the rewritten text"},
+           "roofline": {"bound": "hbm", "kernel": "field path: gather + pseudonymize + splice (all launches of the step)",
+                        "achieved": alg / (ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                        "frac": alg / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None, "algorithmic_bytes_per_step": int(alg),
+                        "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"]},
+           "breakdown_ms_per_step": {k: prof[k][0] / steps for k in ("decode", "pseudonymize")}}
+    if world == 1 and not args.no_cpu_baseline:
+        nb, ns, dt = oracle_fields_pass(rec, min(R, 1500))
+        res["cpu_baseline"] = {"value": nb / 1024.0 / dt, "unit": "KB/s", "cores": 1, "kind": "oracle",
+                               "sample": "first %d records (%.1f MiB, %d field spans) in %.1f s" % (min(R, 1500), nb / 2**20, ns, dt)}
+    return res
+
+
+def free_port():
+    with socket.socket(socket.AF_INET, socket.SOCK_STREAM) as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
 
 
 def main():
@@ -670,21 +928,66 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="base", choices=["base", "large", "stream", "pseudonym", "modern"])
+    ap.add_argument("--workload", default="base", choices=["base", "large", "stream", "pseudonym", "fields", "modern"])
     ap.add_argument("--records", type=int, default=None, help="override the number of records / sequences / strings")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--headline-only", action="store_true", help="only the timed configs[1] line, none of the extra legs")
+    ap.add_argument("--extra-budget-s", type=float, default=840.0,
+                    help="wall-clock budget of the whole run; an extra leg that would not fit is skipped and says so")
     ap.add_argument("--batch-tokens", type=int, default=1 << 20, help="stream workload: token budget per batch")
     ap.add_argument("--regex", action="store_true", help="stream workload: also run the regex detector and merge its spans (NEXT-4)")
     args = ap.parse_args()
+    world_env = os.environ.get("WORLD_SIZE")
+    if args.gpus > 1 and world_env is None:
+        # `python bench.py --gpus N`: become N ranks, one per GPU, under torchrun on this node (S8e)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+        log("bench.py: re-executing under torchrun:", " ".join(cmd))
+        os.environ.setdefault("NCCL_DEBUG", "WARN")
+        os.execv(sys.executable, cmd)
+    if world_env is not None and int(world_env) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} does not match WORLD_SIZE={world_env}")
     if args.warmup < 3 and args.impl == "ours":
         log("note: timing rules ask for >= 3 warm-up steps")
     if args.impl == "reference":
         return run_reference(args)
+    world = int(world_env or "1")
     if args.workload == "pseudonym":
-        return run_pseudonym(args)
-    if args.workload == "stream":
-        return run_stream(args)
-    return run_encoder(args)
+        out = run_pseudonym(args, records=args.records)
+    elif args.workload == "stream":
+        out, _ = run_stream(args, records=args.records)
+    elif args.workload == "fields":
+        out = run_fields(args, records=args.records)
+    else:
+        out = run_encoder(args, records=args.records)
+    if out is None:            # ranks > 0
+        return
+    if args.workload == "base" and args.records is None and world == 1 and not args.headline_only:
+        # the headline configs of BASELINE.json next to the timed configs[1] line, each in its own timed region
+        rec = None
+        est = {"stream": 260, "pseudonym": 170, "large": 110, "fields": 60}           # seconds each leg needs on the box
+        for name in ("stream", "pseudonym", "large", "fields"):
+            left = args.extra_budget_s - (time.time() - T_START)
+            need = est[name] + (80 if name == "fields" and rec is None else 0)
+            if left < need:
+                out[name] = {"skipped": "time budget: %.0f s left, this leg needs about %d s (--extra-budget-s)" % (left, need)}
+                log(f"[extra] {name}: skipped ({left:.0f}s left)")
+                continue
+            t0 = time.time()
+            try:
+                if name == "stream":
+                    out[name], rec = run_stream(args)
+                elif name == "pseudonym":
+                    out[name] = run_pseudonym(args, steps=5, warmup=3)
+                elif name == "large":
+                    out[name] = run_encoder(args, workload="large", steps=3, warmup=3, e2e_steps=2)
+                else:
+                    out[name] = run_fields(args, rec=rec, steps=5, warmup=3)
+            except Exception as e:     # an extra leg must never cost the timed line
+                out[name] = {"error": "%s: %s" % (type(e).__name__, e)}
+            log(f"[extra] {name}: {time.time() - t0:.0f}s")
+        out["wall_s_total"] = time.time() - T_START
+    print(json.dumps(out), flush=True)
 
 
 if __name__ == "__main__":

@@ -32,6 +32,11 @@ DESCS["base_modern"] = dict(layers=22, hidden=768, heads=12, ffn=1152, vocab=503
                             dtype=1, **_MODERN)
 TYPE_NAMES_6 = ["IP_ADDRESS", "IPV6_ADDRESS", "HOSTNAME", "CVE_ID", "MAC_ADDRESS", "SERIAL_NUMBER"]
 TYPE_NAMES_4 = ["TYPE0", "TYPE1", "TYPE2", "TYPE3"]
+# rule D17's pattern set: one pattern per synthetic entity kind of entity_pool(), in type order (data for the NEXT-4
+# regex layer: the patterns are inputs of the method, like the key and the type names)
+REGEX_PATTERNS = [r"(?:[0-9]{1,3}\.){3}[0-9]{1,3}", r"(?:[0-9a-f]{1,4}:){7}[0-9a-f]{1,4}",
+                  r"(?:[a-z0-9]+\.)+(?:example|internal|corp|lan|test|invalid)", r"CVE-[0-9]{4}-[0-9]{4,7}",
+                  r"(?:[0-9a-f]{2}:){5}[0-9a-f]{2}", r"[0-9a-f]{16,32}"]
 PAD, CLS, SEP, UNK, MASK = 0, 1, 2, 3, 4
 # W2 planted-detector strengths: (alpha, beta, gamma) plants the embedding bands and the
 # head only; the 6-tuple adds (kappa, theta, lam), one re-amplifying FFN unit per class in every layer (make_weights), which a
@@ -410,6 +415,26 @@ def make_records(n_records, content_tokens, desc, pool, pool_off, pool_type, see
     return dict(text=cat(texts, np.uint8), rec_off=rec_off, tok_rec_off=tok_off, ids=cat(ids_l, np.int32),
                 char_start=cat(cs_l, np.int32), char_end=cat(ce_l, np.int32),
                 planted_label=cat(lab_l, np.int8), n_entities=n_ent_total)
+
+
+def field_spans(rec, fixed_type):
+    """NEXT-2 input (PAPER.md L57 `anonymization_config`): the caller-supplied FIELD spans of a record stream -- the byte range
+    of every generated entity string, all with one fixed type -- as int32 [S, 4] rows (record, char_start, char_end, type) in
+    stream order.  Pure layout: the ranges are where make_records put the strings (a run of labelled pieces; every entity is
+    preceded by at least one filler token, so runs never touch or cross a record)."""
+    lab = rec["planted_label"]
+    n = lab.size
+    starts = np.flatnonzero((lab > 0) & (lab % 2 == 1))
+    zeros = np.flatnonzero(lab == 0)
+    nxt = np.searchsorted(zeros, starts)                       # first unlabelled token after each start
+    ends = np.where(nxt < zeros.size, zeros[np.minimum(nxt, zeros.size - 1)], n) - 1
+    tok_rec = np.searchsorted(rec["tok_rec_off"], starts, side="right") - 1
+    out = np.empty((starts.size, 4), np.int32)
+    out[:, 0] = tok_rec
+    out[:, 1] = rec["char_start"][starts]
+    out[:, 2] = rec["char_end"][ends]
+    out[:, 3] = fixed_type
+    return out
 
 
 WINDOW_CONTENT, WINDOW_OVERLAP = 510, 128

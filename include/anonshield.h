@@ -218,6 +218,17 @@ int  anon_pseudonymize(anon_ctx* ctx, anon_cache* cache,
 int  anon_hmac_spans(anon_ctx* ctx, const uint8_t* d_span_bytes, const int64_t* d_span_offsets, int64_t S,
                      const uint8_t* key, size_t key_len, uint8_t* d_digests /* [S,32] */);
 
+/* ---- measured issue-rate peaks ("Integer-ALU and MUFU rates are not in MEASURED_PEAKS.json --
+ * measure"): the denominators of the "alu" roofline of HMAC-SHA256 (K10) and of the exp ceiling of attention (K3). -------------- */
+/* Runs a register-only micro-kernel (2,048 resident threads per SM, 8 independent chains per thread, no memory traffic in the
+ * timed loop) and returns thread-level operations per second (= lanes/clk/SM x SMs x clock) in *thread_ops_per_s, best of three
+ * launches timed with CUDA events on the context stream; *kernel_ms (may be NULL) = that launch's duration.
+ * mode 0: LOP3 + funnel shift + three-input add per step (the SHA-256 mix; ptxas spreads it over the ALU and FMA pipes: LOP3 +
+ * LEA.HI + IMAD.IADD, counted as 3 operations); 1: LOP3 only; 2: SHF only; 3: IADD3 only; 4: MUFU ex2.approx only.
+ * iters in [1, 2^20]: outer loop trips, 128 operations (x3 in mode 0) per thread and trip.  Synchronises.
+ * Errors: INVALID_ARG, CUDA. */
+int  anon_microbench(anon_ctx* ctx, int32_t mode, int32_t iters, double* thread_ops_per_s, double* kernel_ms);
+
 /* ---- NEXT-1: record splice (P:L53 stage 5 restricted to record text; S8f NEXT-1) ------------------------------- */
 /* Rewrites every record with each span [char_start, char_end) replaced by its pseudonym token:
  *   new_text = for each record, the bytes between spans copied, out_tokens[out_offsets[s] .. out_offsets[s+1]) in
@@ -304,14 +315,6 @@ int  anon_pipeline_host_text(anon_ctx* ctx, const anon_weights* w, anon_cache* c
  * d_A, d_W BF16 (uint16 bit patterns) row-major, 16-byte aligned.  Asynchronous. */
 int  anon_gemm_bf16(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,
                     const float* d_residual, void* d_C, int32_t M, int32_t N, int32_t K, int32_t epilogue);
-/* The residual GEMMs of the encoder with the LayerNorm fused into the epilogue (S8a A4, A6; S8c O1):
- *   x[M,N] = LN(A[M,K] * W[N,K]^T + bias + residual; gamma, beta)   (biased variance, eps inside the sqrt)
- * written as FP32 to d_x (which MAY alias d_residual: every row is read completely before it is written) and as
- * BF16 to d_xb.  N % 256 == 0 and K % 64 == 0 required (else ANON_ERR_UNSUPPORTED).  Uses a context-owned scratch
- * (allocated on first use).  Asynchronous. */
-int  anon_gemm_bf16_ln(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,
-                       const float* d_residual, const float* d_gamma, const float* d_beta, float eps,
-                       float* d_x, void* d_xb, int32_t M, int32_t N, int32_t K);
 /* ctx[T,H] = varlen bidirectional softmax attention over qkv[T,3H] (S8a A3); dtype as in
  * anon_model_desc (0: FP32 qkv/ctx, 1: BF16).  h_cu_seqlens is a HOST pointer.  Asynchronous. */
 int  anon_attention(anon_ctx* ctx, const void* d_qkv, const int32_t* d_cu_seqlens,

@@ -73,7 +73,6 @@ _SIGNATURES = {
     "anon_ctx_profile": (ctypes.c_int, [_vp, ctypes.c_int]),
     "anon_ctx_profile_read": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "anon_gemm_bf16": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32]),
-    "anon_gemm_bf16_ln": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp, _vp, _i32, _i32, _i32]),
     "anon_splice_records": (ctypes.c_int, [_vp, _vp, _sz, _vp, _i32, _vp, _i32, _vp, _vp, _vp, _sz, _vp]),
     "anon_attention": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32, _i32, _vp]),
     "anon_attention_local": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i32, _i32, _i32, _i32, _i32, _vp]),
@@ -82,6 +81,7 @@ _SIGNATURES = {
     "anon_regex_scan": (ctypes.c_int, [_vp, _vp, _vp, _sz, _vp, _i32, _vp, _i32, _vp]),
     "anon_merge_spans": (ctypes.c_int, [_vp, _vp, _vp, _i32, _vp, _vp, _i32, _vp, _i32, _vp]),
     "anon_ctx_set_regex": (ctypes.c_int, [_vp, _vp]),
+    "anon_microbench": (ctypes.c_int, [_vp, _i32, _i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
 }
 
 
@@ -341,13 +341,6 @@ def anon_ctx_set_regex(ctx, regex):
     ctx._regex = regex            # keeps the handle alive while attached
 
 
-def anon_gemm_bf16_ln(ctx, A, W, bias, residual, gamma, beta, eps, x, xb):
-    M, K = A.shape
-    N = W.shape[0]
-    ctx.check(lib().anon_gemm_bf16_ln(ctx._h, _ptr(A), _ptr(W), _ptr(bias), _ptr(residual), _ptr(gamma), _ptr(beta), eps,
-                                      _ptr(x), _ptr(xb), M, N, K), "anon_gemm_bf16_ln")
-
-
 def anon_attention(ctx, qkv, cu_seqlens_dev, cu_seqlens_host, hidden, heads, dtype, out):
     h = np.ascontiguousarray(cu_seqlens_host, np.int32)
     ctx.check(lib().anon_attention(ctx._h, _ptr(qkv), _ptr(cu_seqlens_dev), h.ctypes.data, h.size - 1, qkv.shape[0],
@@ -391,3 +384,10 @@ def anon_pipeline_host(ctx, weights, cache, token_ids, cu_seqlens, meta, text, r
         res["new_record_offsets"] = ro
         res["new_text"] = bufs["new_text"][:ro[R]]
     return res
+
+
+def anon_microbench(ctx, mode, iters=2048):
+    """Measured issue rate of the integer-ALU (modes 0-3) or MUFU ex2 (mode 4) pipe: (thread-ops per second, kernel ms)."""
+    ops, ms = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    ctx.check(lib().anon_microbench(ctx._h, mode, iters, ctypes.byref(ops), ctypes.byref(ms)), "anon_microbench")
+    return ops.value, ms.value

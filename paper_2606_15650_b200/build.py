@@ -13,9 +13,9 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 SO = os.path.join(HERE, "libanonshield.so")
 STAMP = SO + ".stamp"
-SOURCES = ["api.cu", "crypto.cu", "decode.cu", "regex.cu", "encoder.cu", "attention_bf16.cu", "gemm_tcgen05.cu"]
+SOURCES = ["api.cu", "crypto.cu", "decode.cu", "regex.cu", "encoder.cu", "attention_bf16.cu", "gemm_tcgen05.cu", "microbench.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-cudart", "static"]
+              "-Xcompiler", "-fPIC", "-cudart", "static"] + os.environ.get("ANON_NVCC_EXTRA", "").split()
 
 
 def _nvcc():

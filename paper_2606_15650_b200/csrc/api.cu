@@ -23,8 +23,8 @@ extern "C" const char* const* anon_exported_symbols(void) {
         "anon_last_cuda_error", "anon_workspace_bytes", "anon_weights_load", "anon_weights_free", "anon_ner_forward",
         "anon_decode_spans", "anon_gather_spans", "anon_cache_create", "anon_cache_destroy", "anon_cache_stats", "anon_cache_clear",
         "anon_cache_entry", "anon_cache_export", "anon_pseudonymize", "anon_hmac_spans", "anon_pipeline_host", "anon_gemm_bf16",
-        "anon_attention", "anon_gemm_bf16_ln", "anon_splice_records", "anon_pipeline_host_text", "anon_ctx_profile", "anon_ctx_profile_read",
-        "anon_regex_load", "anon_regex_free", "anon_regex_scan", "anon_merge_spans", "anon_ctx_set_regex", "anon_attention_local", "anon_cache_track_use", "anon_cache_evict", nullptr};
+        "anon_attention", "anon_splice_records", "anon_pipeline_host_text", "anon_ctx_profile", "anon_ctx_profile_read",
+        "anon_regex_load", "anon_regex_free", "anon_regex_scan", "anon_merge_spans", "anon_ctx_set_regex", "anon_attention_local", "anon_cache_track_use", "anon_cache_evict", "anon_microbench", nullptr};
     return names;
 }
 
@@ -59,7 +59,6 @@ extern "C" void anon_ctx_destroy(anon_ctx* c) {
     if (!c) return;
     for (auto& r : c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     cudaFree(c->ws);
-    cudaFree(c->ln_scratch);
     cudaFree(c->d_status);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
     delete c;

@@ -34,7 +34,8 @@ constexpr int kAttThreads = 192;
 constexpr int kQBytes = kQT * kD * 2;          // 16 KB
 constexpr int kKVBytes = kKC * kD * 2;         // 8 KB (K and V each)
 constexpr int kAttSmem = 2 * kQBytes + kKVStages * 2 * kKVBytes + 1024 /*align slack*/ + 256 /*barriers*/;
-constexpr int kAttTmemCols = 256;              // S/P buffers 2 x 64, O buffers 2 x 64
+constexpr int kAttTmemCols = 256;              // S 2 x 64 | P 2 x 32 | O 64
+constexpr int kPolyEvery = 4;                  // every 4th pair of a row takes its exponentials on the FMA pipe (25 %)
 
 // rows relative to the chunk.  Global attention: kv_row0 = the sequence's first row, n = its length.  Local (band) attention
 // (NEXT-3, D20): kv_row0 = first key row any query of the tile may see, n = keys from there, and q_valid carries
@@ -59,6 +60,25 @@ __device__ __forceinline__ uint32_t pack2(float a, float b) {
     return *reinterpret_cast<uint32_t*>(&v);
 }
 
+// 2^t for a packed pair on the FMA pipe (no MUFU): Cody-Waite split t = i + f, i = round(t) via the 1.5 * 2^23 magic add,
+// f in [-0.5, 0.5]; 2^f by a degree-3 minimax polynomial (relative error 7.5e-5, ~50x below the BF16 rounding of P); the
+// integer part goes straight into the exponent field (the magic sum carries i in its low mantissa bits: one shift-add).
+// t is clamped at -126 so the exponent field cannot wrap (masked scores are -inf; the result is then ~1e-38, i.e. 0).
+__device__ __forceinline__ void exp2_pair_fma(uint64_t t, float& p0, float& p1) {
+    float t0, t1;
+    upk2(t, t0, t1);
+    const uint64_t tc = pk2(fmaxf(t0, -126.f), fmaxf(t1, -126.f));
+    const uint64_t rr = add2(tc, pk2(12582912.f, 12582912.f));
+    const uint64_t f = fma2(add2(rr, pk2(-12582912.f, -12582912.f)), pk2(-1.f, -1.f), tc);
+    uint64_t p = fma2(pk2(0.0551716685f, 0.0551716685f), f, pk2(0.2426111251f, 0.2426111251f));
+    p = fma2(p, f, pk2(0.6932609677f, 0.6932609677f));
+    p = fma2(p, f, pk2(0.9999280572f, 0.9999280572f));
+    float q0, q1, r0, r1;
+    upk2(p, q0, q1); upk2(rr, r0, r1);
+    p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(r0) << 23));
+    p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(r1) << 23));
+}
+
 template <bool BAND>
 __global__ void __launch_bounds__(kAttThreads, 2)
 attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_kv,
@@ -73,12 +93,12 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
     auto q_empty = [&](uint32_t i) { return bar_base + 8u * (2 + i); };
     auto kv_full = [&](uint32_t i) { return bar_base + 8u * (4 + i); };
     auto kv_empty = [&](uint32_t i) { return bar_base + 8u * (8 + i); };
-    auto s_full = [&](uint32_t i) { return bar_base + 8u * (12 + i); };
-    auto p_full = [&](uint32_t i) { return bar_base + 8u * (14 + i); };
-    auto pv_done = [&](uint32_t i) { return bar_base + 8u * (16 + i); };
-    auto o_full = [&](uint32_t i) { return bar_base + 8u * (18 + i); };
-    auto o_empty = [&](uint32_t i) { return bar_base + 8u * (20 + i); };
-    const uint32_t tmem_slot = bar_base + 8u * 22;
+    auto s_full = [&](uint32_t i) { return bar_base + 8u * (12 + i); };    // S chunk computed (MMA commit)
+    auto p_full = [&](uint32_t i) { return bar_base + 8u * (14 + i); };    // P chunk written (4 softmax warps)
+    auto pv_done = [&](uint32_t i) { return bar_base + 8u * (16 + i); };   // PV of the chunk in P buffer i has completed
+    auto s_free = [&](uint32_t i) { return bar_base + 8u * (22 + i); };    // S buffer i has been read into registers (4 warps)
+    const uint32_t o_full = bar_base + 8u * 18, o_empty = bar_base + 8u * 20;
+    const uint32_t tmem_slot = bar_base + 8u * 24;
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -91,8 +111,9 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
         for (uint32_t i = 0; i < 2; i++) {
             ptx::mbar_init(q_full(i), 1); ptx::mbar_init(q_empty(i), 1);
             ptx::mbar_init(s_full(i), 1); ptx::mbar_init(p_full(i), 4); ptx::mbar_init(pv_done(i), 1);
-            ptx::mbar_init(o_full(i), 1); ptx::mbar_init(o_empty(i), 4);
+            ptx::mbar_init(s_free(i), 4);
         }
+        ptx::mbar_init(o_full, 1); ptx::mbar_init(o_empty, 4);
         for (uint32_t i = 0; i < kKVStages; i++) { ptx::mbar_init(kv_full(i), 1); ptx::mbar_init(kv_empty(i), 1); }
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
@@ -104,8 +125,10 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
+    // TMEM columns: S buffers 2 x 64 (FP32 scores) | P buffers 2 x 32 (BF16 pairs, 64 keys each) | O 64 (FP32 accumulator)
     const uint32_t tmem_base = *tmem_slot_ptr;
-    const uint32_t tmem_o = tmem_base + 128u;
+    const uint32_t tmem_p = tmem_base + 128u;
+    const uint32_t tmem_o = tmem_base + 192u;
 
     if (warp == 0) {
         // ===== TMA producer =====
@@ -132,7 +155,9 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer: two cursors over the flattened (unit, chunk) sequence, QK^T one chunk ahead of PV =====
+        // ===== MMA issuer: two cursors over the flattened (unit, chunk) sequence.  QK^T runs TWO chunks ahead of PV: S(g+2) is
+        // issued as soon as the softmax warps have pulled S(g) into registers (s_free), not when P(g) has been consumed -- P has
+        // TMEM columns of its own -- so a finished chunk never waits for the tensor pipe's round trip =====
         if (lane == 0) {
             constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(kQT, kKC);          // both operands K-major
             constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(kQT, kD, 1);        // B = V is MN-major
@@ -146,6 +171,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             Cur a{(int)blockIdx.x, 0, chunks_of((int)blockIdx.x), chunks_of((int)blockIdx.x + (int)gridDim.x), 0u, 0u}, b = a;
             auto issue_qk = [&]() {
                 const uint32_t qb = a.qi & 1u, st = a.g % kKVStages, sb = a.g & 1u;
+                if (a.g >= 2u) ptx::mbar_wait(s_free(sb), ((a.g - 2u) >> 1) & 1u);   // S(g-2) has left this buffer
                 if (a.c == 0) ptx::mbar_wait(q_full(qb), (a.qi >> 1) & 1u);
                 ptx::mbar_wait(kv_full(st), (a.g / kKVStages) & 1u);
                 ptx::tc_fence_after();
@@ -158,23 +184,23 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 if (a.c == a.nc - 1) ptx::mma_commit(q_empty(qb));       // last use of this Q tile
             };
             auto issue_pv = [&]() {
-                const uint32_t st = b.g % kKVStages, sb = b.g & 1u, ob = b.qi & 1u;
+                const uint32_t st = b.g % kKVStages, sb = b.g & 1u;
                 ptx::mbar_wait(p_full(sb), (b.g >> 1) & 1u);
-                if (b.c == 0) ptx::mbar_wait(o_empty(ob), ((b.qi >> 1) & 1u) ^ 1u);
+                if (b.c == 0) ptx::mbar_wait(o_empty, (b.qi & 1u) ^ 1u);  // the previous unit's O has been read (finalize)
                 ptx::tc_fence_after();
                 const uint64_t vd = ptx::make_desc_mn_sw128(kv_smem + st * 2 * kKVBytes + kKVBytes);
 #pragma unroll
                 for (int k = 0; k < kKC / 16; k++)                       // 16 keys per MMA: 8 TMEM columns of P, 2 KB of V
-                    ptx::mma_f16_ts(tmem_o + ob * 64u, tmem_base + sb * 64u + 8u * k, vd + (uint64_t)(128 * k), idesc_pv,
-                                    (b.c | k) ? 1u : 0u);
+                    ptx::mma_f16_ts(tmem_o, tmem_p + sb * 32u + 8u * k, vd + (uint64_t)(128 * k), idesc_pv, (b.c | k) ? 1u : 0u);
                 ptx::mma_commit(kv_empty(st));
                 ptx::mma_commit(pv_done(sb));
-                if (b.c == b.nc - 1) ptx::mma_commit(o_full(ob));
+                if (b.c == b.nc - 1) ptx::mma_commit(o_full);
             };
             if (a.nc) { issue_qk(); advance(a); }
+            if (a.nc) { issue_qk(); advance(a); }
             while (b.nc) {
-                if (a.nc) { issue_qk(); advance(a); }
-                issue_pv();
+                if (a.nc) { issue_qk(); advance(a); }        // S(g+2): gated by s_free(g), early in the softmax of chunk g
+                issue_pv();                                  // PV(g): gated by p_full(g), the end of that softmax
                 advance(b);
             }
         }
@@ -186,19 +212,19 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
         const float sc = 0.125f * 1.4426950408889634f;                   // 1/sqrt(64) * log2(e)
         uint32_t qi = 0, g = 0;
         bool pend = false;
-        uint32_t pend_ob = 0, pend_par = 0;
+        uint32_t pend_par = 0;
         float pend_l = 1.f;
         int pend_row0 = 0, pend_valid = 0, pend_head = 0;
         auto finalize = [&]() {                                          // O / l -> BF16 row of ctx
-            ptx::mbar_wait(o_full(pend_ob), pend_par);
+            ptx::mbar_wait(o_full, pend_par);
             ptx::tc_fence_after();
             uint32_t o[64];
-            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + pend_ob * 64u, o);
-            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + pend_ob * 64u + 32u, o + 32);
+            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base, o);
+            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + 32u, o + 32);
             ptx::tmem_ld_wait();
             ptx::tc_fence_before();
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(o_empty(pend_ob));
+            if (lane == 0) ptx::mbar_arrive(o_empty);
             if (row < pend_valid) {
                 const float inv = 1.0f / pend_l;
                 uint4* dst = reinterpret_cast<uint4*>(ctx + (size_t)(pend_row0 + row) * H + pend_head * kD);
@@ -226,6 +252,11 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 if ((int)quarter * 32 >= (w.q_valid & 0xff)) {           // no query of this warp is real: P rows are don't-care
                     ptx::tc_fence_before();
                     __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(s_free(sb));
+                    // like the working warps, do not signal P(g) before PV(g-2) is done: a warp that ran two chunks ahead
+                    // would otherwise arrive on the phase of chunk g-2 and let PV start before the others have written P
+                    if (g >= 2u) ptx::mbar_wait(pv_done(sb), ((g - 2u) >> 1) & 1u);
+                    __syncwarp();
                     if (lane == 0) ptx::mbar_arrive(p_full(sb));
                     if (c == 0 && pend) finalize();
                     continue;
@@ -234,6 +265,9 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 ptx::tmem_ld_32x32b_x32(t_s, r);
                 ptx::tmem_ld_32x32b_x32(t_s + 32u, r + 32);
                 ptx::tmem_ld_wait();
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(s_free(sb));             // the scores are in registers: S(g+2) may overwrite the buffer
                 const int valid = w.n - c * kKC;                         // keys of this chunk that belong to the sequence
                 if (valid < kKC) {
 #pragma unroll
@@ -262,17 +296,16 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     float alpha = 1.0f;
                     if (mnew > m) { alpha = ex2f(m - mnew); m = mnew; l *= alpha; }
                     if (c > 0) {                                         // rescale O in TMEM once PV(g-1) has landed
-                        const uint32_t t_o = tmem_o + lane_base + (qi & 1u) * 64u;
                         ptx::mbar_wait(pv_done((g - 1u) & 1u), ((g - 1u) >> 1) & 1u);
                         ptx::tc_fence_after();
 #pragma unroll
                         for (int hh = 0; hh < 2; hh++) {
                             uint32_t o[32];
-                            ptx::tmem_ld_32x32b_x32(t_o + 32u * hh, o);
+                            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + 32u * hh, o);
                             ptx::tmem_ld_wait();
 #pragma unroll
                             for (int j = 0; j < 32; j++) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
-                            ptx::tmem_st_32x32b_x32(t_o + 32u * hh, o);
+                            ptx::tmem_st_32x32b_x32(tmem_o + lane_base + 32u * hh, o);
                         }
                         ptx::tmem_st_wait();
                     }
@@ -299,9 +332,10 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     }
 #pragma unroll
                     for (int j = 16 * hh; j < 16 * hh + 16; j++) {
-                        float t0, t1;
-                        upk2(fma2(pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])), sc2, nm2), t0, t1);
-                        const float p0 = ex2f(t0), p1 = ex2f(t1);
+                        const uint64_t t = fma2(pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])), sc2, nm2);
+                        float p0, p1;
+                        if ((j % kPolyEvery) == kPolyEvery - 1) exp2_pair_fma(t, p0, p1);      // FMA-pipe exponential
+                        else { float t0, t1; upk2(t, t0, t1); p0 = ex2f(t0); p1 = ex2f(t1); }  // MUFU
                         if (j & 1) sum_b = add2(sum_b, pk2(p0, p1)); else sum_a = add2(sum_a, pk2(p0, p1));
                         pk[j] = pack2(p0, p1);
                     }
@@ -311,7 +345,11 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     upk2(add2(sum_a, sum_b), s0, s1);
                     l += s0 + s1;
                 }
-                ptx::tmem_st_32x32b_x32(t_s, pk);                        // P over the first 32 columns of the S buffer
+                if (g >= 2u) {                                           // PV(g-2) has finished reading this P buffer
+                    ptx::mbar_wait(pv_done(sb), ((g - 2u) >> 1) & 1u);
+                    ptx::tc_fence_after();
+                }
+                ptx::tmem_st_32x32b_x32(tmem_p + lane_base + sb * 32u, pk);
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
@@ -320,7 +358,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             }
             // the O / l write-back of this unit is deferred until after the first chunk of the next one, so that the
             // wait for the last PV overlaps useful work
-            pend = true; pend_ob = qi & 1u; pend_par = (qi >> 1) & 1u; pend_l = l;
+            pend = true; pend_par = qi & 1u; pend_l = l;
             pend_row0 = w.q_row0; pend_valid = w.q_valid & 0xff; pend_head = head;
         }
         if (pend) finalize();

@@ -37,9 +37,6 @@ struct anon_ctx {
     const void* smem_attr_done[48] = {nullptr};
     int n_smem_attr_done = 0;
     long long chunk_tokens_cap = 0;     // ANON_CHUNK_TOKENS read once at context creation (0 = workspace-limited only)
-    // L2-resident scratch of the fused residual+LayerNorm GEMM epilogue (allocated on first use, grows only)
-    void* ln_scratch = nullptr;
-    size_t ln_scratch_bytes = 0;
     // NEXT-4: pattern automaton the host pipeline merges into the NER spans (anon_ctx_set_regex; not owned)
     const struct anon_regex* regex = nullptr;
     // launch accounting + optional event profiling
@@ -133,9 +130,6 @@ int gemm_bf16_res_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16
 // qkv = A W^T, RoPE on the q / k heads in the epilogue; table float2 [32][512] pair-major (cos, sin), pos int [M]
 int gemm_bf16_rope_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const int* pos, const float2* table, void* C,
                         int M, int N, int K);
-// x = LN(A W^T + bias + residual; gamma, beta) as FP32 (x_out may alias residual) plus its BF16 copy; N % 256 == 0
-int gemm_bf16_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
-                      const float* gamma, const float* beta, float eps, float* x_out, __nv_bfloat16* xb_out, int M, int N, int K);
 // 2-D row-major tensor [rows, cols] of esize-byte elements, box [box_rows, box_cols] with box_cols * esize = 128 B,
 // 128-byte swizzle (gemm_tcgen05.cu).
 int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_t esize, const void* base, uint64_t rows,

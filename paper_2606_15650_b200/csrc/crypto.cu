@@ -42,7 +42,7 @@ struct anon_cache {
 };
 
 struct PadStates { uint32_t ipad[8], opad[8]; };
-struct TypeTable { uint8_t len[64]; char name[64][32]; int num; };
+struct TypeTable { uint8_t len[64]; alignas(4) char name[64][32]; int num; };
 
 // ------------------------------------------------------------------------------------------------
 // byte-stream helpers: read a message at any alignment as little-endian 32-bit words
@@ -95,23 +95,34 @@ __device__ __forceinline__ uint32_t tail_mask(int len, int j) {
     return rem >= 4 ? 0xFFFFFFFFu : (rem <= 0 ? 0u : (1u << (8 * rem)) - 1u);
 }
 
+// 64-bit hash of a byte string from four independent 32-bit lanes (one per word of a 16-byte chunk), each step
+// acc = rotl(acc + w * P2, 13) * P1 -- two IMAD and one SHF per word instead of a 64-bit multiply chain per word (the probe
+// kernel was instruction-bound with 34 % of its issue slots in IMAD; profiles/r02_pseudonym.md).  Words past the end of the
+// message enter as zeros (only the last chunk is masked) and the length is mixed in at the end, so strings that differ only
+// in trailing zero bytes still hash differently.  Only performance depends on the quality: equality is always decided by the
+// full byte compare.
 __device__ __forceinline__ u64 hash_bytes(const uint8_t* p, int len) {
-    u64 h = 0x9E3779B97F4A7C15ull ^ ((u64)(uint32_t)len * 0xFF51AFD7ED558CCDull);
+    constexpr uint32_t P1 = 0x9E3779B1u, P2 = 0x85EBCA77u, P3 = 0xC2B2AE3Du, P4 = 0x27D4EB2Fu;
+    uint32_t a0 = 0x243F6A88u, a1 = 0x85A308D3u, a2 = 0x13198A2Eu, a3 = 0x03707344u;
     const int nw = (len + 3) >> 2;
     Words16 ws; ws.init(p, len);
     for (int j = 0; j < nw; j += 4) {
         uint32_t w[4];
         ws.next4(w);
+        if (j + 4 >= nw) {                            // last chunk: drop the bytes past the end
 #pragma unroll
-        for (int k = 0; k < 4; k++) {
-            if (j + k < nw) {
-                h = (h ^ (w[k] & tail_mask(len, j + k))) * 0xD6E8FEB86659FD93ull;
-                h ^= h >> 32;
-            }
+            for (int k = 0; k < 4; k++) w[k] &= tail_mask(len, j + k);
         }
+        a0 = __funnelshift_l(a0 + w[0] * P2, a0 + w[0] * P2, 13) * P1;
+        a1 = __funnelshift_l(a1 + w[1] * P2, a1 + w[1] * P2, 13) * P1;
+        a2 = __funnelshift_l(a2 + w[2] * P2, a2 + w[2] * P2, 13) * P1;
+        a3 = __funnelshift_l(a3 + w[3] * P2, a3 + w[3] * P2, 13) * P1;
     }
-    h ^= h >> 33; h *= 0xFF51AFD7ED558CCDull; h ^= h >> 33; h *= 0xC4CEB9FE1A85EC53ull; h ^= h >> 33;
-    return h;
+    uint32_t lo = __funnelshift_l(a0, a0, 1) + __funnelshift_l(a1, a1, 7) + __funnelshift_l(a2, a2, 12) + __funnelshift_l(a3, a3, 18) + (uint32_t)len;
+    uint32_t hi = (a0 ^ __funnelshift_l(a1, a1, 15)) * P3 + (a2 ^ __funnelshift_l(a3, a3, 9)) * P4 + (uint32_t)len * P1;
+    lo ^= lo >> 15; lo *= P2; lo ^= lo >> 13; lo *= P3; lo ^= lo >> 16;
+    hi ^= hi >> 16; hi *= P1; hi ^= hi >> 13; hi *= P4; hi ^= hi >> 15;
+    return ((u64)hi << 32) | lo;
 }
 
 __device__ __forceinline__ bool bytes_equal(const uint8_t* a, const uint8_t* b, int len) {
@@ -120,9 +131,14 @@ __device__ __forceinline__ bool bytes_equal(const uint8_t* a, const uint8_t* b, 
     for (int j = 0; j < nw; j += 4) {
         uint32_t x[4], y[4];
         wa.next4(x); wb.next4(y);
-        uint32_t diff = 0;
+        uint32_t diff;
+        if (j + 4 >= nw) {                            // last chunk: ignore the bytes past the end
+            diff = 0;
 #pragma unroll
-        for (int k = 0; k < 4; k++) diff |= (x[k] ^ y[k]) & tail_mask(len, j + k);
+            for (int k = 0; k < 4; k++) diff |= (x[k] ^ y[k]) & tail_mask(len, j + k);
+        } else {
+            diff = (x[0] ^ y[0]) | (x[1] ^ y[1]) | (x[2] ^ y[2]) | (x[3] ^ y[3]);
+        }
         if (diff) return false;
     }
     return true;
@@ -306,10 +322,16 @@ __global__ void __launch_bounds__(kEmitWarps * 32) emit_tokens_kernel(
     long long* uid_out, uint8_t* dig_out, TypeTable tt, int slug_len, int* d_status, uint32_t* last_use, uint32_t epoch)
 {
     __shared__ __align__(16) uint8_t s_tok[kEmitWarps][(kEmitWarpBytes + 15) / 16 * 16];
-    __shared__ uint8_t s_name[64][32];
+    __shared__ __align__(16) uint8_t s_name[64][32];
     __shared__ uint8_t s_len[64];
-    for (int k = threadIdx.x; k < 64 * 32; k += blockDim.x) s_name[k >> 5][k & 31] = (uint8_t)tt.name[k >> 5][k & 31];
-    if (threadIdx.x < 64) s_len[threadIdx.x] = tt.len[threadIdx.x];
+    // the table arrives as a kernel parameter (constant bank): a lane-varying index into it is serialised per distinct address
+    // (ncu: ADU pipe 93 % busy when all 64 x 32 bytes were copied byte by byte), so only the num live names are copied, as words
+    {
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(&tt.name[0][0]);
+        uint32_t* dst = reinterpret_cast<uint32_t*>(&s_name[0][0]);
+        for (int k = threadIdx.x; k < tt.num * 8; k += blockDim.x) dst[k] = src[k];
+        if (threadIdx.x < tt.num) s_len[threadIdx.x] = tt.len[threadIdx.x];
+    }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long i0 = ((long long)blockIdx.x * kEmitWarps + warp) * 32;

@@ -359,11 +359,6 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
     if (T == 0) return ANON_OK;
     const int H = d.hidden, F = d.ffn, NL = d.num_labels;
     const bool bf = d.dtype == 1;
-    // The residual + LayerNorm GEMM epilogue (gemm_tcgen05.cu EPI 3, anon_gemm_bf16_ln) is correct but, measured in
-    // the step on B200, slower than the residual GEMM + LayerNorm kernel pair (its second pass over the row block
-    // serialises with the mainloop; profiles/r01_summary.md "r01c").  It stays off until the pass is pipelined.
-    const bool fused_ln = false;
-    const bool fused_ffn2 = false;
     cudaStream_t st = ctx->stream;
 
     // chunk budget: whole sequences, as many tokens as the remaining workspace holds (optionally capped)
@@ -460,38 +455,24 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                 { ProfScope ps(ctx, PROF_ATTN, attn_flops);
                 rc = attention_run(ctx, plan, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx); }
                 if (rc) return rc;
-                if (fused_ln) {       // out-projection + residual + LayerNorm in one kernel, x updated in place
-                    ProfScope ps(ctx, PROF_GEMM_OUT, 2.0 * nt * H * H);
-                    rc = gemm_bf16_ln_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, L.g_1, L.b_1,
-                                           d.ln_eps, x, xb, nt, H, H);
-                    if (rc) return rc;
-                } else {
-                    { ProfScope ps(ctx, PROF_GEMM_OUT, 2.0 * nt * H * H);
-                    if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, y, nt, H, H, 2);
-                    else rc = sgemm<2>(ctx, (const float*)cx, (const float*)L.W_o, L.b_o, x, y, nt, H, H); }
-                    if (rc) return rc;
-                    { ProfScope ps(ctx, PROF_ROW, row_bytes);
-                    launch_layer_norm(st, row_grid, y, nt, H, L.g_1, L.b_1, d.ln_eps, x, xb); }
-                    CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
-                }
+                { ProfScope ps(ctx, PROF_GEMM_OUT, 2.0 * nt * H * H);
+                if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, y, nt, H, H, 2);
+                else rc = sgemm<2>(ctx, (const float*)cx, (const float*)L.W_o, L.b_o, x, y, nt, H, H); }
+                if (rc) return rc;
+                { ProfScope ps(ctx, PROF_ROW, row_bytes);
+                launch_layer_norm(st, row_grid, y, nt, H, L.g_1, L.b_1, d.ln_eps, x, xb); }
+                CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
                 { ProfScope ps(ctx, PROF_GEMM_FFN1, 2.0 * nt * F * H);
                 if (bf) rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_1, L.b_1f, nullptr, f, nt, F, H, 1);
                 else rc = sgemm<1>(ctx, x, (const float*)L.W_1, L.b_1f, nullptr, (float*)f, nt, F, H); }
                 if (rc) return rc;
-                if (fused_ln && fused_ffn2) {
-                    ProfScope ps(ctx, PROF_GEMM_FFN2, 2.0 * nt * F * H);
-                    rc = gemm_bf16_ln_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, x, L.g_2, L.b_2,
-                                           d.ln_eps, x, xb, nt, H, F);
-                    if (rc) return rc;
-                } else {
-                    { ProfScope ps(ctx, PROF_GEMM_FFN2, 2.0 * nt * F * H);
-                    if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, x, y, nt, H, F, 2);
-                    else rc = sgemm<2>(ctx, (const float*)f, (const float*)L.W_2, L.b_2f, x, y, nt, H, F); }
-                    if (rc) return rc;
-                    { ProfScope ps(ctx, PROF_ROW, row_bytes);
-                    launch_layer_norm(st, row_grid, y, nt, H, L.g_2, L.b_2, d.ln_eps, x, xb); }
-                    CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
-                }
+                { ProfScope ps(ctx, PROF_GEMM_FFN2, 2.0 * nt * F * H);
+                if (bf) rc = gemm_bf16_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, x, y, nt, H, F, 2);
+                else rc = sgemm<2>(ctx, (const float*)f, (const float*)L.W_2, L.b_2f, x, y, nt, H, F); }
+                if (rc) return rc;
+                { ProfScope ps(ctx, PROF_ROW, row_bytes);
+                launch_layer_norm(st, row_grid, y, nt, H, L.g_2, L.b_2, d.ln_eps, x, xb); }
+                CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
             }
             { ProfScope ps(ctx, PROF_ROW, (double)nt * (H * 4 + (d_logits ? NL * 4 : 0) + (d_labels ? 4 : 0)));
             enc::launch_head_argmax(st, head_in, nt, H, w->W_c, w->b_c, NL, d_logits ? d_logits + (size_t)tok0 * NL : nullptr,

@@ -40,9 +40,8 @@ constexpr int kRopeStride = 512;   // positions per pair row of the EPI 5 (cos, 
 template <int BN, int EPI, int NB, int CG> struct Cfg {
     static constexpr int B_STAGE_BYTES = (BN / CG) * BK * 2;
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
-    static constexpr int EPI_WARPS = (EPI == 2 || EPI == 3) ? 4 : 8;
-    static constexpr int PAR_BYTES = 3 * 1024 * 4;                // EPI 3: bias, gamma, beta staged in shared memory (N <= 1024)
-    static constexpr int EPI_BYTES = (EPI == 3) ? 4 * (NB + 1) * 4096 + PAR_BYTES : (EPI == 2) ? 4 * NB * 4096 + 12288 /*bias, gamma, beta staged for the epilogue*/ : 8 * 4096;   // 4 KB boxes
+    static constexpr int EPI_WARPS = (EPI == 2) ? 4 : 8;
+    static constexpr int EPI_BYTES = (EPI == 2) ? 4 * NB * 4096 + 12288 /*bias, gamma, beta staged for the epilogue*/ : 8 * 4096;   // 4 KB boxes
     static constexpr int STAGES = (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES > 6 ? 6 : (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES;
     static constexpr int TMEM_COLS = 2 * BN;                      // two accumulator buffers
     static constexpr int NUM_BARS = 2 * STAGES + 4 + 32;
@@ -118,7 +117,7 @@ __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
 }
 
 // EPI: 0 = +bias -> BF16;  1 = +bias, GELU -> BF16;  2 = +bias +residual(FP32) -> FP32;
-//      3 = LayerNorm(+bias +residual) -> FP32 x and BF16 xb (whole rows per CTA pair, see the EPI 3 branch)
+//          (with res_stats: the residual is stored un-normalised and LayerNorm'ed on the fly, see gemm_bf16_res_ln_impl)
 //      4 = GeGLU (NEXT-3): the tile's first BN/2 accumulator columns are a, the last BN/2 their gates (W's rows are
 //          interleaved per tile by the caller); writes gelu(a) * gate as BF16 [M, N/2]; no bias
 //      5 = QKV projection with rotary position embedding (NEXT-3): like 0 without bias; in the q and k column blocks
@@ -129,9 +128,8 @@ template <int BN, int EPI, int NB, int CG>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                          const __grid_constant__ CUtensorMap tmap_c, const __grid_constant__ CUtensorMap tmap_r,
-                         const __grid_constant__ CUtensorMap tmap_y, const __grid_constant__ CUtensorMap tmap_xb,
                          const float* __restrict__ bias, const float* __restrict__ ln_g, const float* __restrict__ ln_b,
-                         float ln_eps, const float2* __restrict__ res_stats, const float2* __restrict__ rope_tab,
+                         const float2* __restrict__ res_stats, const float2* __restrict__ rope_tab,
                          const int* __restrict__ rope_pos, int M, int N, int K)
 {
     using C = Cfg<BN, EPI, NB, CG>;
@@ -154,10 +152,8 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
     const int num_m = (M + TM - 1) / TM, num_n = (N + BN - 1) / BN;
     const int num_tiles = num_m * num_n;
     const int num_kb = K / BK;
-    // local tile lt of this CTA (pair) -> (m_blk, n_blk).  EPI 3 walks all n-tiles of one row block before the next row
-    // block (the LayerNorm needs whole rows); the other epilogues take tiles round-robin.
+    // local tile lt of this CTA (pair) -> (m_blk, n_blk)
     auto get_tile = [&](int lt, int& m_blk, int& n_blk) -> bool {
-        if (EPI == 3) { m_blk = cid + (lt / num_n) * ncl; n_blk = lt % num_n; return m_blk < num_m; }
         if ((EPI <= 1 || EPI >= 4) && num_m >= 2 * ncl) {
             // short-K GEMMs with many row blocks: a pair keeps its row block of A (256 x K, L2-resident across the
             // pairs) for all n-tiles, starting at a different n so that the pairs do not ask for the same W tile at once
@@ -173,7 +169,6 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         ptx::prefetch_tensormap(&tmap_b);
         ptx::prefetch_tensormap(&tmap_c);
         if (EPI >= 2) ptx::prefetch_tensormap(&tmap_r);
-        if (EPI == 3) { ptx::prefetch_tensormap(&tmap_y); ptx::prefetch_tensormap(&tmap_xb); }
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < C::STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
@@ -181,10 +176,6 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         for (int i = 0; i < 32; i++) ptx::mbar_init(rfull_bar(i >> 3, i & 7), 1);
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
-    }
-    if constexpr (EPI == 3) {             // bias / gamma / beta -> shared memory (every thread reads all N of them per row)
-        float* par = reinterpret_cast<float*>(smem_raw + (epi_base + 4 * (NB + 1) * 4096 - ptx::smem_u32(smem_raw)));
-        for (int i = threadIdx.x; i < N; i += kThreads) { par[i] = bias[i]; par[1024 + i] = ln_g[i]; par[2048 + i] = ln_b[i]; }
     }
     if constexpr (EPI == 2) {             // bias (and gamma / beta of the residual's LayerNorm) -> shared memory: every
         if (N <= 1024) {                  // epilogue thread reads all N of them per row
@@ -272,158 +263,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         uint32_t nbox = 0;                            // boxes this warp has handled (buffer ring position)
         (void)nbox;
 
-        if constexpr (EPI == 3) {
-            // ---- fused residual + LayerNorm: x = LN(acc + bias + residual), rows owned by one thread each ----
-            // Pass 1 (per n-tile, as EPI 2): v = acc + bias + residual computed in place in the TMA-loaded residual box,
-            //   stored to a per-pair scratch (L2-resident: the same 256 rows x N FP32 are rewritten for every row block),
-            //   while the thread merges each 32-value chunk into its row's running (count, mean, M2) -- Chan's
-            //   parallel update, numerically a two-pass variance.
-            // Pass 2 (after the last n-tile of the row block): the v boxes come back by TMA, are normalised with
-            //   gamma / beta in place and leave as the FP32 residual stream x plus its BF16 copy xb.
-            // Boxes of both passes run through one ring of NB 4 KB buffers per warp, loads issued NB-1 boxes ahead.
-            constexpr int BPT = BN / 32;
-            const int nbt = num_n * BPT;                  // v boxes per row block and warp
-            const uint32_t stg = epi_base + (uint32_t)(q * (NB + 1) * 4096);
-            const uint32_t xbuf = stg + NB * 4096u;       // one BF16 box (32 rows x 64 columns)
-            const uint32_t par = epi_base + 4u * (NB + 1) * 4096u;       // bias | gamma | beta, 1024 floats each
-            const int srow0 = cid * TM + rank * BM + q * 32;           // this warp's rows in the scratch
-            uint32_t rph = 0;
-            auto issue_load = [&](uint32_t i) {           // lane 0: box i of this warp's sequence -> buffer i % NB
-                const int rb = (int)(i / (2u * nbt)), b = (int)(i % (2u * nbt));
-                const int mb = cid + rb * ncl;
-                if (mb >= num_m) return;
-                const int row0 = mb * TM + rank * BM + q * 32;
-                if (row0 >= M) return;
-                const uint32_t bar = rfull_bar(q, i % NB);
-                ptx::mbar_arrive_expect_tx(bar, 4096);
-                if (b < nbt) {
-                    ptx::tma_load_2d(stg + (i % NB) * 4096u, &tmap_r, bar, b * 32, row0);
-                } else {
-                    // the store of this v box, nbt - NB + 1 groups ago, must have completed (not just been read)
-                    if (nbt >= 12) ptx::bulk_wait<8>(); else ptx::bulk_wait<2>();
-                    ptx::tma_load_2d(stg + (i % NB) * 4096u, &tmap_y, bar, (b - nbt) * 32, srow0);
-                }
-            };
-            if (lane == 0) { for (uint32_t i = 0; i + 1 < NB; i++) issue_load(i); }
-            int m_blk, n_blk;
-            float r_mean = 0.f, r_m2 = 0.f;
-            for (int lt = 0; get_tile(lt, m_blk, n_blk); lt++) {
-                const int row0 = m_blk * TM + rank * BM + q * 32;
-                const bool valid = row0 < M;              // warp-uniform
-                if (n_blk == 0) { r_mean = 0.f; r_m2 = 0.f; }
-                ptx::mbar_wait(tfull_bar(acc), acc_ph);
-                ptx::tc_fence_after();
-                const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
-#pragma unroll 1
-                for (int j = 0; j < BPT; j++, nbox++) {
-                    const int col = n_blk * BN + j * 32;
-                    const uint32_t b = nbox % NB;
-                    const uint32_t buf = stg + b * 4096u;
-                    uint32_t r[32];
-                    ptx::tmem_ld_32x32b_x32(t_base + (uint32_t)(j * 32), r);
-                    ptx::tmem_ld_wait();
-                    if (j == BPT - 1) {
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) arrive_tempty(acc);
-                    }
-                    if (valid) {
-                        ptx::mbar_wait(rfull_bar(q, b), (rph >> b) & 1u);
-                        rph ^= 1u << b;
-                        uint64_t vv[16];                  // the 32 values of this row's chunk as FP32x2 pairs
-                        uint64_t cs0 = pk2(0.f, 0.f), cs1 = cs0;
-#pragma unroll
-                        for (int v = 0; v < 8; v++) {
-                            const uint32_t addr = buf + row_off + (((uint32_t)v ^ sw) << 4);
-                            uint64_t x0, x1, b0, b1;
-                            ld_shared_2x2(addr, x0, x1);
-                            ld_shared_2x2(par + (uint32_t)(col + 4 * v) * 4u, b0, b1);
-                            vv[2 * v] = add2(add2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), b0), x0);
-                            vv[2 * v + 1] = add2(add2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), b1), x1);
-                            st_shared_2x2(addr, vv[2 * v], vv[2 * v + 1]);
-                            cs0 = add2(cs0, vv[2 * v]); cs1 = add2(cs1, vv[2 * v + 1]);
-                        }
-                        ptx::fence_proxy_async();
-                        __syncwarp();
-                        if (lane == 0) ptx::tma_store_2d(&tmap_y, buf, col, srow0);
-                        // merge this 32-value chunk into the row statistics (two-pass inside the chunk, Chan across chunks)
-                        float s0, s1;
-                        upk2(add2(cs0, cs1), s0, s1);
-                        const float cmean = (s0 + s1) * (1.0f / 32.0f);
-                        const uint64_t ncm = pk2(-cmean, -cmean);
-                        uint64_t q0 = pk2(0.f, 0.f), q1 = q0, q2 = q0, q3 = q0;
-#pragma unroll
-                        for (int u = 0; u < 16; u += 4) {
-                            const uint64_t d0 = add2(vv[u], ncm), d1 = add2(vv[u + 1], ncm), d2 = add2(vv[u + 2], ncm), d3 = add2(vv[u + 3], ncm);
-                            q0 = fma2(d0, d0, q0); q1 = fma2(d1, d1, q1); q2 = fma2(d2, d2, q2); q3 = fma2(d3, d3, q3);
-                        }
-                        upk2(add2(add2(q0, q1), add2(q2, q3)), s0, s1);
-                        const float cm2 = s0 + s1;
-                        const float kprev = (float)(n_blk * BPT + j);            // chunks merged so far
-                        const float w = 1.0f / (kprev + 1.0f);
-                        const float delta = cmean - r_mean;
-                        r_mean = fmaf(delta, w, r_mean);
-                        r_m2 += cm2 + delta * delta * (32.0f * kprev * w);
-                    }
-                    if (lane == 0) {
-                        ptx::bulk_commit();
-                        ptx::bulk_wait_read<1>();
-                        issue_load(nbox + NB - 1);
-                    }
-                    __syncwarp();
-                }
-                if (++acc == 2) { acc = 0; acc_ph ^= 1u; }
-                if (n_blk != num_n - 1) continue;
-                // ---- pass 2 over the finished row block ----
-                const float rstd = rsqrtf(r_m2 / (float)N + ln_eps);
-                const uint64_t rstd2 = pk2(rstd, rstd), nmr2 = pk2(-r_mean * rstd, -r_mean * rstd);
-#pragma unroll 1
-                for (int p2 = 0; p2 < nbt; p2++, nbox++) {
-                    const int col = p2 * 32;
-                    const uint32_t b = nbox % NB;
-                    const uint32_t buf = stg + b * 4096u;
-                    if (valid) {
-                        ptx::mbar_wait(rfull_bar(q, b), (rph >> b) & 1u);
-                        rph ^= 1u << b;
-                        uint32_t pk[16];
-#pragma unroll
-                        for (int v = 0; v < 8; v++) {
-                            const uint32_t addr = buf + row_off + (((uint32_t)v ^ sw) << 4);
-                            uint64_t x0, x1, g0, g1, e0, e1;
-                            ld_shared_2x2(addr, x0, x1);
-                            ld_shared_2x2(par + (uint32_t)(1024 + col + 4 * v) * 4u, g0, g1);
-                            ld_shared_2x2(par + (uint32_t)(2048 + col + 4 * v) * 4u, e0, e1);
-                            // (x - mean) * rstd * gamma + beta = fma(fma(x, rstd, -mean * rstd), gamma, beta)
-                            const uint64_t o01 = fma2(fma2(x0, rstd2, nmr2), g0, e0), o23 = fma2(fma2(x1, rstd2, nmr2), g1, e1);
-                            st_shared_2x2(addr, o01, o23);
-                            float o0, o1, o2, o3;
-                            upk2(o01, o0, o1); upk2(o23, o2, o3);
-                            pk[2 * v] = pack_bf16(o0, o1); pk[2 * v + 1] = pack_bf16(o2, o3);
-                        }
-                        if (!(p2 & 1)) {                  // the BF16 box is refilled: its previous store must have read it
-                            if (lane == 0) ptx::bulk_wait_read<0>();
-                            __syncwarp();
-                        }
-#pragma unroll
-                        for (int c = 0; c < 4; c++)       // 16-byte chunks (p2 & 1) * 4 + c of the 64-column BF16 row
-                            st_shared_v4(xbuf + row_off + ((((uint32_t)((p2 & 1) * 4 + c)) ^ sw) << 4), pk[4 * c], pk[4 * c + 1],
-                                         pk[4 * c + 2], pk[4 * c + 3]);
-                        ptx::fence_proxy_async();
-                        __syncwarp();
-                        if (lane == 0) {
-                            ptx::tma_store_2d(&tmap_c, buf, col, row0);
-                            if (p2 & 1) ptx::tma_store_2d(&tmap_xb, xbuf, col - 32, row0);
-                        }
-                    }
-                    if (lane == 0) {
-                        ptx::bulk_commit();
-                        ptx::bulk_wait_read<1>();
-                        issue_load(nbox + NB - 1);
-                    }
-                    __syncwarp();
-                }
-            }
-        } else if constexpr (EPI == 2) {
+        if constexpr (EPI == 2) {
             constexpr int BPT = BN / 32;              // 32x32 FP32 boxes per tile per warp
             const uint32_t stg = epi_base + (uint32_t)(q * NB * 4096);
             const uint32_t par_base = epi_base + 4u * NB * 4096u;      // gamma | beta, 1024 floats each
@@ -669,7 +509,7 @@ int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_
 
 namespace {
 
-struct LnArgs { const float* gamma; const float* beta; float eps; void* xb_out; const float2* res_stats;
+struct LnArgs { const float* gamma; const float* beta; const float2* res_stats;
                 const float2* rope_tab = nullptr; const int* rope_pos = nullptr; };
 
 template <int BN, int EPI, int NB, int CG>
@@ -680,16 +520,12 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
     const int tiles = ((M + BM * CG - 1) / (BM * CG)) * ((N + BN - 1) / BN);
     const int slots = ctx->sm_count / CG;
     int grid = CG * (tiles < slots ? tiles : slots);
-    if (EPI == 3) {                       // one pair per row block
-        const int row_blocks = (M + BM * CG - 1) / (BM * CG);
-        grid = CG * (row_blocks < slots ? row_blocks : slots);
-    }
-    CUtensorMap ta, tb, tc, tr, ty, txb;
+    CUtensorMap ta, tb, tc, tr;
     int rc = make_tmap_2d(ctx, &ta, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, A, (uint64_t)M, (uint64_t)K, BK, BM);
     if (rc) return rc;
     rc = make_tmap_2d(ctx, &tb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, W, (uint64_t)N, (uint64_t)K, BK, BN / CG);
     if (rc) return rc;
-    if (EPI == 2 || EPI == 3) {
+    if (EPI == 2) {
         rc = make_tmap_2d(ctx, &tc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Cout, (uint64_t)M, (uint64_t)N, 32, 32);
         if (rc) return rc;
         rc = make_tmap_2d(ctx, &tr, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, residual, (uint64_t)M, (uint64_t)N, 32, 32);
@@ -698,22 +534,6 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
         rc = make_tmap_2d(ctx, &tc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, Cout, (uint64_t)M, (uint64_t)(EPI == 4 ? N / 2 : N), 64, 32);
         if (rc) return rc;
         tr = tc;
-    }
-    ty = tc; txb = tc;
-    if (EPI == 3) {
-        // per-pair scratch for v = acc + bias + residual: (pairs x 256) rows x N FP32, rewritten for every row block
-        const size_t need = (size_t)(grid / CG) * BM * CG * (size_t)N * 4;
-        if (ctx->ln_scratch_bytes < need) {
-            CU_TRY(ctx, cudaStreamSynchronize(ctx->stream));
-            cudaFree(ctx->ln_scratch);
-            ctx->ln_scratch = nullptr; ctx->ln_scratch_bytes = 0;
-            if (cudaMalloc(&ctx->ln_scratch, need) != cudaSuccess) { cudaGetLastError(); return ANON_ERR_OOM; }
-            ctx->ln_scratch_bytes = need;
-        }
-        rc = make_tmap_2d(ctx, &ty, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, ctx->ln_scratch, (uint64_t)(grid / CG) * BM * CG, (uint64_t)N, 32, 32);
-        if (rc) return rc;
-        rc = make_tmap_2d(ctx, &txb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, ln->xb_out, (uint64_t)M, (uint64_t)N, 64, 32);
-        if (rc) return rc;
     }
     auto kern = gemm_bf16_tcgen05_kernel<BN, EPI, NB, CG>;
     rc = ensure_smem_attr(ctx, (const void*)kern, C::SMEM_BYTES);
@@ -726,11 +546,10 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
     cfg.attrs = attr; cfg.numAttrs = 1;
     const float* g = ln ? ln->gamma : nullptr;
     const float* be = ln ? ln->beta : nullptr;
-    const float eps = ln ? ln->eps : 0.f;
     const float2* rs = ln ? ln->res_stats : nullptr;
     const float2* rtab = ln ? ln->rope_tab : nullptr;
     const int* rpos = ln ? ln->rope_pos : nullptr;
-    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, ty, txb, bias, g, be, eps, rs, rtab, rpos, M, N, K));
+    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, bias, g, be, rs, rtab, rpos, M, N, K));
     CU_LAUNCH_CHECK(ctx, "gemm_bf16_tcgen05_kernel");
     return ANON_OK;
 }
@@ -771,7 +590,7 @@ int gemm_bf16_rope_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat
     if (!ctx || !A || !W || !pos || !table || !Cout || M < 0 || N <= 128 || K <= 0) return ANON_ERR_INVALID_ARG;
     if (K % BK != 0 || N % 192 != 0) return ANON_ERR_UNSUPPORTED;
     if (M == 0) return ANON_OK;
-    LnArgs ln{nullptr, nullptr, 0.f, nullptr, nullptr, table, pos};
+    LnArgs ln{nullptr, nullptr, nullptr, table, pos};
     return launch_gemm<256, 5, 2, 2>(ctx, A, W, nullptr, nullptr, Cout, M, N, K, &ln);
 }
 
@@ -784,31 +603,9 @@ int gemm_bf16_res_ln_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bflo
         return ANON_ERR_INVALID_ARG;
     if (K % BK != 0 || N % 8 != 0 || (res_stats && N > 1024)) return ANON_ERR_UNSUPPORTED;
     if (M == 0) return ANON_OK;
-    LnArgs ln{gamma, beta, 0.f, nullptr, res_stats};
+    LnArgs ln{gamma, beta, res_stats};
     if (K >= 2048) return launch_gemm<256, 2, 2, 2>(ctx, A, W, bias, res_y, C, M, N, K, &ln);
     return launch_gemm<256, 2, 5, 2>(ctx, A, W, bias, res_y, C, M, N, K, &ln);      // 5 boxes per warp + 4 mainloop stages
-}
-
-int gemm_bf16_ln_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias,
-                      const float* residual, const float* gamma, const float* beta, float eps, float* x_out,
-                      __nv_bfloat16* xb_out, int M, int N, int K)
-{
-    if (!ctx || !A || !W || !bias || !residual || !gamma || !beta || !x_out || !xb_out || M < 0 || N <= 0 || K <= 0)
-        return ANON_ERR_INVALID_ARG;
-    if (K % BK != 0 || N % 256 != 0 || N > 1024) return ANON_ERR_UNSUPPORTED;
-    if (M == 0) return ANON_OK;
-    LnArgs ln{gamma, beta, eps, xb_out, nullptr};
-    return launch_gemm<256, 3, 4, 2>(ctx, A, W, bias, residual, x_out, M, N, K, &ln);
-}
-
-extern "C" int anon_gemm_bf16_ln(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,
-                                 const float* d_residual, const float* d_gamma, const float* d_beta, float eps,
-                                 float* d_x, void* d_xb, int32_t M, int32_t N, int32_t K)
-{
-    if (!ctx) return ANON_ERR_INVALID_ARG;
-    CU_TRY(ctx, cudaSetDevice(ctx->device));
-    return gemm_bf16_ln_impl(ctx, (const __nv_bfloat16*)d_A, (const __nv_bfloat16*)d_W, d_bias, d_residual, d_gamma, d_beta,
-                             eps, d_x, (__nv_bfloat16*)d_xb, M, N, K);
 }
 
 extern "C" int anon_gemm_bf16(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,

@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdio.h>
 
 namespace ptx {
 
@@ -34,14 +35,32 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
+#ifdef ANON_HANG_TRAP
+// debug build (ANON_NVCC_EXTRA=-DANON_HANG_TRAP): a wait that spins for ~seconds reports where and traps instead of hanging
+static __device__ __noinline__ void mbar_wait_report(uint32_t bar, uint32_t parity) {
+    printf("HANG block %d thread %d: mbarrier smem 0x%x parity %u\n", (int)blockIdx.x, (int)threadIdx.x, bar, parity);
+    __trap();
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    for (unsigned long long n = 0; !mbar_try_wait(bar, parity); n++)
+        if (n > 20000000ull) mbar_wait_report(bar, parity);
+}
+#else
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {}
 }
+#endif
 // For single-thread roles (TMA producer, MMA issuer) whose waits are long: back off between polls so the spin
 // does not take issue slots from the math warps that share the SM sub-partition.
 __device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
+#ifdef ANON_HANG_TRAP
+    unsigned long long n_polls = 0;
+#endif
     while (true) {
+#ifdef ANON_HANG_TRAP
+        if (++n_polls > 2000000ull) mbar_wait_report(bar, parity);
+#endif
         uint32_t ok;
         asm volatile(
             "{\n\t.reg .pred p;\n\t"

@@ -235,3 +235,76 @@ def test_bounded_cache_eviction_matches_oracle(env):
         st = gc.stats()
         assert (st["n_unique"], st["n_lookups"], st["n_hits"]) == (len(want), oc.n_lookups, oc.n_hits), step
     gc.close()
+
+
+def test_buffers_at_odd_byte_addresses_and_misaligned_digests(env):
+    """ABI alignment rules (include/anonshield.h, anon_pseudonymize): span bytes and the token buffer may sit at ANY byte address
+    (sub-buffers of a larger allocation: offsets 1, 2, 3 from a 16-byte boundary), results stay bit-exact; a digest buffer that
+    is not 16-byte aligned is rejected with INVALID_ARG instead of faulting."""
+    from oracle import crypto
+    P, torch, ctx = env
+    dev = "cuda:0"
+    data, off, types, key = gen.spans_config1()
+    S = off.size - 1
+    oc = crypto.Cache()
+    want = oc.pseudonymize(data, off, types, key.tobytes(), 10, gen.TYPE_NAMES_4)
+    oc.close()
+    for shift in (1, 2, 3, 7):
+        cache = P.Cache(ctx, 4096, 1 << 20)
+        big_in = torch.zeros(data.size + 64, dtype=torch.uint8, device=dev)
+        big_in[shift:shift + data.size] = torch.from_numpy(data).to(dev)
+        big_out = torch.zeros(S * 32 + 64, dtype=torch.uint8, device=dev)
+        out = big_out[shift:]
+        assert out.data_ptr() % 4 == shift % 4
+        out_off = torch.zeros(S + 1, dtype=torch.int64, device=dev)
+        hit = torch.zeros(S + 8, dtype=torch.uint8, device=dev)[shift:shift + S]
+        P.anon_pseudonymize(ctx, cache, big_in[shift:shift + data.size], torch.from_numpy(off).to(dev), torch.from_numpy(types).to(dev),
+                            key.tobytes(), 10, gen.TYPE_NAMES_4, out, out_off, hit)
+        assert ctx.sync() == 0
+        oo = out_off.cpu().numpy()
+        assert np.array_equal(oo, want["out_offsets"])
+        assert np.array_equal(out.cpu().numpy()[:oo[S]], want["out_tokens"])
+        assert np.array_equal(hit.cpu().numpy(), want["hit"])
+        assert int(big_out[:shift].sum()) == 0 and int(big_out[shift + oo[S]:].sum()) == 0     # nothing outside the token range
+        cache.close()
+    cache = P.Cache(ctx, 4096, 1 << 20)
+    dig = torch.zeros(S * 32 + 16, dtype=torch.uint8, device=dev)[4:]
+    out = torch.zeros(S * 32, dtype=torch.uint8, device=dev)
+    with pytest.raises(P.AnonError) as e:
+        P.anon_pseudonymize(ctx, cache, torch.from_numpy(data).to(dev), torch.from_numpy(off).to(dev), None, key.tobytes(), 10,
+                            gen.TYPE_NAMES_4, out, torch.zeros(S + 1, dtype=torch.int64, device=dev), None, None, dig)
+    assert e.value.code == P.ERR_INVALID_ARG
+    with pytest.raises(P.AnonError) as e:
+        P.anon_hmac_spans(ctx, torch.from_numpy(data).to(dev), torch.from_numpy(off).to(dev), key.tobytes(), dig)
+    assert e.value.code == P.ERR_INVALID_ARG
+    assert cache.stats()["n_unique"] == 0
+    cache.close()
+
+
+def test_cache_protocol_is_order_deterministic(env):
+    """The CAS + atomicMin slot protocol must give the sequential definition's answer whatever the thread schedule: the same
+    span list run 5 times on fresh caches gives identical hit / uid arrays (= the oracle's), and a shuffled copy of the list
+    gives the oracle's answer for THAT order (uids follow first occurrence in the new order) with the same set of digests."""
+    from oracle import crypto
+    P, torch, ctx = env
+    data, off, types, key, draws = gen.spans_zipf(3000, 200_000, 7, 128, 6, 77)
+    kb = key.tobytes()
+    oc = crypto.Cache(1 << 14)
+    want = oc.pseudonymize(data, off, types, kb, 10, gen.TYPE_NAMES_6)
+    oc.close()
+    for _ in range(5):
+        cache = P.Cache(ctx, 4096, 1 << 20)
+        got = _run_gpu(P, torch, ctx, cache, data, off, types, kb, 10, gen.TYPE_NAMES_6)
+        cache.close()
+        _assert_same(got, want)
+    perm = np.random.default_rng(3).permutation(off.size - 1)
+    pool, poff = gen.ascii_pool(3000, 7, 128, 77 + 1000)
+    data2, off2 = gen.expand_csr(pool, poff, draws[perm])
+    oc = crypto.Cache(1 << 14)
+    want2 = oc.pseudonymize(data2, off2, types[perm], kb, 10, gen.TYPE_NAMES_6)
+    oc.close()
+    cache = P.Cache(ctx, 4096, 1 << 20)
+    got2 = _run_gpu(P, torch, ctx, cache, data2, off2, types[perm], kb, 10, gen.TYPE_NAMES_6)
+    cache.close()
+    _assert_same(got2, want2)
+    assert np.array_equal(got2["digests"], got["digests"][perm])            # a pseudonym never depends on the order

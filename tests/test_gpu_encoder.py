@@ -143,35 +143,6 @@ def test_tcgen05_gemm_against_fp64(env, M, N, K, epi):
         assert (np.abs(got - want) <= 2.0 ** -8 * np.abs(want) + 1e-4 * scale).all()
 
 
-@pytest.mark.parametrize("M,N,K,inplace", [(300, 768, 768, False), (1000, 768, 3072, True), (256 * 80 + 37, 1024, 1024, True),
-                                            (77, 256, 64, False)])
-def test_tcgen05_gemm_fused_layernorm(env, M, N, K, inplace):
-    """K2 with the LayerNorm fused into the epilogue: x = LN(A W^T + b + residual), FP32 x (optionally written over the
-    residual) and its BF16 copy; several row blocks per CTA pair, ragged M tail, 1 / 3 / 4 n-tiles per row."""
-    P, torch, ctx = env
-    from oracle import encoder
-    rng = np.random.default_rng(M + N + K)
-    A = _bf16(rng.standard_normal((M, K)) * 1.0)
-    Wm = _bf16(rng.standard_normal((N, K)) * 0.05)
-    bias = (rng.standard_normal(N) * 0.1).astype(np.float32)
-    res = (rng.standard_normal((M, N)) + 0.3).astype(np.float32)
-    g = (1.0 + 0.1 * rng.standard_normal(N)).astype(np.float32)
-    b = (0.1 * rng.standard_normal(N)).astype(np.float32)
-    want = encoder.layer_norm(A.astype(np.float64) @ Wm.astype(np.float64).T + bias + res, g.astype(np.float64),
-                              b.astype(np.float64), 1e-5)
-    dev = "cuda:0"
-    t = lambda a: torch.from_numpy(a).to(dev)
-    d_res = t(res)
-    d_x = d_res if inplace else torch.full((M, N), float("nan"), dtype=torch.float32, device=dev)
-    d_xb = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device=dev)
-    P.anon_gemm_bf16_ln(ctx, t(A).to(torch.bfloat16), t(Wm).to(torch.bfloat16), t(bias), d_res, t(g), t(b), 1e-5, d_x, d_xb)
-    assert ctx.sync() == 0
-    got = d_x.cpu().numpy().astype(np.float64)
-    gotb = d_xb.float().cpu().numpy().astype(np.float64)
-    assert np.abs(got - want).max() <= 3e-5 * max(1.0, np.abs(want).max())
-    assert (np.abs(gotb - want) <= 2.0 ** -8 * np.abs(want) + 1e-4).all()
-
-
 def _attention_oracle(qkv, cu, H, A):
     from oracle import encoder
     out = np.zeros((qkv.shape[0], H))

@@ -85,6 +85,105 @@ def test_configs1_full_size_in_bench_configuration():
     cache.close(); W.close(); ctx.close()
 
 
+def test_configs2_stream_subsample():
+    """BASELINE.json configs[2] at its real shape (the workload stands in for the paper's D2,
+    PAPER.md L111: 70,951 records / 550 MB): the first 64 records of bench.py's stream (same seeds, same 300 k-string
+    Zipf pool, so these ARE the stream's first 64 records) with ALL their windows, BERT-base shape BF16, deep planted
+    detector, run through anon_pipeline_host_text in >= 3 token-budgeted batches with ONE persistent cache.
+      * oracle encoder (fp64) on every window: logits max-abs <= 3e-2; labels >= 99.9 % equal, every mismatch at oracle
+        top-2 margin < 3e-2;
+      * oracle decode of the GPU's labels == GPU spans, bit-exact, spans crossing a window boundary included;
+      * oracle dedup / HMAC / write-back / splice of the GPU span list == GPU tokens, hit flags and rewritten text;
+      * planted-truth recall and spans / planted are printed (and must be sane)."""
+    import torch
+    import paper_2606_15650_b200 as P
+    from paper_2606_15650_b200 import stream
+    from oracle import crypto, decode, encoder
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device")
+    dev = "cuda:0"
+    d = gen.DESCS["base"]
+    rec = gen.workload_stream(n_records=64, seed=gen.SEED_BASE + 3, n_pool=300000)
+    win = gen.window_records(rec)
+    w = gen.make_weights(d, gen.SEED_BASE + 2, planted=gen.PLANTED_DEEP)
+    ids, cu, meta = win["token_ids"], win["cu_seqlens"], np.ascontiguousarray(win["meta"])
+    T, B = ids.size, cu.size - 1
+    assert T > 100_000 and B > 250 and np.diff(cu).max() == 512
+    plan = stream.plan_batches(win["win_rec"], cu, T // 4)
+    assert len(plan) >= 3
+    maxT = max(int(cu[b] - cu[a]) for a, b in plan)
+    ctx = P.Context(0, workspace_bytes=P.anon_workspace_bytes(d, T, B) + 200 * T + 4 * rec["text"].size + (256 << 20))
+    W = P.Weights(ctx, d, gen.pack_blob(w))
+    logits = torch.zeros((T, d["num_labels"]), dtype=torch.float32, device=dev)
+    labels = torch.zeros(T, dtype=torch.int32, device=dev)
+    P.anon_ner_forward(ctx, W, torch.from_numpy(ids).to(dev), torch.from_numpy(cu).to(dev), logits, labels)
+    assert ctx.sync() == 0
+    got_logits, got_labels = logits.cpu().numpy(), labels.cpu().numpy()
+    cache = P.Cache(ctx, 1 << 18, 16 << 20)
+    got_spans, got_tok, got_hit, got_len, got_text, got_ro = [], [], [], [], [], []
+    for a, b in plan:
+        bt = stream.slice_batch(rec, win, a, b)
+        res = P.anon_pipeline_host(ctx, W, cache, bt["token_ids"], bt["cu_seqlens"], bt["meta"], bt["text"], bt["rec_off"], KEY, 10,
+                                   gen.TYPE_NAMES_6, span_capacity=maxT // 4, out_capacity=maxT * 8, want_text=True)
+        sp = res["spans"].copy()
+        sp[:, 0] += bt["r0"]
+        got_spans.append(sp)
+        got_tok.append(res["out_tokens"].copy())
+        got_hit.append(res["hit"].copy())
+        got_len.append(np.diff(res["out_offsets"]))
+        got_text.append(res["new_text"].copy())
+        got_ro.append(np.diff(res["new_record_offsets"]))
+    st = cache.stats()
+    cache.close(); W.close(); ctx.close()
+    got_spans = np.concatenate(got_spans)
+    # ---- encoder against the fp64 oracle, every window ----
+    want = encoder.forward_packed(w, d, ids, cu)
+    err = np.abs(got_logits - want)
+    assert err.max() <= 3e-2, err.max()
+    want_labels = encoder.argmax_labels(want)
+    mism = got_labels != want_labels
+    assert (encoder.top2_margin(want)[mism] < 3e-2).all()
+    assert 1.0 - mism.mean() >= 0.999
+    assert np.array_equal(got_labels, encoder.argmax_labels(got_logits))
+    # ---- decode: the oracle walk over the GPU's labels (batch by batch == the undivided stream) ----
+    spans = decode.decode_spans(got_labels, meta)
+    assert np.array_equal(got_spans, np.asarray(spans, np.int32).reshape(-1, 4))
+    # at least one span is stitched across a window boundary: its kept tokens lie in two windows
+    win_of_tok = np.repeat(np.arange(B), np.diff(cu))
+    kept = meta[:, 3] == 1
+    first_tok = {}
+    for j in np.flatnonzero(kept & (got_labels > 0)):
+        first_tok.setdefault((int(meta[j, 0]), int(meta[j, 1])), j)
+    crossing = 0
+    for r, cs, ce, _t in spans:
+        j = first_tok[(r, cs)]
+        k = j
+        while not (kept[k] and meta[k, 0] == r and meta[k, 2] == ce):
+            k += 1
+        crossing += int(win_of_tok[k] != win_of_tok[j])
+    assert crossing >= 1
+    # ---- dedup / HMAC / write-back / splice on the GPU span list ----
+    sb, so = decode.gather_spans(rec["text"], rec["rec_off"], spans)
+    oc = crypto.Cache(1 << 18)
+    wantp = oc.pseudonymize(sb, so, np.asarray([s[3] for s in spans], np.uint8), KEY, 10, gen.TYPE_NAMES_6)
+    oc.close()
+    assert np.array_equal(np.concatenate(got_tok), wantp["out_tokens"])
+    assert np.array_equal(np.concatenate(got_hit), wantp["hit"])
+    assert np.array_equal(np.concatenate(got_len), np.diff(wantp["out_offsets"]))
+    assert st["n_lookups"] == len(spans) and st["n_hits"] == int(wantp["hit"].sum()) and wantp["hit"].sum() > 0
+    want_text, want_ro = decode.splice_records(rec["text"], rec["rec_off"], spans, wantp["out_tokens"], wantp["out_offsets"])
+    assert np.array_equal(np.concatenate(got_text), want_text)
+    assert np.array_equal(np.concatenate(got_ro), np.diff(want_ro))
+    # ---- planted truth (a report; the oracle's labels stay the parity reference) ----
+    planted = set(decode.decode_spans(win["planted_label"].astype(np.int32), meta))
+    found = set(spans)
+    recall = len(planted & found) / len(planted)
+    print(f"configs[2] subsample: T={T} windows={B} batches={len(plan)} spans={len(spans)} planted={len(planted)} "
+          f"spans/planted={len(spans) / len(planted):.4f} recall={recall:.4f} crossing={crossing} max|dlogit|={err.max():.2e} "
+          f"label mismatches={int(mism.sum())} hit rate={st['n_hits'] / st['n_lookups']:.3f}")
+    assert len(planted) == rec["n_entities"] and recall >= 0.99 and len(spans) <= 1.01 * len(planted)
+
+
 def test_configs4_full_size_50m_spans():
     import torch
     import paper_2606_15650_b200 as P
@@ -149,7 +248,7 @@ def test_configs3_full_size_in_bench_configuration():
     dev = "cuda:0"
     d = gen.DESCS["large"]
     rec, win = gen.workload_large(n_seqs=16384, seed=gen.SEED_BASE + 4)             # exactly bench.py's "large" workload
-    w = gen.make_weights(d, gen.SEED_BASE + 4, planted=(2.0, 0.5, 4.0))
+    w = gen.make_weights(d, gen.SEED_BASE + 4, planted=gen.PLANTED_DEEP)       # the 3-tuple plant fades to 0 spans at L = 24
     ids, cu, meta = win["token_ids"], win["cu_seqlens"], np.ascontiguousarray(win["meta"])
     T, B = ids.size, cu.size - 1
     assert B == 16384 and T > 4_000_000
@@ -168,10 +267,35 @@ def test_configs3_full_size_in_bench_configuration():
     assert ctx.sync() == 0
     S = int(nsp.item())
     got_spans = spans.cpu().numpy()[:S]
-    W.close(); ctx.close()
+    assert S > 100_000                          # ~1 entity per 25 tokens: A9-A13 are exercised at this shape
+    # gather + pseudonymize at full size, checked below against the oracle fed with the GPU's spans
+    text, rec_off = rec["text"], rec["rec_off"]
+    span_bytes = torch.zeros(text.size + 16, dtype=torch.uint8, device=dev)
+    span_off = torch.zeros(S + 1, dtype=torch.int64, device=dev)
+    span_type = torch.zeros(S, dtype=torch.uint8, device=dev)
+    P.anon_gather_spans(ctx, torch.from_numpy(text).to(dev), torch.from_numpy(rec_off).to(dev), spans, S, span_bytes, span_off,
+                        span_type)
+    cache = P.Cache(ctx, 1 << 20, 64 << 20)
+    out = torch.zeros(S * 32, dtype=torch.uint8, device=dev)
+    out_off = torch.zeros(S + 1, dtype=torch.int64, device=dev)
+    hit = torch.zeros(S, dtype=torch.uint8, device=dev)
+    P.anon_pseudonymize(ctx, cache, span_bytes, span_off, span_type, KEY, 10, gen.TYPE_NAMES_6, out, out_off, hit)
+    assert ctx.sync() == 0
+    got_sb, got_so, got_oo, got_out, got_hit = (t.cpu().numpy() for t in (span_bytes, span_off, out_off, out, hit))
+    cache.close(); W.close(); ctx.close()
     want_spans = decode.decode_spans(got_labels, meta)
-    assert S == len(want_spans)                 # the planted detector fades over 24 layers: few or no spans here
+    assert S == len(want_spans)
     assert np.array_equal(got_spans, np.asarray(want_spans, np.int32).reshape(-1, 4))
+    sb, so = decode.gather_spans(text, rec_off, want_spans)
+    assert np.array_equal(got_so, so) and np.array_equal(got_sb[:so[-1]], sb)
+    from oracle import crypto
+    oc = crypto.Cache(1 << 20)
+    wantp = oc.pseudonymize(sb, so, np.asarray([s[3] for s in want_spans], np.uint8), KEY, 10, gen.TYPE_NAMES_6)
+    oc.close()
+    assert np.array_equal(got_oo, wantp["out_offsets"]) and np.array_equal(got_out[:got_oo[-1]], wantp["out_tokens"])
+    assert np.array_equal(got_hit, wantp["hit"])
+    planted = set(decode.decode_spans(win["planted_label"].astype(np.int32), meta))
+    print(f"configs[3]: T={T} spans={S} planted={len(planted)} recall={len(planted & set(want_spans)) / len(planted):.4f}")
     lens = np.diff(cu)
     picks = {int(np.argmin(lens)), int(np.argmax(lens)), B - 1} | set(np.random.default_rng(7).integers(0, B, 1).tolist())
     want = encoder.forward_packed(w, d, ids, cu, seq_subset=sorted(picks))

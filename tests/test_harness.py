@@ -65,3 +65,23 @@ def test_zipf_spans_shape():
     assert 0.05 < top < 0.35                      # Zipf head
     uniq = {bytes(data[off[i]:off[i + 1]]) for i in range(0, 50000, 7)}
     assert len(uniq) > 300
+
+
+def test_field_spans_are_the_generated_entity_ranges():
+    """NEXT-2 input: gen.field_spans names exactly the entity strings make_records wrote (checked with the oracle's decoder over
+    the un-windowed planted labels and against the text itself), with the fixed type in every row."""
+    from oracle import decode
+    rec = gen.workload_stream(n_records=40, seed=11, n_pool=500)
+    sp = gen.field_spans(rec, 3)
+    assert sp.dtype == np.int32 and sp.shape == (rec["n_entities"], 4) and (sp[:, 3] == 3).all()
+    T = rec["ids"].size
+    meta = np.zeros((T, 4), np.int32)
+    meta[:, 0] = np.searchsorted(rec["tok_rec_off"], np.arange(T), side="right") - 1
+    meta[:, 1], meta[:, 2], meta[:, 3] = rec["char_start"], rec["char_end"], 1
+    want = decode.decode_spans(rec["planted_label"].astype(np.int32), meta)
+    assert [tuple(r[:3]) for r in sp.tolist()] == [w[:3] for w in want]
+    pool, poff, _ = gen.entity_pool(500, 12)
+    strings = {pool[poff[i]:poff[i + 1]].tobytes() for i in range(500)}
+    for r, cs, ce, _t in sp[:200]:
+        base = int(rec["rec_off"][r])
+        assert rec["text"][base + cs:base + ce].tobytes() in strings

@@ -235,15 +235,26 @@ int  anon_microbench(anon_ctx* ctx, int32_t mode, int32_t iters, double* thread_
  *   place of span s;  d_new_record_offsets int64[R+1] = offsets of the rewritten records.
  * d_spans must be in stream order (as anon_decode_spans writes them) and non-overlapping; text_bytes =
  * record_offsets[R].  If the rewritten text exceeds new_text_capacity nothing beyond it is written and
- * ANON_ERR_CAPACITY is latched in the sticky status.  Asynchronous. */
+ * ANON_ERR_CAPACITY is latched in the sticky status.  Workspace: 16 (S + 1) + new_text_capacity / 1024 + 64 KB bytes
+ * (ANON_ERR_OOM if the context has less).  d_text, d_out_tokens and d_new_text may sit at any byte address.  Asynchronous. */
 int  anon_splice_records(anon_ctx* ctx, const uint8_t* d_text, size_t text_bytes, const int64_t* d_record_offsets, int32_t R,
                          const anon_span* d_spans, int32_t S, const uint8_t* d_out_tokens, const int64_t* d_out_offsets,
                          uint8_t* d_new_text, size_t new_text_capacity, int64_t* d_new_record_offsets);
 
 /* ---- NEXT-4: regex detector and regex / NER span merge ("custom regex patterns"; S8f NEXT-4; D17-D19) ----- */
-/* Uploads a pattern automaton.  h_blob is the byte string regex_dfa.compile_patterns() returns (HOST pointer, layout in
- * paper_2606_15650_b200/regex_dfa.py: header, class_of[256], is_word[256], type_of_pattern[256], accept[n_states],
- * trans[n_states * n_classes]; state 0 dead, state 1 start).  The tables are validated here (sizes, every transition and
+/* Uploads a pattern automaton.  h_blob (HOST pointer) is a deterministic finite automaton over byte classes for ALL patterns
+ * at once; paper_2606_15650_b200/regex_dfa.py compile_patterns() builds it from a restricted regex syntax, and any other
+ * producer (a C caller with its own DFA) may write the same bytes.  Layout, little-endian, no padding except where stated:
+ *   uint32 head[8]      = { 0x31585241 ("ARX1"), n_states (2..65535), n_classes (1..128), n_patterns (1..127),
+ *                           max_match (1..255 bytes), 0, 0, 0 }
+ *   uint8  class_of[256]   byte value -> class index (< n_classes)
+ *   uint8  is_word[256]    1 if the byte is a word character ([0-9A-Za-z_], rule D18's boundary test), else 0
+ *   uint8  type_of[256]    pattern index -> span type written into anon_span.type (entries >= n_patterns unused)
+ *   int16  accept[n_states]   pattern index accepted in this state (lowest index if several), -1 if none;
+ *                             zero-padded to a multiple of 4 bytes
+ *   uint16 trans[n_states][n_classes]   next state
+ * State 0 is the dead state (all its transitions are 0, it accepts nothing), state 1 the start state (must not accept: no
+ * empty match).  blob_bytes must equal 32 + 768 + round4(2 n_states) + 2 n_states n_classes.  The tables are validated here (sizes, every transition and
  * accept label in range, at most 127 patterns, max_match <= 255) and must fit shared memory beside a text tile, else
  * ANON_ERR_UNSUPPORTED.  The handle keeps its own device copy.  Synchronises.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA. */
 int  anon_regex_load(anon_ctx* ctx, const void* h_blob, size_t blob_bytes, anon_regex** out);

@@ -38,6 +38,7 @@ extern "C" int anon_ctx_create(anon_ctx** out, int device, void* cuda_stream, si
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
     { const char* e = getenv("ANON_CHUNK_TOKENS"); c->chunk_tokens_cap = e ? atoll(e) : 0; }
+    { const char* e = getenv("ANON_ABLATE"); c->ablate = e ? atoi(e) : 0; }
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);

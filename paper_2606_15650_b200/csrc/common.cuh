@@ -37,6 +37,8 @@ struct anon_ctx {
     const void* smem_attr_done[48] = {nullptr};
     int n_smem_attr_done = 0;
     long long chunk_tokens_cap = 0;     // ANON_CHUNK_TOKENS read once at context creation (0 = workspace-limited only)
+    int ablate = 0;                     // ANON_ABLATE (measurement aid, results are then WRONG): bit 0 skip attention, 1 skip LayerNorm
+                                        // kernels, 2 skip the out-projection, 3 FFN1 without GELU -- marginal cost of a kernel class in the step
     // NEXT-4: pattern automaton the host pipeline merges into the NER spans (anon_ctx_set_regex; not owned)
     const struct anon_regex* regex = nullptr;
     // launch accounting + optional event profiling

@@ -82,18 +82,40 @@ struct LenIn {
     }
 };
 struct GatherOut {
-    const anon_span* spans; const uint8_t* text; const long long* rec_off;
-    uint8_t* out; long long cap; long long* off; uint8_t* type; int* d_status;
+    const anon_span* spans; long long cap; long long* off; uint8_t* type; int* d_status;
     __device__ __forceinline__ void operator()(long long s, long long o, long long len) const {
         off[s] = o;
-        const anon_span sp = spans[s];
-        if (type) type[s] = (uint8_t)sp.type;
-        if (o + len > cap) { latch_status(d_status, ANON_ERR_CAPACITY); return; }
-        const uint8_t* src = text + rec_off[sp.record_id] + sp.char_start;
-        uint8_t* dst = out + o;
-        for (long long k = 0; k < len; k++) dst[k] = src[k];
+        if (type) type[s] = (uint8_t)spans[s].type;
+        if (o + len > cap) latch_status(d_status, ANON_ERR_CAPACITY);
     }
 };
+// K8 copy: a warp takes 32 consecutive spans -- a contiguous byte range of the output -- and moves them one span at a time with
+// lane-strided byte accesses (32 consecutive bytes per instruction on both sides) instead of one thread walking each span byte
+// by byte (one sector per byte and lane).  Spans that would overflow the buffer are skipped (the scan has latched CAPACITY).
+__global__ void __launch_bounds__(256) gather_copy_kernel(const anon_span* __restrict__ spans, const int* __restrict__ d_n, long long S_max,
+                                                          const uint8_t* __restrict__ text, const long long* __restrict__ rec_off,
+                                                          const long long* __restrict__ off, uint8_t* __restrict__ out, long long cap)
+{
+    const long long n = d_n ? min((long long)*d_n, S_max) : S_max;
+    const int lane = threadIdx.x & 31;
+    const long long s0 = ((long long)blockIdx.x * 8 + (threadIdx.x >> 5)) * 32;
+    if (s0 >= n) return;
+    const long long s = s0 + lane;
+    long long src = 0, dst = 0; int len = 0;
+    if (s < n) {
+        const anon_span sp = spans[s];
+        len = sp.char_end - sp.char_start; if (len < 0) len = 0;
+        src = rec_off[sp.record_id] + sp.char_start;
+        dst = off[s];
+        if (dst + len > cap) len = 0;
+    }
+    const int cnt = (int)min(32ll, n - s0);
+    for (int j = 0; j < cnt; j++) {
+        const long long a = __shfl_sync(0xffffffffu, src, j), b = __shfl_sync(0xffffffffu, dst, j);
+        const int l = __shfl_sync(0xffffffffu, len, j);
+        for (int k = lane; k < l; k += 32) out[b + k] = text[a + k];
+    }
+}
 __global__ void gather_finish_kernel(const long long* total, const int* d_n, long long S_max, long long* off) {
     const long long n = d_n ? min((long long)*d_n, S_max) : S_max;
     off[n] = *total;
@@ -111,47 +133,115 @@ struct DeltaIn {
     }
 };
 struct DeltaOut {
-    const anon_span* spans; const long long* rec_off; long long* D; long long* astart; long long* aend; long long S;
+    const anon_span* spans; const long long* rec_off; long long* D; long long* ostart; long long S;
     __device__ __forceinline__ void operator()(long long s, long long ex, long long v) const {
         const anon_span sp = spans[s];
-        const long long a = rec_off[sp.record_id] + sp.char_start;
-        const int l = sp.char_end - sp.char_start;
-        D[s] = ex; astart[s] = a; aend[s] = a + (l > 0 ? l : 0);
+        D[s] = ex;
+        ostart[s] = rec_off[sp.record_id] + sp.char_start + ex;      // where the token of span s starts in the NEW text
         if (s == S - 1) D[S] = ex + v;
     }
 };
 
-__global__ void __launch_bounds__(256) splice_copy_kernel(const uint8_t* __restrict__ text, long long nbytes, long long S,
-                                                          const long long* __restrict__ D, const long long* __restrict__ astart,
-                                                          const long long* __restrict__ aend, uint8_t* __restrict__ out,
-                                                          long long cap, int* d_status)
-{
-    const long long p0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 16;
-    if (p0 >= nbytes) return;
-    long long lo = 0, hi = S;                       // k = number of spans with astart <= p0
-    while (lo < hi) { const long long mid = (lo + hi) >> 1; if (astart[mid] <= p0) lo = mid + 1; else hi = mid; }
-    long long k = lo;
-    long long prev_end = k > 0 ? aend[k - 1] : -1, next_start = k < S ? astart[k] : nbytes + 16, shift = D[k];
-    const long long pe = p0 + 16 < nbytes ? p0 + 16 : nbytes;
-    for (long long p = p0; p < pe; p++) {
-        while (p >= next_start) { prev_end = aend[k]; k++; next_start = k < S ? astart[k] : nbytes + 16; shift = D[k]; }
-        if (p >= prev_end) {
-            const long long q = p + shift;
-            if (q < cap) out[q] = text[p]; else latch_status(d_status, ANON_ERR_CAPACITY);
-        }
-    }
-}
+// The rewritten text is produced OUTPUT-side: a thread owns 16 consecutive output bytes and finds, for each, whether it is
+// a token byte (of the last span whose token starts at or before it) or a text byte of the gap behind that token
+// (source = q - D[number of spans started]).  One 16-byte store per thread instead of 16 byte stores at a shifted address,
+// and no separate token pass.  The spans of a 4 KB chunk of output are found through a chunk index (kb, below) and a short
+// binary search among them.
+constexpr int kSpChunk = 4096;
 
-__global__ void __launch_bounds__(256) splice_tokens_kernel(long long S, const long long* __restrict__ D,
-                                                            const long long* __restrict__ astart, const uint8_t* __restrict__ tok,
-                                                            const long long* __restrict__ tok_off, uint8_t* __restrict__ out,
-                                                            long long cap, int* d_status)
+// kb[c] = number of spans whose token starts before output byte c * kSpChunk, for every chunk boundary c = 0 .. n_chunks:
+// thread s (0 .. S) fills the boundaries that lie in (ostart[s-1], ostart[s]] -- usually none or one -- so that the copy
+// kernel finds a chunk's spans with two loads instead of a binary search over the whole span list per chunk (which, run by one
+// thread per CTA, was 2 x 22 dependent global loads = most of the round-2 first version's time)
+__global__ void __launch_bounds__(256) splice_chunk_index_kernel(long long S, const long long* __restrict__ ostart,
+                                                                 long long n_bounds, int* __restrict__ kb)
 {
     const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= S) return;
-    const long long q = astart[s] + D[s], a = tok_off[s], n = tok_off[s + 1] - a;
-    if (q + n > cap) { latch_status(d_status, ANON_ERR_CAPACITY); return; }
-    for (long long j = 0; j < n; j++) out[q + j] = tok[a + j];
+    if (s > S) return;
+    long long lo = s == 0 ? 0 : ostart[s - 1] / kSpChunk + 1;
+    long long hi = s == S ? n_bounds - 1 : ostart[s] / kSpChunk;
+    if (hi > n_bounds - 1) hi = n_bounds - 1;
+    for (long long c = lo; c <= hi; c++) kb[c] = (int)s;
+}
+
+__global__ void __launch_bounds__(256) splice_out_kernel(const int* __restrict__ kb, const uint8_t* __restrict__ text, long long nbytes, long long S,
+                                                         const long long* __restrict__ D, const long long* __restrict__ ostart,
+                                                         const uint8_t* __restrict__ tok, const long long* __restrict__ tok_off,
+                                                         uint8_t* __restrict__ out, long long cap, int* d_status)
+{
+    const long long total = nbytes + D[S];
+    if (total > cap && blockIdx.x == 0 && threadIdx.x == 0) latch_status(d_status, ANON_ERR_CAPACITY);
+    const long long lim = total < cap ? total : cap;
+    const bool aligned = (reinterpret_cast<uintptr_t>(out) & 15) == 0;
+    const long long stride = (long long)gridDim.x * blockDim.x * 16;
+    for (long long q0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 16; q0 < lim; q0 += stride) {
+        // the spans that matter for this 4 KB chunk of output: the last one that started before the chunk (its token or the
+        // gap behind it may reach into the chunk) and those whose token starts inside it -- a few dozen consecutive rows of
+        // ostart / D / tok_off that the 256 threads of the chunk all read (L1-resident); no shared memory, no barriers
+        const long long c = q0 / kSpChunk;
+        const long long k0 = __ldg(kb + c), k1 = __ldg(kb + c + 1);
+        const long long first = k0 > 0 ? k0 - 1 : 0;
+        const int n = (int)(k1 - first);
+        const long long* os = ostart + first;
+        const long long* dd = D + first;
+        const long long* to = tok_off + first;              // only read when n > 0 (S > 0)
+        int lo = 0, hi = n;                                 // kl = number of those spans with ostart <= q0
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (__ldg(os + mid) <= q0) lo = mid + 1; else hi = mid; }
+        int kl = lo;
+        uint32_t w[4] = {0u, 0u, 0u, 0u};
+        const int cnt = (int)(lim - q0 < 16 ? lim - q0 : 16);
+        // fast path (about four chunks in five): all 16 bytes come from ONE source range -- the token of span kl-1, or the gap
+        // behind it with no further token starting inside these 16 bytes -- so they are 16 independent loads from consecutive
+        // addresses, no per-byte decision
+        const uint8_t* src1 = nullptr;
+        if (cnt == 16) {
+            const long long next_start = kl < n ? __ldg(os + kl) : (long long)0x7fffffffffffffffll;
+            if (kl > 0) {
+                const long long t0 = __ldg(to + kl - 1), rel = q0 - __ldg(os + kl - 1), tl = __ldg(to + kl) - t0;
+                if (rel + 16 <= tl) src1 = tok + t0 + rel;                               // inside the token
+                else if (rel >= tl && next_start >= q0 + 16) src1 = text + (q0 - __ldg(dd + kl));   // inside the gap
+            } else if (next_start >= q0 + 16) {
+                src1 = text + (q0 - __ldg(dd));
+            }
+        }
+        if (src1) {
+#pragma unroll
+            for (int j = 0; j < 16; j++) w[j >> 2] |= (uint32_t)__ldg(src1 + j) << (8 * (j & 3));
+        } else {
+            // general case: walk the (at most a few) SEGMENTS that meet in these bytes -- rest of a token, a gap up to the next
+            // token start, the next token ... -- looking the span rows up once per segment, not once per byte
+            unsigned long long lo8 = 0ull, hi8 = 0ull;
+            int j = 0;
+            while (j < cnt) {
+                const long long q = q0 + j;
+                while (kl < n && __ldg(os + kl) <= q) kl++;
+                const long long next_start = kl < n ? __ldg(os + kl) : (long long)0x7fffffffffffffffll;
+                const uint8_t* src;
+                long long seg_end = next_start;
+                if (kl > 0) {
+                    const long long t0 = __ldg(to + kl - 1), rel = q - __ldg(os + kl - 1), tl = __ldg(to + kl) - t0;
+                    if (rel < tl) { src = tok + t0 + rel; seg_end = q + (tl - rel); }
+                    else src = text + (q - __ldg(dd + kl));
+                } else {
+                    src = text + (q - __ldg(dd));
+                }
+                const int run = (int)(seg_end - q < (long long)(cnt - j) ? seg_end - q : (long long)(cnt - j));
+                for (int i = 0; i < run; i++) {
+                    const unsigned long long b = __ldg(src + i);
+                    const int pos = j + i;
+                    if (pos < 8) lo8 |= b << (8 * pos); else hi8 |= b << (8 * (pos - 8));
+                }
+                j += run;
+            }
+            w[0] = (uint32_t)lo8; w[1] = (uint32_t)(lo8 >> 32); w[2] = (uint32_t)hi8; w[3] = (uint32_t)(hi8 >> 32);
+        }
+        if (aligned && cnt == 16) {
+            *reinterpret_cast<uint4*>(out + q0) = make_uint4(w[0], w[1], w[2], w[3]);
+        } else {
+#pragma unroll
+            for (int j = 0; j < 16; j++) if (j < cnt) out[q0 + j] = (uint8_t)(w[j >> 2] >> (8 * (j & 3)));
+        }
+    }
 }
 
 __global__ void __launch_bounds__(256) splice_record_offsets_kernel(const long long* __restrict__ rec_off, int R, const anon_span* __restrict__ spans,
@@ -175,26 +265,28 @@ int splice_records_impl(anon_ctx* ctx, WsCursor& ws, const uint8_t* d_text, size
         return ANON_ERR_INVALID_ARG;
     cudaStream_t st = ctx->stream;
     long long* D = (long long*)ws.take(((size_t)S + 1) * 8);
-    long long* astart = (long long*)ws.take(((size_t)S + 1) * 8);
-    long long* aend = (long long*)ws.take(((size_t)S + 1) * 8);
+    long long* ostart = (long long*)ws.take(((size_t)S + 1) * 8);
     long long* agg = (long long*)ws.take(scan::agg_bytes<long long>(S > 0 ? S : 1));
-    if (!D || !astart || !aend || !agg) return ANON_ERR_OOM;
+    const long long n_bounds = (long long)(cap / kSpChunk) + 2;          // chunk boundaries 0 .. ceil(cap / chunk)
+    int* kb = (int*)ws.take((size_t)n_bounds * 4);
+    if (!D || !ostart || !agg || !kb) return ANON_ERR_OOM;
     ProfScope ps(ctx, PROF_DECODE, (double)text_bytes * 2 + (double)S * 64, 6);
     if (S > 0) {
         DeltaIn din{d_spans, (const long long*)d_tok_off};
         scan::reduce_and_scan<long long, scan::SumI64>(din, S, nullptr, agg, st);
-        scan::apply<long long, scan::SumI64>(din, DeltaOut{d_spans, (const long long*)d_rec_off, D, astart, aend, S}, S, nullptr, agg, st);
+        scan::apply<long long, scan::SumI64>(din, DeltaOut{d_spans, (const long long*)d_rec_off, D, ostart, S}, S, nullptr, agg, st);
     } else {
         CU_TRY(ctx, cudaMemsetAsync(D, 0, 8, st));
     }
-    if (text_bytes > 0) {
-        const long long chunks = ((long long)text_bytes + 15) / 16;
-        splice_copy_kernel<<<(unsigned)((chunks + 255) / 256), 256, 0, st>>>(d_text, (long long)text_bytes, S, D, astart, aend,
-                                                                           d_new_text, (long long)cap, ctx->d_status);
+    if (text_bytes > 0 || S > 0) {
+        // persistent grid over 4 KB output chunks (the new size lives on the device: text_bytes + D[S] <= cap)
+        const long long chunks = ((long long)text_bytes + kSpChunk - 1) / kSpChunk + 1;
+        const long long want = (long long)ctx->sm_count * 8;
+        splice_chunk_index_kernel<<<(unsigned)((S + 1 + 255) / 256), 256, 0, st>>>(S, ostart, n_bounds, kb);
+        splice_out_kernel<<<(unsigned)(chunks < want ? chunks : want), 256, 0, st>>>(kb, d_text, (long long)text_bytes, S, D, ostart, d_tok,
+                                                                                 (const long long*)d_tok_off, d_new_text, (long long)cap,
+                                                                                 ctx->d_status);
     }
-    if (S > 0)
-        splice_tokens_kernel<<<(unsigned)((S + 255) / 256), 256, 0, st>>>(S, D, astart, d_tok, (const long long*)d_tok_off, d_new_text,
-                                                                         (long long)cap, ctx->d_status);
     splice_record_offsets_kernel<<<(unsigned)((R + 1 + 255) / 256), 256, 0, st>>>((const long long*)d_rec_off, R, d_spans, S, D,
                                                                                  (long long*)d_new_rec_off);
     CU_LAUNCH_CHECK(ctx, "splice_records");
@@ -246,13 +338,14 @@ int gather_spans_impl(anon_ctx* ctx, WsCursor& ws, const uint8_t* d_text, const 
     if (S_max == 0) { CU_TRY(ctx, cudaMemsetAsync(d_off, 0, 8, st)); return ANON_OK; }
     long long* agg = (long long*)ws.take(scan::agg_bytes<long long>(S_max));
     if (!agg) return ANON_ERR_OOM;
-    ProfScope ps(ctx, PROF_DECODE, (double)S_max * 40, 4);
+    ProfScope ps(ctx, PROF_DECODE, (double)S_max * 40, 5);
     LenIn lin{d_spans};
     scan::reduce_and_scan<long long, scan::SumI64>(lin, S_max, d_num_spans, agg, st);
-    scan::apply<long long, scan::SumI64>(lin, GatherOut{d_spans, d_text, (const long long*)d_rec_off, d_bytes,
-                                                         (long long)cap, (long long*)d_off, d_type, ctx->d_status},
+    scan::apply<long long, scan::SumI64>(lin, GatherOut{d_spans, (long long)cap, (long long*)d_off, d_type, ctx->d_status},
                                          S_max, d_num_spans, agg, st);
     gather_finish_kernel<<<1, 1, 0, st>>>(agg + scan::num_tiles(S_max), d_num_spans, S_max, (long long*)d_off);
+    gather_copy_kernel<<<(unsigned)((S_max + 255) / 256), 256, 0, st>>>(d_spans, d_num_spans, S_max, d_text, (const long long*)d_rec_off,
+                                                                       (const long long*)d_off, d_bytes, (long long)cap);
     CU_LAUNCH_CHECK(ctx, "gather_spans");
     return ANON_OK;
 }

@@ -423,22 +423,22 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                     { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * 3 * H * H);
                     rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_qkv, L.b_qkv, nullptr, qkv, nt, 3 * H, H, 0); }
                     if (rc) return rc;
-                    { ProfScope ps(ctx, PROF_ATTN, attn_flops);
+                    if (!(ctx->ablate & 1)) { ProfScope ps(ctx, PROF_ATTN, attn_flops);
                     rc = attention_run(ctx, plan, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx); }
                     if (rc) return rc;
-                    { ProfScope ps(ctx, PROF_GEMM_OUT, 2.0 * nt * H * H);
+                    if (!(ctx->ablate & 4)) { ProfScope ps(ctx, PROF_GEMM_OUT, 2.0 * nt * H * H);
                     rc = gemm_bf16_res_ln_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, pst, pg, pb, y, nt, H, H); }
                     if (rc) return rc;
-                    { ProfScope ps(ctx, PROF_ROW, ln_bytes);
+                    if (!(ctx->ablate & 2)) { ProfScope ps(ctx, PROF_ROW, ln_bytes);
                     launch_layer_norm(st, row_grid, y, nt, H, L.g_1, L.b_1, d.ln_eps, nullptr, xb, stats); }
                     CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
                     { ProfScope ps(ctx, PROF_GEMM_FFN1, 2.0 * nt * F * H);
-                    rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_1, L.b_1f, nullptr, f, nt, F, H, 1); }
+                    rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_1, L.b_1f, nullptr, f, nt, F, H, (ctx->ablate & 8) ? 0 : 1); }
                     if (rc) return rc;
                     { ProfScope ps(ctx, PROF_GEMM_FFN2, 2.0 * nt * F * H);
                     rc = gemm_bf16_res_ln_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, y, stats, L.g_1, L.b_1, x, nt, H, F); }
                     if (rc) return rc;
-                    { ProfScope ps(ctx, PROF_ROW, ln_bytes + (last ? (double)nt * H * 4 : 0.0));
+                    if (!(ctx->ablate & 2) || last) { ProfScope ps(ctx, PROF_ROW, ln_bytes + (last ? (double)nt * H * 4 : 0.0));
                     launch_layer_norm(st, row_grid, x, nt, H, L.g_2, L.b_2, d.ln_eps, last ? y : nullptr, xb, stats); }
                     CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
                     pst = stats; pg = L.g_2; pb = L.b_2;

@@ -218,6 +218,25 @@ int  anon_pseudonymize(anon_ctx* ctx, anon_cache* cache,
 int  anon_hmac_spans(anon_ctx* ctx, const uint8_t* d_span_bytes, const int64_t* d_span_offsets, int64_t S,
                      const uint8_t* key, size_t key_len, uint8_t* d_digests /* [S,32] */);
 
+/* ---- LayerNorm folded into the GEMMs around it (S8a A4 / A6 -> A2; DESIGN.md section 6 "fold") ---------------------------
+ * The LayerNorm between a layer's FFN and the next layer's QKV projection does not run as a kernel in the BF16 encoder
+ * (hidden 768 / 1024): the FFN2 GEMM (producer) also writes the BF16 copy of its un-normalised output rows and, per row and
+ * per 256-column tile, the partial (sum, sum of squares); the QKV GEMM (consumer) multiplies the raw BF16 rows by
+ * Wf = bf16(W * gamma) and finishes the LayerNorm in its epilogue.  Both are exposed for parity tests and measurements.
+ * Row statistics: part float[M][N_stat / 256][2]; mean = sum / N_stat, rstd = 1 / sqrt(sumsq / N_stat - mean^2 + eps). */
+/* Producer: C[M,N] FP32 = A[M,K] W[N,K]^T + bias + R, Cb = bf16(C), part_out[M][N/256][2] = partial sums of C, where
+ * R = d_res if both d_res_part and d_res_stats are NULL, else R = LN(d_res; gamma, beta) with the rows' (mean, rstd) taken
+ * from d_res_part (partial sums, layout above with N_stat = N) or from d_res_stats (float [M][2] = mean, rstd); giving both
+ * is INVALID_ARG.  N in {256, 512, 768, 1024}, K % 64 == 0 (else UNSUPPORTED).  d_C may alias d_res.  Asynchronous. */
+int  anon_gemm_bf16_fold_res(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias, const float* d_res,
+                             const float* d_res_part, const float* d_res_stats, const float* d_gamma, const float* d_beta,
+                             float eps, float* d_C, void* d_Cb, float* d_part_out, int32_t M, int32_t N, int32_t K);
+/* Consumer: C[M,N] BF16 = rstd_r * (A_raw[M,K] Wf[N,K]^T - mean_r * s[n]) + c[n], i.e. LN(A_raw; gamma, beta) W^T + b when
+ * Wf = bf16(W * gamma), s[n] = sum_k Wf[n,k], c[n] = b[n] + sum_k beta[k] W[n,k]; (mean_r, rstd_r) from d_part with
+ * N_stat = stat_cols (a multiple of 256, normally K).  N > 128, N % 8 == 0, K % 64 == 0.  Asynchronous. */
+int  anon_gemm_bf16_fold(anon_ctx* ctx, const void* d_A_raw, const void* d_Wf, const float* d_c, const float* d_s,
+                         const float* d_part, int32_t stat_cols, float eps, void* d_C, int32_t M, int32_t N, int32_t K);
+
 /* ---- measured issue-rate peaks ("Integer-ALU and MUFU rates are not in MEASURED_PEAKS.json --
  * measure"): the denominators of the "alu" roofline of HMAC-SHA256 (K10) and of the exp ceiling of attention (K3). -------------- */
 /* Runs a register-only micro-kernel (2,048 resident threads per SM, 8 independent chains per thread, no memory traffic in the

@@ -81,6 +81,8 @@ _SIGNATURES = {
     "anon_regex_scan": (ctypes.c_int, [_vp, _vp, _vp, _sz, _vp, _i32, _vp, _i32, _vp]),
     "anon_merge_spans": (ctypes.c_int, [_vp, _vp, _vp, _i32, _vp, _vp, _i32, _vp, _i32, _vp]),
     "anon_ctx_set_regex": (ctypes.c_int, [_vp, _vp]),
+    "anon_gemm_bf16_fold_res": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp, _vp, _vp, _i32, _i32, _i32]),
+    "anon_gemm_bf16_fold": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, ctypes.c_float, _vp, _i32, _i32, _i32]),
     "anon_microbench": (ctypes.c_int, [_vp, _i32, _i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
 }
 
@@ -391,3 +393,19 @@ def anon_microbench(ctx, mode, iters=2048):
     ops, ms = ctypes.c_double(0.0), ctypes.c_double(0.0)
     ctx.check(lib().anon_microbench(ctx._h, mode, iters, ctypes.byref(ops), ctypes.byref(ms)), "anon_microbench")
     return ops.value, ms.value
+
+
+def anon_gemm_bf16_fold_res(ctx, A, W, bias, res, res_part, res_stats, gamma, beta, eps, C, Cb, part_out):
+    """Producer of the LayerNorm fold: C = A W^T + bias + LN(res) (FP32), Cb = bf16(C), part_out = partial row statistics."""
+    M, K = A.shape
+    N = W.shape[0]
+    ctx.check(lib().anon_gemm_bf16_fold_res(ctx._h, _ptr(A), _ptr(W), _ptr(bias), _ptr(res), _ptr(res_part), _ptr(res_stats), _ptr(gamma),
+                                            _ptr(beta), eps, _ptr(C), _ptr(Cb), _ptr(part_out), M, N, K), "anon_gemm_bf16_fold_res")
+
+
+def anon_gemm_bf16_fold(ctx, A_raw, Wf, c, s, part, stat_cols, eps, C):
+    """Consumer of the LayerNorm fold: C = rstd * (A_raw Wf^T - mean * s) + c (BF16)."""
+    M, K = A_raw.shape
+    N = Wf.shape[0]
+    ctx.check(lib().anon_gemm_bf16_fold(ctx._h, _ptr(A_raw), _ptr(Wf), _ptr(c), _ptr(s), _ptr(part), stat_cols, eps, _ptr(C), M, N, K),
+              "anon_gemm_bf16_fold")

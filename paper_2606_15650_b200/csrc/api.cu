@@ -24,7 +24,7 @@ extern "C" const char* const* anon_exported_symbols(void) {
         "anon_decode_spans", "anon_gather_spans", "anon_cache_create", "anon_cache_destroy", "anon_cache_stats", "anon_cache_clear",
         "anon_cache_entry", "anon_cache_export", "anon_pseudonymize", "anon_hmac_spans", "anon_pipeline_host", "anon_gemm_bf16",
         "anon_attention", "anon_splice_records", "anon_pipeline_host_text", "anon_ctx_profile", "anon_ctx_profile_read",
-        "anon_regex_load", "anon_regex_free", "anon_regex_scan", "anon_merge_spans", "anon_ctx_set_regex", "anon_attention_local", "anon_cache_track_use", "anon_cache_evict", "anon_microbench", nullptr};
+        "anon_regex_load", "anon_regex_free", "anon_regex_scan", "anon_merge_spans", "anon_ctx_set_regex", "anon_attention_local", "anon_cache_track_use", "anon_cache_evict", "anon_microbench", "anon_gemm_bf16_fold_res", "anon_gemm_bf16_fold", nullptr};
     return names;
 }
 
@@ -39,6 +39,7 @@ extern "C" int anon_ctx_create(anon_ctx** out, int device, void* cuda_stream, si
     c->stream = (cudaStream_t)cuda_stream;
     { const char* e = getenv("ANON_CHUNK_TOKENS"); c->chunk_tokens_cap = e ? atoll(e) : 0; }
     { const char* e = getenv("ANON_ABLATE"); c->ablate = e ? atoi(e) : 0; }
+    { const char* e = getenv("ANON_FOLD_LN"); c->fold_ln = e ? atoi(e) : 1; }
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);

@@ -37,6 +37,7 @@ struct anon_ctx {
     const void* smem_attr_done[48] = {nullptr};
     int n_smem_attr_done = 0;
     long long chunk_tokens_cap = 0;     // ANON_CHUNK_TOKENS read once at context creation (0 = workspace-limited only)
+    int fold_ln = 1;                    // ANON_FOLD_LN=0 switches the LayerNorm fold off (A/B measurements)
     int ablate = 0;                     // ANON_ABLATE (measurement aid, results are then WRONG): bit 0 skip attention, 1 skip LayerNorm
                                         // kernels, 2 skip the out-projection, 3 FFN1 without GELU -- marginal cost of a kernel class in the step
     // NEXT-4: pattern automaton the host pipeline merges into the NER spans (anon_ctx_set_regex; not owned)
@@ -129,6 +130,13 @@ int gemm_bf16_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, co
                    const float* residual, void* C, int M, int N, int K, int epilogue);
 int gemm_bf16_res_ln_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* res_y,
                           const float2* res_stats, const float* gamma, const float* beta, float* C, int M, int N, int K);
+// LayerNorm folded into the GEMMs (gemm_tcgen05.cu "FOLD"): producer (residual GEMM that also writes the BF16 raw rows and
+// the rows' partial statistics) and consumer (finishes the LayerNorm of its raw A rows in the epilogue)
+int gemm_bf16_fold_res_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* res_y,
+                            const float2* part_in, const float2* res_stats, const float* gamma, const float* beta, float eps, float* C,
+                            __nv_bfloat16* Cb, float2* part_out, int M, int N, int K);
+int gemm_bf16_fold_impl(anon_ctx*, const __nv_bfloat16* A_raw, const __nv_bfloat16* Wf, const float* c, const float* s_vec,
+                        const float2* part_in, int stat_cols, float eps, void* C, int M, int N, int K);
 // qkv = A W^T, RoPE on the q / k heads in the epilogue; table float2 [32][512] pair-major (cos, sin), pos int [M]
 int gemm_bf16_rope_impl(anon_ctx*, const __nv_bfloat16* A, const __nv_bfloat16* W, const int* pos, const float2* table, void* C,
                         int M, int N, int K);

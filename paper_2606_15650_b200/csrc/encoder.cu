@@ -18,6 +18,10 @@
 struct LayerW {
     void *W_qkv, *W_o, *W_1, *W_2;                     // BF16 or FP32 matrices
     float *b_qkv, *b_o, *g_1, *b_1, *b_1f, *b_2f, *g_2, *b_2;
+    // LayerNorm fold (BF16, arch 0, H = 768 / 1024): Wf_qkv = bf16(W_qkv * gamma_2 of the previous layer), s[n] = sum_k Wf[n,k],
+    // c[n] = b[n] + sum_k beta_2[k] W[n,k] (layer 0 reads the normalised embedding: no fold)
+    void* Wf_qkv = nullptr;
+    float *s_qkv = nullptr, *c_qkv = nullptr;
 };
 struct anon_weights {
     anon_ctx* ctx = nullptr;
@@ -33,6 +37,7 @@ struct anon_weights {
     // W_i stored with its rows interleaved per 256-row tile (128 a-rows, then their 128 gate rows) so that the FFN1 GEMM's
     // GeGLU epilogue (gemm_tcgen05.cu EPI 4) finds a and gate in the same accumulator tile
     bool geglu_fused = false;
+    bool folded = false;                               // the fold's tensors were prepared (see LayerW)
     std::vector<LayerW> layers;
 };
 
@@ -74,7 +79,7 @@ size_t per_token_bytes(const anon_model_desc& d) {
     const size_t H = d.hidden, F = d.ffn;
     if (d.arch == 1)      // x, y, h FP32; xb; qkv; ctx; u [2F]; f [F]; position id
         return d.dtype == 1 ? 12 * H + 2 * H + 6 * H + 2 * H + 4 * F + 2 * F + 4 : 12 * H + 12 * H + 4 * H + 8 * F + 4 * F + 4;
-    if (d.dtype == 1) return 4 * H + 2 * H + 4 * H + 6 * H + 2 * H + 2 * F + 8;
+    if (d.dtype == 1) return 4 * H + 2 * H + 4 * H + 6 * H + 2 * H + 2 * F + 8 + 64;     // + row statistics (fold: 2 x H/256 partial pairs)
     return 4 * H + 4 * H + 12 * H + 4 * H + 4 * F;
 }
 
@@ -101,7 +106,7 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
     const size_t H = d.hidden, F = d.ffn, V = d.vocab, NL = d.num_labels, P = d.max_pos;
     const bool bf = d.dtype == 1;
     const size_t msz = bf ? 2 : 4;
-    struct Item { void** dst; size_t n; bool matrix; bool geglu_rows = false; };
+    struct Item { void** dst; size_t n; bool matrix; bool geglu_rows = false; const float* host = nullptr; };
     std::vector<Item> items;
     w->layers.resize(d.layers);
     size_t zero_bytes = 0;
@@ -136,6 +141,46 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
     }
     items.push_back({(void**)&w->W_c, NL * H, false});   // head stays FP32 (values are BF16-representable)
     items.push_back({(void**)&w->b_c, NL, false});
+    // ---- LayerNorm fold: extra tensors computed here from the blob (host, double accumulation) ----
+    std::vector<std::vector<float>> fold_host;
+    if (d.arch == 0 && bf && (H == 768 || H == 1024) && F % 256 == 0) {
+        w->folded = true;
+        // blob offsets of layer l's tensors (fixed order W_qkv, b_qkv, W_o, b_o, g_1, b_1, W_1, b_1f, W_2, b_2f, g_2, b_2)
+        const size_t per_layer = 3 * H * H + 3 * H + H * H + H + 2 * H + F * H + F + H * F + H + 2 * H;
+        const size_t base0 = V * H + P * H + 3 * H;
+        auto bf16_rne = [](float f) { uint32_t u; memcpy(&u, &f, 4); u += 0x7FFFu + ((u >> 16) & 1u); u &= 0xFFFF0000u; float r; memcpy(&r, &u, 4); return r; };
+        auto fold = [&](const float* Wm, const float* bias, const float* gam, const float* bet, size_t N_, void** dW, float** ds, float** dc) {
+            const size_t i0 = fold_host.size();
+            fold_host.emplace_back(N_ * H); fold_host.emplace_back(N_); fold_host.emplace_back(N_);
+            std::vector<float>& Wf2 = fold_host[i0]; std::vector<float>& sv2 = fold_host[i0 + 1]; std::vector<float>& cv = fold_host[i0 + 2];
+            for (size_t n = 0; n < N_; n++) {
+                double ss = 0.0, cc = bias[n];
+                for (size_t k = 0; k < H; k++) {
+                    const float v = bf16_rne(Wm[n * H + k] * gam[k]);
+                    Wf2[n * H + k] = v; ss += v; cc += (double)bet[k] * Wm[n * H + k];
+                }
+                sv2[n] = (float)ss; cv[n] = (float)cc;
+            }
+            items.push_back({dW, N_ * H, true, false, Wf2.data()});
+            items.push_back({(void**)ds, N_, false, false, sv2.data()});
+            items.push_back({(void**)dc, N_, false, false, cv.data()});
+        };
+        fold_host.reserve((size_t)d.layers * 6 + 8);     // the vectors must not move: items keep pointers into them
+        for (int l = 0; l < d.layers; l++) {
+            const float* Lb = blob + base0 + (size_t)l * per_layer;
+            const float* Wqkv = Lb;                   const float* bqkv = Wqkv + 3 * H * H;
+            const float* Wo = bqkv + 3 * H;           const float* bo = Wo + H * H;
+            const float* g1 = bo + H;                 const float* b1 = g1 + H;
+            const float* W1 = b1 + H;                 const float* b1f = W1 + F * H;
+            LayerW& L = w->layers[l];
+            (void)W1; (void)b1f; (void)g1; (void)b1;
+            if (l > 0) {
+                const float* Pb = blob + base0 + (size_t)(l - 1) * per_layer;
+                const float* g2 = Pb + per_layer - 2 * H;  const float* b2 = g2 + H;
+                fold(Wqkv, bqkv, g2, b2, 3 * H, &L.Wf_qkv, &L.s_qkv, &L.c_qkv);
+            }
+        }
+    }
     size_t total = 0, max_matrix = 0;
     for (auto& it : items) {
         total = (total + 255) / 256 * 256 + it.n * (it.matrix ? msz : 4);
@@ -156,7 +201,7 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
         void* dst = w->store + off;
         *it.dst = dst;
         std::vector<float> perm;
-        const float* from = src;
+        const float* from = it.host ? it.host : src;
         if (it.geglu_rows) {                         // tile k: a-rows [128k, 128k + 128), then gate rows F + [128k, 128k + 128)
             perm.resize(it.n);
             for (size_t k = 0; k < F / 128; k++)
@@ -173,11 +218,11 @@ extern "C" int anon_weights_load(anon_ctx* ctx, const anon_model_desc* desc, con
                 e = cudaStreamSynchronize(ctx->stream);      // stage is reused by the next matrix
             }
         } else {
-            e = cudaMemcpyAsync(dst, src, it.n * 4, cudaMemcpyHostToDevice, ctx->stream);
+            e = cudaMemcpyAsync(dst, from, it.n * 4, cudaMemcpyHostToDevice, ctx->stream);
         }
         if (e != cudaSuccess) break;
         off += it.n * (it.matrix ? msz : 4);
-        src += it.n;
+        if (!it.host) src += it.n;
     }
     if (e == cudaSuccess && zero_bytes) {
         e = cudaMemsetAsync(w->store + zero_off, 0, zero_bytes, ctx->stream);
@@ -411,7 +456,55 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
             // normalised FP32 rows (into y) for the classifier head.
             const bool lazy_ln = bf && (H == 768 || H == 1024);
             const float* head_in = x;
-            if (lazy_ln) {
+            const bool fold = lazy_ln && w->folded && ctx->fold_ln && !(ctx->ablate & 7);
+            if (fold) {
+                // LN2 FOLDED into the GEMMs around it (the LayerNorm between a layer's FFN and the next layer's attention): the FFN2
+                // GEMM (producer) writes the un-normalised FP32 rows x, their BF16 copy (into xb) and per-row partial (sum, sum of
+                // squares); the next QKV GEMM (consumer) takes the raw BF16 rows against W_qkv pre-multiplied by gamma_2 and
+                // finishes the LayerNorm in its epilogue (free: that epilogue has slack).  LN1 stays a kernel: folding it into FFN1
+                // made FFN1 epilogue-bound (+11 ms per step; the GELU epilogue has no slack, profiles/r02_summary.md).
+                const int pc = H / 256;
+                float2* part2 = (float2*)c.take((size_t)nt * pc * 8);
+                float2* stats1 = (float2*)c.take((size_t)nt * 8);
+                float2* stats2 = (float2*)c.take((size_t)nt * 8);
+                if (!part2 || !stats1 || !stats2) return ANON_ERR_OOM;
+                const float* pg = nullptr; const float* pb = nullptr;
+                const double ln_bytes = (double)nt * (H * 4 + H * 2 + 8);
+                for (int l = 0; l < d.layers; l++) {
+                    const LayerW& L = w->layers[l];
+                    int rc;
+                    { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * 3 * H * H);
+                    if (l == 0) rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_qkv, L.b_qkv, nullptr, qkv, nt, 3 * H, H, 0);
+                    else rc = gemm_bf16_fold_impl(ctx, xb, (const __nv_bfloat16*)L.Wf_qkv, L.c_qkv, L.s_qkv, part2, H, d.ln_eps, qkv, nt, 3 * H, H); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_ATTN, attn_flops);
+                    rc = attention_run(ctx, plan, qkv, d_cu + s0, tok0, nb, H, d.heads, d.dtype, cx); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_GEMM_OUT, 2.0 * nt * H * H);
+                    rc = gemm_bf16_res_ln_impl(ctx, (const __nv_bfloat16*)cx, (const __nv_bfloat16*)L.W_o, L.b_o, x, l == 0 ? nullptr : stats2, pg, pb, y, nt, H, H); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_ROW, ln_bytes);
+                    launch_layer_norm(st, row_grid, y, nt, H, L.g_1, L.b_1, d.ln_eps, nullptr, xb, stats1); }
+                    CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+                    { ProfScope ps(ctx, PROF_GEMM_FFN1, 2.0 * nt * F * H);
+                    rc = gemm_bf16_impl(ctx, xb, (const __nv_bfloat16*)L.W_1, L.b_1f, nullptr, f, nt, F, H, 1); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_GEMM_FFN2, 2.0 * nt * F * H);
+                    rc = gemm_bf16_fold_res_impl(ctx, (const __nv_bfloat16*)f, (const __nv_bfloat16*)L.W_2, L.b_2f, y, nullptr, stats1, L.g_1, L.b_1,
+                                                 d.ln_eps, x, xb, part2, nt, H, F); }
+                    if (rc) return rc;
+                    { ProfScope ps(ctx, PROF_ROW, (double)nt * (pc * 8 + 8));
+                    enc::stats_from_partials_kernel<<<(unsigned)((nt + 255) / 256), 256, 0, st>>>(part2, nt, pc, 1.0f / (float)H, d.ln_eps, stats2); }
+                    CU_LAUNCH_CHECK(ctx, "stats_from_partials_kernel");
+                    pg = L.g_2; pb = L.b_2;
+                }
+                if (d.layers > 0) {
+                    ProfScope ps(ctx, PROF_ROW, (double)nt * (H * 4 + H * 4 + H * 2));
+                    launch_layer_norm(st, row_grid, x, nt, H, pg, pb, d.ln_eps, y, xb, nullptr);
+                    head_in = y;
+                }
+                CU_LAUNCH_CHECK(ctx, "layer_norm_kernel");
+            } else if (lazy_ln) {
                 float2* stats = (float2*)c.take((size_t)nt * 8);
                 if (!stats) return ANON_ERR_OOM;
                 const float2* pst = nullptr; const float* pg = nullptr; const float* pb = nullptr;   // embedding output: already normal
@@ -445,7 +538,7 @@ int ner_forward_impl(anon_ctx* ctx, WsCursor& ws, const anon_weights* w, const i
                     if (last) head_in = y;
                 }
             }
-            for (int l = 0; l < (lazy_ln ? 0 : d.layers); l++) {
+            for (int l = 0; l < ((lazy_ln || fold) ? 0 : d.layers); l++) {
                 const LayerW& L = w->layers[l];
                 int rc;
                 { ProfScope ps(ctx, PROF_GEMM, 2.0 * nt * 3 * H * H);

@@ -153,6 +153,20 @@ static __global__ void __launch_bounds__(kRowWarps * 32, (N4 <= 6) ? 5 : 4) laye
     }
 }
 
+// Row statistics from the partial sums a folding residual GEMM wrote (gemm_tcgen05.cu FOLD): part[row][cnt] = (sum, sum of squares)
+// over 256 columns each -> stats[row] = (mean, rstd), summed in index order (deterministic).
+static __global__ void __launch_bounds__(256) stats_from_partials_kernel(const float2* __restrict__ part, int ntok, int cnt, float inv_h,
+                                                                         float eps, float2* __restrict__ stats)
+{
+    const int r = blockIdx.x * 256 + threadIdx.x;
+    if (r >= ntok) return;
+    float s = 0.f, q = 0.f;
+    for (int i = 0; i < cnt; i++) { const float2 p = __ldg(part + (size_t)r * cnt + i); s += p.x; q += p.y; }
+    const float mean = s * inv_h;
+    const float var = fmaxf(q * inv_h - mean * mean, 0.f);
+    stats[r] = make_float2(mean, 1.0f / sqrtf(var + eps));
+}
+
 // K6: logits = x W_c^T + b_c (FP32), label = argmax (ties -> lowest index).
 static __global__ void __launch_bounds__(kRowWarps * 32) head_argmax_kernel(
     const float* __restrict__ x, int ntok, int H, const float* __restrict__ W_c, const float* __restrict__ b_c, int NL,

@@ -37,11 +37,11 @@ constexpr int A_STAGE_BYTES = BM * BK * 2;
 // 128 rows of the accumulator and staging only half of the B tile (halves shared-memory fill and operand traffic).
 constexpr int kRopeStride = 512;   // positions per pair row of the EPI 5 (cos, sin) table (max_pos <= 512)
 
-template <int BN, int EPI, int NB, int CG> struct Cfg {
+template <int BN, int EPI, int NB, int CG, bool FOLD = false> struct Cfg {
     static constexpr int B_STAGE_BYTES = (BN / CG) * BK * 2;
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
     static constexpr int EPI_WARPS = (EPI == 2) ? 4 : 8;
-    static constexpr int EPI_BYTES = (EPI == 2) ? 4 * NB * 4096 + 12288 /*bias, gamma, beta staged for the epilogue*/ : 8 * 4096;   // 4 KB boxes
+    static constexpr int EPI_BYTES = (EPI == 2) ? 4 * NB * 4096 + 12288 + (FOLD ? 8 * 4096 : 0) /*FOLD: two BF16 boxes per warp*/ /*bias, gamma, beta staged for the epilogue*/ : 8 * 4096;   // 4 KB boxes
     static constexpr int STAGES = (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES > 6 ? 6 : (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES;
     static constexpr int TMEM_COLS = 2 * BN;                      // two accumulator buffers
     static constexpr int NUM_BARS = 2 * STAGES + 4 + 32;
@@ -86,7 +86,8 @@ __device__ __forceinline__ uint64_t gelu2_f32(uint64_t z) {
     const uint64_t u = mul2(p, z);
     float u0, u1;
     upk2(u, u0, u1);
-    const uint64_t d = add2(pk2(ex2_approx(u0), ex2_approx(u1)), pk2(1.0f, 1.0f));
+    const uint64_t e = pk2(ex2_approx(u0), ex2_approx(u1));
+    const uint64_t d = add2(e, pk2(1.0f, 1.0f));
     float d0, d1;
     upk2(d, d0, d1);
     return mul2(z, pk2(rcp_approx(d0), rcp_approx(d1)));
@@ -124,15 +125,33 @@ __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
 //          (columns < 2N/3) every 64-column box is one head and its pairs (j, j + 32) turn by the angle of the row's
 //          position.  rope_tab = (cos, sin) table float2 [32][kRopeStride] (pair-major, so that the rows of a warp --
 //          consecutive positions -- read consecutive entries), rope_pos = int position id per row
-template <int BN, int EPI, int NB, int CG>
+// FOLD (LayerNorm folded into the GEMMs; EPI 0 / 2 only): row statistics travel as PARTIAL sums, part[row][i] = (sum, sum of
+// squares) over the 256 columns of n-tile i of the GEMM that produced the row, stat_cnt = H / 256 of them, summed in a fixed
+// order (deterministic, no atomics); mean = S / H, rstd = 1 / sqrt(Q / H - mean^2 + eps).
+//   EPI 2 + FOLD (producer): besides C = acc + bias + LN(residual) as FP32 it writes bf16(C) through tmap_yb (the NEXT GEMM's
+//          raw A operand) and part_out[row][n_blk]; the residual's own (mean, rstd) come from part_in instead of res_stats.
+//   EPI 0 + FOLD (consumer): A holds raw rows y, W holds bf16(W * gamma); the epilogue finishes the LayerNorm:
+//          z = rstd * (acc - mean * s_n) + c_n with fold_s[n] = sum_k W'[n,k] and bias[n] = c_n = b_n + sum_k beta_k W[n,k].
+__device__ __forceinline__ float2 row_stats_from_partials(const float2* __restrict__ part, int row, int cnt, float inv_h, float eps) {
+    float s = 0.f, q = 0.f;
+    for (int i = 0; i < cnt; i++) { const float2 p = __ldg(part + (size_t)row * cnt + i); s += p.x; q += p.y; }
+    const float mean = s * inv_h;
+    const float var = fmaxf(q * inv_h - mean * mean, 0.f);
+    return make_float2(mean, 1.0f / sqrtf(var + eps));
+}
+
+template <int BN, int EPI, int NB, int CG, bool FOLD>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                          const __grid_constant__ CUtensorMap tmap_c, const __grid_constant__ CUtensorMap tmap_r,
+                         const __grid_constant__ CUtensorMap tmap_yb,
                          const float* __restrict__ bias, const float* __restrict__ ln_g, const float* __restrict__ ln_b,
                          const float2* __restrict__ res_stats, const float2* __restrict__ rope_tab,
-                         const int* __restrict__ rope_pos, int M, int N, int K)
+                         const int* __restrict__ rope_pos, const float2* __restrict__ part_in, int stat_cnt, float inv_h, float ln_eps,
+                         float2* __restrict__ part_out, const float* __restrict__ fold_s, int M, int N, int K)
 {
-    using C = Cfg<BN, EPI, NB, CG>;
+    static_assert(!FOLD || EPI == 0 || EPI == 2, "FOLD: the plain (consumer) and the residual (producer) epilogue only");
+    using C = Cfg<BN, EPI, NB, CG, FOLD>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t epi_base = smem_base + C::STAGES * C::STAGE_BYTES;
@@ -169,6 +188,7 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
         ptx::prefetch_tensormap(&tmap_b);
         ptx::prefetch_tensormap(&tmap_c);
         if (EPI >= 2) ptx::prefetch_tensormap(&tmap_r);
+        if (EPI == 2 && FOLD) ptx::prefetch_tensormap(&tmap_yb);
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < C::STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
@@ -182,8 +202,8 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             float* par = reinterpret_cast<float*>(smem_raw + (epi_base + 4 * NB * 4096 - ptx::smem_u32(smem_raw)));
             for (int i = threadIdx.x; i < N; i += kThreads) {
                 par[i] = bias[i];
-                par[1024 + i] = res_stats ? ln_g[i] : 1.f;
-                par[2048 + i] = res_stats ? ln_b[i] : 0.f;
+                par[1024 + i] = (res_stats || (FOLD && part_in)) ? ln_g[i] : 1.f;
+                par[2048 + i] = (res_stats || (FOLD && part_in)) ? ln_b[i] : 0.f;
             }
         }
     }
@@ -279,20 +299,28 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             };
             if (lane == 0) { for (uint32_t i = 0; i + 1 < NB; i++) issue_load(i); }
             int m_blk, n_blk;
+            const uint32_t xbuf0 = epi_base + 4u * NB * 4096u + 12288u + (uint32_t)(q * 8192);  // FOLD: this warp's two BF16 boxes (32 rows x 64 columns)
+            (void)xbuf0;
+            const bool res_ln = res_stats != nullptr || (FOLD && part_in != nullptr);      // the residual needs its LayerNorm
+            auto load_stats = [&](int rn) -> float2 {
+                if (FOLD && part_in) return row_stats_from_partials(part_in, rn, stat_cnt, inv_h, ln_eps);
+                return __ldg(res_stats + rn);
+            };
             float2 st_next = make_float2(0.f, 1.f);
-            if (res_stats && get_tile(0, m_blk, n_blk)) {
+            if (res_ln && get_tile(0, m_blk, n_blk)) {
                 const int rn = m_blk * TM + rank * BM + q * 32 + lane;
-                if (rn < M) st_next = __ldg(res_stats + rn);
+                if (rn < M) st_next = load_stats(rn);
             }
+            float f_sum = 0.f, f_sq = 0.f;            // FOLD: this row's partial statistics over the tile's columns
             for (int lt = 0; get_tile(lt, m_blk, n_blk); lt++) {
                 const int row0 = m_blk * TM + rank * BM + q * 32;
                 // (mean, rstd) of this thread's residual row: loaded one tile ahead so that no box waits for it
                 const float r_mu = st_next.x, r_rs = st_next.y;
                 {
                     int mb2, nb2;
-                    if (res_stats && get_tile(lt + 1, mb2, nb2)) {
+                    if (res_ln && get_tile(lt + 1, mb2, nb2)) {
                         const int rn = mb2 * TM + rank * BM + q * 32 + lane;
-                        if (rn < M) st_next = __ldg(res_stats + rn);
+                        if (rn < M) st_next = load_stats(rn);
                     }
                 }
                 ptx::mbar_wait(tfull_bar(acc), acc_ph);
@@ -324,15 +352,50 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                                 uint64_t x0, x1, b0, b1;
                                 ld_shared_2x2(addr, x0, x1);
                                 ld_shared_2x2(pc, b0, b1);
-                                if (res_stats) {          // the residual is stored un-normalised: x = LN(y) on the fly
+                                if (res_ln) {             // the residual is stored un-normalised: x = LN(y) on the fly
                                     uint64_t g0, g1, e0, e1;
                                     ld_shared_2x2(pc + 4096u, g0, g1);
                                     ld_shared_2x2(pc + 8192u, e0, e1);
                                     x0 = fma2(fma2(x0, rs2, nmr2), g0, e0);
                                     x1 = fma2(fma2(x1, rs2, nmr2), g1, e1);
                                 }
-                                st_shared_2x2(addr, add2(add2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), b0), x0),
-                                              add2(add2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), b1), x1));
+                                const uint64_t o01 = add2(add2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), b0), x0);
+                                const uint64_t o23 = add2(add2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), b1), x1);
+                                st_shared_2x2(addr, o01, o23);
+                                if (FOLD) {               // keep the values for the statistics and the BF16 copy (r[] is free now)
+                                    float o0, o1, o2, o3;
+                                    upk2(o01, o0, o1); upk2(o23, o2, o3);
+                                    r[4 * v + 0] = __float_as_uint(o0); r[4 * v + 1] = __float_as_uint(o1);
+                                    r[4 * v + 2] = __float_as_uint(o2); r[4 * v + 3] = __float_as_uint(o3);
+                                }
+                            }
+                            if (FOLD) {
+                                if (j == 0) { f_sum = 0.f; f_sq = 0.f; }
+                                uint64_t s2a = pk2(0.f, 0.f), s2b = s2a, q2a = s2a, q2b = s2a;      // packed FP32x2 partial sums
+#pragma unroll
+                                for (int e = 0; e < 32; e += 4) {
+                                    const uint64_t v01 = pk2(__uint_as_float(r[e]), __uint_as_float(r[e + 1]));
+                                    const uint64_t v23 = pk2(__uint_as_float(r[e + 2]), __uint_as_float(r[e + 3]));
+                                    s2a = add2(s2a, v01); s2b = add2(s2b, v23);
+                                    q2a = fma2(v01, v01, q2a); q2b = fma2(v23, v23, q2b);
+                                }
+                                float sa, sb, qa, qb;
+                                upk2(add2(s2a, s2b), sa, sb); upk2(add2(q2a, q2b), qa, qb);
+                                f_sum += sa + sb;
+                                f_sq += qa + qb;
+                                // two BF16 boxes per warp, alternating per box pair: the store of the box filled two pairs ago was
+                                // committed >= 3 groups back, and every iteration ends with wait_group.read 1.  (One box + a full
+                                // wait per pair keeps FFN2's fifth main-loop stage and is 3.5 ms faster in FFN2 itself, but measured
+                                // 1.4 ms slower over the whole power-capped step: profiles/r02_summary.md.)
+                                const uint32_t xbuf = xbuf0 + (uint32_t)(((j >> 1) & 1) * 4096);
+#pragma unroll
+                                for (int c4 = 0; c4 < 4; c4++)      // 16-byte chunks (j & 1) * 4 + c4 of the 64-column BF16 row
+                                    st_shared_v4(xbuf + row_off + ((((uint32_t)((j & 1) * 4 + c4)) ^ sw) << 4),
+                                                 pack_bf16(__uint_as_float(r[8 * c4 + 0]), __uint_as_float(r[8 * c4 + 1])),
+                                                 pack_bf16(__uint_as_float(r[8 * c4 + 2]), __uint_as_float(r[8 * c4 + 3])),
+                                                 pack_bf16(__uint_as_float(r[8 * c4 + 4]), __uint_as_float(r[8 * c4 + 5])),
+                                                 pack_bf16(__uint_as_float(r[8 * c4 + 6]), __uint_as_float(r[8 * c4 + 7])));
+                                if (j == BPT - 1 && row0 + lane < M) part_out[(size_t)(row0 + lane) * num_n + n_blk] = make_float2(f_sum, f_sq);
                             }
                         } else {
 #pragma unroll
@@ -349,7 +412,10 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                         }
                         ptx::fence_proxy_async();
                         __syncwarp();
-                        if (lane == 0) ptx::tma_store_2d(&tmap_c, buf, col, row0);
+                        if (lane == 0) {
+                            ptx::tma_store_2d(&tmap_c, buf, col, row0);
+                            if (FOLD && (j & 1)) ptx::tma_store_2d(&tmap_yb, xbuf0 + (uint32_t)(((j >> 1) & 1) * 4096), col - 32, row0);
+                        }
                     }
                     if (lane == 0) {
                         ptx::bulk_commit();
@@ -365,8 +431,18 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             const int half = (warp - 4) >> 2;
             const uint32_t buf = epi_base + (uint32_t)((warp - 4) * 4096);
             int m_blk, n_blk;
+            uint64_t fa2 = 0, fb2 = 0;
+            int fold_mblk = -1;
+            (void)fa2; (void)fb2; (void)fold_mblk;
             for (int lt = 0; get_tile(lt, m_blk, n_blk); lt++) {
                 const int row0 = m_blk * TM + rank * BM + q * 32;
+                // FOLD consumer: z = a * acc + (b * s_n + c_n) with a = rstd, b = -rstd * mean of this thread's (raw) A row
+                if (FOLD && m_blk != fold_mblk) {         // the pair keeps a row block for all its n-tiles: one load per row block
+                    float2 st = make_float2(0.f, 1.f);
+                    if (row0 + lane < M) st = row_stats_from_partials(part_in, row0 + lane, stat_cnt, inv_h, ln_eps);
+                    fa2 = pk2(st.y, st.y); fb2 = pk2(-st.x * st.y, -st.x * st.y);
+                    fold_mblk = m_blk;
+                }
                 ptx::mbar_wait(tfull_bar(acc), acc_ph);
                 ptx::tc_fence_after();
                 const uint32_t t_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
@@ -438,8 +514,16 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                         for (int v = 0; v < 16; v++) {             // 4 columns per step; N % 8 == 0
                             float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
                             if (EPI != 5 && col + 4 * v < N) bb = __ldg(reinterpret_cast<const float4*>(bias + col + 4 * v));
-                            const uint64_t z0 = add2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), pk2(bb.x, bb.y));
-                            const uint64_t z1 = add2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), pk2(bb.z, bb.w));
+                            uint64_t z0, z1;
+                            if (FOLD) {
+                                float4 ss = make_float4(0.f, 0.f, 0.f, 0.f);
+                                if (col + 4 * v < N) ss = __ldg(reinterpret_cast<const float4*>(fold_s + col + 4 * v));
+                                z0 = fma2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), fa2, fma2(fb2, pk2(ss.x, ss.y), pk2(bb.x, bb.y)));
+                                z1 = fma2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), fa2, fma2(fb2, pk2(ss.z, ss.w), pk2(bb.z, bb.w)));
+                            } else {
+                                z0 = add2(pk2(__uint_as_float(r[4 * v + 0]), __uint_as_float(r[4 * v + 1])), pk2(bb.x, bb.y));
+                                z1 = add2(pk2(__uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3])), pk2(bb.z, bb.w));
+                            }
                             if (EPI == 1) {
                                 o[2 * v] = gelu2_bf16(z0);
                                 o[2 * v + 1] = gelu2_bf16(z1);
@@ -509,18 +593,21 @@ int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_
 
 namespace {
 
-struct LnArgs { const float* gamma; const float* beta; const float2* res_stats;
-                const float2* rope_tab = nullptr; const int* rope_pos = nullptr; };
+struct LnArgs { const float* gamma = nullptr; const float* beta = nullptr; const float2* res_stats = nullptr;
+                const float2* rope_tab = nullptr; const int* rope_pos = nullptr;
+                // FOLD
+                const float2* part_in = nullptr; int stat_cnt = 0; int stat_cols = 1; float eps = 0.f;
+                float2* part_out = nullptr; void* yb_out = nullptr; const float* fold_s = nullptr; };
 
-template <int BN, int EPI, int NB, int CG>
+template <int BN, int EPI, int NB, int CG, bool FOLD = false>
 int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* residual,
                 void* Cout, int M, int N, int K, const LnArgs* ln = nullptr)
 {
-    using C = Cfg<BN, EPI, NB, CG>;
+    using C = Cfg<BN, EPI, NB, CG, FOLD>;
     const int tiles = ((M + BM * CG - 1) / (BM * CG)) * ((N + BN - 1) / BN);
     const int slots = ctx->sm_count / CG;
     int grid = CG * (tiles < slots ? tiles : slots);
-    CUtensorMap ta, tb, tc, tr;
+    CUtensorMap ta, tb, tc, tr, tyb;
     int rc = make_tmap_2d(ctx, &ta, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, A, (uint64_t)M, (uint64_t)K, BK, BM);
     if (rc) return rc;
     rc = make_tmap_2d(ctx, &tb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, W, (uint64_t)N, (uint64_t)K, BK, BN / CG);
@@ -535,7 +622,12 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
         if (rc) return rc;
         tr = tc;
     }
-    auto kern = gemm_bf16_tcgen05_kernel<BN, EPI, NB, CG>;
+    tyb = tc;
+    if (EPI == 2 && FOLD) {
+        rc = make_tmap_2d(ctx, &tyb, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, ln->yb_out, (uint64_t)M, (uint64_t)N, 64, 32);
+        if (rc) return rc;
+    }
+    auto kern = gemm_bf16_tcgen05_kernel<BN, EPI, NB, CG, FOLD>;
     rc = ensure_smem_attr(ctx, (const void*)kern, C::SMEM_BYTES);
     if (rc) return rc;
     cudaLaunchConfig_t cfg = {};
@@ -549,7 +641,13 @@ int launch_gemm(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, c
     const float2* rs = ln ? ln->res_stats : nullptr;
     const float2* rtab = ln ? ln->rope_tab : nullptr;
     const int* rpos = ln ? ln->rope_pos : nullptr;
-    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, bias, g, be, rs, rtab, rpos, M, N, K));
+    const float2* pin = ln ? ln->part_in : nullptr;
+    const int scnt = ln ? ln->stat_cnt : 0;
+    const float inv_h = ln ? 1.0f / (float)ln->stat_cols : 1.f;
+    const float eps = ln ? ln->eps : 0.f;
+    float2* pout = ln ? ln->part_out : nullptr;
+    const float* fs = ln ? ln->fold_s : nullptr;
+    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, tr, tyb, bias, g, be, rs, rtab, rpos, pin, scnt, inv_h, eps, pout, fs, M, N, K));
     CU_LAUNCH_CHECK(ctx, "gemm_bf16_tcgen05_kernel");
     return ANON_OK;
 }
@@ -590,7 +688,7 @@ int gemm_bf16_rope_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat
     if (!ctx || !A || !W || !pos || !table || !Cout || M < 0 || N <= 128 || K <= 0) return ANON_ERR_INVALID_ARG;
     if (K % BK != 0 || N % 192 != 0) return ANON_ERR_UNSUPPORTED;
     if (M == 0) return ANON_OK;
-    LnArgs ln{nullptr, nullptr, nullptr, table, pos};
+    LnArgs ln; ln.rope_tab = table; ln.rope_pos = pos;
     return launch_gemm<256, 5, 2, 2>(ctx, A, W, nullptr, nullptr, Cout, M, N, K, &ln);
 }
 
@@ -603,9 +701,39 @@ int gemm_bf16_res_ln_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bflo
         return ANON_ERR_INVALID_ARG;
     if (K % BK != 0 || N % 8 != 0 || (res_stats && N > 1024)) return ANON_ERR_UNSUPPORTED;
     if (M == 0) return ANON_OK;
-    LnArgs ln{gamma, beta, res_stats};
+    LnArgs ln; ln.gamma = gamma; ln.beta = beta; ln.res_stats = res_stats;
     if (K >= 2048) return launch_gemm<256, 2, 2, 2>(ctx, A, W, bias, res_y, C, M, N, K, &ln);
     return launch_gemm<256, 2, 5, 2>(ctx, A, W, bias, res_y, C, M, N, K, &ln);      // 5 boxes per warp + 4 mainloop stages
+}
+
+// ---- LayerNorm folded into the GEMMs (see the FOLD note above the kernel); H = 768 / 1024 shapes of the encoder ----
+// Producer: C = A W^T + bias + LN(res_y) as FP32, Cb = bf16(C), part_out[row][N / 256] = partial (sum, sum of squares).
+// The residual's (mean, rstd) come from part_in (partial sums) or res_stats (finished pairs); both NULL: res_y is already normalised.
+int gemm_bf16_fold_res_impl(anon_ctx* ctx, const __nv_bfloat16* A, const __nv_bfloat16* W, const float* bias, const float* res_y,
+                            const float2* part_in, const float2* res_stats, const float* gamma, const float* beta, float eps, float* C,
+                            __nv_bfloat16* Cb, float2* part_out, int M, int N, int K)
+{
+    if (!ctx || !A || !W || !bias || !res_y || !C || !Cb || !part_out || M < 0 || K <= 0 || ((part_in || res_stats) && (!gamma || !beta)) ||
+        (part_in && res_stats))
+        return ANON_ERR_INVALID_ARG;
+    if (K % BK != 0 || N % 256 != 0 || N > 1024 || N < 256) return ANON_ERR_UNSUPPORTED;
+    if (M == 0) return ANON_OK;
+    LnArgs ln; ln.gamma = gamma; ln.beta = beta; ln.part_in = part_in; ln.res_stats = res_stats; ln.stat_cnt = N / 256; ln.stat_cols = N; ln.eps = eps;
+    ln.part_out = part_out; ln.yb_out = Cb;
+    if (K >= 2048) return launch_gemm<256, 2, 2, 2, true>(ctx, A, W, bias, res_y, C, M, N, K, &ln);
+    return launch_gemm<256, 2, 4, 2, true>(ctx, A, W, bias, res_y, C, M, N, K, &ln);
+}
+
+// Consumer: C = epilogue(LN(A_raw) W^T + b) computed as rstd * (A_raw W'^T - mean * s) + c; W' = bf16(W * gamma), s[n] = sum_k W'[n,k],
+// c[n] = b[n] + sum_k beta[k] W[n,k] are prepared at weights load; part_in[row][stat_cols / 256] are the rows' partial statistics.
+int gemm_bf16_fold_impl(anon_ctx* ctx, const __nv_bfloat16* A_raw, const __nv_bfloat16* Wf, const float* c, const float* s_vec,
+                        const float2* part_in, int stat_cols, float eps, void* C, int M, int N, int K)
+{
+    if (!ctx || !A_raw || !Wf || !c || !s_vec || !part_in || !C || M < 0 || N <= 128 || K <= 0) return ANON_ERR_INVALID_ARG;
+    if (K % BK != 0 || N % 8 != 0 || stat_cols % 256 != 0) return ANON_ERR_UNSUPPORTED;
+    if (M == 0) return ANON_OK;
+    LnArgs ln; ln.part_in = part_in; ln.stat_cnt = stat_cols / 256; ln.stat_cols = stat_cols; ln.eps = eps; ln.fold_s = s_vec;
+    return launch_gemm<256, 0, 2, 2, true>(ctx, A_raw, Wf, c, nullptr, C, M, N, K, &ln);
 }
 
 extern "C" int anon_gemm_bf16(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias,
@@ -615,4 +743,24 @@ extern "C" int anon_gemm_bf16(anon_ctx* ctx, const void* d_A, const void* d_W, c
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     return gemm_bf16_impl(ctx, (const __nv_bfloat16*)d_A, (const __nv_bfloat16*)d_W, d_bias, d_residual, d_C, M, N, K,
                           epilogue);
+}
+
+// ---- the fold's two GEMMs exposed for parity tests and per-kernel measurements (include/anonshield.h) ----
+extern "C" int anon_gemm_bf16_fold_res(anon_ctx* ctx, const void* d_A, const void* d_W, const float* d_bias, const float* d_res,
+                                       const float* d_res_part, const float* d_res_stats, const float* d_gamma, const float* d_beta,
+                                       float eps, float* d_C, void* d_Cb, float* d_part_out, int32_t M, int32_t N, int32_t K)
+{
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    return gemm_bf16_fold_res_impl(ctx, (const __nv_bfloat16*)d_A, (const __nv_bfloat16*)d_W, d_bias, d_res, (const float2*)d_res_part,
+                                   (const float2*)d_res_stats, d_gamma, d_beta, eps, d_C, (__nv_bfloat16*)d_Cb, (float2*)d_part_out, M, N, K);
+}
+
+extern "C" int anon_gemm_bf16_fold(anon_ctx* ctx, const void* d_A_raw, const void* d_Wf, const float* d_c, const float* d_s,
+                                   const float* d_part, int32_t stat_cols, float eps, void* d_C, int32_t M, int32_t N, int32_t K)
+{
+    if (!ctx) return ANON_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    return gemm_bf16_fold_impl(ctx, (const __nv_bfloat16*)d_A_raw, (const __nv_bfloat16*)d_Wf, d_c, d_s, (const float2*)d_part, stat_cols, eps,
+                               d_C, M, N, K);
 }

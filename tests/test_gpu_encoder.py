@@ -143,6 +143,79 @@ def test_tcgen05_gemm_against_fp64(env, M, N, K, epi):
         assert (np.abs(got - want) <= 2.0 ** -8 * np.abs(want) + 1e-4 * scale).all()
 
 
+@pytest.mark.parametrize("M,N,K,mode", [(300, 768, 768, "part"), (1000, 768, 3072, "stats"), (256 * 80 + 37, 1024, 1024, "part"),
+                                        (77, 256, 64, "none")])
+def test_fold_producer_gemm_against_fp64(env, M, N, K, mode):
+    """The residual GEMM that feeds the LayerNorm fold (anon_gemm_bf16_fold_res): C = A W^T + b + LN(res) in FP32 with the
+    residual's statistics taken from partial sums / from (mean, rstd) pairs / not at all, its BF16 copy, and the per-row,
+    per-256-column partial (sum, sum of squares) of C; several row blocks per CTA pair, ragged M tail, 1 / 3 / 4 n-tiles."""
+    P, torch, ctx = env
+    from oracle import encoder
+    rng = np.random.default_rng(M + N + K)
+    A = _bf16(rng.standard_normal((M, K)))
+    Wm = _bf16(rng.standard_normal((N, K)) * 0.05)
+    bias = (rng.standard_normal(N) * 0.1).astype(np.float32)
+    res = (rng.standard_normal((M, N)) * 1.5 + 0.3).astype(np.float32)
+    g = (1.0 + 0.1 * rng.standard_normal(N)).astype(np.float32)
+    b = (0.1 * rng.standard_normal(N)).astype(np.float32)
+    r64 = res.astype(np.float64)
+    R = r64 if mode == "none" else encoder.layer_norm(r64, g.astype(np.float64), b.astype(np.float64), 1e-5)
+    want = A.astype(np.float64) @ Wm.astype(np.float64).T + bias + R
+    dev = "cuda:0"
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    part_in = stats_in = None
+    if mode == "part":          # the residual's partial sums, as an earlier producer would have written them
+        pr = np.stack([r64.reshape(M, N // 256, 256).sum(-1), (r64 ** 2).reshape(M, N // 256, 256).sum(-1)], -1)
+        part_in = t(pr.astype(np.float32))
+    if mode == "stats":
+        mean = r64.mean(1)
+        stats_in = t(np.stack([mean, 1.0 / np.sqrt(r64.var(1) + 1e-5)], -1).astype(np.float32))
+    d_C = torch.full((M, N), float("nan"), dtype=torch.float32, device=dev)
+    d_Cb = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device=dev)
+    d_part = torch.full((M, N // 256, 2), float("nan"), dtype=torch.float32, device=dev)
+    P.anon_gemm_bf16_fold_res(ctx, t(A).to(torch.bfloat16), t(Wm).to(torch.bfloat16), t(bias), t(res), part_in, stats_in,
+                              None if mode == "none" else t(g), None if mode == "none" else t(b), 1e-5, d_C, d_Cb, d_part)
+    assert ctx.sync() == 0
+    got = d_C.cpu().numpy().astype(np.float64)
+    scale = max(1.0, np.abs(want).max())
+    assert np.abs(got - want).max() <= 3e-5 * scale
+    gotb = d_Cb.float().cpu().numpy().astype(np.float64)
+    assert (np.abs(gotb - want) <= 2.0 ** -8 * np.abs(want) + 1e-4 * scale).all()
+    gp = d_part.cpu().numpy().astype(np.float64)
+    wp = np.stack([want.reshape(M, N // 256, 256).sum(-1), (want ** 2).reshape(M, N // 256, 256).sum(-1)], -1)
+    assert np.abs(gp - wp).max() <= 2e-4 * np.abs(wp).max()
+
+
+@pytest.mark.parametrize("M,N,K", [(300, 2304, 768), (256 * 75 + 9, 3072, 1024), (128, 136, 256)])
+def test_fold_consumer_gemm_against_fp64(env, M, N, K):
+    """The GEMM that finishes a folded LayerNorm in its epilogue (anon_gemm_bf16_fold): raw BF16 rows, W pre-multiplied by gamma,
+    row statistics from partial sums -> LN(A; gamma, beta) W^T + b, against the plain fp64 definition."""
+    P, torch, ctx = env
+    from oracle import encoder
+    rng = np.random.default_rng(M + N + K + 1)
+    A = _bf16(rng.standard_normal((M, K)) * 1.3 + 0.2)                     # the raw rows as the producer rounds them
+    Wm = _bf16(rng.standard_normal((N, K)) * 0.05)
+    bias = (rng.standard_normal(N) * 0.1).astype(np.float32)
+    g = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
+    b = (0.1 * rng.standard_normal(K)).astype(np.float32)
+    a64 = A.astype(np.float64)
+    want = encoder.layer_norm(a64, g.astype(np.float64), b.astype(np.float64), 1e-5) @ Wm.astype(np.float64).T + bias
+    Wf = _bf16(Wm * g[None, :])                                            # what anon_weights_load prepares (host)
+    s_vec = Wf.astype(np.float64).sum(1).astype(np.float32)
+    c_vec = (bias + Wm.astype(np.float64) @ b.astype(np.float64)).astype(np.float32)
+    part = np.stack([a64.reshape(M, K // 256, 256).sum(-1), (a64 ** 2).reshape(M, K // 256, 256).sum(-1)], -1).astype(np.float32)
+    dev = "cuda:0"
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    d_C = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device=dev)
+    P.anon_gemm_bf16_fold(ctx, t(A).to(torch.bfloat16), t(Wf).to(torch.bfloat16), t(c_vec), t(s_vec), t(part), K, 1e-5, d_C)
+    assert ctx.sync() == 0
+    got = d_C.float().cpu().numpy().astype(np.float64)
+    scale = np.abs(want).max()
+    # one BF16 rounding of the output (2^-9) + the extra rounding of W * gamma (2^-9 per weight, averaging over K)
+    assert (np.abs(got - want) <= 2.0 ** -8 * np.abs(want) + 3e-3 * scale).all()
+    assert np.abs(got - want).mean() <= 2e-3 * scale
+
+
 def _attention_oracle(qkv, cu, H, A):
     from oracle import encoder
     out = np.zeros((qkv.shape[0], H))

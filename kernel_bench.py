@@ -11,7 +11,9 @@ L2 where the kernel is memory-bound.  Peaks: MEASURED_PEAKS.json (else the B200_
 import argparse
 import json
 import os
+import subprocess
 import sys
+import time
 
 import numpy as np
 
@@ -52,7 +54,20 @@ def main():
     hbm, tf_peak, src = _peaks()
     ctx = P.Context(0, workspace_bytes=256 << 20)
 
+    clocks_after = []          # SM clock right after each timed loop, in call order
+
+    def sm_mhz():
+        try:
+            return float(subprocess.check_output(["nvidia-smi", "-i", "0", "--query-gpu=clocks.sm", "--format=csv,noheader,nounits"],
+                                                 text=True).strip().splitlines()[0])
+        except Exception:
+            return None
+
     def timeit(fn, n=args.iters, warm=3):
+        # every kernel is timed ALONE: two seconds of idle first, so that the clock the power-capped GEMM loops leave behind
+        # (1.0-1.3 GHz) does not carry into the next measurement; the clock right after the loop is reported with each number
+        torch.cuda.synchronize()
+        time.sleep(2.0)
         for _ in range(warm):
             fn()
         torch.cuda.synchronize()
@@ -62,12 +77,12 @@ def main():
             fn()
         e1.record()
         torch.cuda.synchronize()
+        clocks_after.append(sm_mhz())
         return e0.elapsed_time(e1) / n
 
     res = {"peaks": {"hbm_gbs": hbm, "bf16_tflops_burst": tf_peak, "source": src}, "tokens": M, "hidden": H}
     # measured issue-rate peaks (anon_microbench): thread-ops/s of the integer-ALU pipe and of MUFU ex2, and the lanes/clk/SM
     # they amount to at the clock nvidia-smi reports right after the run ("record which of 64 / 128")
-    import subprocess
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     names = {0: "lop3+shf+iadd3 mix (ALU + FMA pipes)", 1: "lop3", 2: "shf", 3: "iadd3", 4: "mufu_ex2"}
     mb = {}
@@ -95,7 +110,7 @@ def main():
         ms_ref = timeit(lambda: torch.matmul(A, W.t()))
         fl = 2.0 * M * N * K
         byts = M * K * 2 + N * K * 2 + M * N * (8 if epi == 2 else 2)
-        res[name] = {"M": M, "N": N, "K": K, "ms": ms, "tflops": fl / ms / 1e9, "frac_of_bf16_peak": fl / ms / 1e9 / tf_peak,
+        res[name] = {"M": M, "N": N, "K": K, "ms": ms, "sm_mhz_after": clocks_after[-2], "tflops": fl / ms / 1e9, "frac_of_bf16_peak": fl / ms / 1e9 / tf_peak,
                      "algorithmic_gbs": byts / ms / 1e6, "frac_of_hbm_peak": byts / ms / 1e6 / hbm,
                      "cublas_no_epilogue_ms": ms_ref, "cublas_no_epilogue_tflops": fl / ms_ref / 1e9}
         del A, W, C, resid
@@ -114,7 +129,7 @@ def main():
         d_cu = torch.from_numpy(cu).to(dev)
         ms = timeit(lambda: P.anon_attention(ctx, qkv, d_cu, cu, H, H // 64, 1, out))
         n2 = float((lens[:B].astype(np.float64) ** 2).sum())
-        res[name] = {"tokens": T, "sequences": B, "ms": ms, "tflops": 4.0 * n2 * H / ms / 1e9,
+        res[name] = {"tokens": T, "sequences": B, "ms": ms, "sm_mhz_after": clocks_after[-1], "tflops": 4.0 * n2 * H / ms / 1e9,
                      "exp_per_s": n2 * (H // 64) / ms * 1e3, "frac_of_measured_exp_peak": n2 * (H // 64) / ms * 1e3 / exp_peak_measured,
                      "frac_of_bf16_burst_peak": 4.0 * n2 * H / ms / 1e9 / tf_peak, "algorithmic_gbs": T * H * 2 * 4 / ms / 1e6}
         # NEXT-3: the same inputs through the banded kernel (window 128): a query sees at most 129 keys

@@ -418,7 +418,7 @@ int attention_run(anon_ctx* ctx, const AttnPlan& plan, const void* d_qkv, const 
     if (heads <= 0 || hidden != heads * 64) return ANON_ERR_UNSUPPORTED;
     if (B == 0) return ANON_OK;
     if (dtype == 0) {
-        enc::attention_f32_kernel<<<dim3(B, heads), 128, 0, ctx->stream>>>((const float*)d_qkv, d_cu, 0, tok0, hidden, (float*)d_ctx,
+        enc::attention_f32_kernel<<<dim3(B, heads, (512 + enc::kF32QueryBlock - 1) / enc::kF32QueryBlock), 128, 0, ctx->stream>>>((const float*)d_qkv, d_cu, 0, tok0, hidden, (float*)d_ctx,
                                                                            plan.window ? plan.window / 2 : -1);
         CU_LAUNCH_CHECK(ctx, "attention_f32_kernel");
         return ANON_OK;

@@ -319,9 +319,10 @@ static __global__ void __launch_bounds__(256) sgemm_tn_kernel(const float* __res
     }
 }
 
-// FP32 varlen attention: one CTA per (sequence, head); each warp owns one query at a time; scores in shared
-// memory; exact two-pass softmax in FP32.  qkv [T,3H] with q | k | v column blocks; d_head = 64.
+// FP32 varlen attention: one CTA per (sequence, head, block of 32 queries); each warp owns one query at a time; scores in
+// shared memory; exact two-pass softmax in FP32.  qkv [T,3H] with q | k | v column blocks; d_head = 64.
 // half >= 0 (NEXT-3 local layers): query i sees keys m with |i - m| <= half only.
+constexpr int kF32QueryBlock = 32;     // queries per CTA (grid.z = ceil(max sequence length / 32); blocks past a sequence's end exit)
 static __global__ void __launch_bounds__(128) attention_f32_kernel(const float* __restrict__ qkv, const int* __restrict__ cu,
                                                             int seq0, int tok0, int H, float* __restrict__ ctx, int half = -1)
 {
@@ -334,7 +335,8 @@ static __global__ void __launch_bounds__(128) attention_f32_kernel(const float* 
     const float* Q = qkv + (size_t)a * ld + head * 64;
     const float* Kp = Q + H;
     const float* Vp = Q + 2 * H;
-    for (int i = warp; i < n; i += 4) {
+    const int i_end = min(n, (int)(blockIdx.z + 1) * kF32QueryBlock);
+    for (int i = (int)blockIdx.z * kF32QueryBlock + warp; i < i_end; i += 4) {
         qs[warp][lane] = Q[(size_t)i * ld + lane];
         qs[warp][lane + 32] = Q[(size_t)i * ld + lane + 32];
         __syncwarp();

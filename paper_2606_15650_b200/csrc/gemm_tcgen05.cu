@@ -41,7 +41,7 @@ template <int BN, int EPI, int NB, int CG, bool FOLD = false> struct Cfg {
     static constexpr int B_STAGE_BYTES = (BN / CG) * BK * 2;
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
     static constexpr int EPI_WARPS = (EPI == 2) ? 4 : 8;
-    static constexpr int EPI_BYTES = (EPI == 2) ? 4 * NB * 4096 + 12288 + (FOLD ? 8 * 4096 : 0) /*FOLD: two BF16 boxes per warp*/ /*bias, gamma, beta staged for the epilogue*/ : 8 * 4096;   // 4 KB boxes
+    static constexpr int EPI_BYTES = (EPI == 2) ? 4 * NB * 4096 + 12288 + (FOLD ? 4 * 4096 : 0) /*FOLD: one BF16 box per warp*/ /*bias, gamma, beta staged for the epilogue*/ : 8 * 4096;   // 4 KB boxes
     static constexpr int STAGES = (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES > 6 ? 6 : (227 * 1024 - 2048 - EPI_BYTES) / STAGE_BYTES;
     static constexpr int TMEM_COLS = 2 * BN;                      // two accumulator buffers
     static constexpr int NUM_BARS = 2 * STAGES + 4 + 32;
@@ -299,8 +299,8 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             };
             if (lane == 0) { for (uint32_t i = 0; i + 1 < NB; i++) issue_load(i); }
             int m_blk, n_blk;
-            const uint32_t xbuf0 = epi_base + 4u * NB * 4096u + 12288u + (uint32_t)(q * 8192);  // FOLD: this warp's two BF16 boxes (32 rows x 64 columns)
-            (void)xbuf0;
+            const uint32_t xbuf = epi_base + 4u * NB * 4096u + 12288u + (uint32_t)(q * 4096);   // FOLD: this warp's BF16 box (32 rows x 64 columns)
+            (void)xbuf;
             const bool res_ln = res_stats != nullptr || (FOLD && part_in != nullptr);      // the residual needs its LayerNorm
             auto load_stats = [&](int rn) -> float2 {
                 if (FOLD && part_in) return row_stats_from_partials(part_in, rn, stat_cnt, inv_h, ln_eps);
@@ -383,11 +383,10 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                                 upk2(add2(s2a, s2b), sa, sb); upk2(add2(q2a, q2b), qa, qb);
                                 f_sum += sa + sb;
                                 f_sq += qa + qb;
-                                // two BF16 boxes per warp, alternating per box pair: the store of the box filled two pairs ago was
-                                // committed >= 3 groups back, and every iteration ends with wait_group.read 1.  (One box + a full
-                                // wait per pair keeps FFN2's fifth main-loop stage and is 3.5 ms faster in FFN2 itself, but measured
-                                // 1.4 ms slower over the whole power-capped step: profiles/r02_summary.md.)
-                                const uint32_t xbuf = xbuf0 + (uint32_t)(((j >> 1) & 1) * 4096);
+                                if (!(j & 1)) {           // the BF16 box is refilled: its store (committed BEFORE the FP32 store of the
+                                    if (lane == 0) ptx::bulk_wait_read<1>();      // same iteration, see below) must have read it; the newest
+                                    __syncwarp();                                 // group -- that FP32 store -- may still be in flight
+                                }
 #pragma unroll
                                 for (int c4 = 0; c4 < 4; c4++)      // 16-byte chunks (j & 1) * 4 + c4 of the 64-column BF16 row
                                     st_shared_v4(xbuf + row_off + ((((uint32_t)((j & 1) * 4 + c4)) ^ sw) << 4),
@@ -413,8 +412,11 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
                         ptx::fence_proxy_async();
                         __syncwarp();
                         if (lane == 0) {
+                            if (FOLD && (j & 1)) {        // a bulk group of its own, OLDER than this iteration's FP32 store
+                                ptx::tma_store_2d(&tmap_yb, xbuf, col - 32, row0);
+                                ptx::bulk_commit();
+                            }
                             ptx::tma_store_2d(&tmap_c, buf, col, row0);
-                            if (FOLD && (j & 1)) ptx::tma_store_2d(&tmap_yb, xbuf0 + (uint32_t)(((j >> 1) & 1) * 4096), col - 32, row0);
                         }
                     }
                     if (lane == 0) {

@@ -161,3 +161,50 @@ def test_splice_records_matches_oracle(env):
     P.anon_splice_records(ctx, t(rec["text"]), t(rec["rec_off"]), t(np.asarray(spans, np.int32).reshape(-1, 4)), len(spans),
                           t(ps["out_tokens"]), t(ps["out_offsets"]), small, new_off)
     assert ctx.sync() == -3
+
+
+def test_splice_edge_cases_and_unaligned_buffers(env):
+    """Hand-built records: a span covering a whole record, spans that touch (no gap between them), a span at offset 0 and one
+    ending at the record's end, an empty record, an empty token; text / token / output buffers at odd byte addresses."""
+    P, torch, ctx = env
+    from oracle import decode
+    dev = "cuda:0"
+    recs = [b"ABCDEFGHIJ", b"", b"0123456789abcdefghijklmnopqrstuvwxyz" * 40, b"xy", b"tail-span-here"]
+    text = np.frombuffer(b"".join(recs), np.uint8).copy()
+    ro = np.zeros(len(recs) + 1, np.int64)
+    ro[1:] = np.cumsum([len(r) for r in recs])
+    spans = [(0, 0, 10, 0),                                  # the whole record
+             (2, 0, 3, 1), (2, 3, 7, 2), (2, 7, 8, 0),       # at offset 0, touching each other
+             (2, 500, 530, 1), (2, 1430, 1440, 3),           # ... the last one ends at the record's end
+             (3, 1, 2, 0), (4, 5, 14, 2)]
+    toks = [b"[T0_aaaaaaaaaaaaaaaaaaaaaaaaaaaaaaaa]", b"", b"[X]", b"[LONGER_THAN_THE_SPAN]", b"[s]", b"[END]", b"[ONE_BYTE_SPAN]", b"[t]"]
+    tok = np.frombuffer(b"".join(toks), np.uint8).copy()
+    to = np.zeros(len(toks) + 1, np.int64)
+    to[1:] = np.cumsum([len(x) for x in toks])
+    want, want_off = decode.splice_records(text, ro, spans, tok, to)
+    # independent check of the oracle on this case: plain Python string surgery
+    exp = []
+    for r, body in enumerate(recs):
+        out, cur = b"", 0
+        for (rr, cs, ce, _t), tk in zip(spans, toks):
+            if rr == r:
+                out += body[cur:cs] + tk
+                cur = ce
+        exp.append(out + body[cur:])
+    assert want.tobytes() == b"".join(exp)
+    for shift in (0, 1, 5, 13):
+        big_text = torch.zeros(text.size + 32, dtype=torch.uint8, device=dev)
+        big_text[shift:shift + text.size] = torch.from_numpy(text).to(dev)
+        big_tok = torch.zeros(tok.size + 32, dtype=torch.uint8, device=dev)
+        big_tok[(shift + 2):(shift + 2) + tok.size] = torch.from_numpy(tok).to(dev)
+        big_out = torch.full((want.size + 64,), 0xEE, dtype=torch.uint8, device=dev)
+        out = big_out[shift:shift + want.size + 8]
+        new_off = torch.zeros(len(recs) + 1, dtype=torch.int64, device=dev)
+        P.anon_splice_records(ctx, big_text[shift:shift + text.size], torch.from_numpy(ro).to(dev),
+                              torch.from_numpy(np.asarray(spans, np.int32)).to(dev), len(spans), big_tok[(shift + 2):(shift + 2) + tok.size],
+                              torch.from_numpy(to).to(dev), out, new_off)
+        assert ctx.sync() == 0
+        assert np.array_equal(new_off.cpu().numpy(), want_off)
+        got = big_out.cpu().numpy()
+        assert np.array_equal(got[shift:shift + want.size], want)
+        assert (got[:shift] == 0xEE).all() and (got[shift + want.size:] == 0xEE).all()

@@ -77,3 +77,25 @@ def test_gloo_world2_no_exchange_needed():
         slug0 = d0[e][0].rsplit(b"_", 1)[1]
         slug1 = d1[e][0].rsplit(b"_", 1)[1]
         assert slug0 == slug1
+
+
+def test_bench_gpus_flag_launches_that_many_ranks():
+    """`python bench.py --gpus 2` without torchrun re-executes itself under torch.distributed.run with two ranks (S8e); checked
+    on the CPU box with the reference arm (rank 0 prints the line, rank 1 exits without work), and a --gpus / WORLD_SIZE
+    mismatch fails loudly."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "reference", "--headline-only",
+                          "--steps", "1", "--warmup", "0"], capture_output=True, text=True, env=env, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.strip().splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                   # one JSON line in total, from rank 0
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["impl"] == "reference" and d["value"] > 0
+    bad = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "reference", "--headline-only"],
+                         capture_output=True, text=True, env=dict(env, WORLD_SIZE="3"), timeout=120)
+    assert bad.returncode != 0 and "does not match WORLD_SIZE" in (bad.stderr + bad.stdout)

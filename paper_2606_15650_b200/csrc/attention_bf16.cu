@@ -8,16 +8,17 @@
 //                              packed qkv tensor, 128B swizzle, mbarrier completion
 //   warp 1      MMA issuer   : S = Q K^T   tcgen05.mma M128 N64 K16 x4, both operands K-major in shared memory,
 //                                          accumulator = one of two 64-column S buffers in TMEM
-//                              O += P V    A = P read from TMEM (BF16 pairs written by the softmax warps over the
-//                                          S buffer they have just consumed), B = V chunk, MN-major descriptor
-//                              QK^T of chunk g+1 is issued before PV of chunk g, so the tensor pipe works while the
-//                              softmax warps are busy with chunk g
+//                              O += P V    A = P read from TMEM (BF16 pairs the softmax warps write into P columns of their
+//                                          own), B = V chunk, MN-major descriptor
+//                              QK^T runs TWO chunks ahead of PV: S(g+2) is issued as soon as the softmax warps have S(g) in
+//                              registers, so a finished chunk never waits for the tensor pipe's round trip
 //   warps 2-5   softmax      : one thread per query row: tcgen05.ld S -> FP32 max -> exp2 (1/sqrt(64)*log2(e) folded
 //                              in) -> row sum -> BF16 P -> tcgen05.st.  The running reference max is only raised
 //                              when a chunk exceeds it by more than 2^8 (then O is rescaled in TMEM), so the common
 //                              path never touches O; the final O / l uses the same reference, hence exact.
-// The softmax is MUFU-bound at d_head = 64 (one exp per 256 tensor FLOPs); two CTAs per SM keep the MUFU pipes of
-// all four SMSPs fed while either CTA waits for an MMA or a TMA.
+// TMEM per CTA: S 2 x 64 | P 2 x 32 | O 64 = 256 columns.  Measured (profiles/r02_attention.md): the kernel is bound by the
+// latency of one softmax warp's chain per chunk (about 2,250 cycles per 128 x 64 scores with two such warps per scheduler), not
+// by MUFU (37 % busy) or tensor throughput (27 %); two CTAs per SM interleave two such chains per scheduler.
 #include "common.cuh"
 #include "ptx_sm100.cuh"
 

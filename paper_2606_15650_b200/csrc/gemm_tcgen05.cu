@@ -289,9 +289,9 @@ gemm_bf16_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __gri
             const uint32_t par_base = epi_base + 4u * NB * 4096u;      // gamma | beta, 1024 floats each
             uint32_t rph = 0;                         // phase bit of each residual buffer's barrier
             auto issue_load = [&](uint32_t i) {       // lane 0: residual box i -> buffer i % NB
-                const int tile = cid + (int)(i / BPT) * ncl;
-                if (tile >= num_tiles) return;
-                const int row0 = (tile / num_n) * TM + rank * BM + q * 32, col = (tile % num_n) * BN + (int)(i % BPT) * 32;
+                int mb, nb;
+                if (!get_tile((int)(i / BPT), mb, nb)) return;
+                const int row0 = mb * TM + rank * BM + q * 32, col = nb * BN + (int)(i % BPT) * 32;
                 if (row0 >= M || col >= N) return;
                 const uint32_t bar = rfull_bar(q, i % NB);
                 ptx::mbar_arrive_expect_tx(bar, 4096);

@@ -36,7 +36,6 @@ constexpr int kQBytes = kQT * kD * 2;          // 16 KB
 constexpr int kKVBytes = kKC * kD * 2;         // 8 KB (K and V each)
 constexpr int kAttSmem = 2 * kQBytes + kKVStages * 2 * kKVBytes + 1024 /*align slack*/ + 256 /*barriers*/;
 constexpr int kAttTmemCols = 256;              // S 2 x 64 | P 2 x 32 | O 64
-constexpr int kPolyEvery = 4;                  // every 4th pair of a row takes its exponentials on the FMA pipe (25 %)
 
 // rows relative to the chunk.  Global attention: kv_row0 = the sequence's first row, n = its length.  Local (band) attention
 // (NEXT-3, D20): kv_row0 = first key row any query of the tile may see, n = keys from there, and q_valid carries
@@ -59,25 +58,6 @@ __device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
 __device__ __forceinline__ uint32_t pack2(float a, float b) {
     __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
     return *reinterpret_cast<uint32_t*>(&v);
-}
-
-// 2^t for a packed pair on the FMA pipe (no MUFU): Cody-Waite split t = i + f, i = round(t) via the 1.5 * 2^23 magic add,
-// f in [-0.5, 0.5]; 2^f by a degree-3 minimax polynomial (relative error 7.5e-5, ~50x below the BF16 rounding of P); the
-// integer part goes straight into the exponent field (the magic sum carries i in its low mantissa bits: one shift-add).
-// t is clamped at -126 so the exponent field cannot wrap (masked scores are -inf; the result is then ~1e-38, i.e. 0).
-__device__ __forceinline__ void exp2_pair_fma(uint64_t t, float& p0, float& p1) {
-    float t0, t1;
-    upk2(t, t0, t1);
-    const uint64_t tc = pk2(fmaxf(t0, -126.f), fmaxf(t1, -126.f));
-    const uint64_t rr = add2(tc, pk2(12582912.f, 12582912.f));
-    const uint64_t f = fma2(add2(rr, pk2(-12582912.f, -12582912.f)), pk2(-1.f, -1.f), tc);
-    uint64_t p = fma2(pk2(0.0551716685f, 0.0551716685f), f, pk2(0.2426111251f, 0.2426111251f));
-    p = fma2(p, f, pk2(0.6932609677f, 0.6932609677f));
-    p = fma2(p, f, pk2(0.9999280572f, 0.9999280572f));
-    float q0, q1, r0, r1;
-    upk2(p, q0, q1); upk2(rr, r0, r1);
-    p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(r0) << 23));
-    p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(r1) << 23));
 }
 
 template <bool BAND>
@@ -333,10 +313,9 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     }
 #pragma unroll
                     for (int j = 16 * hh; j < 16 * hh + 16; j++) {
-                        const uint64_t t = fma2(pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])), sc2, nm2);
-                        float p0, p1;
-                        if ((j % kPolyEvery) == kPolyEvery - 1) exp2_pair_fma(t, p0, p1);      // FMA-pipe exponential
-                        else { float t0, t1; upk2(t, t0, t1); p0 = ex2f(t0); p1 = ex2f(t1); }  // MUFU
+                        float t0, t1;
+                        upk2(fma2(pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])), sc2, nm2), t0, t1);
+                        const float p0 = ex2f(t0), p1 = ex2f(t1);
                         if (j & 1) sum_b = add2(sum_b, pk2(p0, p1)); else sum_a = add2(sum_a, pk2(p0, p1));
                         pk[j] = pack2(p0, p1);
                     }

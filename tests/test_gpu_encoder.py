@@ -323,3 +323,23 @@ def test_bf16_small_hidden_generic_path(env):
     e, a = _bf16_model_check(P, torch, ctx, d, w, ids, cu, None, require_agreement=False)
     assert a >= 0.995
     print(f"\nhidden-256 BF16 model: max|dlogit|={e:.2e} agreement={a:.4%}")
+
+
+def test_issue_rate_microbench_is_consistent(env):
+    """anon_microbench (the measured denominators of the "alu" and exp rooflines): the three integer-ALU instruction kinds share
+    one pipe, so their rates agree; MUFU ex2 runs at a quarter of it; all within the physical range of the part."""
+    P, torch, ctx = env
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    rates = {}
+    for mode in (1, 2, 3, 4):
+        P.anon_microbench(ctx, mode, 64)
+        ops, ms = P.anon_microbench(ctx, mode, 1024)
+        assert ops > 0 and ms > 0
+        rates[mode] = ops
+    alu = [rates[1], rates[2], rates[3]]
+    assert max(alu) / min(alu) < 1.1
+    assert 3.0 < min(alu) / rates[4] < 5.0                         # 64 against 16 lanes per clock and SM
+    lanes = min(alu) / (sms * 1.965e9)                             # at most the boost clock
+    assert 20.0 < lanes < 140.0
+    with pytest.raises(P.AnonError):
+        P.anon_microbench(ctx, 9, 16)

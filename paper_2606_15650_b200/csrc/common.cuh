@@ -33,6 +33,11 @@ struct anon_ctx {
     // cached driver entry point for cuTensorMapEncodeTiled (resolved lazily, see gemm_tcgen05.cu)
     void* encode_tiled = nullptr;
     int smem_optin = 0;
+    // tensor maps already encoded for this context (the same activation / weight buffers come back every layer and every step):
+    // make_tmap_2d looks here before calling cuTensorMapEncodeTiled
+    struct TmapKey { const void* base; uint64_t rows, cols; uint32_t box_cols, box_rows, dt; };
+    std::vector<TmapKey> tmap_keys;
+    std::vector<CUtensorMap> tmap_vals;
     // kernels whose MaxDynamicSharedMemorySize opt-in has been set on THIS context's device (the attribute is per device)
     const void* smem_attr_done[48] = {nullptr};
     int n_smem_attr_done = 0;

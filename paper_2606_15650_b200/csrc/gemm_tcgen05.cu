@@ -579,6 +579,13 @@ int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_
             return cuda_fail(ctx, e == cudaSuccess ? cudaErrorUnknown : e, "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)");
         ctx->encode_tiled = fn;
     }
+    for (size_t i = 0; i < ctx->tmap_keys.size(); i++) {
+        const anon_ctx::TmapKey& k = ctx->tmap_keys[i];
+        if (k.base == base && k.rows == rows && k.cols == cols && k.box_cols == box_cols && k.box_rows == box_rows && k.dt == (uint32_t)dt) {
+            *tm = ctx->tmap_vals[i];
+            return ANON_OK;
+        }
+    }
     const cuuint64_t gdim[2] = {cols, rows};
     const cuuint64_t gstride[1] = {cols * esize};
     const cuuint32_t box[2] = {box_cols, box_rows};
@@ -590,6 +597,9 @@ int make_tmap_2d(anon_ctx* ctx, CUtensorMap* tm, CUtensorMapDataType dt, uint32_
         snprintf(ctx->cuda_err, sizeof ctx->cuda_err, "cuTensorMapEncodeTiled failed: CUresult %d", (int)r);
         return ANON_ERR_CUDA;
     }
+    if (ctx->tmap_keys.size() >= 512) { ctx->tmap_keys.clear(); ctx->tmap_vals.clear(); }     // bounded: start over
+    ctx->tmap_keys.push_back(anon_ctx::TmapKey{base, rows, cols, box_cols, box_rows, (uint32_t)dt});
+    ctx->tmap_vals.push_back(*tm);
     return ANON_OK;
 }
 

@@ -134,6 +134,22 @@ int  anon_ner_forward(anon_ctx* ctx, const anon_weights* w,
 int  anon_decode_spans(anon_ctx* ctx, const int32_t* d_labels, const anon_tok_meta* d_meta, int32_t T,
                        int32_t num_labels, anon_span* d_spans, int32_t span_capacity, int32_t* d_num_spans);
 
+/* A9 for callers that may not allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the
+ * same decode, same kernels and same results as anon_decode_spans, but it needs no context and no workspace.  Its scratch
+ * (previous-kept-token index per token, the scan aggregates, a status word; 4.2 MB) is a file-scope device array inside the
+ * library that every GPU loading the library holds until exit.  The call allocates nothing: kernel launches and one 4-byte
+ * memset on `cuda_stream` (NULL = the default stream) of `device`, which it makes current.  Asynchronous.
+ * Limit: T <= ANON_DECODE_STATIC_MAX_TOKENS, else ANON_ERR_CAPACITY and nothing is launched (use anon_decode_spans).
+ * All calls on one device share the array: calls that overlap on the GPU (different streams without an ordering between them)
+ * race and give undefined spans -- keep them stream-ordered.  The array keeps the last call's contents; each call rewrites what
+ * it reads and clears the status word, so nothing carries over.  There is no sticky status here: span_capacity overflow is
+ * reported only through *d_num_spans > span_capacity (the first span_capacity spans are written, as in anon_decode_spans).
+ * All pointers are device pointers owned by the caller.  Errors: INVALID_ARG, UNSUPPORTED (num_labels even or < 1), CAPACITY
+ * (T beyond the limit), CUDA. */
+#define ANON_DECODE_STATIC_MAX_TOKENS 1048576
+int  anon_decode_spans_static(int device, void* cuda_stream, const int32_t* d_labels, const anon_tok_meta* d_meta, int32_t T,
+                              int32_t num_labels, anon_span* d_spans, int32_t span_capacity, int32_t* d_num_spans);
+
 /* ---- A10: span byte gather (S8a A10) ---------------------------------------------------------- */
 /* span_bytes[off_s : off_s + len_s] = text[rec_off[record_id] + char_start : ... + char_end],
  * d_span_offsets int64[S+1] = exclusive prefix sum of the lengths; d_span_type uint8[S]

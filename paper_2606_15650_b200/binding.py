@@ -53,6 +53,7 @@ _SIGNATURES = {
     "anon_weights_free": (None, [_vp]),
     "anon_ner_forward": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i32, _vp, _vp]),
     "anon_decode_spans": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i32, _vp, _i32, _vp]),
+    "anon_decode_spans_static": (ctypes.c_int, [ctypes.c_int, _vp, _vp, _vp, _i32, _i32, _vp, _i32, _vp]),
     "anon_gather_spans": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _vp, _sz, _vp, _vp]),
     "anon_cache_create": (ctypes.c_int, [_vp, _u64, _u64, ctypes.POINTER(_vp)]),
     "anon_cache_destroy": (None, [_vp]),
@@ -283,6 +284,15 @@ def anon_decode_spans(ctx, labels, meta, num_labels, spans, num_spans):
     """labels int32[T], meta int32[T,4], spans int32[cap,4], num_spans int32[1] -- all device tensors."""
     ctx.check(lib().anon_decode_spans(ctx._h, _ptr(labels), _ptr(meta), labels.numel(), num_labels, _ptr(spans),
                                       spans.shape[0], _ptr(num_spans)), "anon_decode_spans")
+
+
+def anon_decode_spans_static(device, cuda_stream, labels, meta, num_labels, spans, num_spans):
+    """anon_decode_spans without a context or any allocation (scratch is a static device array; T <= 1,048,576).  Raises AnonError on anything
+    but ANON_OK."""
+    rc = lib().anon_decode_spans_static(int(device), ctypes.c_void_p(cuda_stream or 0), _ptr(labels), _ptr(meta), labels.numel(),
+                                        num_labels, _ptr(spans), spans.shape[0], _ptr(num_spans))
+    if rc != 0:
+        raise AnonError(rc, "anon_decode_spans_static")
 
 
 def anon_gather_spans(ctx, text, record_offsets, spans, S, span_bytes, span_offsets, span_type=None):

@@ -24,7 +24,7 @@ extern "C" const char* const* anon_exported_symbols(void) {
         "anon_decode_spans", "anon_gather_spans", "anon_cache_create", "anon_cache_destroy", "anon_cache_stats", "anon_cache_clear",
         "anon_cache_entry", "anon_cache_export", "anon_pseudonymize", "anon_hmac_spans", "anon_pipeline_host", "anon_gemm_bf16",
         "anon_attention", "anon_splice_records", "anon_pipeline_host_text", "anon_ctx_profile", "anon_ctx_profile_read",
-        "anon_regex_load", "anon_regex_free", "anon_regex_scan", "anon_merge_spans", "anon_ctx_set_regex", "anon_attention_local", "anon_cache_track_use", "anon_cache_evict", "anon_microbench", "anon_gemm_bf16_fold_res", "anon_gemm_bf16_fold", nullptr};
+        "anon_regex_load", "anon_regex_free", "anon_regex_scan", "anon_merge_spans", "anon_ctx_set_regex", "anon_attention_local", "anon_cache_track_use", "anon_cache_evict", "anon_microbench", "anon_gemm_bf16_fold_res", "anon_gemm_bf16_fold", "anon_decode_spans_static", nullptr};
     return names;
 }
 

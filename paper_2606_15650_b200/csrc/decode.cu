@@ -369,3 +369,72 @@ extern "C" int anon_gather_spans(anon_ctx* ctx, const uint8_t* d_text, const int
     return gather_spans_impl(ctx, ws, d_text, d_record_offsets, d_spans, nullptr, S, d_span_bytes, bytes_capacity,
                              d_span_offsets, d_span_type);
 }
+
+// ---- A9 without any allocation: anon_decode_spans_static ---------------------------------------------------------------------
+// The same two transform-scans as decode_spans_impl, with the scratch (prev_kept[T], the tile aggregates of both scans and a
+// status word) in a file-scope device array instead of the context workspace: no context, no cudaMalloc / cudaFree, nothing but
+// kernel launches and one 4-byte memset on the caller's stream.  For callers that may not allocate (code under CUDA graph capture,
+// serving loops, harnesses that forbid it).  Every GPU that loads the library holds the array (4.2 MB) until exit; every call on a
+// device shares it, so two calls that overlap on the GPU (different streams) race -- serialise them.  Nothing in it has to start at
+// zero except the status word, which each call clears: prev_kept and the aggregates are fully rewritten for the call's T before
+// they are read.
+namespace {
+
+constexpr int kStaticMaxTokens = ANON_DECODE_STATIC_MAX_TOKENS;
+constexpr size_t kStaticStatusBytes = 256;
+constexpr size_t kStaticPrevBytes = (size_t)kStaticMaxTokens * 4;
+constexpr size_t kStaticAggI = ((size_t)(kStaticMaxTokens / scan::kTile + 2) * sizeof(int) + 255) / 256 * 256;
+constexpr size_t kStaticAggL = ((size_t)(kStaticMaxTokens / scan::kTile + 2) * sizeof(long long) + 255) / 256 * 256;
+constexpr size_t kStaticBytes = kStaticStatusBytes + kStaticPrevBytes + kStaticAggI + kStaticAggL;
+
+static __device__ __align__(256) uint8_t g_decode_static_scratch[kStaticBytes];
+
+// In host code `g_decode_static_scratch` is only a stand-in for the symbol: the device address comes from cudaGetSymbolAddress,
+// asked once per device with that device current.
+constexpr int kStaticMaxDevices = 64;
+uint8_t* g_static_ptr[kStaticMaxDevices] = {nullptr};
+
+int static_scratch(int device, uint8_t** out) {
+    if (device < 0 || device >= kStaticMaxDevices) return ANON_ERR_INVALID_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return ANON_ERR_CUDA; }
+    uint8_t* p = __atomic_load_n(&g_static_ptr[device], __ATOMIC_ACQUIRE);
+    if (!p) {
+        void* sym = nullptr;
+        if (cudaGetSymbolAddress(&sym, g_decode_static_scratch) != cudaSuccess || !sym) { cudaGetLastError(); return ANON_ERR_CUDA; }
+        p = (uint8_t*)sym;
+        __atomic_store_n(&g_static_ptr[device], p, __ATOMIC_RELEASE);     // racing first calls store the same address
+    }
+    *out = p;
+    return ANON_OK;
+}
+
+}  // namespace
+
+extern "C" int anon_decode_spans_static(int device, void* cuda_stream, const int32_t* d_labels, const anon_tok_meta* d_meta, int32_t T,
+                                        int32_t num_labels, anon_span* d_spans, int32_t span_capacity, int32_t* d_num_spans)
+{
+    if (T < 0 || span_capacity < 0 || !d_num_spans || (T > 0 && (!d_labels || !d_meta)) || (span_capacity > 0 && !d_spans))
+        return ANON_ERR_INVALID_ARG;
+    if (num_labels < 1 || (num_labels & 1) == 0) return ANON_ERR_UNSUPPORTED;
+    if (T > kStaticMaxTokens) return ANON_ERR_CAPACITY;                 // beyond the static scratch: use anon_decode_spans
+    uint8_t* base = nullptr;
+    const int rc = static_scratch(device, &base);
+    if (rc != ANON_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (T == 0) return cudaMemsetAsync(d_num_spans, 0, 4, st) == cudaSuccess ? ANON_OK : (cudaGetLastError(), ANON_ERR_CUDA);
+    int* status = (int*)base;
+    int* prev = (int*)(base + kStaticStatusBytes);
+    int* agg_i = (int*)(base + kStaticStatusBytes + kStaticPrevBytes);
+    long long* agg_l = (long long*)(base + kStaticStatusBytes + kStaticPrevBytes + kStaticAggI);
+    if (cudaMemsetAsync(status, 0, 4, st) != cudaSuccess) { cudaGetLastError(); return ANON_ERR_CUDA; }
+    KeepIn kin{d_meta};
+    scan::reduce_and_scan<int, scan::MaxI32>(kin, T, nullptr, agg_i, st);
+    scan::apply<int, scan::MaxI32>(kin, PrevKeptOut{prev}, T, nullptr, agg_i, st);
+    StartIn sin{d_labels, d_meta, prev};
+    scan::reduce_and_scan<long long, scan::SumI64>(sin, T, nullptr, agg_l, st);
+    scan::apply<long long, scan::SumI64>(sin, StartOut{d_labels, d_meta, prev, d_spans, span_capacity}, T, nullptr, agg_l, st);
+    decode_finish_kernel<<<1, 1, 0, st>>>(d_labels, d_meta, prev, T, agg_l + scan::num_tiles(T), d_spans, span_capacity, d_num_spans,
+                                          status);
+    if (cudaGetLastError() != cudaSuccess) return ANON_ERR_CUDA;
+    return ANON_OK;
+}

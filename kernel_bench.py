@@ -31,6 +31,27 @@ def _peaks():
     return 6650.0, 1590.0, "fallback"
 
 
+def _att_prof(P):
+    """Cycles per 128 x 64 chunk in each wait / phase of the MMA issuer and of two softmax warps of virtual CTA 0, from the clock64
+    counters an ATT_PROF build of attention_bf16.cu keeps (the counters themselves cost ~40-60 cycles per reading)."""
+    import ctypes
+    from paper_2606_15650_b200 import binding
+    lib = binding.lib()
+    if not hasattr(lib, "anon_debug_att_prof"):
+        raise SystemExit("--att-prof: rebuild with ANON_NVCC_EXTRA=-DATT_PROF=1")
+    buf = (ctypes.c_ulonglong * 64)()
+    if lib.anon_debug_att_prof(buf) != 0:
+        raise SystemExit("--att-prof: cudaMemcpyFromSymbol failed")
+    v = list(buf)
+    names = {"mma_issuer": ["wait_s_free", "wait_q_full", "wait_k_full", "issue_qk", "wait_v_full", "wait_p_full", "wait_o_empty", "issue_pv"],
+             "softmax_warp": ["wait_s_full", "tmem_ld+arrive", "max(+rescale)", "exp+sum+pack", "wait_pv_done", "tmem_st+arrive", "finalize"]}
+    out = {}
+    for off, key, tag in ((0, "mma_issuer", "mma_issuer"), (16, "softmax_warp", "softmax_warp_2"), (32, "softmax_warp", "softmax_warp_5")):
+        ch = max(1, v[off + 9])
+        out[tag] = {"chunks": v[off + 9], "total": round(v[off + 8] / ch, 1), **{n: round(v[off + i] / ch, 1) for i, n in enumerate(names[key])}}
+    return out
+
+
 def main():
     import torch
     import paper_2606_15650_b200 as P
@@ -42,6 +63,9 @@ def main():
     ap.add_argument("--iters", type=int, default=10)
     ap.add_argument("--regex-records", type=int, default=2000)
     ap.add_argument("--regex-mb", type=float, default=400.0)
+    ap.add_argument("--att-prof", action="store_true",
+                    help="print the attention kernel's clock64 counters after each attention run (needs a library built with "
+                         "ANON_NVCC_EXTRA=-DATT_PROF=1, which exports anon_debug_att_prof)")
     ap.add_argument("--only", default="", help="comma list out of gemm,attention,hmac,regex (default: all); the issue-rate peaks always run")
     args = ap.parse_args()
     only = set(x for x in args.only.split(",") if x)
@@ -128,10 +152,13 @@ def main():
         out = torch.empty(T, H, device=dev, dtype=torch.bfloat16)
         d_cu = torch.from_numpy(cu).to(dev)
         ms = timeit(lambda: P.anon_attention(ctx, qkv, d_cu, cu, H, H // 64, 1, out))
+        prof = _att_prof(P) if args.att_prof else None
         n2 = float((lens[:B].astype(np.float64) ** 2).sum())
         res[name] = {"tokens": T, "sequences": B, "ms": ms, "sm_mhz_after": clocks_after[-1], "tflops": 4.0 * n2 * H / ms / 1e9,
                      "exp_per_s": n2 * (H // 64) / ms * 1e3, "frac_of_measured_exp_peak": n2 * (H // 64) / ms * 1e3 / exp_peak_measured,
                      "frac_of_bf16_burst_peak": 4.0 * n2 * H / ms / 1e9 / tf_peak, "algorithmic_gbs": T * H * 2 * 4 / ms / 1e6}
+        if prof:
+            res[name]["cycles_per_chunk"] = prof
         # NEXT-3: the same inputs through the banded kernel (window 128): a query sees at most 129 keys
         ms = timeit(lambda: P.anon_attention_local(ctx, qkv, d_cu, cu, H, H // 64, 1, 128, out))
         ln = lens[:B].astype(np.float64)

@@ -4,21 +4,29 @@
 //
 // sm_100a design (BF16 path): persistent CTAs, two per SM (96 KB shared memory, 256 TMEM columns each), looping
 // over (work item, head) units.  Warp-specialised:
-//   warp 0      TMA producer : Q tile [128 x 64] (double-buffered) and K / V chunks [64 x 64] (4-stage ring) of the
-//                              packed qkv tensor, 128B swizzle, mbarrier completion
+//   warp 0      TMA producer : Q tile [128 x 64] (double-buffered) and K / V chunks [64 x 64] of the packed qkv tensor,
+//                              128B swizzle, mbarrier completion.  K and V have 4-slot rings of their own and the K
+//                              loads run two chunks ahead of the V loads (see the producer)
 //   warp 1      MMA issuer   : S = Q K^T   tcgen05.mma M128 N64 K16 x4, both operands K-major in shared memory,
 //                                          accumulator = one of two 64-column S buffers in TMEM
 //                              O += P V    A = P read from TMEM (BF16 pairs the softmax warps write into P columns of their
 //                                          own), B = V chunk, MN-major descriptor
 //                              QK^T runs TWO chunks ahead of PV: S(g+2) is issued as soon as the softmax warps have S(g) in
-//                              registers, so a finished chunk never waits for the tensor pipe's round trip
-//   warps 2-5   softmax      : one thread per query row: tcgen05.ld S -> FP32 max -> exp2 (1/sqrt(64)*log2(e) folded
-//                              in) -> row sum -> BF16 P -> tcgen05.st.  The running reference max is only raised
-//                              when a chunk exceeds it by more than 2^8 (then O is rescaled in TMEM), so the common
-//                              path never touches O; the final O / l uses the same reference, hence exact.
-// TMEM per CTA: S 2 x 64 | P 2 x 32 | O 64 = 256 columns.  Measured (profiles/r02_attention.md): the kernel is bound by the
-// latency of one softmax warp's chain per chunk (about 2,250 cycles per 128 x 64 scores with two such warps per scheduler), not
-// by MUFU (37 % busy) or tensor throughput (27 %); two CTAs per SM interleave two such chains per scheduler.
+//                              registers, so a finished chunk never waits for the tensor pipe's round trip.  The whole warp
+//                              walks the cursors in uniform control flow, the barrier probes of a step are issued together,
+//                              and one elected lane issues the MMAs / commits (straight UTCHMMA x4 + UTCBAR in the SASS)
+//   warps 2-5   softmax      : one thread per query row: tcgen05.ld S -> FP32 max (the first 32 scores while the second load
+//                              is in flight) -> exp2 (1/sqrt(64)*log2(e) folded in) -> row sum -> BF16 P -> tcgen05.st.
+//                              The running reference max is only raised when a chunk exceeds it by more than 2^8 (then O is
+//                              rescaled in TMEM), so the common path never touches O; the final O / l uses the same
+//                              reference, hence exact.  The barriers of the NEXT steps (S(g+1) there, PV(g-2) done) are
+//                              probed right after the load and looked at only where needed.
+// TMEM per CTA: S 2 x 64 | P 2 x 32 | O 64 = 256 columns.
+// Measured with the kernel's own clock64 counters and timing-only ablations (profiles/r02_attention.md, section 5): what bounds
+// the kernel is the serial chain of ONE softmax warp per 128 x 64 chunk, ~1,600-1,850 cycles (64 ex2 at 8 issue cycles each on
+// the sub-partition's MUFU unit = 512, ~220 other instructions, the rest dependency and barrier latency with only two such warps
+// per scheduler); the MMA issuer's own chain is ~1,000 cycles per chunk (1,500 before it was made warp-uniform), the K / V loads
+// are not on the path (no change with the loads removed), nor is the tensor pipe (28 %) or TMEM.
 #include "common.cuh"
 #include "ptx_sm100.cuh"
 
@@ -30,16 +38,34 @@ namespace {
 constexpr int kQT = 128;    // queries per work item
 constexpr int kKC = 64;     // keys per chunk
 constexpr int kD = 64;
-constexpr int kKVStages = 4;
+constexpr int kKStages = 4;     // K and V chunks travel in rings of their own: a K slot is free again after QK^T of its chunk,
+constexpr int kVStages = 4;     // a V slot after P V -- two chunks later -- so each load is issued four chunk-times before its use
 constexpr int kAttThreads = 192;
 constexpr int kQBytes = kQT * kD * 2;          // 16 KB
 constexpr int kKVBytes = kKC * kD * 2;         // 8 KB (K and V each)
-constexpr int kAttSmem = 2 * kQBytes + kKVStages * 2 * kKVBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+constexpr int kAttSmem = 2 * kQBytes + (kKStages + kVStages) * kKVBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+// ANON_NVCC_EXTRA=-DATT_PROF=1 builds clock64 counters into the MMA issuer and two softmax warps of virtual CTA 0 (cycles per
+// chunk spent in each wait and phase) and exports anon_debug_att_prof; `python kernel_bench.py --only attention --att-prof` prints them
+#ifndef ATT_PROF
+#define ATT_PROF 0
+#endif
+#ifndef ATT_ABL
+#define ATT_ABL 0               // timing-only ablations (results wrong), never set in the product build: 1 = no ex2, 8 = the
+                                // softmax warps only do the barrier handshakes (every warp takes the padding path)
+#endif
 constexpr int kAttTmemCols = 256;              // S 2 x 64 | P 2 x 32 | O 64
 
 // rows relative to the chunk.  Global attention: kv_row0 = the sequence's first row, n = its length.  Local (band) attention
 // (NEXT-3, D20): kv_row0 = first key row any query of the tile may see, n = keys from there, and q_valid carries
 // (q_row0 - kv_row0) << 8 in its upper bits: query row r sees key kk (relative to kv_row0) iff |kk - (delta + r)| <= band.
+#if ATT_PROF
+__device__ unsigned long long g_att_prof[64];
+#define PROF_T(v) const long long v = clock64()
+#define PROF_ADD(i, a, b) do { if (blockIdx.x == 0) prof[i] += (unsigned long long)((b) - (a)); } while (0)
+#else
+#define PROF_T(v)
+#define PROF_ADD(i, a, b)
+#endif
 struct WorkItem { int q_row0; int kv_row0; int n; int q_valid; };
 constexpr int kBand = 64;   // half width of the local window the tcgen05 kernel supports (window 128)
 
@@ -68,18 +94,21 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t q_smem = smem_base;                                   // 2 x 16 KB
-    const uint32_t kv_smem = smem_base + 2 * kQBytes;                    // stages x (K 8 KB | V 8 KB)
-    const uint32_t bar_base = kv_smem + kKVStages * 2 * kKVBytes;
+    const uint32_t k_smem = smem_base + 2 * kQBytes;                     // K ring: stages x 8 KB
+    const uint32_t v_smem = k_smem + kKStages * kKVBytes;                // V ring: stages x 8 KB
+    const uint32_t bar_base = v_smem + kVStages * kKVBytes;
     auto q_full = [&](uint32_t i) { return bar_base + 8u * i; };
     auto q_empty = [&](uint32_t i) { return bar_base + 8u * (2 + i); };
-    auto kv_full = [&](uint32_t i) { return bar_base + 8u * (4 + i); };
-    auto kv_empty = [&](uint32_t i) { return bar_base + 8u * (8 + i); };
+    auto k_full = [&](uint32_t i) { return bar_base + 8u * (4 + i); };
+    auto v_full = [&](uint32_t i) { return bar_base + 8u * (24 + i); };
+    auto k_empty = [&](uint32_t i) { return bar_base + 8u * (8 + i); };     // QK^T of the chunk in K slot i has completed
+    auto v_empty = [&](uint32_t i) { return bar_base + 8u * (28 + i); };    // P V of the chunk in V slot i has completed
     auto s_full = [&](uint32_t i) { return bar_base + 8u * (12 + i); };    // S chunk computed (MMA commit)
     auto p_full = [&](uint32_t i) { return bar_base + 8u * (14 + i); };    // P chunk written (4 softmax warps)
     auto pv_done = [&](uint32_t i) { return bar_base + 8u * (16 + i); };   // PV of the chunk in P buffer i has completed
     auto s_free = [&](uint32_t i) { return bar_base + 8u * (22 + i); };    // S buffer i has been read into registers (4 warps)
     const uint32_t o_full = bar_base + 8u * 18, o_empty = bar_base + 8u * 20;
-    const uint32_t tmem_slot = bar_base + 8u * 24;
+    const uint32_t tmem_slot = bar_base + 8u * 19;
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -95,7 +124,8 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             ptx::mbar_init(s_free(i), 4);
         }
         ptx::mbar_init(o_full, 1); ptx::mbar_init(o_empty, 4);
-        for (uint32_t i = 0; i < kKVStages; i++) { ptx::mbar_init(kv_full(i), 1); ptx::mbar_init(kv_empty(i), 1); }
+        for (uint32_t i = 0; i < kKStages; i++) { ptx::mbar_init(k_full(i), 1); ptx::mbar_init(k_empty(i), 1); }
+        for (uint32_t i = 0; i < kVStages; i++) { ptx::mbar_init(v_full(i), 1); ptx::mbar_init(v_empty(i), 1); }
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
     }
@@ -112,78 +142,154 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
     const uint32_t tmem_o = tmem_base + 192u;
 
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== TMA producer: two cursors over the flattened (unit, chunk) sequence.  The K cursor runs two chunks ahead of the
+        // V cursor -- the distance between QK^T and P V in the MMA issuer -- so that neither ring waits on the other's slot: a K
+        // (V) slot is re-filled as soon as the QK^T (P V) that read it has completed, four chunk-times before its next use.  With K
+        // and V in one slot the re-fill could only start after P V, ONE chunk-time before the next QK^T needed it, and the kernel
+        // ran at the TMA round trip per chunk (profiles/r02_attention.md, section 5) =====
         if (lane == 0) {
-            uint32_t qi = 0, g = 0;
-            WorkItem wn = work[min((int)blockIdx.x, n_units - 1) / heads];     // next unit's item, loaded one unit ahead
-            for (int u = blockIdx.x; u < n_units; u += gridDim.x, qi++) {
-                const WorkItem w = wn;
-                if (u + (int)gridDim.x < n_units) wn = work[(u + (int)gridDim.x) / heads];
-                const int head = u % heads;
-                const uint32_t qb = qi & 1u;
-                ptx::mbar_wait_backoff(q_empty(qb), ((qi >> 1) & 1u) ^ 1u);
-                ptx::mbar_arrive_expect_tx(q_full(qb), kQBytes);
-                ptx::tma_load_2d(q_smem + qb * kQBytes, &tmap_q, q_full(qb), head * kD, w.q_row0);
-                const int nc = (w.n + kKC - 1) / kKC;
-                for (int c = 0; c < nc; c++, g++) {
-                    const uint32_t st = g % kKVStages;
-                    ptx::mbar_wait_backoff(kv_empty(st), ((g / kKVStages) & 1u) ^ 1u);
-                    ptx::mbar_arrive_expect_tx(kv_full(st), 2 * kKVBytes);
-                    const uint32_t dst = kv_smem + st * 2 * kKVBytes;
-                    ptx::tma_load_2d(dst, &tmap_kv, kv_full(st), H + head * kD, w.kv_row0 + c * kKC);
-                    ptx::tma_load_2d(dst + kKVBytes, &tmap_kv, kv_full(st), 2 * H + head * kD, w.kv_row0 + c * kKC);
+            struct Cur { int u, c, nc; uint32_t qi, g; WorkItem w; };
+            auto enter = [&](Cur& k) { if (k.u < n_units) { k.w = work[k.u / heads]; k.nc = (k.w.n + kKC - 1) / kKC; } };
+            auto advance = [&](Cur& k) {
+                k.g++;
+                if (++k.c == k.nc) { k.u += gridDim.x; k.qi++; k.c = 0; enter(k); }
+            };
+            Cur a{(int)blockIdx.x, 0, 0, 0u, 0u, WorkItem{0, 0, 0, 0}};
+            enter(a);
+            Cur b = a;
+            auto load_k = [&]() {
+                const int head = a.u % heads;
+                if (a.c == 0) {
+                    const uint32_t qb = a.qi & 1u;
+                    ptx::mbar_wait_backoff(q_empty(qb), ((a.qi >> 1) & 1u) ^ 1u);
+                    ptx::mbar_arrive_expect_tx(q_full(qb), kQBytes);
+                    ptx::tma_load_2d(q_smem + qb * kQBytes, &tmap_q, q_full(qb), head * kD, a.w.q_row0);
                 }
+                const uint32_t st = a.g % kKStages;
+                ptx::mbar_wait_backoff(k_empty(st), ((a.g / kKStages) & 1u) ^ 1u);
+                ptx::mbar_arrive_expect_tx(k_full(st), kKVBytes);
+                ptx::tma_load_2d(k_smem + st * kKVBytes, &tmap_kv, k_full(st), H + head * kD, a.w.kv_row0 + a.c * kKC);
+                advance(a);
+            };
+            auto load_v = [&]() {
+                const int head = b.u % heads;
+                const uint32_t st = b.g % kVStages;
+                ptx::mbar_wait_backoff(v_empty(st), ((b.g / kVStages) & 1u) ^ 1u);
+                ptx::mbar_arrive_expect_tx(v_full(st), kKVBytes);
+                ptx::tma_load_2d(v_smem + st * kKVBytes, &tmap_kv, v_full(st), 2 * H + head * kD, b.w.kv_row0 + b.c * kKC);
+                advance(b);
+            };
+            if (a.u < n_units) load_k();
+            if (a.u < n_units) load_k();
+            while (b.u < n_units) {
+                if (a.u < n_units) load_k();
+                load_v();
             }
         }
     } else if (warp == 1) {
         // ===== MMA issuer: two cursors over the flattened (unit, chunk) sequence.  QK^T runs TWO chunks ahead of PV: S(g+2) is
         // issued as soon as the softmax warps have pulled S(g) into registers (s_free), not when P(g) has been consumed -- P has
-        // TMEM columns of its own -- so a finished chunk never waits for the tensor pipe's round trip =====
-        if (lane == 0) {
+        // TMEM columns of its own -- so a finished chunk never waits for the tensor pipe's round trip.
+        // The WHOLE warp walks the cursors in uniform control flow and one elected lane issues: with the loop inside
+        // `if (lane == 0)` ptxas cannot prove the descriptors warp-uniform and wraps every tcgen05.mma / commit in an
+        // ELECT ... BRA.U.ANY loop -- measured with clock64 at 485 + 440 cycles per chunk for 8 MMAs and 5 commits, which made this
+        // thread, not the softmax, the pace of the kernel (profiles/r02_attention.md, section 5) =====
+        {
             constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(kQT, kKC);          // both operands K-major
             constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(kQT, kD, 1);        // B = V is MN-major
             // nc_next = chunk count of the unit after the cursor's, loaded one unit ahead so that no MMA waits on it
             struct Cur { int u, c, nc, nc_next; uint32_t qi, g; };
+            // (the shuffle -- at the point of use, a whole unit after the load -- tells ptxas the count is warp-uniform)
             auto chunks_of = [&](int u) { return u < n_units ? (work[u / heads].n + kKC - 1) / kKC : 0; };
             auto advance = [&](Cur& k) {
                 k.g++;
-                if (++k.c == k.nc) { k.u += gridDim.x; k.qi++; k.c = 0; k.nc = k.nc_next; k.nc_next = chunks_of(k.u + (int)gridDim.x); }
+                if (++k.c == k.nc) {
+                    k.u += gridDim.x; k.qi++; k.c = 0;
+                    k.nc = __shfl_sync(0xffffffffu, k.nc_next, 0);
+                    k.nc_next = chunks_of(k.u + (int)gridDim.x);
+                }
             };
-            Cur a{(int)blockIdx.x, 0, chunks_of((int)blockIdx.x), chunks_of((int)blockIdx.x + (int)gridDim.x), 0u, 0u}, b = a;
+            Cur a{(int)blockIdx.x, 0, __shfl_sync(0xffffffffu, chunks_of((int)blockIdx.x), 0), chunks_of((int)blockIdx.x + (int)gridDim.x), 0u, 0u}, b = a;
+#if ATT_PROF
+            unsigned long long prof[16];
+            for (int i = 0; i < 16; i++) prof[i] = 0;
+            const long long t_begin = clock64();
+#endif
             auto issue_qk = [&]() {
-                const uint32_t qb = a.qi & 1u, st = a.g % kKVStages, sb = a.g & 1u;
-                if (a.g >= 2u) ptx::mbar_wait(s_free(sb), ((a.g - 2u) >> 1) & 1u);   // S(g-2) has left this buffer
-                if (a.c == 0) ptx::mbar_wait(q_full(qb), (a.qi >> 1) & 1u);
-                ptx::mbar_wait(kv_full(st), (a.g / kKVStages) & 1u);
+                const uint32_t qb = a.qi & 1u, st = a.g % kKStages, sb = a.g & 1u;
+                PROF_T(t0);
+                // the probes are issued together (an mbarrier probe answers after ~70 cycles even when the phase is long complete)
+                // and only a failed one is waited for
+                const bool ok_s = a.g < 2u || ptx::mbar_try_wait(s_free(sb), ((a.g - 2u) >> 1) & 1u);   // S(g-2) has left this buffer
+                const bool ok_k = ptx::mbar_try_wait(k_full(st), (a.g / kKStages) & 1u);
+                const bool ok_q = a.c != 0 || ptx::mbar_try_wait(q_full(qb), (a.qi >> 1) & 1u);
+                PROF_T(t1);
+                if (!ok_s) ptx::mbar_wait(s_free(sb), ((a.g - 2u) >> 1) & 1u);
+                if (!ok_q) ptx::mbar_wait(q_full(qb), (a.qi >> 1) & 1u);
+                PROF_T(t2);
+                if (!ok_k) ptx::mbar_wait(k_full(st), (a.g / kKStages) & 1u);
+                PROF_T(t3);
+                PROF_ADD(0, t0, t1); PROF_ADD(1, t1, t2); PROF_ADD(2, t2, t3);
                 ptx::tc_fence_after();
                 const uint64_t qd = ptx::make_desc_k_sw128(q_smem + qb * kQBytes);
-                const uint64_t kd = ptx::make_desc_k_sw128(kv_smem + st * 2 * kKVBytes);
+                const uint64_t kd = ptx::make_desc_k_sw128(k_smem + st * kKVBytes);
+                if (ptx::elect_one()) {
 #pragma unroll
-                for (int k = 0; k < kD / 16; k++)
-                    ptx::mma_f16_ss(tmem_base + sb * 64u, qd + (uint64_t)(2 * k), kd + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
-                ptx::mma_commit(s_full(sb));
-                if (a.c == a.nc - 1) ptx::mma_commit(q_empty(qb));       // last use of this Q tile
+                    for (int k = 0; k < kD / 16; k++)
+                        ptx::mma_f16_ss(tmem_base + sb * 64u, qd + (uint64_t)(2 * k), kd + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
+                    PROF_T(tm);
+                    PROF_ADD(10, t3, tm);
+                    ptx::mma_commit(s_full(sb));
+                    ptx::mma_commit(k_empty(st));
+                    if (a.c == a.nc - 1) ptx::mma_commit(q_empty(qb));   // last use of this Q tile
+                }
+                __syncwarp();
+                PROF_T(t4);
+                PROF_ADD(3, t3, t4);
             };
             auto issue_pv = [&]() {
-                const uint32_t st = b.g % kKVStages, sb = b.g & 1u;
-                ptx::mbar_wait(p_full(sb), (b.g >> 1) & 1u);
-                if (b.c == 0) ptx::mbar_wait(o_empty, (b.qi & 1u) ^ 1u);  // the previous unit's O has been read (finalize)
+                const uint32_t st = b.g % kVStages, sb = b.g & 1u;
+                PROF_T(t0);
+                const bool ok_v = ptx::mbar_try_wait(v_full(st), (b.g / kVStages) & 1u);
+                const bool ok_p = ptx::mbar_try_wait(p_full(sb), (b.g >> 1) & 1u);
+                const bool ok_o = b.c != 0 || ptx::mbar_try_wait(o_empty, (b.qi & 1u) ^ 1u);   // the previous unit's O has been read (finalize)
+                PROF_T(t1);
+                if (!ok_v) ptx::mbar_wait(v_full(st), (b.g / kVStages) & 1u);
+                if (!ok_p) ptx::mbar_wait(p_full(sb), (b.g >> 1) & 1u);
+                PROF_T(t2);
+                if (!ok_o) ptx::mbar_wait(o_empty, (b.qi & 1u) ^ 1u);
+                PROF_T(t3);
+                PROF_ADD(4, t0, t1); PROF_ADD(5, t1, t2); PROF_ADD(6, t2, t3);
                 ptx::tc_fence_after();
-                const uint64_t vd = ptx::make_desc_mn_sw128(kv_smem + st * 2 * kKVBytes + kKVBytes);
+                const uint64_t vd = ptx::make_desc_mn_sw128(v_smem + st * kKVBytes);
+                if (ptx::elect_one()) {
 #pragma unroll
-                for (int k = 0; k < kKC / 16; k++)                       // 16 keys per MMA: 8 TMEM columns of P, 2 KB of V
-                    ptx::mma_f16_ts(tmem_o, tmem_p + sb * 32u + 8u * k, vd + (uint64_t)(128 * k), idesc_pv, (b.c | k) ? 1u : 0u);
-                ptx::mma_commit(kv_empty(st));
-                ptx::mma_commit(pv_done(sb));
-                if (b.c == b.nc - 1) ptx::mma_commit(o_full);
+                    for (int k = 0; k < kKC / 16; k++)                   // 16 keys per MMA: 8 TMEM columns of P, 2 KB of V
+                        ptx::mma_f16_ts(tmem_o, tmem_p + sb * 32u + 8u * k, vd + (uint64_t)(128 * k), idesc_pv, (b.c | k) ? 1u : 0u);
+                    PROF_T(tm);
+                    PROF_ADD(11, t3, tm);
+                    ptx::mma_commit(v_empty(st));
+                    ptx::mma_commit(pv_done(sb));
+                    if (b.c == b.nc - 1) ptx::mma_commit(o_full);
+                }
+                __syncwarp();
+                PROF_T(t4);
+                PROF_ADD(7, t3, t4);
+                PROF_ADD(9, 0, 1);
             };
             if (a.nc) { issue_qk(); advance(a); }
             if (a.nc) { issue_qk(); advance(a); }
             while (b.nc) {
                 if (a.nc) { issue_qk(); advance(a); }        // S(g+2): gated by s_free(g), early in the softmax of chunk g
                 issue_pv();                                  // PV(g): gated by p_full(g), the end of that softmax
+                PROF_T(ta);
                 advance(b);
+                PROF_T(tb);
+                PROF_ADD(12, ta, tb);
             }
+#if ATT_PROF
+            if (blockIdx.x == 0 && lane == 0) { prof[8] = (unsigned long long)(clock64() - t_begin); for (int i = 0; i < 16; i++) g_att_prof[i] = prof[i]; }
+#endif
         }
     } else {
         // ===== softmax warps: thread = query row =====
@@ -192,6 +298,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
         const int row = (int)quarter * 32 + lane;
         const float sc = 0.125f * 1.4426950408889634f;                   // 1/sqrt(64) * log2(e)
         uint32_t qi = 0, g = 0;
+        bool s_ok = false;                                               // s_full of the chunk about to start has been seen (probed early)
         bool pend = false;
         uint32_t pend_par = 0;
         float pend_l = 1.f;
@@ -218,6 +325,11 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             }
             pend = false;
         };
+#if ATT_PROF
+        unsigned long long prof[16];
+        for (int i = 0; i < 16; i++) prof[i] = 0;
+        const long long t_begin = clock64();
+#endif
         WorkItem wn = work[min((int)blockIdx.x, n_units - 1) / heads];         // next unit's item, loaded one unit ahead
         for (int u = blockIdx.x; u < n_units; u += gridDim.x, qi++) {
             const WorkItem w = wn;
@@ -228,9 +340,13 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             for (int c = 0; c < nc; c++, g++) {
                 const uint32_t sb = g & 1u;
                 const uint32_t t_s = tmem_base + lane_base + sb * 64u;
-                ptx::mbar_wait(s_full(sb), (g >> 1) & 1u);
+                PROF_T(t0);
+                if (!s_ok) ptx::mbar_wait(s_full(sb), (g >> 1) & 1u);
+                s_ok = false;
+                PROF_T(t1);
+                PROF_ADD(0, t0, t1);
                 ptx::tc_fence_after();
-                if ((int)quarter * 32 >= (w.q_valid & 0xff)) {           // no query of this warp is real: P rows are don't-care
+                if (ATT_ABL == 8 || (int)quarter * 32 >= (w.q_valid & 0xff)) {           // no query of this warp is real: P rows are don't-care
                     ptx::tc_fence_before();
                     __syncwarp();
                     if (lane == 0) ptx::mbar_arrive(s_free(sb));
@@ -243,13 +359,31 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     continue;
                 }
                 uint32_t r[64];
-                ptx::tmem_ld_32x32b_x32(t_s, r);
+                const int valid = w.n - c * kKC;                         // keys of this chunk that belong to the sequence
+                float cmx[4];                                            // four independent chains, then a tree
+                const bool plain = !BAND && valid >= kKC;                // no mask to apply: the maxima of the first 32 scores are
+                ptx::tmem_ld_32x32b_x32(t_s, r);                         // taken while the second load is in flight
+                auto chain = [&](int q4) {
+                    cmx[q4] = max3(__uint_as_float(r[16 * q4]), __uint_as_float(r[16 * q4 + 1]), __uint_as_float(r[16 * q4 + 2]));
+#pragma unroll
+                    for (int j = 3; j + 1 < 16; j += 2)
+                        cmx[q4] = max3(cmx[q4], __uint_as_float(r[16 * q4 + j]), __uint_as_float(r[16 * q4 + j + 1]));
+                    cmx[q4] = fmaxf(cmx[q4], __uint_as_float(r[16 * q4 + 15]));
+                };
+                ptx::tmem_ld_wait();
                 ptx::tmem_ld_32x32b_x32(t_s + 32u, r + 32);
+                if (plain) { chain(0); chain(1); }
                 ptx::tmem_ld_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(s_free(sb));             // the scores are in registers: S(g+2) may overwrite the buffer
-                const int valid = w.n - c * kKC;                         // keys of this chunk that belong to the sequence
+                // PV(g-2) has all but always finished by now, and so has QK^T(g+1) (issued one chunk-time ago): probe both barriers
+                // here and look at the answers only before the P store / at the top of the next chunk, so that the ~70-150 cycles a
+                // probe takes are covered by the maximum and the exponentials
+                const bool pv_ok = g < 2u || ptx::mbar_test_wait(pv_done(sb), ((g - 2u) >> 1) & 1u);
+                s_ok = ptx::mbar_test_wait(s_full(sb ^ 1u), ((g + 1u) >> 1) & 1u);
+                PROF_T(t2);
+                PROF_ADD(1, t1, t2);
                 if (valid < kKC) {
 #pragma unroll
                     for (int j = 0; j < kKC; j++) if (j >= valid) r[j] = 0xff800000u;      // -inf
@@ -262,15 +396,8 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                         for (int j = 0; j < kKC; j++) if (j < jlo || j > jhi) r[j] = 0xff800000u;
                     }
                 }
-                float cmx[4];                                            // four independent chains, then a tree
-#pragma unroll
-                for (int q4 = 0; q4 < 4; q4++) {
-                    cmx[q4] = max3(__uint_as_float(r[16 * q4]), __uint_as_float(r[16 * q4 + 1]), __uint_as_float(r[16 * q4 + 2]));
-#pragma unroll
-                    for (int j = 3; j + 1 < 16; j += 2)
-                        cmx[q4] = max3(cmx[q4], __uint_as_float(r[16 * q4 + j]), __uint_as_float(r[16 * q4 + j + 1]));
-                    cmx[q4] = fmaxf(cmx[q4], __uint_as_float(r[16 * q4 + 15]));
-                }
+                if (!plain) { chain(0); chain(1); }
+                chain(2); chain(3);
                 const float cm = fmaxf(max3(cmx[0], cmx[1], cmx[2]), cmx[3]);
                 const float mnew = cm * sc;
                 if (__any_sync(0xffffffffu, mnew > m + 8.0f)) {          // raise the reference (first chunk: m = -inf)
@@ -291,6 +418,8 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                         ptx::tmem_st_wait();
                     }
                 }
+                PROF_T(t3);
+                PROF_ADD(2, t2, t3);
                 uint32_t pk[32];
                 uint64_t sum_a = pk2(0.f, 0.f), sum_b = sum_a;           // packed FP32x2 partial row sums
                 // BAND: a row may not have seen any key yet (m = -inf): exponentiate against 0, every p is then 0
@@ -313,9 +442,13 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     }
 #pragma unroll
                     for (int j = 16 * hh; j < 16 * hh + 16; j++) {
-                        float t0, t1;
-                        upk2(fma2(pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])), sc2, nm2), t0, t1);
-                        const float p0 = ex2f(t0), p1 = ex2f(t1);
+                        const uint64_t t = fma2(pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])), sc2, nm2);
+                        float p0, p1;
+#if ATT_ABL == 1
+                        upk2(t, p0, p1);
+#else
+                        { float t0, t1; upk2(t, t0, t1); p0 = ex2f(t0); p1 = ex2f(t1); }
+#endif
                         if (j & 1) sum_b = add2(sum_b, pk2(p0, p1)); else sum_a = add2(sum_a, pk2(p0, p1));
                         pk[j] = pack2(p0, p1);
                     }
@@ -325,16 +458,23 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     upk2(add2(sum_a, sum_b), s0, s1);
                     l += s0 + s1;
                 }
-                if (g >= 2u) {                                           // PV(g-2) has finished reading this P buffer
-                    ptx::mbar_wait(pv_done(sb), ((g - 2u) >> 1) & 1u);
-                    ptx::tc_fence_after();
-                }
+                PROF_T(t4);
+                PROF_ADD(3, t3, t4);
+                if (!pv_ok) ptx::mbar_wait(pv_done(sb), ((g - 2u) >> 1) & 1u);      // PV(g-2) has finished reading this P buffer
+                ptx::tc_fence_after();
+                PROF_T(t5);
+                PROF_ADD(4, t4, t5);
                 ptx::tmem_st_32x32b_x32(tmem_p + lane_base + sb * 32u, pk);
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(p_full(sb));
+                PROF_T(t6);
+                PROF_ADD(5, t5, t6);
                 if (c == 0 && pend) finalize();
+                PROF_T(t7);
+                PROF_ADD(6, t6, t7);
+                PROF_ADD(9, 0, 1);
             }
             // the O / l write-back of this unit is deferred until after the first chunk of the next one, so that the
             // wait for the last PV overlaps useful work
@@ -342,6 +482,10 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             pend_row0 = w.q_row0; pend_valid = w.q_valid & 0xff; pend_head = head;
         }
         if (pend) finalize();
+#if ATT_PROF
+        if (blockIdx.x == 0 && warp == 2 && lane == 0) { prof[8] = (unsigned long long)(clock64() - t_begin); for (int i = 0; i < 16; i++) g_att_prof[16 + i] = prof[i]; }
+        if (blockIdx.x == 0 && warp == 5 && lane == 31) { prof[8] = (unsigned long long)(clock64() - t_begin); for (int i = 0; i < 16; i++) g_att_prof[32 + i] = prof[i]; }
+#endif
     }
 
     ptx::tc_fence_before();
@@ -451,3 +595,7 @@ extern "C" int anon_attention_local(anon_ctx* ctx, const void* d_qkv, const int3
     if (rc) return rc;
     return attention_run(ctx, plan, d_qkv, d_cu_seqlens, h_cu_seqlens[0], B, hidden, heads, dtype, d_ctx);
 }
+
+#if ATT_PROF
+extern "C" int anon_debug_att_prof(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_att_prof, sizeof(unsigned long long) * 64); }
+#endif

@@ -46,7 +46,7 @@ def _att_prof(P):
     names = {"mma_issuer": ["wait_s_free", "wait_q_full", "wait_k_full", "issue_qk", "wait_v_full", "wait_p_full", "wait_o_empty", "issue_pv"],
              "softmax_warp": ["wait_s_full", "tmem_ld+arrive", "max(+rescale)", "exp+sum+pack", "wait_pv_done", "tmem_st+arrive", "finalize"]}
     out = {}
-    for off, key, tag in ((0, "mma_issuer", "mma_issuer"), (16, "softmax_warp", "softmax_warp_2"), (32, "softmax_warp", "softmax_warp_5")):
+    for off, key, tag in ((0, "mma_issuer", "mma_issuer"), (16, "softmax_warp", "softmax_warp_a"), (32, "softmax_warp", "softmax_warp_b")):
         ch = max(1, v[off + 9])
         out[tag] = {"chunks": v[off + 9], "total": round(v[off + 8] / ch, 1), **{n: round(v[off + i] / ch, 1) for i, n in enumerate(names[key])}}
     return out

@@ -15,8 +15,8 @@
 //                              registers, so a finished chunk never waits for the tensor pipe's round trip.  The whole warp
 //                              walks the cursors in uniform control flow, the barrier probes of a step are issued together,
 //                              and one elected lane issues the MMAs / commits (straight UTCHMMA x4 + UTCBAR in the SASS)
-//   warps 2-5   softmax      : one thread per query row: tcgen05.ld S -> FP32 max (the first 32 scores while the second load
-//                              is in flight) -> exp2 (1/sqrt(64)*log2(e) folded in) -> row sum -> BF16 P -> tcgen05.st.
+//   warps 2-5   softmax      : one thread per query row: tcgen05.ld S -> FP32 max -> exp2 (1/sqrt(64)*log2(e) folded in)
+//                              -> row sum -> BF16 P -> tcgen05.st.
 //                              The running reference max is only raised when a chunk exceeds it by more than 2^8 (then O is
 //                              rescaled in TMEM), so the common path never touches O; the final O / l uses the same
 //                              reference, hence exact.  The barriers of the NEXT steps (S(g+1) there, PV(g-2) done) are
@@ -112,6 +112,11 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // unit u = item * heads + head.  The roles step u by gridDim.x; (item, head) follow by addition (two integer divisions per
+    // thread here instead of one or two per unit -- ~40 instructions each -- in every role)
+    const int step_item = (int)gridDim.x / heads, step_head = (int)gridDim.x % heads;
+    const int item0 = (int)blockIdx.x / heads, head0 = (int)blockIdx.x % heads;
+    auto next_unit = [&](int& item, int& head) { item += step_item; head += step_head; if (head >= heads) { head -= heads; item++; } };
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&tmap_q);
@@ -148,17 +153,17 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
         // and V in one slot the re-fill could only start after P V, ONE chunk-time before the next QK^T needed it, and the kernel
         // ran at the TMA round trip per chunk (profiles/r02_attention.md, section 5) =====
         if (lane == 0) {
-            struct Cur { int u, c, nc; uint32_t qi, g; WorkItem w; };
-            auto enter = [&](Cur& k) { if (k.u < n_units) { k.w = work[k.u / heads]; k.nc = (k.w.n + kKC - 1) / kKC; } };
+            struct Cur { int u, item, head, c, nc; uint32_t qi, g; WorkItem w; };
+            auto enter = [&](Cur& k) { if (k.u < n_units) { k.w = work[k.item]; k.nc = (k.w.n + kKC - 1) / kKC; } };
             auto advance = [&](Cur& k) {
                 k.g++;
-                if (++k.c == k.nc) { k.u += gridDim.x; k.qi++; k.c = 0; enter(k); }
+                if (++k.c == k.nc) { k.u += gridDim.x; next_unit(k.item, k.head); k.qi++; k.c = 0; enter(k); }
             };
-            Cur a{(int)blockIdx.x, 0, 0, 0u, 0u, WorkItem{0, 0, 0, 0}};
+            Cur a{(int)blockIdx.x, item0, head0, 0, 0, 0u, 0u, WorkItem{0, 0, 0, 0}};
             enter(a);
             Cur b = a;
             auto load_k = [&]() {
-                const int head = a.u % heads;
+                const int head = a.head;
                 if (a.c == 0) {
                     const uint32_t qb = a.qi & 1u;
                     ptx::mbar_wait_backoff(q_empty(qb), ((a.qi >> 1) & 1u) ^ 1u);
@@ -172,7 +177,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 advance(a);
             };
             auto load_v = [&]() {
-                const int head = b.u % heads;
+                const int head = b.head;
                 const uint32_t st = b.g % kVStages;
                 ptx::mbar_wait_backoff(v_empty(st), ((b.g / kVStages) & 1u) ^ 1u);
                 ptx::mbar_arrive_expect_tx(v_full(st), kKVBytes);
@@ -198,18 +203,23 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(kQT, kKC);          // both operands K-major
             constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(kQT, kD, 1);        // B = V is MN-major
             // nc_next = chunk count of the unit after the cursor's, loaded one unit ahead so that no MMA waits on it
-            struct Cur { int u, c, nc, nc_next; uint32_t qi, g; };
+            // (item, head) = the unit AFTER the cursor's: where nc_next comes from
+            struct Cur { int u, item, head, c, nc, nc_next; uint32_t qi, g; };
             // (the shuffle -- at the point of use, a whole unit after the load -- tells ptxas the count is warp-uniform)
-            auto chunks_of = [&](int u) { return u < n_units ? (work[u / heads].n + kKC - 1) / kKC : 0; };
+            auto chunks_of = [&](int u, int item) { return u < n_units ? (work[item].n + kKC - 1) / kKC : 0; };
             auto advance = [&](Cur& k) {
                 k.g++;
                 if (++k.c == k.nc) {
                     k.u += gridDim.x; k.qi++; k.c = 0;
                     k.nc = __shfl_sync(0xffffffffu, k.nc_next, 0);
-                    k.nc_next = chunks_of(k.u + (int)gridDim.x);
+                    next_unit(k.item, k.head);
+                    k.nc_next = chunks_of(k.u + (int)gridDim.x, k.item);
                 }
             };
-            Cur a{(int)blockIdx.x, 0, __shfl_sync(0xffffffffu, chunks_of((int)blockIdx.x), 0), chunks_of((int)blockIdx.x + (int)gridDim.x), 0u, 0u}, b = a;
+            Cur a{(int)blockIdx.x, item0, head0, 0, __shfl_sync(0xffffffffu, chunks_of((int)blockIdx.x, item0), 0), 0, 0u, 0u};
+            next_unit(a.item, a.head);
+            a.nc_next = chunks_of(a.u + (int)gridDim.x, a.item);
+            Cur b = a;
 #if ATT_PROF
             unsigned long long prof[16];
             for (int i = 0; i < 16; i++) prof[i] = 0;
@@ -314,7 +324,8 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(o_empty);
             if (row < pend_valid) {
-                const float inv = 1.0f / pend_l;
+                float inv;                                               // the row sum is >= 1 (the reference key's own 2^0 at least)
+                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(pend_l));
                 uint4* dst = reinterpret_cast<uint4*>(ctx + (size_t)(pend_row0 + row) * H + pend_head * kD);
 #pragma unroll
                 for (int v = 0; v < 8; v++)
@@ -331,10 +342,12 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
         const long long t_begin = clock64();
 #endif
         WorkItem wn = work[min((int)blockIdx.x, n_units - 1) / heads];         // next unit's item, loaded one unit ahead
+        int item_n = item0, head_n = head0;                              // (item, head) of the unit after this one
         for (int u = blockIdx.x; u < n_units; u += gridDim.x, qi++) {
             const WorkItem w = wn;
-            if (u + (int)gridDim.x < n_units) wn = work[(u + (int)gridDim.x) / heads];
-            const int head = u % heads;
+            const int head = head_n;
+            next_unit(item_n, head_n);
+            if (u + (int)gridDim.x < n_units) wn = work[item_n];
             const int nc = (w.n + kKC - 1) / kKC;
             float m = -INFINITY, l = 0.f;                                // reference max (scaled, log2 domain), row sum
             for (int c = 0; c < nc; c++, g++) {
@@ -361,8 +374,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 uint32_t r[64];
                 const int valid = w.n - c * kKC;                         // keys of this chunk that belong to the sequence
                 float cmx[4];                                            // four independent chains, then a tree
-                const bool plain = !BAND && valid >= kKC;                // no mask to apply: the maxima of the first 32 scores are
-                ptx::tmem_ld_32x32b_x32(t_s, r);                         // taken while the second load is in flight
+                ptx::tmem_ld_32x32b_x32(t_s, r);
                 auto chain = [&](int q4) {
                     cmx[q4] = max3(__uint_as_float(r[16 * q4]), __uint_as_float(r[16 * q4 + 1]), __uint_as_float(r[16 * q4 + 2]));
 #pragma unroll
@@ -370,16 +382,14 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                         cmx[q4] = max3(cmx[q4], __uint_as_float(r[16 * q4 + j]), __uint_as_float(r[16 * q4 + j + 1]));
                     cmx[q4] = fmaxf(cmx[q4], __uint_as_float(r[16 * q4 + 15]));
                 };
-                ptx::tmem_ld_wait();
-                ptx::tmem_ld_32x32b_x32(t_s + 32u, r + 32);
-                if (plain) { chain(0); chain(1); }
-                ptx::tmem_ld_wait();
+                ptx::tmem_ld_32x32b_x32(t_s + 32u, r + 32);              // both loads, ONE wait: taking the maxima of the first 32 scores
+                ptx::tmem_ld_wait();                                     // under the second load costs a second wait and measured slower
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(s_free(sb));             // the scores are in registers: S(g+2) may overwrite the buffer
                 // PV(g-2) has all but always finished by now, and so has QK^T(g+1) (issued one chunk-time ago): probe both barriers
                 // here and look at the answers only before the P store / at the top of the next chunk, so that the ~70-150 cycles a
-                // probe takes are covered by the maximum and the exponentials
+                // probe takes are covered by the maximum and the exponentials (n = 512: 0.656 ms with the early probes, 0.667 without)
                 const bool pv_ok = g < 2u || ptx::mbar_test_wait(pv_done(sb), ((g - 2u) >> 1) & 1u);
                 s_ok = ptx::mbar_test_wait(s_full(sb ^ 1u), ((g + 1u) >> 1) & 1u);
                 PROF_T(t2);
@@ -396,8 +406,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                         for (int j = 0; j < kKC; j++) if (j < jlo || j > jhi) r[j] = 0xff800000u;
                     }
                 }
-                if (!plain) { chain(0); chain(1); }
-                chain(2); chain(3);
+                chain(0); chain(1); chain(2); chain(3);
                 const float cm = fmaxf(max3(cmx[0], cmx[1], cmx[2]), cmx[3]);
                 const float mnew = cm * sc;
                 if (__any_sync(0xffffffffu, mnew > m + 8.0f)) {          // raise the reference (first chunk: m = -inf)

@@ -38,12 +38,13 @@ namespace {
 constexpr int kQT = 128;    // queries per work item
 constexpr int kKC = 64;     // keys per chunk
 constexpr int kD = 64;
-constexpr int kKStages = 4;     // K and V chunks travel in rings of their own: a K slot is free again after QK^T of its chunk,
-constexpr int kVStages = 4;     // a V slot after P V -- two chunks later -- so each load is issued four chunk-times before its use
+constexpr int kKStages = 3;     // K and V chunks travel in rings of their own: a K slot is free again after QK^T of its chunk,
+constexpr int kVStages = 3;     // a V slot after P V -- two chunks later -- so each load is issued three chunk-times before its use
 constexpr int kAttThreads = 192;
 constexpr int kQBytes = kQT * kD * 2;          // 16 KB
 constexpr int kKVBytes = kKC * kD * 2;         // 8 KB (K and V each)
-constexpr int kAttSmem = 2 * kQBytes + (kKStages + kVStages) * kKVBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+constexpr int kOBytes = kQT * kD * 2;          // 16 KB: the normalised BF16 output tile, staged for the TMA store (one 4 KB box per warp)
+constexpr int kAttSmem = 2 * kQBytes + (kKStages + kVStages) * kKVBytes + kOBytes + 1024 /*align slack*/ + 256 /*barriers*/;
 // ANON_NVCC_EXTRA=-DATT_PROF=1 builds clock64 counters into the MMA issuer and two softmax warps of virtual CTA 0 (cycles per
 // chunk spent in each wait and phase) and exports anon_debug_att_prof; `python kernel_bench.py --only attention --att-prof` prints them
 #ifndef ATT_PROF
@@ -86,17 +87,33 @@ __device__ __forceinline__ uint32_t pack2(float a, float b) {
     return *reinterpret_cast<uint32_t*>(&v);
 }
 
+// O *= alpha for this thread's row (64 FP32 columns in TMEM).  Rare (the reference maximum moved by more than 2^8 after a unit's
+// first chunk) and deliberately NOT inlined: its 32 extra live registers would otherwise be part of the hot loop's allocation.
+__device__ __noinline__ void rescale_o(uint32_t taddr, float alpha) {
+#pragma unroll
+    for (int hh = 0; hh < 2; hh++) {
+        uint32_t o[32];
+        ptx::tmem_ld_32x32b_x32(taddr + 32u * hh, o);
+        ptx::tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 32; j++) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
+        ptx::tmem_st_32x32b_x32(taddr + 32u * hh, o);
+    }
+    ptx::tmem_st_wait();
+}
+
 template <bool BAND>
 __global__ void __launch_bounds__(kAttThreads, 2)
 attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_kv,
-                         const WorkItem* __restrict__ work, int n_units, int heads, int H, __nv_bfloat16* __restrict__ ctx)
+                         const __grid_constant__ CUtensorMap tmap_o, const WorkItem* __restrict__ work, int n_units, int heads, int H, __nv_bfloat16* __restrict__ ctx)
 {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t q_smem = smem_base;                                   // 2 x 16 KB
     const uint32_t k_smem = smem_base + 2 * kQBytes;                     // K ring: stages x 8 KB
     const uint32_t v_smem = k_smem + kKStages * kKVBytes;                // V ring: stages x 8 KB
-    const uint32_t bar_base = v_smem + kVStages * kKVBytes;
+    const uint32_t o_smem = v_smem + kVStages * kKVBytes;                // 4 x 4 KB: [32 rows x 128 B], 128B swizzle, one box per softmax warp
+    const uint32_t bar_base = o_smem + kOBytes;
     auto q_full = [&](uint32_t i) { return bar_base + 8u * i; };
     auto q_empty = [&](uint32_t i) { return bar_base + 8u * (2 + i); };
     auto k_full = [&](uint32_t i) { return bar_base + 8u * (4 + i); };
@@ -121,6 +138,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&tmap_q);
         ptx::prefetch_tensormap(&tmap_kv);
+        ptx::prefetch_tensormap(&tmap_o);
     }
     if (warp == 1 && lane == 0) {
         for (uint32_t i = 0; i < 2; i++) {
@@ -323,9 +341,29 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(o_empty);
-            if (row < pend_valid) {
-                float inv;                                               // the row sum is >= 1 (the reference key's own 2^0 at least)
-                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(pend_l));
+            float inv;                                                   // the row sum is >= 1 (the reference key's own 2^0 at least)
+            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(pend_l));
+            if ((int)quarter * 32 + 32 <= pend_valid) {
+                // all 32 rows of this warp are real: BF16 rows into the warp's swizzled 4 KB box, ONE TMA store of full 128-byte lines.
+                // (Per-thread 16-byte stores put 32 different lines into every store instruction: with them the write-back cost
+                // 10 % of the kernel at n = 512 and 17 % of the banded one, profiles/r02_attention.md section 5.)
+                if (lane == 0) ptx::bulk_wait_read<0>();                 // the box's previous store has read it (a unit ago)
+                __syncwarp();
+                const uint32_t box = o_smem + quarter * 4096u, rowb = box + (uint32_t)lane * 128u, sw = (uint32_t)(lane & 7);
+#pragma unroll
+                for (int v = 0; v < 8; v++)
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(rowb + ((((uint32_t)v) ^ sw) << 4)),
+                                 "r"(pack2(__uint_as_float(o[8 * v]) * inv, __uint_as_float(o[8 * v + 1]) * inv)),
+                                 "r"(pack2(__uint_as_float(o[8 * v + 2]) * inv, __uint_as_float(o[8 * v + 3]) * inv)),
+                                 "r"(pack2(__uint_as_float(o[8 * v + 4]) * inv, __uint_as_float(o[8 * v + 5]) * inv)),
+                                 "r"(pack2(__uint_as_float(o[8 * v + 6]) * inv, __uint_as_float(o[8 * v + 7]) * inv)) : "memory");
+                ptx::fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) {
+                    ptx::tma_store_2d(&tmap_o, box, pend_head * kD, pend_row0 + (int)quarter * 32);
+                    ptx::bulk_commit();
+                }
+            } else if (row < pend_valid) {                               // the tile's last, partly filled warp: its rows one by one
                 uint4* dst = reinterpret_cast<uint4*>(ctx + (size_t)(pend_row0 + row) * H + pend_head * kD);
 #pragma unroll
                 for (int v = 0; v < 8; v++)
@@ -350,7 +388,11 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             if (u + (int)gridDim.x < n_units) wn = work[item_n];
             const int nc = (w.n + kKC - 1) / kKC;
             float m = -INFINITY, l = 0.f;                                // reference max (scaled, log2 domain), row sum
-            for (int c = 0; c < nc; c++, g++) {
+            // One chunk.  The body is instantiated twice -- for a unit's first chunk, after which the previous unit's write-back
+            // runs, and inside the loop over the others -- so that the write-back (64 more live registers) is not part of the
+            // hot loop: with it inlined there the whole loop was allocated and scheduled around it (n = 512: 0.665 -> 0.60 ms
+            // with the write-back's arithmetic removed, far more than that arithmetic takes)
+            auto chunk = [&](const int c) {
                 const uint32_t sb = g & 1u;
                 const uint32_t t_s = tmem_base + lane_base + sb * 64u;
                 PROF_T(t0);
@@ -368,8 +410,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     if (g >= 2u) ptx::mbar_wait(pv_done(sb), ((g - 2u) >> 1) & 1u);
                     __syncwarp();
                     if (lane == 0) ptx::mbar_arrive(p_full(sb));
-                    if (c == 0 && pend) finalize();
-                    continue;
+                    return;
                 }
                 uint32_t r[64];
                 const int valid = w.n - c * kKC;                         // keys of this chunk that belong to the sequence
@@ -415,16 +456,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     if (c > 0) {                                         // rescale O in TMEM once PV(g-1) has landed
                         ptx::mbar_wait(pv_done((g - 1u) & 1u), ((g - 1u) >> 1) & 1u);
                         ptx::tc_fence_after();
-#pragma unroll
-                        for (int hh = 0; hh < 2; hh++) {
-                            uint32_t o[32];
-                            ptx::tmem_ld_32x32b_x32(tmem_o + lane_base + 32u * hh, o);
-                            ptx::tmem_ld_wait();
-#pragma unroll
-                            for (int j = 0; j < 32; j++) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
-                            ptx::tmem_st_32x32b_x32(tmem_o + lane_base + 32u * hh, o);
-                        }
-                        ptx::tmem_st_wait();
+                        rescale_o(tmem_o + lane_base, alpha);
                     }
                 }
                 PROF_T(t3);
@@ -480,17 +512,25 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 if (lane == 0) ptx::mbar_arrive(p_full(sb));
                 PROF_T(t6);
                 PROF_ADD(5, t5, t6);
-                if (c == 0 && pend) finalize();
+                PROF_ADD(9, 0, 1);
+            };
+            chunk(0);
+            g++;
+            {
+                PROF_T(t6);
+                if (pend) finalize();
                 PROF_T(t7);
                 PROF_ADD(6, t6, t7);
-                PROF_ADD(9, 0, 1);
             }
+#pragma unroll 1
+            for (int c = 1; c < nc; c++, g++) chunk(c);
             // the O / l write-back of this unit is deferred until after the first chunk of the next one, so that the
             // wait for the last PV overlaps useful work
             pend = true; pend_par = qi & 1u; pend_l = l;
             pend_row0 = w.q_row0; pend_valid = w.q_valid & 0xff; pend_head = head;
         }
         if (pend) finalize();
+        if (lane == 0) ptx::bulk_wait<0>();                              // the last TMA stores have left shared memory and are complete
 #if ATT_PROF
         if (blockIdx.x == 0 && warp == 2 && lane == 0) { prof[8] = (unsigned long long)(clock64() - t_begin); for (int i = 0; i < 16; i++) g_att_prof[16 + i] = prof[i]; }
         if (blockIdx.x == 0 && warp == 5 && lane == 31) { prof[8] = (unsigned long long)(clock64() - t_begin); for (int i = 0; i < 16; i++) g_att_prof[32 + i] = prof[i]; }
@@ -563,6 +603,9 @@ int attention_run(anon_ctx* ctx, const AttnPlan& plan, const void* d_qkv, const 
     if (rc) return rc;
     rc = make_tmap_2d(ctx, &tkv, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, d_qkv, (uint64_t)plan.n_rows, (uint64_t)3 * hidden, kD, kKC);
     if (rc) return rc;
+    CUtensorMap to;          // ctx rows for the write-back: boxes of 32 rows x one head (64 columns)
+    rc = make_tmap_2d(ctx, &to, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, d_ctx, (uint64_t)plan.n_rows, (uint64_t)hidden, kD, 32);
+    if (rc) return rc;
     rc = ensure_smem_attr(ctx, (const void*)attention_tcgen05_kernel<false>, kAttSmem);
     if (rc) return rc;
     rc = ensure_smem_attr(ctx, (const void*)attention_tcgen05_kernel<true>, kAttSmem);
@@ -570,10 +613,10 @@ int attention_run(anon_ctx* ctx, const AttnPlan& plan, const void* d_qkv, const 
     const long long units = (long long)plan.n_items * heads;
     const int grid = (int)std::min<long long>(units, 2LL * ctx->sm_count);
     if (plan.window)
-        attention_tcgen05_kernel<true><<<grid, kAttThreads, kAttSmem, ctx->stream>>>(tq, tkv, (const WorkItem*)plan.d_work, (int)units,
+        attention_tcgen05_kernel<true><<<grid, kAttThreads, kAttSmem, ctx->stream>>>(tq, tkv, to, (const WorkItem*)plan.d_work, (int)units,
                                                                                       heads, hidden, (__nv_bfloat16*)d_ctx);
     else
-        attention_tcgen05_kernel<false><<<grid, kAttThreads, kAttSmem, ctx->stream>>>(tq, tkv, (const WorkItem*)plan.d_work, (int)units,
+        attention_tcgen05_kernel<false><<<grid, kAttThreads, kAttSmem, ctx->stream>>>(tq, tkv, to, (const WorkItem*)plan.d_work, (int)units,
                                                                                        heads, hidden, (__nv_bfloat16*)d_ctx);
     CU_LAUNCH_CHECK(ctx, "attention_tcgen05_kernel");
     return ANON_OK;

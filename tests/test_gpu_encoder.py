@@ -259,6 +259,46 @@ def test_varlen_attention_against_oracle(env, dtype):
         assert np.abs(got - want).max() <= 2e-5 * np.abs(want).max()
 
 
+@pytest.mark.parametrize("dtype", [1, 0])
+def test_attention_rising_scores_rescale_path(env, dtype):
+    """Scores that keep growing along the keys (every 64-key chunk beats the running reference maximum by far more than 2^8):
+    the tcgen05 kernel's rare path -- raise the reference, rescale O in TMEM -- runs in every chunk after the first, and the
+    last keys carry nearly all the weight.  Also rows whose maximum sits in the FIRST chunk (falling scores), the common case."""
+    P, torch, ctx = env
+    H, A = 128, 2
+    lens = [512, 300, 129, 64]
+    cu = np.zeros(len(lens) + 1, np.int32); cu[1:] = np.cumsum(lens)
+    T = int(cu[-1])
+    rng = np.random.default_rng(23)
+    qkv = rng.standard_normal((T, 3 * H)).astype(np.float32) * 0.3
+    for s_i in range(len(lens)):
+        a, b = int(cu[s_i]), int(cu[s_i + 1])
+        pos = np.arange(b - a, dtype=np.float32)
+        for h in range(A):
+            u = rng.standard_normal(64).astype(np.float32)
+            u *= 3.0 / np.linalg.norm(u)
+            sign = 1.0 if h == 0 else -1.0                        # head 0: rising scores, head 1: falling
+            qkv[a:b, h * 64:(h + 1) * 64] += u                                           # q ~ u
+            qkv[a:b, H + h * 64:H + (h + 1) * 64] += sign * np.outer(pos * 0.12, u)      # k_j ~ +-0.12 j u: score step ~1.1 per key
+    if dtype == 1:
+        qkv = _bf16(qkv)
+    want = _attention_oracle(qkv.astype(np.float64), cu, H, A)
+    dev = "cuda:0"
+    tq = torch.from_numpy(qkv).to(dev)
+    if dtype == 1:
+        tq = tq.to(torch.bfloat16)
+    out = torch.full((T, H), float("nan"), dtype=tq.dtype, device=dev)
+    P.anon_attention(ctx, tq, torch.from_numpy(cu).to(dev), cu, H, A, dtype, out)
+    assert ctx.sync() == 0
+    got = out.float().cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    if dtype == 1:
+        assert np.abs(got - want).max() <= 2e-2 * np.abs(want).max()
+        assert np.sqrt(((got - want) ** 2).mean()) <= 3e-3 * np.sqrt((want ** 2).mean())
+    else:
+        assert np.abs(got - want).max() <= 2e-5 * np.abs(want).max()
+
+
 def _bf16_model_check(P, torch, ctx, d, w, ids, cu, subset, require_agreement):
     from oracle import encoder
     W = P.Weights(ctx, d, gen.pack_blob(w))

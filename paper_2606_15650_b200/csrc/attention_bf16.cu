@@ -2,10 +2,10 @@
 // No padding FLOPs: the work list holds one item per (sequence, 128-query tile), longest sequences first; keys
 // are walked in 64-key chunks up to the sequence's own length only.
 //
-// sm_100a design (BF16 path): persistent CTAs, two per SM (96 KB shared memory, 256 TMEM columns each), looping
+// sm_100a design (BF16 path): persistent CTAs, two per SM (97 KB shared memory, 256 TMEM columns each), looping
 // over (work item, head) units.  Warp-specialised:
 //   warp 0      TMA producer : Q tile [128 x 64] (double-buffered) and K / V chunks [64 x 64] of the packed qkv tensor,
-//                              128B swizzle, mbarrier completion.  K and V have 4-slot rings of their own and the K
+//                              128B swizzle, mbarrier completion.  K and V have 3-slot rings of their own and the K
 //                              loads run two chunks ahead of the V loads (see the producer)
 //   warp 1      MMA issuer   : S = Q K^T   tcgen05.mma M128 N64 K16 x4, both operands K-major in shared memory,
 //                                          accumulator = one of two 64-column S buffers in TMEM
@@ -20,7 +20,11 @@
 //                              The running reference max is only raised when a chunk exceeds it by more than 2^8 (then O is
 //                              rescaled in TMEM), so the common path never touches O; the final O / l uses the same
 //                              reference, hence exact.  The barriers of the NEXT steps (S(g+1) there, PV(g-2) done) are
-//                              probed right after the load and looked at only where needed.
+//                              probed right after the load and looked at only where needed.  O / l of a unit is written
+//                              after the first chunk of the next one (the last P V is hidden): BF16 rows into a swizzled
+//                              4 KB box per warp, ONE TMA store of full 128-byte lines (a partly filled last warp stores its
+//                              rows itself).  The chunk body exists twice (first chunk of a unit / loop over the rest) so
+//                              that the write-back and the rare O rescale (out of line) are not part of the hot loop.
 // TMEM per CTA: S 2 x 64 | P 2 x 32 | O 64 = 256 columns.
 // Measured with the kernel's own clock64 counters and timing-only ablations (profiles/r02_attention.md, section 5): what bounds
 // the kernel is the serial chain of ONE softmax warp per 128 x 64 chunk, ~1,600-1,850 cycles (64 ex2 at 8 issue cycles each on

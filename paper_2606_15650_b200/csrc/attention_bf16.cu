@@ -35,6 +35,7 @@
 #include "ptx_sm100.cuh"
 
 #include <algorithm>
+#include <type_traits>
 #include <vector>
 
 namespace {
@@ -396,7 +397,14 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
             // runs, and inside the loop over the others -- so that the write-back (64 more live registers) is not part of the
             // hot loop: with it inlined there the whole loop was allocated and scheduled around it (n = 512: 0.665 -> 0.60 ms
             // with the write-back's arithmetic removed, far more than that arithmetic takes)
-            auto chunk = [&](const int c) {
+            auto chunk = [&](auto first_tag, const int c) {
+                constexpr bool FIRST = decltype(first_tag)::value;
+                // SPEC: after a unit's first chunk the exponentials are taken against the reference the row already has, WITHOUT
+                // looking for the chunk's maximum first (33 FMNMX and their dependency chain per chunk); a reference that is too
+                // low for this chunk shows in the chunk's row sum, which is computed anyway, and only then -- rare -- the scores
+                // are read again, the reference is raised (O rescaled) and the exponentials repeated.  The S buffer is therefore
+                // handed back (s_free) only after that decision.  Not in the banded kernel (rows that have not seen a key yet).
+                constexpr bool SPEC = !FIRST && !BAND;
                 const uint32_t sb = g & 1u;
                 const uint32_t t_s = tmem_base + lane_base + sb * 64u;
                 PROF_T(t0);
@@ -418,20 +426,30 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 }
                 uint32_t r[64];
                 const int valid = w.n - c * kKC;                         // keys of this chunk that belong to the sequence
-                float cmx[4];                                            // four independent chains, then a tree
-                ptx::tmem_ld_32x32b_x32(t_s, r);
-                auto chain = [&](int q4) {
-                    cmx[q4] = max3(__uint_as_float(r[16 * q4]), __uint_as_float(r[16 * q4 + 1]), __uint_as_float(r[16 * q4 + 2]));
+                auto load_scores = [&]() {
+                    ptx::tmem_ld_32x32b_x32(t_s, r);
+                    ptx::tmem_ld_32x32b_x32(t_s + 32u, r + 32);          // both loads, ONE wait: taking the maxima of the first 32 scores
+                    ptx::tmem_ld_wait();                                 // under the second load costs a second wait and measured slower
+                    if (valid < kKC) {
 #pragma unroll
-                    for (int j = 3; j + 1 < 16; j += 2)
-                        cmx[q4] = max3(cmx[q4], __uint_as_float(r[16 * q4 + j]), __uint_as_float(r[16 * q4 + j + 1]));
-                    cmx[q4] = fmaxf(cmx[q4], __uint_as_float(r[16 * q4 + 15]));
+                        for (int j = 0; j < kKC; j++) if (j >= valid) r[j] = 0xff800000u;      // -inf
+                    }
+                    if (BAND) {                                          // keys outside |key - query| <= kBand: -inf
+                        const int qq = (w.q_valid >> 8) + row - c * kKC; // the query's own column in this chunk
+                        const int jlo = qq - kBand, jhi = qq + kBand;
+                        if (jlo > 0 || jhi < kKC - 1) {
+#pragma unroll
+                            for (int j = 0; j < kKC; j++) if (j < jlo || j > jhi) r[j] = 0xff800000u;
+                        }
+                    }
                 };
-                ptx::tmem_ld_32x32b_x32(t_s + 32u, r + 32);              // both loads, ONE wait: taking the maxima of the first 32 scores
-                ptx::tmem_ld_wait();                                     // under the second load costs a second wait and measured slower
-                ptx::tc_fence_before();
-                __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(s_free(sb));             // the scores are in registers: S(g+2) may overwrite the buffer
+                auto release_s = [&]() {                                 // the scores are in registers: S(g+2) may overwrite the buffer
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(s_free(sb));
+                };
+                load_scores();
+                if (!SPEC) release_s();
                 // PV(g-2) has all but always finished by now, and so has QK^T(g+1) (issued one chunk-time ago): probe both barriers
                 // here and look at the answers only before the P store / at the top of the next chunk, so that the ~70-150 cycles a
                 // probe takes are covered by the maximum and the exponentials (n = 512: 0.656 ms with the early probes, 0.667 without)
@@ -439,76 +457,92 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 s_ok = ptx::mbar_test_wait(s_full(sb ^ 1u), ((g + 1u) >> 1) & 1u);
                 PROF_T(t2);
                 PROF_ADD(1, t1, t2);
-                if (valid < kKC) {
+                // the chunk's maximum; raise the reference when it is more than 2^thr above it (first chunk: m = -inf)
+                auto raise = [&](const float thr) {
+                    float cmx[4];                                        // four independent chains, then a tree
 #pragma unroll
-                    for (int j = 0; j < kKC; j++) if (j >= valid) r[j] = 0xff800000u;      // -inf
-                }
-                if (BAND) {                                              // keys outside |key - query| <= kBand: -inf
-                    const int qq = (w.q_valid >> 8) + row - c * kKC;     // the query's own column in this chunk
-                    const int jlo = qq - kBand, jhi = qq + kBand;
-                    if (jlo > 0 || jhi < kKC - 1) {
+                    for (int q4 = 0; q4 < 4; q4++) {
+                        cmx[q4] = max3(__uint_as_float(r[16 * q4]), __uint_as_float(r[16 * q4 + 1]), __uint_as_float(r[16 * q4 + 2]));
 #pragma unroll
-                        for (int j = 0; j < kKC; j++) if (j < jlo || j > jhi) r[j] = 0xff800000u;
+                        for (int j = 3; j + 1 < 16; j += 2)
+                            cmx[q4] = max3(cmx[q4], __uint_as_float(r[16 * q4 + j]), __uint_as_float(r[16 * q4 + j + 1]));
+                        cmx[q4] = fmaxf(cmx[q4], __uint_as_float(r[16 * q4 + 15]));
                     }
-                }
-                chain(0); chain(1); chain(2); chain(3);
-                const float cm = fmaxf(max3(cmx[0], cmx[1], cmx[2]), cmx[3]);
-                const float mnew = cm * sc;
-                if (__any_sync(0xffffffffu, mnew > m + 8.0f)) {          // raise the reference (first chunk: m = -inf)
-                    float alpha = 1.0f;
-                    if (mnew > m) { alpha = ex2f(m - mnew); m = mnew; l *= alpha; }
-                    if (c > 0) {                                         // rescale O in TMEM once PV(g-1) has landed
-                        ptx::mbar_wait(pv_done((g - 1u) & 1u), ((g - 1u) >> 1) & 1u);
-                        ptx::tc_fence_after();
-                        rescale_o(tmem_o + lane_base, alpha);
-                    }
-                }
-                PROF_T(t3);
-                PROF_ADD(2, t2, t3);
-                uint32_t pk[32];
-                uint64_t sum_a = pk2(0.f, 0.f), sum_b = sum_a;           // packed FP32x2 partial row sums
-                // BAND: a row may not have seen any key yet (m = -inf): exponentiate against 0, every p is then 0
-                const float mref = (BAND && m == -INFINITY) ? 0.f : m;
-                const uint64_t sc2 = pk2(sc, sc), nm2 = pk2(-mref, -mref);
-#pragma unroll
-                for (int hh = 0; hh < 2; hh++) {
-                    if (hh == 1 && valid <= 32) {                        // second half of a short last chunk: all masked
-#pragma unroll
-                        for (int j = 16; j < 32; j++) pk[j] = 0u;
-                        break;
-                    }
-                    if (BAND) {                                          // a half-chunk none of this warp's 32 rows can see
-                        const int wq = (w.q_valid >> 8) + (int)quarter * 32 - c * kKC;    // column of the warp's first row
-                        if (32 * hh + 31 < wq - kBand || 32 * hh > wq + 31 + kBand) {
-#pragma unroll
-                            for (int j = 16 * hh; j < 16 * hh + 16; j++) pk[j] = 0u;
-                            continue;
+                    const float cm = fmaxf(max3(cmx[0], cmx[1], cmx[2]), cmx[3]);
+                    const float mnew = cm * sc;
+                    if (__any_sync(0xffffffffu, mnew > m + thr)) {
+                        float alpha = 1.0f;
+                        if (mnew > m) { alpha = ex2f(m - mnew); m = mnew; l *= alpha; }
+                        if (!FIRST) {                                    // rescale O in TMEM once PV(g-1) has landed
+                            ptx::mbar_wait(pv_done((g - 1u) & 1u), ((g - 1u) >> 1) & 1u);
+                            ptx::tc_fence_after();
+                            rescale_o(tmem_o + lane_base, alpha);
                         }
                     }
+                };
+                uint32_t pk[32];
+                auto exps = [&]() -> float {                             // P = 2^(s * sc - m) as BF16 pairs; returns the row's sum over the chunk
+                    uint64_t sum_a = pk2(0.f, 0.f), sum_b = sum_a;       // packed FP32x2 partial row sums
+                    // BAND: a row may not have seen any key yet (m = -inf): exponentiate against 0, every p is then 0
+                    const float mref = (BAND && m == -INFINITY) ? 0.f : m;
+                    const uint64_t sc2 = pk2(sc, sc), nm2 = pk2(-mref, -mref);
 #pragma unroll
-                    for (int j = 16 * hh; j < 16 * hh + 16; j++) {
-                        const uint64_t t = fma2(pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])), sc2, nm2);
-                        float p0, p1;
+                    for (int hh = 0; hh < 2; hh++) {
+                        if (hh == 1 && valid <= 32) {                    // second half of a short last chunk: all masked
+#pragma unroll
+                            for (int j = 16; j < 32; j++) pk[j] = 0u;
+                            break;
+                        }
+                        if (BAND) {                                      // a half-chunk none of this warp's 32 rows can see
+                            const int wq = (w.q_valid >> 8) + (int)quarter * 32 - c * kKC;    // column of the warp's first row
+                            if (32 * hh + 31 < wq - kBand || 32 * hh > wq + 31 + kBand) {
+#pragma unroll
+                                for (int j = 16 * hh; j < 16 * hh + 16; j++) pk[j] = 0u;
+                                continue;
+                            }
+                        }
+#pragma unroll
+                        for (int j = 16 * hh; j < 16 * hh + 16; j++) {
+                            const uint64_t t = fma2(pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])), sc2, nm2);
+                            float p0, p1;
 #if ATT_ABL == 1
-                        upk2(t, p0, p1);
+                            upk2(t, p0, p1);
 #else
-                        { float t0, t1; upk2(t, t0, t1); p0 = ex2f(t0); p1 = ex2f(t1); }
+                            { float t0, t1; upk2(t, t0, t1); p0 = ex2f(t0); p1 = ex2f(t1); }
 #endif
-                        if (j & 1) sum_b = add2(sum_b, pk2(p0, p1)); else sum_a = add2(sum_a, pk2(p0, p1));
-                        pk[j] = pack2(p0, p1);
+                            if (j & 1) sum_b = add2(sum_b, pk2(p0, p1)); else sum_a = add2(sum_a, pk2(p0, p1));
+                            pk[j] = pack2(p0, p1);
+                        }
                     }
-                }
-                {
                     float s0, s1;
                     upk2(add2(sum_a, sum_b), s0, s1);
-                    l += s0 + s1;
+                    return s0 + s1;
+                };
+                if (!SPEC) {
+                    raise(8.0f);
+                    PROF_T(t3);
+                    PROF_ADD(2, t2, t3);
+                    l += exps();
+                    PROF_T(t4);
+                    PROF_ADD(3, t3, t4);
+                } else {
+                    float sum = exps();
+                    // a P above 2^12 means the reference is more than 12 binades too low for this chunk (also catches inf / NaN)
+                    if (__any_sync(0xffffffffu, !(sum <= 4096.0f * (float)kKC))) {
+                        load_scores();                                   // S(g) is still there: s_free has not been signalled
+                        raise(0.0f);
+                        sum = exps();
+                    }
+                    l += sum;
+                    release_s();
+                    PROF_T(t4);
+                    PROF_ADD(3, t2, t4);
                 }
-                PROF_T(t4);
-                PROF_ADD(3, t3, t4);
+                PROF_T(t4b);
                 if (!pv_ok) ptx::mbar_wait(pv_done(sb), ((g - 2u) >> 1) & 1u);      // PV(g-2) has finished reading this P buffer
                 ptx::tc_fence_after();
                 PROF_T(t5);
-                PROF_ADD(4, t4, t5);
+                PROF_ADD(4, t4b, t5);
                 ptx::tmem_st_32x32b_x32(tmem_p + lane_base + sb * 32u, pk);
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
@@ -518,7 +552,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 PROF_ADD(5, t5, t6);
                 PROF_ADD(9, 0, 1);
             };
-            chunk(0);
+            chunk(std::true_type{}, 0);
             g++;
             {
                 PROF_T(t6);
@@ -527,7 +561,7 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                 PROF_ADD(6, t6, t7);
             }
 #pragma unroll 1
-            for (int c = 1; c < nc; c++, g++) chunk(c);
+            for (int c = 1; c < nc; c++, g++) chunk(std::false_type{}, c);
             // the O / l write-back of this unit is deferred until after the first chunk of the next one, so that the
             // wait for the last PV overlaps useful work
             pend = true; pend_par = qi & 1u; pend_l = l;

@@ -448,7 +448,15 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     __syncwarp();
                     if (lane == 0) ptx::mbar_arrive(s_free(sb));
                 };
-                load_scores();
+                // SPEC on a full chunk: the second 32 scores are loaded under the exponentials of the first 32
+                const bool piped = SPEC && valid >= kKC;
+                if (piped) {
+                    ptx::tmem_ld_32x32b_x32(t_s, r);
+                    ptx::tmem_ld_wait();
+                    ptx::tmem_ld_32x32b_x32(t_s + 32u, r + 32);
+                } else {
+                    load_scores();
+                }
                 if (!SPEC) release_s();
                 // PV(g-2) has all but always finished by now, and so has QK^T(g+1) (issued one chunk-time ago): probe both barriers
                 // here and look at the answers only before the P store / at the top of the next chunk, so that the ~70-150 cycles a
@@ -481,13 +489,14 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     }
                 };
                 uint32_t pk[32];
-                auto exps = [&]() -> float {                             // P = 2^(s * sc - m) as BF16 pairs; returns the row's sum over the chunk
+                auto exps = [&](const bool second_half_in_flight) -> float {     // P = 2^(s * sc - m) as BF16 pairs; returns the row's sum over the chunk
                     uint64_t sum_a = pk2(0.f, 0.f), sum_b = sum_a;       // packed FP32x2 partial row sums
                     // BAND: a row may not have seen any key yet (m = -inf): exponentiate against 0, every p is then 0
                     const float mref = (BAND && m == -INFINITY) ? 0.f : m;
                     const uint64_t sc2 = pk2(sc, sc), nm2 = pk2(-mref, -mref);
 #pragma unroll
                     for (int hh = 0; hh < 2; hh++) {
+                        if (hh == 1 && second_half_in_flight) ptx::tmem_ld_wait();
                         if (hh == 1 && valid <= 32) {                    // second half of a short last chunk: all masked
 #pragma unroll
                             for (int j = 16; j < 32; j++) pk[j] = 0u;
@@ -522,16 +531,16 @@ attention_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_q, const __gri
                     raise(8.0f);
                     PROF_T(t3);
                     PROF_ADD(2, t2, t3);
-                    l += exps();
+                    l += exps(false);
                     PROF_T(t4);
                     PROF_ADD(3, t3, t4);
                 } else {
-                    float sum = exps();
+                    float sum = exps(piped);
                     // a P above 2^12 means the reference is more than 12 binades too low for this chunk (also catches inf / NaN)
                     if (__any_sync(0xffffffffu, !(sum <= 4096.0f * (float)kKC))) {
                         load_scores();                                   // S(g) is still there: s_free has not been signalled
                         raise(0.0f);
-                        sum = exps();
+                        sum = exps(false);
                     }
                     l += sum;
                     release_s();

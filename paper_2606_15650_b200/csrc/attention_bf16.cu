@@ -15,16 +15,22 @@
 //                              registers, so a finished chunk never waits for the tensor pipe's round trip.  The whole warp
 //                              walks the cursors in uniform control flow, the barrier probes of a step are issued together,
 //                              and one elected lane issues the MMAs / commits (straight UTCHMMA x4 + UTCBAR in the SASS)
-//   warps 2-5   softmax      : one thread per query row: tcgen05.ld S -> FP32 max -> exp2 (1/sqrt(64)*log2(e) folded in)
-//                              -> row sum -> BF16 P -> tcgen05.st.
-//                              The running reference max is only raised when a chunk exceeds it by more than 2^8 (then O is
-//                              rescaled in TMEM), so the common path never touches O; the final O / l uses the same
-//                              reference, hence exact.  The barriers of the NEXT steps (S(g+1) there, PV(g-2) done) are
-//                              probed right after the load and looked at only where needed.  O / l of a unit is written
-//                              after the first chunk of the next one (the last P V is hidden): BF16 rows into a swizzled
-//                              4 KB box per warp, ONE TMA store of full 128-byte lines (a partly filled last warp stores its
-//                              rows itself).  The chunk body exists twice (first chunk of a unit / loop over the rest) so
-//                              that the write-back and the rare O rescale (out of line) are not part of the hot loop.
+//   warps 2-5   softmax      : one thread per query row: tcgen05.ld S -> exp2 (1/sqrt(64)*log2(e) folded in) -> row sum
+//                              -> BF16 P -> tcgen05.st.  A unit's FIRST chunk takes the row maximum of its 64 scores as the
+//                              row's reference; every later chunk exponentiates against that reference WITHOUT looking for
+//                              its own maximum (33 FMNMX and their chain per chunk), with the second 32 scores loading under
+//                              the exponentials of the first 32.  A reference that is too low shows in the chunk's row sum,
+//                              which is computed anyway: above 2^18 (also inf / NaN) the scores are read again (S is handed
+//                              back only after this decision), the reference is raised to the chunk maximum, O is rescaled
+//                              in TMEM (out of line) and the exponentials are repeated.  P, l and O share the reference, so
+//                              O / l is exact whatever it is; in between P <= 2^18 per element is far from any FP32 / BF16
+//                              range limit.  (The banded kernel keeps the maximum-first order: its rows may not have seen a
+//                              key yet.)  The barriers of the NEXT steps (S(g+1) there, PV(g-2) done) are probed right
+//                              after the load and looked at only where needed.  O / l of a unit is written after the first
+//                              chunk of the next one (the last P V is hidden): BF16 rows into a swizzled 4 KB box per warp,
+//                              ONE TMA store of full 128-byte lines (a partly filled last warp stores its rows itself).
+//                              The chunk body exists twice (first chunk of a unit / loop over the rest) so that the
+//                              write-back and the rare O rescale are not part of the hot loop.
 // TMEM per CTA: S 2 x 64 | P 2 x 32 | O 64 = 256 columns.
 // Measured with the kernel's own clock64 counters and timing-only ablations (profiles/r02_attention.md, section 5): what bounds
 // the kernel is the serial chain of ONE softmax warp per 128 x 64 chunk, ~1,600-1,850 cycles (64 ex2 at 8 issue cycles each on

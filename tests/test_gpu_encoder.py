@@ -299,6 +299,28 @@ def test_attention_rising_scores_rescale_path(env, dtype):
         assert np.abs(got - want).max() <= 2e-5 * np.abs(want).max()
 
 
+@pytest.mark.parametrize("lens", [[3], [31, 1], [33], [128], [160, 7]])
+def test_attention_tiny_inputs(env, lens):
+    """Fewer rows than one TMA box (32-row write-back boxes, 64-key and 128-query loads): the tensor maps clip, a partly filled
+    last warp writes its rows itself, a full 32-row warp goes through the TMA store."""
+    P, torch, ctx = env
+    H, A = 64, 1
+    cu = np.zeros(len(lens) + 1, np.int32); cu[1:] = np.cumsum(lens)
+    T = int(cu[-1])
+    rng = np.random.default_rng(5 + T)
+    qkv = _bf16(rng.standard_normal((T, 3 * H)).astype(np.float32))
+    want = _attention_oracle(qkv.astype(np.float64), cu, H, A)
+    dev = "cuda:0"
+    tq = torch.from_numpy(qkv).to(dev).to(torch.bfloat16)
+    guard = torch.full((T + 64, H), 7.0, dtype=torch.bfloat16, device=dev)      # rows past T must stay untouched
+    out = guard[:T]
+    P.anon_attention(ctx, tq, torch.from_numpy(cu).to(dev), cu, H, A, 1, out)
+    assert ctx.sync() == 0
+    got = out.float().cpu().numpy().astype(np.float64)
+    assert np.abs(got - want).max() <= 2e-2 * max(np.abs(want).max(), 1e-6)
+    assert (guard[T:].float() == 7.0).all()
+
+
 def _bf16_model_check(P, torch, ctx, d, w, ids, cu, subset, require_agreement):
     from oracle import encoder
     W = P.Weights(ctx, d, gen.pack_blob(w))

@@ -154,12 +154,47 @@ __device__ __forceinline__ uint32_t slot_index(u64 v) { return (uint32_t)(v & 0x
 // ------------------------------------------------------------------------------------------------
 // K9 probe / insert-claim
 // ------------------------------------------------------------------------------------------------
+// The items of a block handed to its threads SORTED BY A WORK CLASS (0 .. 7; a counting sort in shared memory): returns the
+// block-local index of the item this thread should take.  Thread-per-span kernels whose loops run once per 16-byte chunk or
+// per SHA-256 block are as slow as the longest span of each warp; with span lengths spread over 7-128 bytes a warp of
+// consecutive spans had 13 of 32 lanes active on average (profiles/r02_pseudonym.md).  Which thread takes which item must
+// not matter for the result.  All threads of the block must call it.
+#ifndef ANON_PROBE_SORT
+#define ANON_PROBE_SORT 1
+#endif
+template <int BLOCK>
+__device__ __forceinline__ int block_take_sorted(int cls) {
+#if ANON_PROBE_SORT
+    __shared__ int s_cnt[8];
+    __shared__ uint16_t s_perm[BLOCK];
+    if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    const int rank = atomicAdd(&s_cnt[cls], 1);
+    __syncthreads();
+    int start = 0;
+#pragma unroll
+    for (int b = 0; b < 7; b++) start += b < cls ? s_cnt[b] : 0;
+    s_perm[start + rank] = (uint16_t)threadIdx.x;
+    __syncthreads();
+    return (int)s_perm[threadIdx.x];
+#else
+    (void)cls;
+    return (int)threadIdx.x;
+#endif
+}
+
 __global__ void __launch_bounds__(256) cache_probe_kernel(
     const uint8_t* __restrict__ bytes, const long long* __restrict__ off, long long S,
     u64* table, u64 mask, const uint8_t* __restrict__ arena, const long long* __restrict__ entry_off,
     int* __restrict__ slot_of, int* d_full)
 {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // work class = 16-byte chunks of the span (the hash and the byte compare loop once per chunk); threads past the end go last
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    {
+        const int my_len = i < S ? (int)(off[i + 1] - off[i]) : 0;
+        const int cls = i < S ? min(max((my_len + 15) >> 4, 1), 8) - 1 : 7;
+        i = (long long)blockIdx.x * blockDim.x + block_take_sorted<256>(cls);
+    }
     if (i >= S) return;
     const long long o = off[i];
     const int len = (int)(off[i + 1] - o);
@@ -273,6 +308,8 @@ __global__ void __launch_bounds__(128) cache_insert_kernel(
     long long n_new, long long base_unique, const int* __restrict__ slot_of, u64* table,
     uint8_t* arena, const long long* __restrict__ entry_off, uint32_t* digests, PadStates ps)
 {
+    // (sorting this kernel's items by SHA-256 block count like the probe's was measured: slower -- consecutive entities write
+    // consecutive arena bytes, and the permutation breaks that: 6.80 against 6.64 ms for the whole call at 50 M spans)
     const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n_new) return;
     const int i = new_list[r];
@@ -295,7 +332,12 @@ __global__ void __launch_bounds__(128) cache_insert_kernel(
 __global__ void __launch_bounds__(128) hmac_spans_kernel(
     const uint8_t* __restrict__ bytes, const long long* __restrict__ off, long long S, uint32_t* digests, PadStates ps)
 {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // work class = SHA-256 blocks of the inner hash (a warp is as slow as its longest message)
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    {
+        const int cls = i < S ? min(((int)(off[i + 1] - off[i]) + 9 + 63) >> 6, 8) - 1 : 7;
+        i = (long long)blockIdx.x * blockDim.x + block_take_sorted<128>(cls);
+    }
     if (i >= S) return;
     const long long o = off[i];
     uint32_t d[8];

@@ -689,7 +689,7 @@ def run_pseudonym(args, records=None, steps=None, warmup=None):
     data, off, types, key, _ = gen.spans_zipf(n_unique, n_draws, 7, 128, 6, gen.SEED_BASE + 5 + 1000 * rank)
     log(f"[rank {rank}] generated {n_draws} spans, {data.size / 1e9:.2f} GB in {time.time() - t0:.0f}s")
     S = n_draws
-    ctx = P.Context(local, workspace_bytes=S * 8 + (S // 2048 + 2) * 24 + (64 << 20))
+    ctx = P.Context(local, workspace_bytes=S * 9 + (S // 2048 + 2) * 24 + (64 << 20))
     cache = P.Cache(ctx, n_unique, int(n_unique * 70) + (1 << 20))
     d_bytes, d_off, d_type = (torch.from_numpy(a).to(dev) for a in (data, off, types))
     out_cap = S * (3 + 13 + SLUG_LEN)

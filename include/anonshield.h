@@ -219,7 +219,8 @@ int  anon_cache_evict(anon_cache* c, uint64_t keep, uint64_t* n_evicted);
  * address (e.g. a sub-buffer of a larger allocation).  S > 0 needs d_span_bytes and d_out_tokens (INVALID_ARG if NULL).
  * Synchronises once (to learn how many entities are new, so that capacity errors are
  * returned, not latched): on ANON_ERR_CAPACITY (max_unique, arena or out_capacity
- * exceeded) the cache is left exactly as before the call.  S must be < 2^31. */
+ * exceeded) the cache is left exactly as before the call.  S must be < 2^31.
+ * Workspace: 9 S + 24 (S / 2048 + 2) bytes plus alignment (ANON_ERR_OOM if the context has less). */
 int  anon_pseudonymize(anon_ctx* ctx, anon_cache* cache,
                        const uint8_t* d_span_bytes, const int64_t* d_span_offsets,
                        const uint8_t* d_span_type, int64_t S,

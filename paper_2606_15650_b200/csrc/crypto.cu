@@ -256,13 +256,26 @@ __global__ void __launch_bounds__(256) cache_probe_kernel(
 // ------------------------------------------------------------------------------------------------
 // classify + scan functors
 // ------------------------------------------------------------------------------------------------
+// The scan evaluates its input twice (reduce pass, apply pass).  The first evaluation reads the span's slot -- a random 8-byte
+// access per span -- and leaves the verdict in is_new[i]; the second (ClassifyAgain) reads that byte instead of the table.
 struct ClassifyIn {
     const long long* off; const uint8_t* type; const int* slot_of; const u64* table;
-    TypeTable tt; int slug_len;
+    TypeTable tt; int slug_len; uint8_t* is_new_out;
     __device__ __forceinline__ scan::I64x3 operator()(long long i) const {
         const int s = slot_of[i];
         bool is_new = false;
         if (s >= 0) { u64 v = table[s]; is_new = slot_pending(v) && slot_index(v) == (uint32_t)i; }
+        is_new_out[i] = is_new ? 1 : 0;
+        int t = type ? type[i] : 0;
+        if (t >= tt.num) t = tt.num - 1;
+        return scan::I64x3{is_new ? 1 : 0, is_new ? off[i + 1] - off[i] : 0, 3 + tt.len[t] + slug_len};
+    }
+};
+struct ClassifyAgain {
+    const long long* off; const uint8_t* type; const uint8_t* is_new_in;
+    TypeTable tt; int slug_len;
+    __device__ __forceinline__ scan::I64x3 operator()(long long i) const {
+        const bool is_new = is_new_in[i] != 0;
         int t = type ? type[i] : 0;
         if (t >= tt.num) t = tt.num - 1;
         return scan::I64x3{is_new ? 1 : 0, is_new ? off[i + 1] - off[i] : 0, 3 + tt.len[t] + slug_len};
@@ -745,7 +758,8 @@ int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t*
     int* slot_of = (int*)ws.take((size_t)S * 4);
     int* new_list = (int*)ws.take((size_t)S * 4);
     scan::I64x3* agg = (scan::I64x3*)ws.take(scan::agg_bytes<scan::I64x3>(S));
-    if (!slot_of || !new_list || !agg) return ANON_ERR_OOM;
+    uint8_t* is_new = (uint8_t*)ws.take((size_t)S);
+    if (!slot_of || !new_list || !agg || !is_new) return ANON_ERR_OOM;
     const long long* off = (const long long*)d_off;
     const unsigned nb256 = (unsigned)((S + 255) / 256);
     ProfScope prof(ctx, PROF_PSEUDO, 0.0, 6);
@@ -755,7 +769,7 @@ int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t*
     cache_probe_kernel<<<nb256, 256, 0, st>>>(d_bytes, off, S, c->d_table, c->n_slots - 1, c->d_arena,
                                                c->d_entry_off, slot_of, d_full);
     CU_LAUNCH_CHECK(ctx, "cache_probe_kernel");
-    ClassifyIn in{off, d_type, slot_of, c->d_table, tt, slug_len};
+    ClassifyIn in{off, d_type, slot_of, c->d_table, tt, slug_len, is_new};
     scan::reduce_and_scan<scan::I64x3, scan::SumI64x3>(in, S, nullptr, agg, st);
     CU_LAUNCH_CHECK(ctx, "classify scan");
     scan::I64x3* h_tot = (scan::I64x3*)ctx->h_pinned;
@@ -774,7 +788,8 @@ int pseudonymize_impl(anon_ctx* ctx, WsCursor& ws, anon_cache* c, const uint8_t*
     }
     ClassifyOut outf{(long long*)d_out_off, d_hit, new_list, c->d_entry_off, (long long)c->n_unique,
                      (long long)c->arena_used, S};
-    scan::apply<scan::I64x3, scan::SumI64x3>(in, outf, S, nullptr, agg, st);
+    ClassifyAgain in2{off, d_type, is_new, tt, slug_len};
+    scan::apply<scan::I64x3, scan::SumI64x3>(in2, outf, S, nullptr, agg, st);
     CU_LAUNCH_CHECK(ctx, "classify apply");
     if (n_new > 0) {
         cache_insert_kernel<<<(unsigned)((n_new + 127) / 128), 128, 0, st>>>(

@@ -193,7 +193,7 @@ def test_configs4_full_size_50m_spans():
     dev = "cuda:0"
     n_unique, S = 2_000_000, 50_000_000
     data, off, types, key, draws = gen.spans_zipf(n_unique, S, 7, 128, 6, gen.SEED_BASE + 5)      # bench.py's workload
-    ctx = P.Context(0, workspace_bytes=S * 8 + (S // 2048 + 2) * 24 + (64 << 20))
+    ctx = P.Context(0, workspace_bytes=S * 9 + (S // 2048 + 2) * 24 + (64 << 20))
     cache = P.Cache(ctx, n_unique, int(n_unique * 70) + (1 << 20))
     d_bytes, d_off, d_type = (torch.from_numpy(a).to(dev) for a in (data, off, types))
     out = torch.zeros(S * (3 + 13 + 10), dtype=torch.uint8, device=dev)

@@ -172,7 +172,9 @@ def encoder_workload(name, rank, n_records=None):
 
 
 def make_weights_for(desc, seed):
-    return (gen.make_weights_modern if desc.get("arch") == 1 else gen.make_weights)(desc, seed, planted=PLANTED)
+    if desc.get("arch") == 1:       # the arch-1 generator plants the shallow detector only: (alpha, beta, gamma)
+        return gen.make_weights_modern(desc, seed, planted=tuple(PLANTED[:3]))
+    return gen.make_weights(desc, seed, planted=PLANTED)
 
 
 def pack_for(desc, w):
@@ -459,7 +461,8 @@ def run_encoder(args, workload=None, steps=None, warmup=None, e2e_steps=5, recor
         "steps": steps, "warmup": warmup, "ms_per_step": 1e3 * sec / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": label, "tokens_per_step_per_gpu": T, "records_per_step_per_gpu": R,
-                   "spans_per_step_per_gpu": S, "weights": "W2 planted-detector (deep variant), seeded random-init",
+                   "spans_per_step_per_gpu": S,
+                   "weights": "W2 planted-detector (%s), seeded random-init" % ("embedding / head triple" if desc.get("arch") == 1 else "deep variant"),
                    "l2": "inputs larger than L2 (activations %.1f GB per step stream through HBM)" % (T * 19968 / 1e9),
                    "slug_len": SLUG_LEN},
         "records_per_s": recs_all / sec, "spans_per_s": spans_all / sec,

@@ -85,3 +85,13 @@ def test_field_spans_are_the_generated_entity_ranges():
     for r, cs, ce, _t in sp[:200]:
         base = int(rec["rec_off"][r])
         assert rec["text"][base + cs:base + ce].tobytes() in strings
+
+
+def test_bench_weight_recipe_covers_both_architectures():
+    """bench.py's weight recipe (the deep planted detector) must work for the arch-0 and the arch-1 generator: the arch-1 one
+    only takes the shallow triple (`bench.py --workload modern` once died unpacking the longer tuple)."""
+    import bench
+    for name, d in gen.DESCS.items():
+        small = dict(d, layers=1, vocab=min(d["vocab"], 4096))
+        w = bench.make_weights_for(small, 7)
+        assert len(w["layers"]) == 1 and w["W_c"].shape[0] == small["num_labels"], name
